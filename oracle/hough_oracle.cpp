@@ -1,0 +1,401 @@
+// hough_oracle.cpp -- CPU ORACLE for the Hough track-finding hot path of arXiv 1311.2769.
+//
+// *** TEST INFRASTRUCTURE ONLY ***  Only tests/, __graft_entry__.smoke() and bench.py's
+// cpu_baseline / --impl reference legs may load this.  The product (paper_1311_2769_b200/) never does,
+// and this file shares no code, header, table or constant generator with the CUDA path.
+//
+// Plain, slow, single-threaded, obviously-correct restatement of what the path computes:
+//   * PAPER.md:37 (section 3): "Each possible instance of a feature starts with zero votes in the
+//     parameter space, and then, for each piece of input data, votes are added to the feature
+//     instances that would include that input data ... looking for local maxima in the parameter
+//     space ... further computations ... confirm the existence of the track".
+//   * PAPER.md:45 (section 3): two-parameter space for curved tracks through the origin; curved
+//     displaced tracks need three parameters.
+//   * BASELINE.json north_star (B:L5): parameters phi0, signed q/pT, d0; one vote per (phi0, d0)
+//     column; 3x3(x3) local maximum above a threshold; hit association + duplicate removal; bin
+//     indices from one prescribed IEEE fp32 formula (host: -ffp-contract=off).
+// The paper prints no formula, so every definition below is a reading recorded in DESIGN.md
+// ("Readings", D1-D9 / S1-S20 of SURVEY.md section 8(c)).  Each function names the reading it follows.
+//
+// There is no windowing, sorting, blocking or fusion here: the vote is a full scan over every
+// (hit, phi0 column, d0 slice).  Build: g++ -O2 -ffp-contract=off (no -ffast-math, no -march=native).
+//
+// Pins (tests/test_oracle_*.py, run with -m "not gpu"): V1 brute force in double from the
+// tangent-chord construction, V2 noiseless helix -> its own bin, V3 closed-form vote count,
+// V4 linearity/permutation, V5 2-D special case, V6 quarter-turn shift, V7 peak definition on
+// constructed volumes, V8 brute-force vs indexed assignment.  No function here is "parity unpinned".
+
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+
+extern "C" {
+
+typedef struct {
+    int32_t n_phi, n_qpt, n_d0;
+    float qpt_min, qpt_max;   // GeV^-1, half-open [min, max)
+    float d0_min, d0_max;     // cm; ignored when n_d0 == 1
+} orc_binning;
+
+typedef struct {
+    int32_t event, k, i, j, votes;
+    float phi0, qpt, d0;
+} orc_candidate;              // 32 bytes
+
+}  // extern "C"
+
+namespace {
+
+const double kPi = 3.14159265358979323846;
+const double kGeVPerTeslaCm = 0.00299792458;   // pT[GeV] = K * Bz[T] * R[cm]   (D1)
+
+// D2 -- plan constants, double -> fp32.
+struct Tables {
+    std::vector<float> cosT, sinT;     // [n_phi]  phi0 column centres
+    std::vector<float> d0c, td0, d0sq; // [n_d0]
+    float A_f, qmin, inv_wq;
+};
+
+bool valid_binning(const orc_binning* b) {
+    return b && b->n_phi > 0 && b->n_phi % 4 == 0 && b->n_qpt > 0 && b->n_d0 > 0 &&
+           b->qpt_max > b->qpt_min && (b->n_d0 == 1 || b->d0_max > b->d0_min);
+}
+
+Tables make_tables(const orc_binning& b, float bz) {
+    Tables t;
+    t.A_f = (float)(0.5 * kGeVPerTeslaCm * (double)bz);
+    t.qmin = b.qpt_min;
+    t.inv_wq = (float)((double)b.n_qpt / ((double)b.qpt_max - (double)b.qpt_min));
+    const int n = b.n_phi, q = n / 4;
+    t.cosT.resize(n);
+    t.sinT.resize(n);
+    for (int i = 0; i < q; ++i) {                    // first quadrant from libm, in double
+        const double theta = ((double)i + 0.5) * (2.0 * kPi / (double)n);
+        t.cosT[i] = (float)std::cos(theta);
+        t.sinT[i] = (float)std::sin(theta);
+    }
+    for (int i = 0; i + q < n; ++i) {                // other quadrants by exact symmetry (S6)
+        t.cosT[i + q] = -t.sinT[i];
+        t.sinT[i + q] = t.cosT[i];
+    }
+    t.d0c.resize(b.n_d0);
+    t.td0.resize(b.n_d0);
+    t.d0sq.resize(b.n_d0);
+    for (int k = 0; k < b.n_d0; ++k) {
+        if (b.n_d0 == 1) {
+            t.d0c[k] = 0.0f;
+        } else {
+            t.d0c[k] = (float)((double)b.d0_min +
+                               ((double)k + 0.5) * ((double)b.d0_max - (double)b.d0_min) / (double)b.n_d0);
+        }
+        t.td0[k] = 2.0f * t.d0c[k];
+        t.d0sq[k] = t.d0c[k] * t.d0c[k];
+    }
+    return t;
+}
+
+// D3 -- the q/pT bin of hit (x, y, r2) in column (i, k), or -1 when the hit casts no vote there.
+// Every fp32 operation is individually rounded (no FMA: -ffp-contract=off), in exactly this order.
+inline int vote_bin(const Tables& t, int n_qpt, float x, float y, float r2, int i, int k) {
+    const float c = t.cosT[i], s = t.sinT[i];
+    const float yc = y * c;
+    const float xs = x * s;
+    const float w = yc - xs;                 // w = p . n_hat
+    const float xc = x * c;
+    const float ys = y * s;
+    const float f = xc + ys;                 // f = p . t_hat
+    if (!(f > 0.0f)) return -1;              // forward branch only (S4)
+    const float num = t.d0c[k] - w;
+    const float tw = t.td0[k] * w;
+    const float d1 = r2 - tw;
+    const float den = d1 + t.d0sq[k];
+    const float g = t.A_f * den;
+    const float rinv = 1.0f / g;             // IEEE-correct reciprocal
+    const float v = num * rinv;
+    const float dv = v - t.qmin;
+    const float tt = dv * t.inv_wq;
+    if (!(tt >= 0.0f && tt < (float)n_qpt)) return -1;   // range test; NaN/inf fall out here (S5)
+    return (int)tt;                          // tt >= 0: truncation == floor
+}
+
+inline float hit_r2(float x, float y) {
+    const float xx = x * x;
+    const float yy = y * y;
+    return xx + yy;
+}
+
+// D5 -- offset order: (dk, di, dj) lexicographically below (0,0,0)?
+inline bool offset_is_before(int dk, int di, int dj) {
+    if (dk != 0) return dk < 0;
+    if (di != 0) return di < 0;
+    return dj < 0;
+}
+
+}  // namespace
+
+extern "C" {
+
+// D2: export the plan constants (for the pins that check table symmetry / exact representability).
+// consts = {A_f, qmin, inv_wq}.  Any output pointer may be null.
+int orc_tables(const orc_binning* b, float bz, float* cosT, float* sinT, float* d0c, float* td0,
+               float* d0sq, float* consts) {
+    if (!valid_binning(b)) return -1;
+    Tables t = make_tables(*b, bz);
+    if (cosT) std::memcpy(cosT, t.cosT.data(), sizeof(float) * b->n_phi);
+    if (sinT) std::memcpy(sinT, t.sinT.data(), sizeof(float) * b->n_phi);
+    if (d0c) std::memcpy(d0c, t.d0c.data(), sizeof(float) * b->n_d0);
+    if (td0) std::memcpy(td0, t.td0.data(), sizeof(float) * b->n_d0);
+    if (d0sq) std::memcpy(d0sq, t.d0sq.data(), sizeof(float) * b->n_d0);
+    if (consts) { consts[0] = t.A_f; consts[1] = t.qmin; consts[2] = t.inv_wq; }
+    return 0;
+}
+
+// D3/D4 -- vote.  accum is int32 [n_events][k_hi-k_lo][n_phi][n_qpt] (j fastest), OVERWRITTEN
+// ("starts with zero votes").  [k_lo, k_hi) restricts the d0 slices computed; the full
+// accumulator is (0, n_d0).  Returns the number of votes cast, or <0 on bad arguments.
+long long orc_vote(const orc_binning* b, float bz, const float* hits_xy, int32_t n_hits,
+                   const int32_t* event_offsets, int32_t n_events, int32_t k_lo, int32_t k_hi,
+                   int32_t* accum) {
+    if (!valid_binning(b) || n_hits < 0 || n_events < 0 || !event_offsets || !accum) return -1;
+    if (k_lo < 0 || k_hi > b->n_d0 || k_lo >= k_hi) return -1;
+    if (n_hits > 0 && !hits_xy) return -1;
+    const Tables t = make_tables(*b, bz);
+    const int nk = k_hi - k_lo;
+    const size_t per_event = (size_t)nk * b->n_phi * b->n_qpt;
+    std::memset(accum, 0, sizeof(int32_t) * per_event * (size_t)n_events);
+    long long votes = 0;
+    for (int e = 0; e < n_events; ++e) {
+        int32_t* acc = accum + per_event * (size_t)e;
+        for (int h = event_offsets[e]; h < event_offsets[e + 1]; ++h) {
+            const float x = hits_xy[2 * (size_t)h], y = hits_xy[2 * (size_t)h + 1];
+            const float r2 = hit_r2(x, y);
+            for (int i = 0; i < b->n_phi; ++i) {
+                for (int k = k_lo; k < k_hi; ++k) {
+                    const int j = vote_bin(t, b->n_qpt, x, y, r2, i, k);
+                    if (j < 0) continue;
+                    acc[((size_t)(k - k_lo) * b->n_phi + i) * b->n_qpt + j] += 1;
+                    ++votes;
+                }
+            }
+        }
+    }
+    return votes;
+}
+
+// D3 for sampled columns: rows[s][0..n_qpt) = accumulator column (event, k, i) of sample s,
+// computed one by one (full-size parity on sampled outputs).  cols = int32 [n_samples][3] = (e, k, i).
+int orc_vote_columns(const orc_binning* b, float bz, const float* hits_xy, int32_t n_hits,
+                     const int32_t* event_offsets, int32_t n_events, const int32_t* cols,
+                     int32_t n_samples, int32_t* rows) {
+    if (!valid_binning(b) || !event_offsets || !cols || !rows) return -1;
+    (void)n_hits;
+    const Tables t = make_tables(*b, bz);
+    std::memset(rows, 0, sizeof(int32_t) * (size_t)n_samples * b->n_qpt);
+    for (int s = 0; s < n_samples; ++s) {
+        const int e = cols[3 * s], k = cols[3 * s + 1], i = cols[3 * s + 2];
+        if (e < 0 || e >= n_events || k < 0 || k >= b->n_d0 || i < 0 || i >= b->n_phi) return -1;
+        for (int h = event_offsets[e]; h < event_offsets[e + 1]; ++h) {
+            const float x = hits_xy[2 * (size_t)h], y = hits_xy[2 * (size_t)h + 1];
+            const int j = vote_bin(t, b->n_qpt, x, y, hit_r2(x, y), i, k);
+            if (j >= 0) rows[(size_t)s * b->n_qpt + j] += 1;
+        }
+    }
+    return 0;
+}
+
+// D3 per hit: number of (i, k) columns in which hit h votes (the independent counter of pin V3).
+int orc_votes_per_hit(const orc_binning* b, float bz, const float* hits_xy, int32_t n_hits,
+                      int32_t* votes_per_hit) {
+    if (!valid_binning(b) || !votes_per_hit) return -1;
+    const Tables t = make_tables(*b, bz);
+    for (int h = 0; h < n_hits; ++h) {
+        const float x = hits_xy[2 * (size_t)h], y = hits_xy[2 * (size_t)h + 1];
+        const float r2 = hit_r2(x, y);
+        int n = 0;
+        for (int i = 0; i < b->n_phi; ++i)
+            for (int k = 0; k < b->n_d0; ++k)
+                if (vote_bin(t, b->n_qpt, x, y, r2, i, k) >= 0) ++n;
+        votes_per_hit[h] = n;
+    }
+    return 0;
+}
+
+// D5/D6/D7 -- peaks.  accum: int32 [n_events][k_hi-k_lo][n_phi][n_qpt] holding global slices
+// [k_lo, k_hi).  Peaks are reported for slices [ko_lo, ko_hi), which requires every EXISTING
+// neighbour slice (ko_lo-1 .. ko_hi, clipped to [0, n_d0)) to lie inside [k_lo, k_hi).
+// Full volume: k_lo = ko_lo = 0, k_hi = ko_hi = n_d0.
+// cand_offsets [n_events+1] = exclusive scan of the TRUE per-event counts; records are written only
+// for global rank < capacity (S12).  Returns the total number of peaks, or <0 on bad arguments.
+long long orc_find_peaks(const orc_binning* b, const int32_t* accum, int32_t n_events, int32_t k_lo,
+                         int32_t k_hi, int32_t ko_lo, int32_t ko_hi, int32_t threshold,
+                         orc_candidate* cands, long long capacity, int32_t* cand_offsets) {
+    if (!valid_binning(b) || !accum || !cand_offsets || n_events < 0) return -1;
+    if (k_lo < 0 || k_hi > b->n_d0 || k_lo >= k_hi || ko_lo < k_lo || ko_hi > k_hi || ko_lo > ko_hi) return -1;
+    if (ko_lo < ko_hi) {
+        const int need_lo = ko_lo - 1 < 0 ? 0 : ko_lo - 1;
+        const int need_hi = ko_hi + 1 > b->n_d0 ? b->n_d0 : ko_hi + 1;
+        if (need_lo < k_lo || need_hi > k_hi) return -1;
+    }
+    const int nphi = b->n_phi, nq = b->n_qpt, nd = b->n_d0;
+    const int nk = k_hi - k_lo;
+    const size_t per_event = (size_t)nk * nphi * nq;
+    const float wq = (float)(((double)b->qpt_max - (double)b->qpt_min) / (double)nq);
+    const float wphi = (float)((2.0 * kPi) / (double)nphi);
+    const float wd = (float)(((double)b->d0_max - (double)b->d0_min) / (double)nd);
+    const float two_pi_f = (float)(2.0 * kPi);
+    long long total = 0;
+    for (int e = 0; e < n_events; ++e) {
+        cand_offsets[e] = (int32_t)total;
+        const int32_t* acc = accum + per_event * (size_t)e;
+        for (int k = ko_lo; k < ko_hi; ++k)
+            for (int i = 0; i < nphi; ++i)
+                for (int j = 0; j < nq; ++j) {
+                    const int32_t a = acc[((size_t)(k - k_lo) * nphi + i) * nq + j];
+                    if (a < threshold) continue;                                   // S9: a >= threshold
+                    bool peak = true;
+                    long long S = 0, Sj = 0, Si = 0, Sk = 0;
+                    for (int dk = -1; dk <= 1 && peak; ++dk) {
+                        const int kk = k + dk;
+                        if (kk < 0 || kk >= nd) continue;                          // clipped in d0 (S10)
+                        for (int di = -1; di <= 1 && peak; ++di) {
+                            const int ii = (i + di + nphi) % nphi;                 // phi0 is cyclic (S10)
+                            for (int dj = -1; dj <= 1; ++dj) {
+                                const int jj = j + dj;
+                                if (jj < 0 || jj >= nq) continue;                  // clipped in q/pT
+                                const int32_t v = acc[((size_t)(kk - k_lo) * nphi + ii) * nq + jj];
+                                S += v; Sj += (long long)v * dj; Si += (long long)v * di; Sk += (long long)v * dk;
+                                if (dk == 0 && di == 0 && dj == 0) continue;
+                                if (offset_is_before(dk, di, dj)) { if (!(a > v)) { peak = false; break; } }
+                                else                              { if (!(a >= v)) { peak = false; break; } }
+                            }
+                        }
+                    }
+                    if (!peak) continue;
+                    if (cands && total < capacity) {
+                        orc_candidate& c = cands[total];
+                        c.event = e; c.k = k; c.i = i; c.j = j; c.votes = a;
+                        const float fS = (float)S;                                  // D7 centroid
+                        const float oj = (float)Sj / fS;
+                        const float oi = (float)Si / fS;
+                        const float ok = (float)Sk / fS;
+                        const float tj = ((float)j + 0.5f) + oj;
+                        c.qpt = b->qpt_min + tj * wq;
+                        const float ti = ((float)i + 0.5f) + oi;
+                        float ph = ti * wphi;
+                        if (ph < 0.0f) ph = ph + two_pi_f;
+                        else if (ph >= two_pi_f) ph = ph - two_pi_f;
+                        c.phi0 = ph;
+                        if (nd == 1) {
+                            c.d0 = 0.0f;
+                        } else {
+                            const float tk = ((float)k + 0.5f) + ok;
+                            c.d0 = b->d0_min + tk * wd;
+                        }
+                    }
+                    ++total;
+                }
+    }
+    cand_offsets[n_events] = (int32_t)total;
+    return total;
+}
+
+// D8 key: (votes, -|dj|, -index) lexicographic, as a 64-bit integer.
+static inline uint64_t assign_key(int32_t votes, int adj, long long index) {
+    return ((uint64_t)(uint32_t)votes << 40) | ((uint64_t)(255 - adj) << 32) |
+           (uint64_t)(0xFFFFFFFFu - (uint32_t)index);
+}
+
+// D9 applied to a filled hit_to_cand.
+static void dedup(int32_t n_hits, long long n_cands, int32_t min_hits, int32_t* hit_to_cand,
+                  int32_t* cand_nhits, uint8_t* cand_keep) {
+    for (long long c = 0; c < n_cands; ++c) cand_nhits[c] = 0;
+    for (int h = 0; h < n_hits; ++h)
+        if (hit_to_cand[h] >= 0) cand_nhits[hit_to_cand[h]] += 1;
+    for (long long c = 0; c < n_cands; ++c) cand_keep[c] = cand_nhits[c] >= min_hits ? 1 : 0;
+    for (int h = 0; h < n_hits; ++h)
+        if (hit_to_cand[h] >= 0 && !cand_keep[hit_to_cand[h]]) hit_to_cand[h] = -1;   // no re-assignment
+}
+
+// D8/D9 -- brute force over (hit, candidate) pairs.  n_cands = min(total, capacity) records present.
+// apply_dedup = 0 returns the raw best candidate per hit (before the min_hits cut).
+int orc_assign_brute(const orc_binning* b, float bz, const float* hits_xy, int32_t n_hits,
+                     const int32_t* event_offsets, int32_t n_events, const orc_candidate* cands,
+                     const int32_t* cand_offsets, long long capacity, int32_t assoc_dj, int32_t min_hits,
+                     int32_t apply_dedup, int32_t* hit_to_cand, int32_t* cand_nhits, uint8_t* cand_keep) {
+    if (!valid_binning(b) || !event_offsets || !cand_offsets || !hit_to_cand) return -1;
+    const Tables t = make_tables(*b, bz);
+    for (int e = 0; e < n_events; ++e) {
+        long long c0 = cand_offsets[e], c1 = cand_offsets[e + 1];
+        if (c1 > capacity) c1 = capacity;
+        for (int h = event_offsets[e]; h < event_offsets[e + 1]; ++h) {
+            const float x = hits_xy[2 * (size_t)h], y = hits_xy[2 * (size_t)h + 1];
+            const float r2 = hit_r2(x, y);
+            uint64_t best = 0;
+            int32_t best_c = -1;
+            for (long long c = c0; c < c1; ++c) {
+                const int jh = vote_bin(t, b->n_qpt, x, y, r2, cands[c].i, cands[c].k);
+                if (jh < 0) continue;
+                const int adj = jh > cands[c].j ? jh - cands[c].j : cands[c].j - jh;
+                if (adj > assoc_dj) continue;
+                const uint64_t key = assign_key(cands[c].votes, adj, c);
+                if (best_c < 0 || key > best) { best = key; best_c = (int32_t)c; }
+            }
+            hit_to_cand[h] = best_c;
+        }
+    }
+    if (apply_dedup) {
+        if (!cand_nhits || !cand_keep) return -1;
+        long long n_cands = cand_offsets[n_events] < capacity ? cand_offsets[n_events] : capacity;
+        dedup(n_hits, n_cands, min_hits, hit_to_cand, cand_nhits, cand_keep);
+    }
+    return 0;
+}
+
+// D8/D9 -- independent indexed version: a dense per-event volume mapping bin -> candidate index,
+// then every hit re-traces ALL its columns (full scan) and probes j in [jh-dj, jh+dj].
+int orc_assign_indexed(const orc_binning* b, float bz, const float* hits_xy, int32_t n_hits,
+                       const int32_t* event_offsets, int32_t n_events, const orc_candidate* cands,
+                       const int32_t* cand_offsets, long long capacity, int32_t assoc_dj, int32_t min_hits,
+                       int32_t apply_dedup, int32_t* hit_to_cand, int32_t* cand_nhits, uint8_t* cand_keep) {
+    if (!valid_binning(b) || !event_offsets || !cand_offsets || !hit_to_cand) return -1;
+    const Tables t = make_tables(*b, bz);
+    const int nphi = b->n_phi, nq = b->n_qpt, nd = b->n_d0;
+    std::vector<int32_t> index((size_t)nd * nphi * nq, -1);
+    for (int e = 0; e < n_events; ++e) {
+        long long c0 = cand_offsets[e], c1 = cand_offsets[e + 1];
+        if (c1 > capacity) c1 = capacity;
+        for (long long c = c0; c < c1; ++c)
+            index[((size_t)cands[c].k * nphi + cands[c].i) * nq + cands[c].j] = (int32_t)c;
+        for (int h = event_offsets[e]; h < event_offsets[e + 1]; ++h) {
+            const float x = hits_xy[2 * (size_t)h], y = hits_xy[2 * (size_t)h + 1];
+            const float r2 = hit_r2(x, y);
+            uint64_t best = 0;
+            int32_t best_c = -1;
+            for (int i = 0; i < nphi; ++i)
+                for (int k = 0; k < nd; ++k) {
+                    const int jh = vote_bin(t, nq, x, y, r2, i, k);
+                    if (jh < 0) continue;
+                    for (int j = jh - assoc_dj; j <= jh + assoc_dj; ++j) {
+                        if (j < 0 || j >= nq) continue;
+                        const int32_t c = index[((size_t)k * nphi + i) * nq + j];
+                        if (c < 0) continue;
+                        const int adj = jh > j ? jh - j : j - jh;
+                        const uint64_t key = assign_key(cands[c].votes, adj, c);
+                        if (best_c < 0 || key > best) { best = key; best_c = c; }
+                    }
+                }
+            hit_to_cand[h] = best_c;
+        }
+        for (long long c = c0; c < c1; ++c)
+            index[((size_t)cands[c].k * nphi + cands[c].i) * nq + cands[c].j] = -1;
+    }
+    if (apply_dedup) {
+        if (!cand_nhits || !cand_keep) return -1;
+        long long n_cands = cand_offsets[n_events] < capacity ? cand_offsets[n_events] : capacity;
+        dedup(n_hits, n_cands, min_hits, hit_to_cand, cand_nhits, cand_keep);
+    }
+    return 0;
+}
+
+}  // extern "C"

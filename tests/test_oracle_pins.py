@@ -1,0 +1,453 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix (no GPU, no CUDA path).
+
+V-numbers follow SURVEY.md section 8(c) "What pins the oracle".  Each pin is chosen so that a
+plausible mistake in oracle/hough_oracle.cpp (dropped term, wrong sign, transposed operand, wrong
+index order, off-by-one in a neighbourhood) fails at least one of them.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from oracle import Oracle
+from workloads import (LAYERS_10, LAYERS_14, generate_events, get_workload, helix_hits)
+
+from helpers import K, brute_peaks, geometric_bins
+
+BZ = 3.8
+
+
+# ----------------------------------------------------------------------------- golden (textbook)
+def _golden_cases(golden_dir):
+    rows = []
+    with open(os.path.join(golden_dir, "circle_chord_cases.txt")) as f:
+        for line in f:
+            line = line.strip()
+            if not line or line.startswith("#"):
+                continue
+            n_phi, i, R, a_deg, q, exp = line.split()
+            rows.append((int(n_phi), int(i), float(R), float(a_deg), int(q), float(exp)))
+    return rows
+
+
+def test_golden_tangent_chord(golden_dir):
+    """tests/golden/circle_chord_cases.txt: pT = 0.3 B R and the tangent-chord theorem."""
+    n_qpt = 256
+    for n_phi, i, R, a_deg, q, exp in _golden_cases(golden_dir):
+        theta = (i + 0.5) * 2.0 * math.pi / n_phi
+        a = math.radians(a_deg)
+        r = 2.0 * R * math.sin(a)
+        ang = theta - q * a
+        hit = np.array([[r * math.cos(ang), r * math.sin(ang)]], np.float32)
+        o = Oracle(n_phi, n_qpt, 1, -1.0, 1.0, bz_tesla=BZ)
+        rows = o.vote_columns(hit, None, [[0, 0, i]])[0]
+        if -1.0 <= exp < 1.0:
+            j = int(math.floor((exp + 1.0) / (2.0 / n_qpt)))
+            assert rows.sum() == 1 and rows[j] == 1, (n_phi, i, R, a_deg, q, exp, np.nonzero(rows))
+        else:
+            assert rows.sum() == 0
+        # mirror column (phi0 + pi) is the backward branch and must not be voted (S4)
+        assert o.vote_columns(hit, None, [[0, 0, (i + n_phi // 2) % n_phi]]).sum() == 0
+
+
+def test_plan_constants():
+    """D2: A = K Bz / 2 = 0.005696056702 for 3.8 T, exact table symmetry, exact d0 tables."""
+    o = Oracle(256, 128, 64, bz_tesla=BZ)
+    t = o.tables()
+    # bz enters as fp32 (3.8f = 3.7999999523...), so A_f is the fp32 nearest 0.5*K*(double)3.8f: one ulp
+    # below fp32(0.005696056702); R(1 GeV) = 1/(2A) = 87.78 cm
+    assert t["A_f"] == np.float32(0.5 * K * float(np.float32(3.8)))
+    assert abs(float(t["A_f"]) - 0.005696056702) < 6e-10 and abs(1.0 / (2.0 * float(t["A_f"])) - 87.78) < 0.01
+    assert t["inv_wq"] == np.float32(64.0) and t["qmin"] == np.float32(-1.0)
+    n = 256
+    th = (np.arange(n) + 0.5) * 2 * np.pi / n
+    assert np.abs(t["cosT"] - np.cos(th)).max() < 1e-7 and np.abs(t["sinT"] - np.sin(th)).max() < 1e-7
+    q = n // 4
+    assert np.array_equal(t["cosT"][q:], -t["sinT"][:-q]) and np.array_equal(t["sinT"][q:], t["cosT"][:-q])
+    d0 = -20.0 + (np.arange(64) + 0.5) * 40.0 / 64
+    assert np.array_equal(t["d0c"].astype(np.float64), d0)           # exactly representable
+    assert np.array_equal(t["td0"].astype(np.float64), 2 * d0)
+    assert np.array_equal(t["d0sq"].astype(np.float64), d0 * d0)
+    t2 = Oracle(64, 32, 1, bz_tesla=BZ).tables()
+    assert t2["d0c"][0] == 0 and t2["td0"][0] == 0 and t2["d0sq"][0] == 0
+
+
+# ----------------------------------------------------------------------------- V1
+@pytest.mark.parametrize("seed", [0, 1, 2, 3])
+@pytest.mark.parametrize("shape", [(8, 8, 1), (8, 8, 4), (16, 12, 3)])
+def test_v1_bruteforce_double_geometry(seed, shape):
+    n_phi, n_qpt, n_d0 = shape
+    rng = np.random.default_rng(100 + seed)
+    r = rng.uniform(4.0, 110.0, 8)
+    ph = rng.uniform(0, 2 * np.pi, 8)
+    hits = np.stack([r * np.cos(ph), r * np.sin(ph)], 1).astype(np.float32)
+    qr = (1.0, 3.0)[seed % 2]          # the wider range makes inner-layer hits vote in many columns
+    o = Oracle(n_phi, n_qpt, n_d0, -qr, qr, -20.0, 20.0, BZ)
+    n_checked = 0
+    for h in range(hits.shape[0]):
+        acc, _ = o.vote(hits[h:h + 1])
+        for (_, k, i, j, safe) in geometric_bins(hits[h:h + 1], n_phi, n_qpt, n_d0, -qr, qr, -20.0, 20.0, BZ):
+            if not safe:
+                continue
+            col = acc[0, k, i]
+            if j < 0:
+                assert col.sum() == 0, (h, k, i)
+            else:
+                assert col.sum() == 1 and col[j] == 1, (h, k, i, j, np.nonzero(col))
+            n_checked += 1
+    assert n_checked > 0.9 * hits.shape[0] * n_phi * n_d0
+
+
+# ----------------------------------------------------------------------------- V2
+@pytest.mark.parametrize("shape,ijk", [((256, 256, 1), (37, 200, 0)), ((256, 128, 64), (201, 30, 40)),
+                                       ((256, 128, 64), (5, 100, 12)), ((1024, 512, 128), (700, 260, 64))])
+def test_v2_noiseless_helix_peaks_in_its_own_bin(shape, ijk):
+    n_phi, n_qpt, n_d0 = shape
+    i, j, k = ijk
+    phi0 = (i + 0.5) * 2 * math.pi / n_phi
+    qpt = -1.0 + (j + 0.5) * 2.0 / n_qpt
+    d0 = 0.0 if n_d0 == 1 else -20.0 + (k + 0.5) * 40.0 / n_d0
+    hits = helix_hits(phi0, qpt, d0, LAYERS_10, BZ)
+    n = hits.shape[0]
+    assert n >= 7            # layers inside |d0| are never crossed
+    o = Oracle(n_phi, n_qpt, n_d0, bz_tesla=BZ)
+    k_lo, k_hi = max(0, k - 2), min(n_d0, k + 3)
+    acc, _ = o.vote(hits, k_range=(k_lo, k_hi))
+    assert acc[0, k - k_lo, i, j] == n                       # every hit votes for the true bin
+    assert (acc == n).sum() == 1 and acc.max() == n          # and it is the unique maximum
+    ko = (max(k_lo, k - 1) if k_lo > 0 else 0, min(k_hi, k + 2) if k_hi < n_d0 else n_d0)
+    c = o.find_peaks(acc, n, k_range=(k_lo, k_hi), k_out=ko)
+    assert c.total == 1
+    rec = c.records[0]
+    assert (rec["k"], rec["i"], rec["j"], rec["votes"]) == (k, i, j, n)
+    assert abs(rec["qpt"] - qpt) <= 0.5 * 2.0 / n_qpt
+    assert abs(rec["phi0"] - phi0) <= 0.5 * 2 * math.pi / n_phi
+    if n_d0 > 1:
+        assert abs(rec["d0"] - d0) <= 0.5 * 40.0 / n_d0
+    if n_d0 <= 64 and n_phi <= 256:
+        full, _ = o.vote(hits)
+        cf = o.find_peaks(full, n)
+        assert cf.total == 1 and cf.records[0] == rec
+        h2c, nh, keep = o.assign_brute(hits, None, cf, 1, n)
+        assert (h2c == 0).all() and nh[0] == n and keep[0] == 1
+
+
+# ----------------------------------------------------------------------------- V3
+def test_v3_closed_form_vote_count():
+    w = get_workload(0)
+    b = generate_events(w)
+    o = Oracle.from_binning(w.binning, w.bz_tesla)
+    acc, votes = o.vote(b.hits_xy, b.event_offsets)
+    vph = o.votes_per_hit(b.hits_xy)
+    assert votes == int(acc.sum()) == int(vph.sum())
+    A = 0.5 * K * w.bz_tesla
+    r = np.hypot(b.hits_xy[:, 0].astype(np.float64), b.hits_xy[:, 1].astype(np.float64))
+    arg = np.minimum(A * r * 1.0, 1.0)
+    expect = w.binning.n_phi * np.arcsin(arg) / np.pi
+    assert np.abs(vph - expect).max() <= 1.0
+    # every in-range column of a hit gets exactly one vote, never two
+    one, _ = o.vote(b.hits_xy[:1])
+    assert one.sum(axis=-1).max() == 1
+
+
+def test_v3_3d_count_matches_counter_and_geometry():
+    rng = np.random.default_rng(7)
+    r = np.array(LAYERS_10)[rng.integers(0, 10, 24)]
+    ph = rng.uniform(0, 2 * np.pi, 24)
+    hits = np.stack([r * np.cos(ph), r * np.sin(ph)], 1).astype(np.float32)
+    o = Oracle(32, 16, 8, bz_tesla=BZ)
+    acc, votes = o.vote(hits)
+    assert votes == acc.sum() == o.votes_per_hit(hits).sum()
+    g = geometric_bins(hits, 32, 16, 8, -1.0, 1.0, -20.0, 20.0, BZ)
+    n_geo = sum(1 for (_, _, _, j, _) in g if j >= 0)
+    n_unsafe = sum(1 for (_, _, _, _, s) in g if not s)
+    assert abs(n_geo - votes) <= n_unsafe
+
+
+# ----------------------------------------------------------------------------- V4
+def test_v4_linearity_permutation_batching():
+    w = get_workload(1)
+    b = generate_events(w)
+    o = Oracle(64, 32, 8, bz_tesla=BZ)
+    hits = b.hits_xy[:400]
+    acc, _ = o.vote(hits)
+    a1, _ = o.vote(hits[:150])
+    a2, _ = o.vote(hits[150:])
+    assert np.array_equal(acc, a1 + a2)
+    perm = np.random.default_rng(3).permutation(hits.shape[0])
+    ap, _ = o.vote(hits[perm])
+    assert np.array_equal(acc, ap)
+    off = np.array([0, 150, 150, 400], np.int32)          # includes an empty event
+    ab, _ = o.vote(hits, off)
+    assert np.array_equal(ab[0], a1[0]) and np.array_equal(ab[2], a2[0]) and ab[1].sum() == 0
+    # k-range restriction is a pure slice
+    ak, _ = o.vote(hits, k_range=(2, 5))
+    assert np.array_equal(ak[0], acc[0, 2:5])
+    cols = [[0, 3, 17], [0, 0, 63], [0, 7, 0]]
+    rows = o.vote_columns(hits, None, cols)
+    for s, (_, k, i) in enumerate(cols):
+        assert np.array_equal(rows[s], acc[0, k, i])
+
+
+# ----------------------------------------------------------------------------- V5
+def _tables_py(n_phi):
+    q = n_phi // 4
+    c = np.zeros(n_phi, np.float32)
+    s = np.zeros(n_phi, np.float32)
+    for i in range(q):
+        th = (i + 0.5) * (2.0 * 3.14159265358979323846 / n_phi)
+        c[i] = np.float32(math.cos(th))
+        s[i] = np.float32(math.sin(th))
+    for i in range(n_phi - q):
+        c[i + q] = -s[i]
+        s[i + q] = c[i]
+    return c, s
+
+
+def _vote_2d_numpy(hits, n_phi, n_qpt, qmin, qmax, bz):
+    """Hand-written 2-D special case: v = (0 - w) * (1 / (A r2)), numpy float32 (each op rounded)."""
+    f32 = np.float32
+    c, s = _tables_py(n_phi)
+    A = f32(0.5 * K * bz)
+    inv_wq = f32(n_qpt / (float(qmax) - float(qmin)))
+    acc = np.zeros((n_phi, n_qpt), np.int32)
+    x = hits[:, 0:1].astype(f32)
+    y = hits[:, 1:2].astype(f32)
+    r2 = x * x + y * y
+    w = y * c[None, :] - x * s[None, :]
+    f = x * c[None, :] + y * s[None, :]
+    with np.errstate(all="ignore"):
+        v = (f32(0.0) - w) * (f32(1.0) / (A * r2))
+        t = (v - f32(qmin)) * inv_wq
+    ok = (f > 0) & (t >= 0) & (t < f32(n_qpt))
+    hh, ii = np.nonzero(ok)
+    np.add.at(acc, (ii, t[hh, ii].astype(np.int32)), 1)
+    return acc
+
+
+def test_v5_2d_special_case_bit_exact():
+    w = get_workload(0)
+    b = generate_events(w)
+    bn = w.binning
+    o2 = Oracle.from_binning(bn, w.bz_tesla)
+    acc2, _ = o2.vote(b.hits_xy)
+    ref = _vote_2d_numpy(b.hits_xy, bn.n_phi, bn.n_qpt, bn.qpt_min, bn.qpt_max, w.bz_tesla)
+    assert np.array_equal(acc2[0, 0], ref)
+    # slice with d0 centre exactly 0 of an odd-n_d0 plan == the 2-D accumulator
+    o3 = Oracle(bn.n_phi, bn.n_qpt, 5, bn.qpt_min, bn.qpt_max, -20.0, 20.0, w.bz_tesla)
+    assert o3.tables()["d0c"][2] == 0.0
+    acc3, _ = o3.vote(b.hits_xy, k_range=(2, 3))
+    assert np.array_equal(acc3[0, 0], acc2[0, 0])
+    # and the other slices differ (d0 really enters)
+    accn, _ = o3.vote(b.hits_xy, k_range=(1, 2))
+    assert not np.array_equal(accn[0, 0], acc2[0, 0])
+
+
+# ----------------------------------------------------------------------------- V6
+@pytest.mark.parametrize("cfg,shape", [(0, (256, 256, 1)), (1, (64, 32, 8))])
+def test_v6_quarter_turn_shifts_accumulator_exactly(cfg, shape):
+    w = get_workload(cfg)
+    hits = generate_events(w).hits_xy[:300]
+    o = Oracle(*shape, bz_tesla=BZ)
+    acc, _ = o.vote(hits)
+    rot = hits.copy()
+    for m in (1, 2, 3):
+        rot = np.stack([-rot[:, 1], rot[:, 0]], 1)        # (x, y) -> (-y, x), exact in fp32
+        am, _ = o.vote(rot)
+        assert np.array_equal(am, np.roll(acc, m * shape[0] // 4, axis=2))
+
+
+def test_v6_integer_bin_rotation_statistical():
+    w = get_workload(0)
+    hits = generate_events(w).hits_xy.astype(np.float64)
+    o = Oracle(256, 256, 1, bz_tesla=BZ)
+    acc, votes = o.vote(hits.astype(np.float32))
+    m = 37
+    a = m * 2 * np.pi / 256
+    rot = np.stack([np.cos(a) * hits[:, 0] - np.sin(a) * hits[:, 1],
+                    np.sin(a) * hits[:, 0] + np.cos(a) * hits[:, 1]], 1).astype(np.float32)
+    am, _ = o.vote(rot)
+    l1 = np.abs(am - np.roll(acc, m, axis=2)).sum()
+    assert l1 <= max(8, 4e-3 * votes)      # a handful of edge votes move by one bin; a wrong shift gives ~2*votes
+    assert l1 < 0.02 * votes
+
+
+# ----------------------------------------------------------------------------- V7
+def test_v7_single_cell_and_plateaus():
+    o = Oracle(8, 6, 4, bz_tesla=BZ)
+    T = 5
+    acc = np.zeros((1, 4, 8, 6), np.int32)
+    acc[0, 2, 3, 4] = T
+    c = o.find_peaks(acc, T)
+    assert c.total == 1 and tuple(c.records[0][["k", "i", "j", "votes"]]) == (2, 3, 4, T)
+    assert c.records[0]["qpt"] == np.float32(-1.0 + 4.5 * (2.0 / 6))       # lone cell: centroid = centre
+    assert o.find_peaks(acc, T + 1).total == 0                            # S9: a >= threshold
+    # constant volume: every bin has an equal neighbour "before" it (phi wraps) -> no peak
+    assert o.find_peaks(np.full((1, 4, 8, 6), 3, np.int32), 1).total == 0
+    # two-bin plateaus: exactly one winner, the FIRST in (k, i, j) order
+    for d in [(0, 0, 1), (0, 1, 0), (1, 0, 0), (0, 1, -1), (1, -1, 1), (1, 1, -1)]:
+        acc = np.zeros((1, 4, 8, 6), np.int32)
+        p = (1, 3, 3)
+        q = (1 + d[0], 3 + d[1], 3 + d[2])
+        acc[0][p] = 4
+        acc[0][q] = 4
+        c = o.find_peaks(acc, 1)
+        assert c.total == 1 and tuple(c.records[0][["k", "i", "j"]]) == min(p, q), d
+    # wrap-around in phi0: peak at i = 0 sees i = n_phi-1
+    acc = np.zeros((1, 4, 8, 6), np.int32)
+    acc[0, 1, 0, 2] = 5
+    acc[0, 1, 7, 2] = 6
+    c = o.find_peaks(acc, 1)
+    assert c.total == 1 and tuple(c.records[0][["k", "i", "j"]]) == (1, 7, 2)
+    # centroid wraps into [0, 2pi)
+    assert 0.0 <= c.records[0]["phi0"] < 2 * math.pi
+    # faces in j and k: no wrap there
+    acc = np.zeros((1, 4, 8, 6), np.int32)
+    acc[0, 0, 2, 0] = 5
+    acc[0, 3, 2, 5] = 5
+    acc[0, 0, 5, 5] = 5
+    c = o.find_peaks(acc, 1)
+    assert c.total == 3
+    assert [tuple(r) for r in c.records[["k", "i", "j"]]] == [(0, 2, 0), (0, 5, 5), (3, 2, 5)]   # D6 order
+
+
+@pytest.mark.parametrize("shape", [(1, 8, 8), (3, 8, 5), (4, 12, 7), (2, 4, 9)])
+def test_v7_random_volumes_vs_definition(shape):
+    nd, nphi, nq = shape
+    o = Oracle(nphi, nq, nd, bz_tesla=BZ)
+    rng = np.random.default_rng(nd * 100 + nphi)
+    for trial in range(6):
+        acc = rng.integers(0, 4 + trial, size=(2, nd, nphi, nq)).astype(np.int32)   # many ties
+        thr = 2
+        c = o.find_peaks(acc, thr)
+        exp = []
+        for e in range(2):
+            exp += [(e,) + p for p in brute_peaks(acc[e], thr)]
+        got = [tuple(int(v) for v in r) for r in c.records[["event", "k", "i", "j"]]]
+        assert got == exp
+        assert c.offsets[0] == 0 and c.offsets[2] == len(exp) == c.total
+        assert c.offsets[1] == sum(1 for p in exp if p[0] == 0)
+        for r in c.records:
+            assert r["votes"] == acc[r["event"], r["k"], r["i"], r["j"]]
+        # capacity truncation keeps true counts (S12)
+        if c.total > 2:
+            ct = o.find_peaks(acc, thr, capacity=2)
+            assert ct.total == c.total and len(ct.records) == 2 and np.array_equal(ct.records, c.records[:2])
+            assert np.array_equal(ct.offsets, c.offsets)
+
+
+def test_v7_centroid_integer_moments():
+    o = Oracle(8, 8, 1, bz_tesla=BZ)
+    acc = np.zeros((1, 1, 8, 8), np.int32)
+    acc[0, 0, 4, 4] = 6
+    acc[0, 0, 4, 5] = 2          # +dj
+    acc[0, 0, 3, 4] = 1          # -di
+    c = o.find_peaks(acc, 6)
+    assert c.total == 1
+    r = c.records[0]
+    S = 9.0
+    assert abs(r["qpt"] - (-1.0 + (4.5 + 2.0 / S) * 0.25)) < 1e-6
+    assert abs(r["phi0"] - ((4.5 - 1.0 / S) * 2 * math.pi / 8)) < 1e-6
+    assert r["d0"] == 0.0
+
+
+def test_v7_slab_peaks_equal_full_volume():
+    w = get_workload(1)
+    hits = generate_events(w).hits_xy
+    o = Oracle(64, 32, 16, bz_tesla=BZ)
+    acc, _ = o.vote(hits)
+    full = o.find_peaks(acc, 5)
+    sub = full.records[(full.records["k"] >= 4) & (full.records["k"] < 9)]
+    slab, _ = o.vote(hits, k_range=(3, 10))
+    part = o.find_peaks(slab, 5, k_range=(3, 10), k_out=(4, 9))
+    assert part.total == len(sub) and np.array_equal(part.records, sub)
+
+
+# ----------------------------------------------------------------------------- V8
+@pytest.mark.parametrize("cfg", [0, 1])
+def test_v8_assignment_bruteforce_vs_indexed_and_invariants(cfg):
+    w = get_workload(cfg)
+    b = generate_events(w)
+    o = Oracle.from_binning(w.binning, w.bz_tesla)
+    acc, _ = o.vote(b.hits_xy, b.event_offsets)
+    c = o.find_peaks(acc, w.threshold)
+    raw_b, _, _ = o.assign_brute(b.hits_xy, b.event_offsets, c, 1, w.min_hits, apply_dedup=False)
+    raw_i, _, _ = o.assign_indexed(b.hits_xy, b.event_offsets, c, 1, w.min_hits, apply_dedup=False)
+    assert np.array_equal(raw_b, raw_i)
+    h2c_b, nh_b, keep_b = o.assign_brute(b.hits_xy, b.event_offsets, c, 1, w.min_hits)
+    h2c_i, nh_i, keep_i = o.assign_indexed(b.hits_xy, b.event_offsets, c, 1, w.min_hits)
+    assert np.array_equal(h2c_b, h2c_i) and np.array_equal(nh_b, nh_i) and np.array_equal(keep_b, keep_i)
+    # invariants
+    assert nh_b.sum() == (raw_b >= 0).sum()
+    assert np.array_equal(nh_b, np.bincount(raw_b[raw_b >= 0], minlength=c.total))
+    assert np.array_equal(keep_b.astype(bool), nh_b >= w.min_hits)
+    assert np.array_equal(h2c_b, np.where((raw_b >= 0) & keep_b.astype(bool)[np.maximum(raw_b, 0)], raw_b, -1))
+    # every assigned hit is compatible with its candidate: its own vote column holds a bin within dj
+    for h in np.nonzero(raw_b >= 0)[0][:200]:
+        r = c.records[raw_b[h]]
+        col = o.vote_columns(b.hits_xy[h:h + 1], None, [[0, r["k"], r["i"]]])[0]
+        jh = np.nonzero(col)[0]
+        assert len(jh) == 1 and abs(int(jh[0]) - int(r["j"])) <= 1
+
+
+def test_v8_best_candidate_key_order():
+    """D8: more votes wins; then smaller |dj|; then the smaller index."""
+    w = get_workload(0)
+    o = Oracle(256, 256, 1, bz_tesla=BZ)
+    i = 40
+    phi0 = (i + 0.5) * 2 * math.pi / 256
+    qpt = -1.0 + 100.5 * 2.0 / 256
+    hits = helix_hits(phi0, qpt, 0.0, LAYERS_10, BZ)[:1]
+    from oracle import CAND_DTYPE, OracleCandidates
+
+    def cands(lst):
+        rec = np.zeros(len(lst), CAND_DTYPE)
+        for n, (ii, jj, vv) in enumerate(lst):
+            rec[n]["i"], rec[n]["j"], rec[n]["votes"] = ii, jj, vv
+        return OracleCandidates(rec, np.array([0, len(lst)], np.int32), len(lst))
+
+    def best(lst, dj=1):
+        return int(o.assign_brute(hits, None, cands(lst), dj, 0, apply_dedup=False)[0][0])
+
+    assert best([(i, 100, 5)]) == 0
+    assert best([(i, 102, 9)]) == -1 and best([(i, 102, 9)], dj=2) == 0
+    assert best([(i, 101, 5), (i, 100, 5)]) == 1            # smaller |dj| wins at equal votes
+    assert best([(i, 101, 6), (i, 100, 5)]) == 0            # votes dominate |dj|
+    assert best([(i, 99, 5), (i, 101, 5)]) == 0             # equal key -> smaller index
+    assert best([((i + 128) % 256, 100, 50)]) == -1         # backward column is never compatible
+    for lst in ([(i, 101, 5), (i, 100, 5)], [(i, 99, 5), (i, 101, 5)], [(i, 101, 6), (i, 100, 5)]):
+        assert best(lst) == int(o.assign_indexed(hits, None, cands(lst), 1, 0, apply_dedup=False)[0][0])
+
+
+def test_v8_capacity_limits_participants():
+    w = get_workload(1)
+    b = generate_events(w)
+    o = Oracle.from_binning(w.binning, w.bz_tesla)
+    acc, _ = o.vote(b.hits_xy)
+    c = o.find_peaks(acc, w.threshold)
+    cap = c.total // 2
+    ct = o.find_peaks(acc, w.threshold, capacity=cap)
+    h_b, nh_b, _ = o.assign_brute(b.hits_xy, None, ct, 1, w.min_hits, capacity=cap)
+    h_i, nh_i, _ = o.assign_indexed(b.hits_xy, None, ct, 1, w.min_hits, capacity=cap)
+    assert np.array_equal(h_b, h_i) and np.array_equal(nh_b, nh_i) and h_b.max() < cap and len(nh_b) == cap
+
+
+# ----------------------------------------------------------------------------- workload sanity
+def test_workload_shapes_match_baseline():
+    """Hit counts of the generated configs sit where BASELINE.json says ("about 210", "about 33k" ...)."""
+    exp = {0: (205, 215), 1: (1900, 2010), 2: (32000, 34000), 4: (155000, 170000)}
+    for cfg, (lo, hi) in exp.items():
+        w = get_workload(cfg)
+        b = generate_events(w)
+        assert lo <= b.n_hits <= hi, (cfg, b.n_hits)
+        r = np.hypot(b.hits_xy[:, 0].astype(np.float64), b.hits_xy[:, 1])
+        lay = np.array(w.layers)
+        assert np.abs(r[:, None] - lay[None, :]).min(axis=1).max() < 1e-4     # every hit sits on a layer
+    w3 = get_workload(3)
+    b3 = generate_events(w3, events=range(4))
+    per = np.diff(b3.event_offsets)
+    assert ((per > 8000) & (per < 9100)).all()
+    # event e is the same whether generated alone or in a batch (per-event Philox key)
+    assert np.array_equal(generate_events(w3, events=[2]).hits_xy, b3.event(2))
+    assert len(LAYERS_14) == 14
