@@ -1,0 +1,158 @@
+/* hough.h -- C ABI of libhough_b200: Hough-transform track finding (arXiv 1311.2769) on one B200 (sm_100a).
+ *
+ * The paper states the method in words only (section 3):
+ *   "Each possible instance of a feature starts with zero votes in the parameter space, and then, for each
+ *    piece of input data, votes are added to the feature instances that would include that input data.
+ *    After all input data has been processed ... looking for local maxima in the parameter space.  After
+ *    the initial identification, further computations ... confirm the existence of the track."
+ * and PAPER.md:45: the two-parameter space finds curved tracks through the origin; curved displaced tracks
+ * need three parameters.  BASELINE.json `north_star` (B:L5) fixes the parameters (phi0, signed q/pT, d0),
+ * the call names and the bit-exact fp32 contract.  Every formula below is a reading recorded in DESIGN.md
+ * ("Readings" D1-D9, taken from SURVEY.md section 8(c)).
+ *
+ * Conventions
+ *   - Every function returns an int status (HOUGH_OK = 0, errors < 0), never throws, never exits.
+ *   - Pointers named d_*  are DEVICE pointers owned by the caller (the library never frees them and keeps
+ *     none after the call returns).  Pointers named h_* are HOST pointers.  Plain names are host structs.
+ *   - `cuda_stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).
+ *   - Device-side calls only ENQUEUE work on `cuda_stream` and return: no device synchronisation, no
+ *     device->host read (they can be captured into a CUDA graph).  A plan owns one workspace, so one plan
+ *     serves one stream at a time.
+ *   - Host-detectable argument errors return a negative status and enqueue nothing.
+ *   - Accumulator layout: accum[event][k (d0)][i (phi0)][j (q/pT)], j fastest, tightly packed, int32_t
+ *     (HOUGH_ACC_I32) or uint16_t (HOUGH_ACC_U16).  U16 precondition: no bin exceeds 65535.
+ *   - Hit layout: float xy[n_hits][2] in cm, events concatenated; int32 event_offsets[n_events + 1] with
+ *     event_offsets[0] = 0, event_offsets[n_events] = n_hits, non-decreasing.  Hit order inside an event is
+ *     arbitrary and affects no output.  d_hits_xy must be 8-byte aligned.
+ */
+#ifndef HOUGH_B200_H_
+#define HOUGH_B200_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { HOUGH_OK = 0, HOUGH_ERR_INVALID_ARG = -1, HOUGH_ERR_CUDA = -2, HOUGH_ERR_ALLOC = -3, HOUGH_ERR_UNSUPPORTED = -4 };
+enum { HOUGH_ACC_I32 = 0, HOUGH_ACC_U16 = 1 };
+
+/* Parameter-space binning (B:L5; D2).  n_phi % 4 == 0 (quadrant-symmetric trig tables).  n_d0 == 1 is the
+ * two-parameter space of PAPER.md:45 (single d0 slice with centre exactly 0; d0_min/d0_max ignored). */
+typedef struct {
+    int32_t n_phi, n_qpt, n_d0;
+    float qpt_min, qpt_max;       /* GeV^-1, half-open [min, max) */
+    float d0_min, d0_max;         /* cm */
+    int32_t accum_dtype;          /* HOUGH_ACC_I32 | HOUGH_ACC_U16 */
+} hough_binning;
+
+/* Detector description.  bz_tesla enters the vote formula (A = K*Bz/2, K = 0.00299792458 GeV/(T cm)).
+ * layer_radius_cm (host pointer, copied; may be NULL with n_layers = 0) is used ONLY to size work
+ * (radius classes for hit staging); it never changes a result (S19). */
+typedef struct {
+    float bz_tesla;
+    int32_t n_layers;
+    const float* layer_radius_cm;
+} hough_geometry;
+
+/* Track candidate = local maximum of the accumulator (D5-D7).  32 bytes. */
+typedef struct {
+    int32_t event, k, i, j;       /* bin indices: d0 slice k, phi0 column i, q/pT bin j */
+    int32_t votes;
+    float phi0, qpt, d0;          /* integer-moment centroid over the 3x3(x3) neighbourhood (D7) */
+} hough_candidate;
+
+typedef struct hough_plan hough_plan;   /* opaque: device tables + workspace */
+
+/* hough_plan_create (B:L5 "hough_plan_create(binning, detector geometry)"; D2).
+ * Validates, builds the fp32 tables (cos/sin of the phi0 column centres from libm in double with exact
+ * quadrant symmetry, d0 centres, 2*d0, d0^2, A, qmin, n_qpt/(qmax-qmin)), copies them to the current CUDA
+ * device and allocates workspace for at most max_hits hits in at most max_events events per call.
+ * Errors: INVALID_ARG (null pointers, n_phi % 4, empty ranges, unknown dtype, non-positive sizes),
+ * UNSUPPORTED (bins per event > 2^31-1), ALLOC/CUDA.  *out is untouched on error. */
+int hough_plan_create(const hough_binning* binning, const hough_geometry* geometry, int32_t max_hits,
+                      int32_t max_events, hough_plan** out);
+int hough_plan_destroy(hough_plan* plan);
+
+/* Bytes of an accumulator for n_events events with this plan's binning and dtype (0 if plan is NULL). */
+size_t hough_accum_bytes(const hough_plan* plan, int32_t n_events);
+
+/* hough_vote ("votes are added to the feature instances that would include that input data"; D3/D4).
+ * OVERWRITES d_accum (n_events accumulators) with the votes of exactly these hits: for every hit and every
+ * (phi0 column i, d0 slice k) the one compatible q/pT is solved with the prescribed fp32 sequence
+ *     r2 = x*x + y*y;  w = y*cos_i - x*sin_i;  f = x*cos_i + y*sin_i;  vote only if f > 0;
+ *     num = d0_k - w;  den = (r2 - 2d0_k*w) + d0_k^2;  v = num * (1/(A*den));  t = (v - qmin)*inv_wq;
+ *     vote only if 0 <= t < n_qpt;  j = (int)t;  accum[e][k][i][j] += 1
+ * (each operation rounded to nearest-even, no FMA contraction, IEEE reciprocal).
+ * Errors: INVALID_ARG (null pointers, n_hits > max_hits, n_events > max_events, negative sizes), CUDA. */
+int hough_vote(hough_plan* plan, const float* d_hits_xy, int32_t n_hits, const int32_t* d_event_offsets,
+               int32_t n_events, void* d_accum, void* cuda_stream);
+
+/* hough_find_peaks ("looking for local maxima in the parameter space"; D5-D7).
+ * A bin is a peak iff a >= threshold and, over its 3x3 (n_d0 == 1) or 3x3x3 neighbourhood (phi0 cyclic,
+ * q/pT and d0 clipped), a > b for neighbours at lexicographically smaller offset (dk,di,dj) and a >= b for
+ * the others.  Records are written in ascending (event, k, i, j) order for global rank < capacity;
+ * d_cand_offsets[n_events + 1] always receives the exclusive scan of the TRUE per-event counts (overflow is
+ * not an error: compare d_cand_offsets[n_events] with capacity).  d_cands may be NULL when capacity == 0. */
+int hough_find_peaks(hough_plan* plan, const void* d_accum, int32_t n_events, int32_t threshold,
+                     hough_candidate* d_cands, int32_t capacity, int32_t* d_cand_offsets, void* cuda_stream);
+
+/* hough_assign_hits ("further computations ... confirm the existence of the track"; "cleaned to
+ * ... eliminate duplicate tracks"; D8/D9).
+ * d_hit_to_cand[h] = the candidate of the hit's own event, among those with rank < capacity, whose column
+ * (i,k) the hit votes in at a bin jh with |jh - j| <= assoc_dj, maximising (votes, -|jh-j|, -index); -1 if
+ * none.  d_cand_nhits[c] = hits whose best candidate is c; d_cand_keep[c] = (nhits >= min_hits); hits of a
+ * dropped candidate become -1 (single pass, no re-assignment).  d_cand_nhits / d_cand_keep hold `capacity`
+ * entries; entries at or beyond min(total, capacity) are zeroed.  0 <= assoc_dj <= 15. */
+int hough_assign_hits(hough_plan* plan, const float* d_hits_xy, int32_t n_hits, const int32_t* d_event_offsets,
+                      int32_t n_events, const hough_candidate* d_cands, const int32_t* d_cand_offsets,
+                      int32_t capacity, int32_t assoc_dj, int32_t min_hits, int32_t* d_hit_to_cand,
+                      int32_t* d_cand_nhits, uint8_t* d_cand_keep, void* cuda_stream);
+
+/* Plan options (debug / tuning; results never change).  key "fullscan": 1 = evaluate every (hit,i,k) with
+ * no windowing and vote straight into global memory (the bisecting path of SURVEY section 5).
+ * Also read once at plan creation from the environment: HOUGH_DEBUG_FULLSCAN=1. */
+int hough_plan_set_option(hough_plan* plan, const char* key, int32_t value);
+
+/* Batched multi-event pipeline (B:L5 "a batched multi-event path using CUDA streams and graphs"; B:L10).
+ * Runs vote -> find_peaks -> assign_hits over HOST buffers: events are cut into tiles of tile_events, tiles
+ * are dealt round-robin to n_streams streams, each with its own plan, accumulator and staging buffers; each
+ * stream's tile sequence (H2D hits, kernels, D2H results) is captured once as a CUDA graph and replayed.
+ * h_hits_xy / h_event_offsets and the outputs should be pinned for copies to overlap.
+ * Outputs (host): h_hit_to_cand[n_hits] (indices are GLOBAL candidate ranks, events concatenated, -1 = none),
+ * h_cand_offsets[n_events + 1], h_cands[cand_capacity] (records of rank < cand_capacity),
+ * h_cand_nhits / h_cand_keep [cand_capacity].  Per-tile candidate capacity is tile_cand_capacity; a tile
+ * that overflows it sets *h_overflowed (results for that tile are truncated as in hough_find_peaks). */
+typedef struct hough_pipeline hough_pipeline;
+int hough_pipeline_create(const hough_binning* binning, const hough_geometry* geometry, int32_t tile_events,
+                          int32_t max_hits_per_tile, int32_t tile_cand_capacity, int32_t n_streams,
+                          hough_pipeline** out);
+int hough_pipeline_destroy(hough_pipeline* p);
+int hough_pipeline_run_host(hough_pipeline* p, const float* h_hits_xy, int32_t n_hits,
+                            const int32_t* h_event_offsets, int32_t n_events, int32_t threshold,
+                            int32_t assoc_dj, int32_t min_hits, int32_t* h_hit_to_cand,
+                            int32_t* h_cand_offsets, hough_candidate* h_cands, int32_t cand_capacity,
+                            int32_t* h_cand_nhits, uint8_t* h_cand_keep, int32_t* h_overflowed);
+
+/* Measurement support (K6): peak-rate microbenchmarks for the roofline denominators that
+ * MEASURED_PEAKS.json lacks.  Each runs `iters` launches on cuda_stream, synchronises, and writes the
+ * average operations per second of the best launch to *ops_per_s.  kind:
+ *   0 = shared-memory atomicAdd(u32), conflict-free (lane -> distinct bank), all SMs
+ *   1 = shared-memory atomicAdd(u32), random addresses in a 64 KB tile
+ *   2 = shared-memory load+add+store (non-atomic RMW), conflict-free
+ *   3 = global red.add.u32 to random addresses in a region of `region_bytes` (L2- or HBM-resident)
+ *   4 = fp32 issue rate of the D3 vote sequence (no memory), evaluations per second            */
+int hough_microbench(int32_t kind, size_t region_bytes, int32_t iters, double* ops_per_s, void* cuda_stream);
+
+/* Process-wide number of CUDA kernel launches this library has issued so far (memsets/copies excluded). */
+int64_t hough_kernel_launches(void);
+
+const char* hough_status_string(int status);
+/* Library build identity: "libhough_b200 <version> sm_100a". */
+const char* hough_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HOUGH_B200_H_ */

@@ -1,0 +1,168 @@
+// assign.cu -- A5: hit-to-candidate association and duplicate removal (D8/D9).
+//
+// K4-index : candidate list -> dense lookup (1 bit per bin + rank of the first set bit of each word)
+// K4a      : per hit, re-trace its vote columns (D3) and probe bins jh-dj..jh+dj; 64-bit best key
+// K4b      : decode best key -> hit_to_cand, count hits per candidate
+// K4c      : keep = nhits >= min_hits; hits of dropped candidates -> -1
+#include "common.cuh"
+
+namespace {
+
+__device__ __forceinline__ int find_event_a(const int32_t* __restrict__ off, int n_events, int h) {
+    int lo = 0, hi = n_events;
+    while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (off[mid] <= h) lo = mid; else hi = mid;
+    }
+    return lo;
+}
+
+__global__ void __launch_bounds__(256) cand_index_kernel(HoughConsts c, const hough_candidate* __restrict__ cands,
+                                                         const int32_t* __restrict__ cand_offsets, int n_events,
+                                                         int capacity, uint32_t* __restrict__ mask,
+                                                         int32_t* __restrict__ word_rank) {
+    const int total = min(cand_offsets[n_events], capacity);
+    for (int ci = blockIdx.x * blockDim.x + threadIdx.x; ci < total; ci += gridDim.x * blockDim.x) {
+        const int4 a = __ldg(reinterpret_cast<const int4*>(cands + ci));        // event, k, i, j
+        const int b = (a.y * c.n_phi + a.z) * c.n_qpt + a.w;
+        const size_t word = (size_t)a.x * c.words_per_event + (b >> 5);
+        atomicOr(mask + word, 1u << (b & 31));
+        bool first = ci == 0;
+        if (!first) {
+            const int4 q = __ldg(reinterpret_cast<const int4*>(cands + ci - 1));
+            const int bq = (q.y * c.n_phi + q.z) * c.n_qpt + q.w;
+            first = q.x != a.x || (bq >> 5) != (b >> 5);
+        }
+        if (first) word_rank[word] = ci;
+    }
+}
+
+__device__ __forceinline__ unsigned long long make_key(int votes, int adj, int index) {
+    return ((unsigned long long)(unsigned)votes << 40) | ((unsigned long long)(255 - adj) << 32) |
+           (unsigned long long)(0xFFFFFFFFu - (unsigned)index);
+}
+
+// full-scan association: one thread per (hit, phi0 column)
+__global__ void __launch_bounds__(256) assign_fullscan_kernel(HoughConsts c, const float2* __restrict__ hits, int n_hits,
+                                                              const int32_t* __restrict__ off, int n_events,
+                                                              const hough_candidate* __restrict__ cands,
+                                                              const uint32_t* __restrict__ mask,
+                                                              const int32_t* __restrict__ word_rank, int assoc_dj,
+                                                              unsigned long long* __restrict__ best_key) {
+    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const int h = (int)(t / c.n_phi);
+    const int i = (int)(t - (long long)h * c.n_phi);
+    if (h >= n_hits) return;
+    const float2 p = hits[h];
+    const float2 cs = c.cs[i];
+    float w, f;
+    d3_wf(p.x, p.y, cs.x, cs.y, w, f);
+    if (!(f > 0.0f)) return;
+    const float r2 = d3_r2(p.x, p.y);
+    const int e = find_event_a(off, n_events, h);
+    const uint32_t* emask = mask + (size_t)e * c.words_per_event;
+    const int32_t* erank = word_rank + (size_t)e * c.words_per_event;
+    unsigned long long best = 0ull;
+    for (int k = 0; k < c.n_d0; ++k) {
+        const float4 d = c.d0t[k];
+        const int jh = d3_bin_from_w(w, r2, d.x, d.y, d.z, c.A_f, c.qmin, c.inv_wq, c.nq_f);
+        if (jh < 0) continue;
+        const int row = (k * c.n_phi + i) * c.n_qpt;
+        const int j0 = max(jh - assoc_dj, 0), j1 = min(jh + assoc_dj, c.n_qpt - 1);
+        for (int j = j0; j <= j1; ++j) {
+            const int b = row + j;
+            const uint32_t m = __ldg(emask + (b >> 5));
+            if (!((m >> (b & 31)) & 1u)) continue;
+            const int ci = __ldg(erank + (b >> 5)) + __popc(m & ((1u << (b & 31)) - 1u));
+            const int votes = __ldg(&cands[ci].votes);
+            const unsigned long long key = make_key(votes, abs(jh - j), ci);
+            best = key > best ? key : best;
+        }
+    }
+    if (best) atomicMax(best_key + h, best);
+}
+
+__global__ void __launch_bounds__(256) assign_decode_kernel(const unsigned long long* __restrict__ best_key, int n_hits,
+                                                            int32_t* __restrict__ hit_to_cand,
+                                                            int32_t* __restrict__ cand_nhits) {
+    const int h = blockIdx.x * blockDim.x + threadIdx.x;
+    if (h >= n_hits) return;
+    const unsigned long long key = best_key[h];
+    int ci = -1;
+    if (key) {
+        ci = (int)(0xFFFFFFFFu - (unsigned)(key & 0xFFFFFFFFull));
+        atomicAdd(cand_nhits + ci, 1);
+    }
+    hit_to_cand[h] = ci;
+}
+
+__global__ void __launch_bounds__(256) cand_keep_kernel(const int32_t* __restrict__ cand_nhits, int capacity, int min_hits,
+                                                        const int32_t* __restrict__ cand_offsets, int n_events,
+                                                        uint8_t* __restrict__ cand_keep) {
+    const int total = min(cand_offsets[n_events], capacity);
+    for (int ci = blockIdx.x * blockDim.x + threadIdx.x; ci < capacity; ci += gridDim.x * blockDim.x)
+        cand_keep[ci] = (ci < total && cand_nhits[ci] >= min_hits) ? 1 : 0;
+}
+
+__global__ void __launch_bounds__(256) unassign_kernel(int n_hits, const uint8_t* __restrict__ cand_keep,
+                                                       int32_t* __restrict__ hit_to_cand) {
+    const int h = blockIdx.x * blockDim.x + threadIdx.x;
+    if (h >= n_hits) return;
+    const int ci = hit_to_cand[h];
+    if (ci >= 0 && !cand_keep[ci]) hit_to_cand[h] = -1;
+}
+
+}  // namespace
+
+extern "C" int hough_assign_hits(hough_plan* p, const float* d_hits_xy, int32_t n_hits, const int32_t* d_event_offsets,
+                                 int32_t n_events, const hough_candidate* d_cands, const int32_t* d_cand_offsets,
+                                 int32_t capacity, int32_t assoc_dj, int32_t min_hits, int32_t* d_hit_to_cand,
+                                 int32_t* d_cand_nhits, uint8_t* d_cand_keep, void* cuda_stream) {
+    if (!p || !d_event_offsets || !d_cand_offsets) return HOUGH_ERR_INVALID_ARG;
+    if (n_hits < 0 || n_events < 0 || n_hits > p->max_hits || n_events > p->max_events) return HOUGH_ERR_INVALID_ARG;
+    if (capacity < 0 || assoc_dj < 0 || assoc_dj > 15) return HOUGH_ERR_INVALID_ARG;
+    if (n_hits > 0 && (!d_hits_xy || !d_hit_to_cand)) return HOUGH_ERR_INVALID_ARG;
+    if (capacity > 0 && (!d_cands || !d_cand_nhits || !d_cand_keep)) return HOUGH_ERR_INVALID_ARG;
+    if ((reinterpret_cast<uintptr_t>(d_hits_xy) & 7u) || (reinterpret_cast<uintptr_t>(d_cands) & 15u))
+        return HOUGH_ERR_INVALID_ARG;
+    if (n_events == 0) return n_hits == 0 ? HOUGH_OK : HOUGH_ERR_INVALID_ARG;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+    const size_t n_words = (size_t)n_events * p->c.words_per_event;
+    HOUGH_CUDA_TRY(cudaMemsetAsync(p->d_mask, 0, sizeof(uint32_t) * n_words, st));
+    if (capacity > 0) HOUGH_CUDA_TRY(cudaMemsetAsync(d_cand_nhits, 0, sizeof(int32_t) * (size_t)capacity, st));
+    if (n_hits > 0) HOUGH_CUDA_TRY(cudaMemsetAsync(p->d_best_key, 0, sizeof(unsigned long long) * (size_t)n_hits, st));
+    if (capacity > 0) {
+        const int blocks = min((capacity + 255) / 256, p->sm_count * 8);
+        cand_index_kernel<<<blocks, 256, 0, st>>>(p->c, d_cands, d_cand_offsets, n_events, capacity, p->d_mask,
+                                                  p->d_word_rank);
+        HOUGH_CUDA_TRY(cudaGetLastError());
+        hough_count_launches(1);
+    }
+    if (n_hits > 0) {
+        const float2* hits = reinterpret_cast<const float2*>(d_hits_xy);
+        const long long threads = (long long)n_hits * p->c.n_phi;
+        const long long blocks = (threads + 255) / 256;
+        if (blocks > 0x7fffffffLL) return HOUGH_ERR_UNSUPPORTED;
+        if (capacity > 0) {
+            assign_fullscan_kernel<<<(unsigned)blocks, 256, 0, st>>>(p->c, hits, n_hits, d_event_offsets, n_events, d_cands,
+                                                                     p->d_mask, p->d_word_rank, assoc_dj, p->d_best_key);
+            HOUGH_CUDA_TRY(cudaGetLastError());
+            hough_count_launches(1);
+        }
+        assign_decode_kernel<<<(n_hits + 255) / 256, 256, 0, st>>>(p->d_best_key, n_hits, d_hit_to_cand, d_cand_nhits);
+        HOUGH_CUDA_TRY(cudaGetLastError());
+        hough_count_launches(1);
+    }
+    if (capacity > 0) {
+        const int blocks = min((capacity + 255) / 256, p->sm_count * 8);
+        cand_keep_kernel<<<blocks, 256, 0, st>>>(d_cand_nhits, capacity, min_hits, d_cand_offsets, n_events, d_cand_keep);
+        HOUGH_CUDA_TRY(cudaGetLastError());
+        hough_count_launches(1);
+        if (n_hits > 0) {
+            unassign_kernel<<<(n_hits + 255) / 256, 256, 0, st>>>(n_hits, d_cand_keep, d_hit_to_cand);
+            HOUGH_CUDA_TRY(cudaGetLastError());
+            hough_count_launches(1);
+        }
+    }
+    return HOUGH_OK;
+}

@@ -1,0 +1,93 @@
+// common.cuh -- shared declarations of libhough_b200 (sm_100a only).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include "../../include/hough.h"
+
+#ifndef __CUDA_ARCH__
+#define HOUGH_HOST_ONLY 1
+#endif
+
+#define HOUGH_CUDA_TRY(expr)                         \
+    do {                                             \
+        cudaError_t _e = (expr);                     \
+        if (_e != cudaSuccess) {                     \
+            hough_set_last_cuda_error(_e, #expr);    \
+            return HOUGH_ERR_CUDA;                   \
+        }                                            \
+    } while (0)
+
+void hough_set_last_cuda_error(cudaError_t e, const char* what);
+void hough_count_launches(int n);   // process-wide count of kernel launches issued by the library
+
+// Plan constants passed by value to kernels (D2).
+struct HoughConsts {
+    int32_t n_phi, n_qpt, n_d0;
+    int32_t bins_per_event;       // n_d0 * n_phi * n_qpt
+    int32_t words_per_event;      // ceil(bins_per_event / 32)  (peak bitmask)
+    int32_t is_u16;
+    float A_f, qmin, inv_wq, nq_f;
+    float qpt_min, d0_min;        // centroid (D7)
+    float wq, wphi, wd, two_pi_f;
+    const float2* cs;             // [n_phi] {cos, sin} of the column centres
+    const float4* d0t;            // [n_d0]  {d0c, 2*d0c, d0c^2, 0}
+};
+
+struct hough_plan {
+    hough_binning b;
+    float bz;
+    int32_t max_hits, max_events;
+    int device, sm_count;
+    int fullscan;
+    HoughConsts c;
+    // geometry (work sizing only)
+    int32_t n_layers;
+    float layer_r[64];
+    // device tables
+    float2* d_cs;
+    float4* d_d0t;
+    // workspace: peaks
+    int32_t peak_blocks_per_event;     // blocks of PEAK_BLOCK_BINS bins
+    int32_t* d_peak_block_cnt;         // [max_events * peak_blocks_per_event] counts, scanned in place per event
+    int32_t* d_event_cnt;              // [max_events + 1]
+    uint32_t* d_mask;                  // [max_events * words_per_event] peak bitmask (find_peaks) / candidate bitmask (assign)
+    int32_t* d_word_rank;              // [max_events * words_per_event] rank of the first set bit of each word
+    unsigned long long* d_best_key;    // [max_hits]
+    // workspace: staged hits (K1)
+    float4* d_staged;                  // [max_hits] {x, y, r2, bitcast(original index)}
+    int32_t* d_stage_cnt;              // histogram / offsets
+    size_t stage_cnt_len;
+};
+
+constexpr int PEAK_BLOCK_BINS = 4096;  // bins per peak-scan block (multiple of 32)
+
+// ---------------------------------------------------------------------------------------------
+// D3: the prescribed fp32 vote sequence.  Intrinsics (__f*_rn) are never contracted into FMAs and
+// __frcp_rn is the IEEE-correct reciprocal, so the result is independent of compiler flags.
+// Returns the q/pT bin or -1.
+__device__ __forceinline__ void d3_wf(float x, float y, float c, float s, float& w, float& f) {
+    w = __fsub_rn(__fmul_rn(y, c), __fmul_rn(x, s));
+    f = __fadd_rn(__fmul_rn(x, c), __fmul_rn(y, s));
+}
+
+__device__ __forceinline__ int d3_bin_from_w(float w, float r2, float d0c, float td0, float d0sq, float A_f,
+                                             float qmin, float inv_wq, float nq_f) {
+    const float num = __fsub_rn(d0c, w);
+    const float den = __fadd_rn(__fsub_rn(r2, __fmul_rn(td0, w)), d0sq);
+    const float g = __fmul_rn(A_f, den);
+    const float rinv = __frcp_rn(g);
+    const float v = __fmul_rn(num, rinv);
+    const float t = __fmul_rn(__fsub_rn(v, qmin), inv_wq);
+    if (!(t >= 0.0f && t < nq_f)) return -1;
+    return (int)t;
+}
+
+__device__ __forceinline__ float d3_r2(float x, float y) { return __fadd_rn(__fmul_rn(x, x), __fmul_rn(y, y)); }
+
+// internal entry points (defined in the .cu files)
+int hough_vote_fullscan(hough_plan* p, const float* d_hits_xy, int32_t n_hits, const int32_t* d_event_offsets,
+                        int32_t n_events, void* d_accum, cudaStream_t st);
+int hough_vote_tiled(hough_plan* p, const float* d_hits_xy, int32_t n_hits, const int32_t* d_event_offsets,
+                     int32_t n_events, void* d_accum, cudaStream_t st);

@@ -1,0 +1,169 @@
+// plan.cu -- hough_plan_create / destroy, plan constants (D2), status strings.
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+#include <atomic>
+#include <vector>
+
+#include "common.cuh"
+
+namespace {
+thread_local char g_last_cuda[256] = "";
+std::atomic<long long> g_launches{0};
+}
+
+void hough_count_launches(int n) { g_launches.fetch_add(n, std::memory_order_relaxed); }
+extern "C" int64_t hough_kernel_launches(void) { return (int64_t)g_launches.load(std::memory_order_relaxed); }
+
+void hough_set_last_cuda_error(cudaError_t e, const char* what) {
+    snprintf(g_last_cuda, sizeof(g_last_cuda), "%s: %s", what, cudaGetErrorString(e));
+    if (getenv("HOUGH_VERBOSE")) fprintf(stderr, "[libhough_b200] CUDA error: %s\n", g_last_cuda);
+    (void)cudaGetLastError();
+}
+
+extern "C" const char* hough_status_string(int status) {
+    switch (status) {
+        case HOUGH_OK: return "ok";
+        case HOUGH_ERR_INVALID_ARG: return "invalid argument";
+        case HOUGH_ERR_CUDA: return g_last_cuda[0] ? g_last_cuda : "CUDA error";
+        case HOUGH_ERR_ALLOC: return "allocation failed";
+        case HOUGH_ERR_UNSUPPORTED: return "unsupported configuration";
+        default: return "unknown status";
+    }
+}
+
+extern "C" const char* hough_version(void) { return "libhough_b200 0.1 sm_100a"; }
+
+static void plan_free(hough_plan* p) {
+    if (!p) return;
+    cudaFree(p->d_cs);
+    cudaFree(p->d_d0t);
+    cudaFree(p->d_peak_block_cnt);
+    cudaFree(p->d_event_cnt);
+    cudaFree(p->d_mask);
+    cudaFree(p->d_word_rank);
+    cudaFree(p->d_best_key);
+    cudaFree(p->d_staged);
+    cudaFree(p->d_stage_cnt);
+    delete p;
+}
+
+extern "C" int hough_plan_create(const hough_binning* b, const hough_geometry* g, int32_t max_hits,
+                                 int32_t max_events, hough_plan** out) {
+    if (!b || !g || !out) return HOUGH_ERR_INVALID_ARG;
+    if (b->n_phi <= 0 || b->n_phi % 4 != 0 || b->n_qpt <= 0 || b->n_d0 <= 0) return HOUGH_ERR_INVALID_ARG;
+    if (!(b->qpt_max > b->qpt_min)) return HOUGH_ERR_INVALID_ARG;
+    if (b->n_d0 > 1 && !(b->d0_max > b->d0_min)) return HOUGH_ERR_INVALID_ARG;
+    if (b->accum_dtype != HOUGH_ACC_I32 && b->accum_dtype != HOUGH_ACC_U16) return HOUGH_ERR_INVALID_ARG;
+    if (max_hits <= 0 || max_events <= 0) return HOUGH_ERR_INVALID_ARG;
+    if (g->n_layers < 0 || g->n_layers > 64 || (g->n_layers > 0 && !g->layer_radius_cm)) return HOUGH_ERR_INVALID_ARG;
+    if (!(g->bz_tesla == g->bz_tesla)) return HOUGH_ERR_INVALID_ARG;
+    const long long bins = (long long)b->n_phi * b->n_qpt * b->n_d0;
+    if (bins > 0x7fffffffLL || b->n_qpt >= (1 << 24) || b->n_phi > (1 << 20) || b->n_d0 > (1 << 16))
+        return HOUGH_ERR_UNSUPPORTED;
+
+    hough_plan* p = new (std::nothrow) hough_plan();
+    if (!p) return HOUGH_ERR_ALLOC;
+    memset(p, 0, sizeof(*p));
+    p->b = *b;
+    p->bz = g->bz_tesla;
+    p->max_hits = max_hits;
+    p->max_events = max_events;
+    p->n_layers = g->n_layers;
+    for (int l = 0; l < g->n_layers; ++l) p->layer_r[l] = g->layer_radius_cm[l];
+    const char* env = getenv("HOUGH_DEBUG_FULLSCAN");
+    p->fullscan = (env && env[0] == '1') ? 1 : 0;
+
+    cudaError_t ce = cudaGetDevice(&p->device);
+    if (ce == cudaSuccess) ce = cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, p->device);
+    if (ce != cudaSuccess) { hough_set_last_cuda_error(ce, "cudaGetDevice"); delete p; return HOUGH_ERR_CUDA; }
+
+    // ---- D2: constants, double -> fp32 ----
+    const double kPi = 3.14159265358979323846;
+    HoughConsts& c = p->c;
+    c.n_phi = b->n_phi; c.n_qpt = b->n_qpt; c.n_d0 = b->n_d0;
+    c.bins_per_event = (int32_t)bins;
+    c.words_per_event = (int32_t)((bins + 31) / 32);
+    c.is_u16 = b->accum_dtype == HOUGH_ACC_U16;
+    c.A_f = (float)(0.5 * 0.00299792458 * (double)g->bz_tesla);
+    c.qmin = b->qpt_min;
+    c.inv_wq = (float)((double)b->n_qpt / ((double)b->qpt_max - (double)b->qpt_min));
+    c.nq_f = (float)b->n_qpt;
+    c.qpt_min = b->qpt_min;
+    c.d0_min = b->d0_min;
+    c.wq = (float)(((double)b->qpt_max - (double)b->qpt_min) / (double)b->n_qpt);
+    c.wphi = (float)((2.0 * kPi) / (double)b->n_phi);
+    c.wd = (float)(((double)b->d0_max - (double)b->d0_min) / (double)b->n_d0);
+    c.two_pi_f = (float)(2.0 * kPi);
+
+    std::vector<float2> cs(b->n_phi);
+    const int q = b->n_phi / 4;
+    for (int i = 0; i < q; ++i) {
+        const double th = ((double)i + 0.5) * (2.0 * kPi / (double)b->n_phi);
+        cs[i].x = (float)cos(th);
+        cs[i].y = (float)sin(th);
+    }
+    for (int i = 0; i + q < b->n_phi; ++i) {   // quarter-turn symmetry, exact
+        cs[i + q].x = -cs[i].y;
+        cs[i + q].y = cs[i].x;
+    }
+    std::vector<float4> d0t(b->n_d0);
+    for (int k = 0; k < b->n_d0; ++k) {
+        float d0c = 0.0f;
+        if (b->n_d0 > 1)
+            d0c = (float)((double)b->d0_min + ((double)k + 0.5) * ((double)b->d0_max - (double)b->d0_min) / (double)b->n_d0);
+        d0t[k].x = d0c;
+        d0t[k].y = 2.0f * d0c;
+        d0t[k].z = d0c * d0c;
+        d0t[k].w = 0.0f;
+    }
+
+    p->peak_blocks_per_event = (int32_t)((bins + PEAK_BLOCK_BINS - 1) / PEAK_BLOCK_BINS);
+    const size_t n_words = (size_t)max_events * c.words_per_event;
+    p->stage_cnt_len = (size_t)max_events * 64 * 64 + 1024;
+
+    bool ok = true;
+    auto A = [&](void** ptr, size_t bytes) {
+        if (!ok) return;
+        if (cudaMalloc(ptr, bytes ? bytes : 4) != cudaSuccess) { ok = false; (void)cudaGetLastError(); }
+    };
+    A((void**)&p->d_cs, sizeof(float2) * b->n_phi);
+    A((void**)&p->d_d0t, sizeof(float4) * b->n_d0);
+    A((void**)&p->d_peak_block_cnt, sizeof(int32_t) * (size_t)max_events * p->peak_blocks_per_event);
+    A((void**)&p->d_event_cnt, sizeof(int32_t) * ((size_t)max_events + 1));
+    A((void**)&p->d_mask, sizeof(uint32_t) * n_words);
+    A((void**)&p->d_word_rank, sizeof(int32_t) * n_words);
+    A((void**)&p->d_best_key, sizeof(unsigned long long) * (size_t)max_hits);
+    A((void**)&p->d_staged, sizeof(float4) * (size_t)max_hits);
+    A((void**)&p->d_stage_cnt, sizeof(int32_t) * p->stage_cnt_len);
+    if (!ok) { plan_free(p); return HOUGH_ERR_ALLOC; }
+    if (cudaMemcpy(p->d_cs, cs.data(), sizeof(float2) * b->n_phi, cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(p->d_d0t, d0t.data(), sizeof(float4) * b->n_d0, cudaMemcpyHostToDevice) != cudaSuccess) {
+        hough_set_last_cuda_error(cudaGetLastError(), "table upload");
+        plan_free(p);
+        return HOUGH_ERR_CUDA;
+    }
+    c.cs = p->d_cs;
+    c.d0t = p->d_d0t;
+    *out = p;
+    return HOUGH_OK;
+}
+
+extern "C" int hough_plan_destroy(hough_plan* p) {
+    if (!p) return HOUGH_ERR_INVALID_ARG;
+    plan_free(p);
+    return HOUGH_OK;
+}
+
+extern "C" size_t hough_accum_bytes(const hough_plan* p, int32_t n_events) {
+    if (!p || n_events < 0) return 0;
+    return (size_t)n_events * (size_t)p->c.bins_per_event * (p->c.is_u16 ? 2 : 4);
+}
+
+extern "C" int hough_plan_set_option(hough_plan* p, const char* key, int32_t value) {
+    if (!p || !key) return HOUGH_ERR_INVALID_ARG;
+    if (strcmp(key, "fullscan") == 0) { p->fullscan = value ? 1 : 0; return HOUGH_OK; }
+    return HOUGH_ERR_INVALID_ARG;
+}

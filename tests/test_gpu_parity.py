@@ -1,0 +1,215 @@
+"""-m gpu: the CUDA path through the C ABI vs the CPU oracle, element by element, on the same seeded inputs.
+
+Bar (B:L5): accumulators, peak lists and hit assignments bit-exact; centroids within 1e-5 relative.
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import Oracle
+from workloads import HoughBinning, generate_events, get_workload, helix_hits, LAYERS_10
+from workloads.configs import ACC_I32, ACC_U16
+
+pytestmark = pytest.mark.gpu
+
+from gpu_util import (assert_centroids_close, oracle_peaks_parallel, oracle_vote_parallel, run_cuda)  # noqa: E402
+
+
+def _narrow(acc_i32, binning):
+    if binning.accum_dtype == ACC_U16:
+        assert acc_i32.max() <= 65535          # U16 precondition, asserted on the oracle's int32 counts (D4)
+        return acc_i32.astype(np.uint16)
+    return acc_i32
+
+
+def _compare_all(w, batch, binning=None, capacity=None, fullscan=False, oracle_parallel=False):
+    bn = binning or w.binning
+    o = Oracle.from_binning(bn, w.bz_tesla)
+    if oracle_parallel:
+        acc, votes = oracle_vote_parallel(o, batch.hits_xy, batch.event_offsets)
+        ref = oracle_peaks_parallel(o, acc, w.threshold)
+    else:
+        acc, votes = o.vote(batch.hits_xy, batch.event_offsets)
+        ref = o.find_peaks(acc, w.threshold)
+    cap = ref.total + 7 if capacity is None else capacity
+    got = run_cuda(bn, w.bz_tesla, w.layers, batch.hits_xy, batch.event_offsets, w.threshold, w.assoc_dj, w.min_hits,
+                   cap, fullscan=fullscan)
+    assert np.array_equal(got.accum, _narrow(acc, bn)), "accumulator differs"
+    assert int(got.accum.astype(np.int64).sum()) == votes
+    assert got.total == ref.total and np.array_equal(got.offsets, ref.offsets)
+    n_c = min(cap, ref.total)
+    for f in ("event", "k", "i", "j", "votes"):
+        assert np.array_equal(got.records[f], ref.records[f][:n_c]), f
+    assert_centroids_close(got.records, ref.records[:n_c], bn)
+    ref_c = ref if n_c == ref.total else o.find_peaks(acc, w.threshold, capacity=cap)
+    h2c, nh, keep = o.assign_indexed(batch.hits_xy, batch.event_offsets, ref_c, w.assoc_dj, w.min_hits, capacity=cap)
+    assert np.array_equal(got.hit_to_cand, h2c), "hit_to_cand differs"
+    assert np.array_equal(got.cand_nhits[:n_c], nh) and np.array_equal(got.cand_keep[:n_c], keep)
+    assert not got.cand_nhits[n_c:].any() and not got.cand_keep[n_c:].any()
+    return got, ref
+
+
+@pytest.mark.parametrize("fullscan", [False, True])
+@pytest.mark.parametrize("cfg", [0, 1])
+def test_config_0_1_bit_exact(cfg, fullscan):
+    w = get_workload(cfg)
+    got, ref = _compare_all(w, generate_events(w), fullscan=fullscan)
+    assert ref.total > 0
+
+
+def test_config_2_bit_exact():
+    w = get_workload(2)
+    _compare_all(w, generate_events(w), oracle_parallel=True)
+
+
+def test_config_3_subset_of_events_bit_exact():
+    w = get_workload(3)
+    batch = generate_events(w, events=[0, 1, 513, 1023, 7])
+    _compare_all(w, batch)
+
+
+def test_config_3_fullscan_matches_tiled_on_more_events():
+    """Both CUDA code paths agree with the oracle on a ragged 3-event batch (different hit counts)."""
+    w = get_workload(3)
+    batch = generate_events(w, events=[11, 12, 13])
+    _compare_all(w, batch, fullscan=True)
+
+
+def test_config_4_reduced_bins_bit_exact():
+    """Config-4 hits (162k) into a reduced accumulator the oracle finishes in seconds: many tiles + ragged tail."""
+    w = get_workload(4)
+    batch = generate_events(w)
+    bn = HoughBinning(128, 64, 16, accum_dtype=ACC_U16)
+    o = Oracle.from_binning(bn, w.bz_tesla)
+    acc, votes = oracle_vote_parallel(o, batch.hits_xy, batch.event_offsets)
+    assert acc.max() <= 65535
+    got = run_cuda(bn, w.bz_tesla, w.layers, batch.hits_xy, batch.event_offsets, 10 ** 6, 1, 1, 16)
+    assert np.array_equal(got.accum, acc.astype(np.uint16))
+    assert got.total == 0 and (got.hit_to_cand == -1).all()
+
+
+def test_config_4_full_size_sampled_columns_and_slab_peaks():
+    """Full config-4 size in the launch configuration bench.py uses; outputs the oracle computes one by one."""
+    w = get_workload(4)
+    bn = w.binning
+    batch = generate_events(w)
+    o = Oracle.from_binning(bn, w.bz_tesla)
+    cap = bn.n_bins // 16
+    got = run_cuda(bn, w.bz_tesla, w.layers, batch.hits_xy, batch.event_offsets, w.threshold, w.assoc_dj, w.min_hits, cap)
+    rng = np.random.default_rng(4)
+    cols = np.stack([np.zeros(48, np.int64), rng.integers(0, bn.n_d0, 48), rng.integers(0, bn.n_phi, 48)], 1)
+    cols[0] = (0, 0, 0)
+    cols[1] = (0, bn.n_d0 - 1, bn.n_phi - 1)
+    rows = o.vote_columns(batch.hits_xy, batch.event_offsets, cols)
+    for s, (_, k, i) in enumerate(cols):
+        assert np.array_equal(got.accum[0, k, i].astype(np.int32), rows[s]), (k, i)
+    # peaks in a d0 slab: the oracle votes slices 61..66 and reports peaks of slices 62..64
+    slab, _ = o.vote(batch.hits_xy, batch.event_offsets, k_range=(61, 66))
+    assert np.array_equal(got.accum[0, 61:66].astype(np.int32), slab[0])
+    part = o.find_peaks(slab, w.threshold, k_range=(61, 66), k_out=(62, 65))
+    sel = (got.records["k"] >= 62) & (got.records["k"] < 65)
+    assert got.total <= cap
+    sub = got.records[sel]
+    assert len(sub) == part.total
+    for f in ("event", "k", "i", "j", "votes"):
+        assert np.array_equal(sub[f], part.records[f]), f
+    assert_centroids_close(sub, part.records, bn)
+    # properties that hold at any size
+    lin = (got.records["k"].astype(np.int64) * bn.n_phi + got.records["i"]) * bn.n_qpt + got.records["j"]
+    assert np.all(np.diff(lin) > 0)                                   # D6 order, no duplicates
+    assert np.array_equal(got.records["votes"],
+                          got.accum[0][got.records["k"], got.records["i"], got.records["j"]].astype(np.int32))
+    assert got.records["votes"].min() >= w.threshold
+    raw_assigned = got.cand_nhits[:got.total].sum()
+    assert np.array_equal(got.cand_keep[:got.total].astype(bool), got.cand_nhits[:got.total] >= w.min_hits)
+    kept_hits = np.bincount(got.hit_to_cand[got.hit_to_cand >= 0], minlength=got.total)
+    assert np.array_equal(kept_hits, np.where(got.cand_keep[:got.total] > 0, got.cand_nhits[:got.total], 0))
+    assert raw_assigned <= batch.n_hits
+
+
+# ----------------------------------------------------------------------------- edge cases
+def test_empty_inputs_and_empty_events():
+    w = get_workload(1)
+    bn = HoughBinning(64, 32, 8)
+    # no hits at all
+    got = run_cuda(bn, w.bz_tesla, w.layers, np.zeros((0, 2), np.float32), np.array([0, 0], np.int32), 1, 1, 1, 8)
+    assert got.accum.sum() == 0 and got.total == 0 and list(got.offsets) == [0, 0]
+    # events 0 and 2 empty
+    hits = generate_events(w).hits_xy[:300]
+    off = np.array([0, 0, 300, 300], np.int32)
+    o = Oracle.from_binning(bn, w.bz_tesla)
+    acc, _ = o.vote(hits, off)
+    ref = o.find_peaks(acc, 3)
+    got = run_cuda(bn, w.bz_tesla, w.layers, hits, off, 3, 1, 3, ref.total + 1)
+    assert np.array_equal(got.accum, acc) and np.array_equal(got.offsets, ref.offsets)
+    h2c, nh, keep = o.assign_brute(hits, off, ref, 1, 3)
+    assert np.array_equal(got.hit_to_cand, h2c) and np.array_equal(got.cand_nhits[:ref.total], nh)
+
+
+def test_degenerate_hits():
+    """Hit at the origin (r2 = 0 -> 1/0), hits far outside, denormal coordinates: no vote, no crash, same bits."""
+    bn = HoughBinning(32, 16, 4)
+    hits = np.array([[0.0, 0.0], [1e-30, -1e-30], [1e6, 1e6], [4.0, 0.0], [0.0, -110.0], [1e-42, 3.0]], np.float32)
+    off = np.array([0, hits.shape[0]], np.int32)
+    o = Oracle.from_binning(bn, 3.8)
+    acc, _ = o.vote(hits, off)
+    got = run_cuda(bn, 3.8, LAYERS_10, hits, off, 1, 1, 1, 64)
+    assert np.array_equal(got.accum, acc)
+    ref = o.find_peaks(acc, 1)
+    assert got.total == ref.total and np.array_equal(got.records["j"], ref.records["j"])
+
+
+@pytest.mark.parametrize("dtype", [ACC_I32, ACC_U16])
+def test_capacity_overflow_and_zero_capacity(dtype):
+    w = get_workload(1)
+    bn = HoughBinning(256, 128, 64, accum_dtype=dtype)
+    batch = generate_events(w)
+    _compare_all(w, batch, binning=bn, capacity=100)          # fewer slots than peaks (S12)
+    o = Oracle.from_binning(bn, w.bz_tesla)
+    acc, _ = o.vote(batch.hits_xy)
+    ref = o.find_peaks(acc, w.threshold)
+    got = run_cuda(bn, w.bz_tesla, w.layers, batch.hits_xy, batch.event_offsets, w.threshold, 1, w.min_hits, 0)
+    assert got.total == ref.total and (got.hit_to_cand == -1).all()
+
+
+def test_plateaus_and_wraparound_via_constructed_hits():
+    """Duplicated hits give multi-vote bins and equal-valued neighbours; phi0 near 0/2pi exercises the wrap."""
+    bn = HoughBinning(64, 64, 1)
+    base = np.concatenate([helix_hits(0.01, 0.3, 0.0, LAYERS_10, 3.8), helix_hits(6.27, -0.3, 0.0, LAYERS_10, 3.8),
+                           helix_hits(3.1, 0.8, 0.0, LAYERS_10, 3.8)])
+    hits = np.concatenate([base, base, base[::2]])
+    off = np.array([0, hits.shape[0]], np.int32)
+    o = Oracle.from_binning(bn, 3.8)
+    acc, _ = o.vote(hits, off)
+    ref = o.find_peaks(acc, 2)
+    got = run_cuda(bn, 3.8, LAYERS_10, hits, off, 2, 2, 2, ref.total)
+    assert np.array_equal(got.accum, acc) and got.total == ref.total
+    for f in ("k", "i", "j", "votes"):
+        assert np.array_equal(got.records[f], ref.records[f])
+    h2c, nh, keep = o.assign_brute(hits, off, ref, 2, 2)
+    assert np.array_equal(got.hit_to_cand, h2c) and np.array_equal(got.cand_keep[:ref.total], keep)
+
+
+def test_hit_order_does_not_matter_and_vote_overwrites():
+    w = get_workload(1)
+    batch = generate_events(w)
+    bn = w.binning
+    a = run_cuda(bn, w.bz_tesla, w.layers, batch.hits_xy, batch.event_offsets, w.threshold, 1, w.min_hits, 4096)
+    perm = np.random.default_rng(0).permutation(batch.n_hits)
+    b = run_cuda(bn, w.bz_tesla, w.layers, batch.hits_xy[perm], batch.event_offsets, w.threshold, 1, w.min_hits, 4096)
+    assert np.array_equal(a.accum, b.accum) and np.array_equal(a.records, b.records)
+    assert np.array_equal(a.hit_to_cand[perm], b.hit_to_cand)
+
+
+def test_invalid_arguments_are_rejected():
+    from paper_1311_2769_b200 import HoughPlan, HoughError
+    with pytest.raises(HoughError):
+        HoughPlan(255, 128, 1)                      # n_phi % 4
+    with pytest.raises(HoughError):
+        HoughPlan(256, 128, 1, qpt_min=1.0, qpt_max=-1.0)
+    plan = HoughPlan(64, 32, 1, max_hits=10, max_events=1)
+    hits = torch.zeros((11, 2), dtype=torch.float32, device="cuda")
+    off = torch.tensor([0, 11], dtype=torch.int32, device="cuda")
+    with pytest.raises(HoughError):
+        plan.vote(hits, off, plan.alloc_accum(1))   # n_hits > max_hits
+    plan.close()
