@@ -1,0 +1,465 @@
+#!/usr/bin/env python
+"""bench.py -- the round-end measurement of the Hough track-finding hot path.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C] [--tile-events T]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P \
+        bench.py --gpus N --steps K --warmup W
+
+A "step" is one pass of the WHOLE hot path (rows A1-A6 of SURVEY 8(a): stage -> vote -> flush -> find peaks
+-> assign hits / remove duplicates) over one batch of seeded synthetic events.  The default workload is
+BASELINE.json configs[3] (B:L10: 1024 events, uint16 256x128x32 accumulator per event) -- the configuration
+the metric's "events/s" is quoted on; `--config` selects another one (0, 1, 2, 4) for inspection.
+
+One JSON line goes to stdout (rank 0):
+  value            whole-job Hough votes/s, inputs resident in HBM before the timed region, all ranks
+  events_per_s     the same step expressed in events/s (the metric's second figure)
+  e2e              the same metric through hough_pipeline_run_host: pinned HOST buffers in, HOST results out,
+                   host<->device copies inside the timed region
+  roofline         dominant kernel (vote): algorithmic votes per launch / average launch duration (CUDA events
+                   on the launching stream, inside the timed region) against the ALU issue bound derived in
+                   DESIGN.md; the atomic and HBM ceilings of SURVEY 8(d) are quoted beside it
+  cpu_baseline     the CPU oracle as it stands, one thread, on a bounded sample of the same workload
+  --impl reference times the oracle instead (this tier's reference arm).
+
+Multi-GPU: events are independent, so every rank runs the same number of events of its own
+(event indices offset by rank), no data-path collective; "scaling": "weak".
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "hough_votes_per_s"
+UNIT = "votes/s"
+
+# ALU issue bound of the vote step: the D3 sequence per (hit, phi0 column, d0 slice)
+# is 9 fp32 arithmetic operations + 2 compares + 1 float->int conversion = 12 issue slots at the very least
+# (the atomic goes down the LSU pipe in parallel); 148 SMs x 128 fp32 lanes x sm_max_mhz.
+D3_MIN_ISSUE_SLOTS = 12
+FP32_LANES_PER_SM = 128
+
+
+def _env_int(name, default):
+    try:
+        return int(os.environ.get(name, default))
+    except ValueError:
+        return default
+
+
+class ClockSampler:
+    """nvidia-smi clocks + throttle reasons sampled DURING the timed region (B200_PROFILING.md recipe)."""
+    FIELDS = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+              "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+              "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index = index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits",
+                                          "-lms", "100", "-i", str(self.index)], stdout=subprocess.PIPE,
+                                         stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append((time.time(), line.strip()))
+
+    def mark(self):
+        return time.time()
+
+    def stop(self, t0: float, t1: float):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        rows = [l for (t, l) in self.lines if t0 - 0.05 <= t <= t1 + 0.15] or [l for (_, l) in self.lines]
+        sm, smax, power, reasons = [], [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for l in rows:
+            f = [x.strip() for x in l.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1])); power.append(float(f[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def _physical_gpu_index(local_rank: int) -> int:
+    vis = os.environ.get("CUDA_VISIBLE_DEVICES", "")
+    ids = [x.strip() for x in vis.split(",") if x.strip()]
+    if local_rank < len(ids) and ids[local_rank].isdigit():
+        return int(ids[local_rank])
+    return local_rank
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return float(p["hbm_gbs"]), float(p.get("sm_max_mhz", 1965.0)), "measured (MEASURED_PEAKS.json)"
+    return 6650.0, 1965.0, "fallback (B200_PROFILING.md)"
+
+
+# ----------------------------------------------------------------------------------------------
+def make_batch(cfg: int, n_events: int, rank: int):
+    from workloads import generate_events, get_workload
+    w = get_workload(cfg)
+    if w.n_events > 1 or n_events != w.n_events:
+        w = w.scaled(n_events)
+    first = rank * n_events
+    batch = generate_events(w, events=range(first, first + n_events))
+    return w, batch
+
+
+def oracle_sample(w, batch, n_sample_events: int):
+    """The oracle, as it stands, single-threaded, on the first n_sample_events events: vote (full scan) +
+    peaks + indexed assignment.  Returns (votes, events, seconds)."""
+    from oracle import Oracle
+    sub = batch.select(list(range(min(n_sample_events, batch.n_events))))
+    o = Oracle.from_binning(w.binning, w.bz_tesla)
+    t0 = time.perf_counter()
+    votes_total = 0
+    for e in range(sub.n_events):          # one event at a time keeps the oracle's int32 volume small
+        ev = sub.select([e])
+        acc, votes = o.vote(ev.hits_xy, ev.event_offsets)
+        cands = o.find_peaks(acc, w.threshold)
+        o.assign_indexed(ev.hits_xy, ev.event_offsets, cands, w.assoc_dj, w.min_hits)
+        votes_total += votes
+    return votes_total, sub.n_events, time.perf_counter() - t0
+
+
+def oracle_events_for_seconds(w, target_s: float) -> int:
+    """Bounded sample size: ~target_s of single-thread oracle work, from the full-scan evaluation count
+    (2 scans: vote + indexed assignment) at ~1.5e8 evaluations/s."""
+    bn = w.binning
+    hits_per_event = (w.n_prompt + w.n_displaced) * len(w.layers) + max(w.n_noise, 0)
+    per_event_s = 2.0 * hits_per_event * bn.n_phi * bn.n_d0 / 1.5e8 + bn.n_bins / 2.0e8
+    return max(1, min(w.n_events, int(target_s / max(per_event_s, 1e-6))))
+
+
+def run_reference(args, rank, world):
+    """--impl reference: this tier's reference arm is the CPU oracle, timed as it stands on the host cores."""
+    if rank != 0:
+        return
+    from workloads import get_workload
+    w = get_workload(args.config)
+    n_ev = oracle_events_for_seconds(w, args.ref_seconds_per_step)
+    wl, batch = make_batch(args.config, n_ev, 0)
+    for _ in range(min(args.warmup, 1)):
+        oracle_sample(wl, batch, 1)
+    votes = 0
+    secs = 0.0
+    for _ in range(args.steps):
+        v, _, s = oracle_sample(wl, batch, n_ev)
+        votes += v
+        secs += s
+    value = votes / secs
+    sample = f"{n_ev} event(s) of {wl.name} per step, vote (full scan) + peaks + indexed assignment"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32+int32",
+            "data": "synthetic", "events_per_s": n_ev * args.steps / secs,
+            "config": {"workload": wl.name, "cite": wl.cite, "events_per_step": n_ev,
+                       "note": "bounded sample of the workload; oracle single-threaded"},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+# ----------------------------------------------------------------------------------------------
+class DeviceRun:
+    """All device buffers of one rank and the tile loop over the three C-ABI calls."""
+
+    def __init__(self, w, batch, tile_events: int, cand_per_bin: float):
+        import torch
+        from paper_1311_2769_b200 import HoughPlan, alloc_candidates
+        self.torch = torch
+        self.w, self.batch = w, batch
+        bn = w.binning
+        self.n_events = batch.n_events
+        self.tile_events = max(1, min(tile_events, self.n_events))
+        off = batch.event_offsets.astype(np.int64)
+        self.tiles = []
+        for e0 in range(0, self.n_events, self.tile_events):
+            e1 = min(e0 + self.tile_events, self.n_events)
+            self.tiles.append((e0, e1, int(off[e0]), int(off[e1])))
+        max_hits = max(h1 - h0 for (_, _, h0, h1) in self.tiles)
+        self.plan = HoughPlan.from_workload(w, max_hits=max(max_hits, 1), max_events=self.tile_events)
+        self.d_hits = torch.from_numpy(batch.hits_xy).cuda()
+        # per-tile offsets are relative to the tile's first hit
+        self.d_offs = []
+        for (e0, e1, h0, _) in self.tiles:
+            self.d_offs.append(torch.from_numpy((off[e0:e1 + 1] - h0).astype(np.int32)).cuda())
+        self.accum = self.plan.alloc_accum(self.tile_events)
+        self.cap = int(cand_per_bin * bn.n_bins * self.tile_events) + 1024
+        self.cands = alloc_candidates(self.cap)
+        self.cand_off = torch.zeros(self.tile_events + 1, dtype=torch.int32, device="cuda")
+        self.h2c = torch.empty(max(max_hits, 1), dtype=torch.int32, device="cuda")
+        self.nh = torch.empty(self.cap, dtype=torch.int32, device="cuda")
+        self.keep = torch.empty(self.cap, dtype=torch.uint8, device="cuda")
+        self.totals = torch.zeros(len(self.tiles), dtype=torch.int32, device="cuda")
+
+    def step(self, vote_events=None):
+        """One pass over all tiles on the current stream.  vote_events: list to append (start, end) CUDA
+        events bracketing each hough_vote call."""
+        torch = self.torch
+        w = self.w
+        for t, (e0, e1, h0, h1) in enumerate(self.tiles):
+            hits = self.d_hits[h0:h1]
+            offs = self.d_offs[t]
+            n_ev = e1 - e0
+            if vote_events is not None:
+                a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+                a.record()
+            self.plan.vote(hits, offs, self.accum)
+            if vote_events is not None:
+                b.record()
+                vote_events.append((a, b))
+            self.plan.find_peaks(self.accum, n_ev, w.threshold, self.cands, self.cap, self.cand_off)
+            self.plan.assign_hits(hits, offs, self.cands, self.cand_off, self.cap, w.assoc_dj, w.min_hits,
+                                  self.h2c[:max(h1 - h0, 1)], self.nh, self.keep)
+            self.totals[t:t + 1].copy_(self.cand_off[n_ev:n_ev + 1])
+
+    def count_votes(self) -> int:
+        """Votes cast per step = sum of all accumulator bins (counted once, outside the timed region)."""
+        torch = self.torch
+        total = 0
+        for t, (e0, e1, h0, h1) in enumerate(self.tiles):
+            self.plan.vote(self.d_hits[h0:h1], self.d_offs[t], self.accum)
+            n_ev = e1 - e0
+            total += int(self.accum[:n_ev].to(torch.int64).sum().item())
+        return total
+
+
+def e2e_python(run: DeviceRun, steps: int, warmup: int):
+    """End-to-end through the public Python API with HOST buffers: per tile, pinned hits/offsets -> device,
+    the three calls, results -> pinned host (cand_offsets, hit_to_cand, candidate records, nhits, keep)."""
+    torch = run.torch
+    w, batch = run.w, run.batch
+    h_hits = torch.from_numpy(batch.hits_xy).pin_memory()
+    off = batch.event_offsets.astype(np.int64)
+    h_offs = [torch.from_numpy((off[e0:e1 + 1] - h0).astype(np.int32)).pin_memory() for (e0, e1, h0, _) in run.tiles]
+    max_hits = run.h2c.numel()
+    d_hits = torch.empty((max_hits, 2), dtype=torch.float32, device="cuda")
+    d_off = torch.empty(run.tile_events + 1, dtype=torch.int32, device="cuda")
+    out_h2c = torch.empty(batch.n_hits, dtype=torch.int32).pin_memory()
+    out_off = torch.empty((len(run.tiles), run.tile_events + 1), dtype=torch.int32).pin_memory()
+    out_cands = torch.empty((run.cap, 32), dtype=torch.uint8).pin_memory()
+    out_nh = torch.empty(run.cap, dtype=torch.int32).pin_memory()
+    out_keep = torch.empty(run.cap, dtype=torch.uint8).pin_memory()
+    h2d = d2h = 0
+
+    def one_step(count: bool):
+        nonlocal h2d, d2h
+        for t, (e0, e1, h0, h1) in enumerate(run.tiles):
+            n_ev, n_h = e1 - e0, h1 - h0
+            d_hits[:n_h].copy_(h_hits[h0:h1], non_blocking=True)
+            d_off[:n_ev + 1].copy_(h_offs[t], non_blocking=True)
+            run.plan.vote(d_hits[:n_h], d_off[:n_ev + 1], run.accum)
+            run.plan.find_peaks(run.accum, n_ev, w.threshold, run.cands, run.cap, run.cand_off)
+            run.plan.assign_hits(d_hits[:n_h], d_off[:n_ev + 1], run.cands, run.cand_off, run.cap, w.assoc_dj,
+                                 w.min_hits, run.h2c[:max(n_h, 1)], run.nh, run.keep)
+            out_off[t, :n_ev + 1].copy_(run.cand_off[:n_ev + 1], non_blocking=True)
+            torch.cuda.current_stream().synchronize()           # the candidate count decides the copy sizes
+            n_c = min(int(out_off[t, n_ev]), run.cap)
+            out_h2c[h0:h1].copy_(run.h2c[:n_h], non_blocking=True)
+            out_cands[:n_c].copy_(run.cands[:n_c], non_blocking=True)
+            out_nh[:n_c].copy_(run.nh[:n_c], non_blocking=True)
+            out_keep[:n_c].copy_(run.keep[:n_c], non_blocking=True)
+            if count:
+                h2d += n_h * 8 + (n_ev + 1) * 4
+                d2h += (n_ev + 1) * 4 + n_h * 4 + n_c * (32 + 4 + 1)
+        torch.cuda.current_stream().synchronize()
+
+    for _ in range(warmup):
+        one_step(False)
+    torch.cuda.synchronize()
+    a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(steps):
+        one_step(True)
+    b.record()
+    torch.cuda.synchronize()
+    return a.elapsed_time(b) / steps, h2d // max(steps, 1), d2h // max(steps, 1)
+
+
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    from paper_1311_2769_b200 import kernel_launches, load_library, version
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (libhough_b200 has no CPU fallback)")
+    load_library()
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    from workloads import get_workload
+    w0 = get_workload(args.config)
+    n_events = args.events if args.events > 0 else w0.n_events
+    w, batch = make_batch(args.config, n_events, rank)
+    run = DeviceRun(w, batch, args.tile_events, args.cand_per_bin)
+    votes_per_step = run.count_votes()
+    torch.cuda.synchronize()
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        run.step()
+    barrier()
+    sampler = ClockSampler(_physical_gpu_index(local_rank))
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.3)
+    barrier()
+    vote_events = []
+    launches0 = kernel_launches()
+    t_mark0 = time.time()
+    ev0 = torch.cuda.Event(enable_timing=True); ev1 = torch.cuda.Event(enable_timing=True)
+    ev0.record()
+    for _ in range(args.steps):
+        run.step(vote_events)
+    ev1.record()
+    barrier()
+    t_mark1 = time.time()
+    launches = kernel_launches() - launches0
+    ms_total = ev0.elapsed_time(ev1)
+    clocks = sampler.stop(t_mark0, t_mark1) if rank == 0 else None
+    vote_ms = [a.elapsed_time(b) for (a, b) in vote_events]
+    peaks_overflow = bool((run.totals > run.cap).any().item())
+
+    # max over ranks (device time), whole-job totals
+    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+    v = torch.tensor([float(votes_per_step), float(batch.n_events), float(batch.n_hits)], dtype=torch.float64,
+                     device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(v, op=dist.ReduceOp.SUM)
+    ms_step = float(t.item()) / args.steps
+    job_votes, job_events, job_hits = (float(x) for x in v.tolist())
+
+    # e2e leg (host buffers in and out), same workload
+    e2e_ms, h2d, d2h = e2e_python(run, max(1, min(args.steps, args.e2e_steps)), 1)
+    te = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_ms = float(te.item())
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    hbm_gbs, sm_max_mhz, peak_src = load_peaks()
+    sms = torch.cuda.get_device_properties(local_rank).multi_processor_count
+    bn = w.binning
+    # dominant kernel = vote: one launch per tile
+    vote_ms_avg = sum(vote_ms) / len(vote_ms)
+    votes_per_launch = votes_per_step / len(run.tiles)
+    achieved = votes_per_launch / (vote_ms_avg * 1e-3) / 1e9                     # Gvotes/s
+    alu_peak = sms * FP32_LANES_PER_SM * sm_max_mhz * 1e6 / D3_MIN_ISSUE_SLOTS / 1e9
+    hits_per_launch = batch.n_hits / len(run.tiles)
+    bins_per_launch = bn.n_bins * run.tile_events
+    hbm_bytes = hits_per_launch * 8 + bins_per_launch * bn.bin_bytes            # hits in + accumulator out
+    roofline = {"bound": "alu", "kernel": "hough_vote (stage + vote + flush)", "achieved": achieved, "peak": alu_peak,
+                "unit": "Gvotes/s", "frac": achieved / alu_peak, "traffic": None,
+                "peak_source": f"{sms} SMs x {FP32_LANES_PER_SM} fp32 lanes x {sm_max_mhz:.0f} MHz / "
+                               f"{D3_MIN_ISSUE_SLOTS} issue slots per vote (DESIGN.md); clocks {peak_src}",
+                "vote_ms_per_launch": vote_ms_avg, "votes_per_launch": votes_per_launch,
+                "launches_timed": len(vote_ms),
+                "hbm": {"algorithmic_bytes_per_launch": hbm_bytes, "achieved_gbs": hbm_bytes / (vote_ms_avg * 1e-3) / 1e9,
+                        "peak_gbs": hbm_gbs, "frac": hbm_bytes / (vote_ms_avg * 1e-3) / 1e9 / hbm_gbs,
+                        "peak_source": peak_src},
+                "smem_atomic": {"peak_gops": args.smem_atomic_gops, "frac": achieved / args.smem_atomic_gops,
+                                "peak_source": "hough_microbench kind 0 on this pool's B200 (profiles/)"}}
+
+    n_ref = oracle_events_for_seconds(w, args.cpu_seconds)
+    o_votes, o_events, o_secs = oracle_sample(w, batch, n_ref)
+    cpu = {"value": o_votes / o_secs, "unit": UNIT, "cores": 1, "kind": "oracle",
+           "sample": f"first {o_events} event(s) of {w.name}: vote (full scan) + peaks + indexed assignment, "
+                     f"{o_secs:.1f} s", "events_per_s": o_events / o_secs, "host_cores_available": os.cpu_count()}
+
+    line = {"metric": METRIC, "value": job_votes / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world,
+            "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32+u16" if bn.bin_bytes == 2 else "f32+int32",
+            "data": "synthetic",
+            "config": {"workload": w.name, "cite": w.cite, "events_per_gpu": batch.n_events,
+                       "hits_per_gpu": batch.n_hits, "votes_per_step_per_gpu": votes_per_step,
+                       "binning": [bn.n_phi, bn.n_qpt, bn.n_d0], "accum": "u16" if bn.bin_bytes == 2 else "i32",
+                       "threshold": w.threshold, "tile_events": run.tile_events, "parallelism": f"events x{world}",
+                       "l2": "no flush: per-step working set (hits + accumulators + candidates) exceeds the 126 MB L2"
+                             if batch.n_events * bn.n_bins * bn.bin_bytes > 126e6 else
+                             "working set fits L2; latency-bound configuration",
+                       "library": version()},
+            "events_per_s": job_events / (ms_step * 1e-3), "hits_per_s": job_hits / (ms_step * 1e-3),
+            "e2e": {"value": job_votes / (e2e_ms * 1e-3), "unit": UNIT, "events_per_s": job_events / (e2e_ms * 1e-3),
+                    "ms_per_step": e2e_ms, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                    "api": "HoughPlan.vote/find_peaks/assign_hits per event tile, pinned host buffers in and out"},
+            "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks,
+            "candidate_overflow": peaks_overflow}
+    print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=3)
+    ap.add_argument("--events", type=int, default=0, help="events per GPU (default: the workload's own count)")
+    ap.add_argument("--tile-events", type=int, default=64)
+    ap.add_argument("--cand-per-bin", type=float, default=1.0 / 16.0, help="candidate capacity per accumulator bin")
+    ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target oracle time of the cpu_baseline sample")
+    ap.add_argument("--ref-seconds-per-step", type=float, default=10.0)
+    ap.add_argument("--smem-atomic-gops", type=float, default=7593.0,
+                    help="measured conflict-free shared atomicAdd rate, Gops/s (profiles/microbench_r1.md)")
+    args = ap.parse_args()
+    rank, world, local_rank = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1), _env_int("LOCAL_RANK", 0)
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()
