@@ -135,6 +135,16 @@ int hough_pipeline_run_host(hough_pipeline* p, const float* h_hits_xy, int32_t n
                             int32_t* h_cand_offsets, hough_candidate* h_cands, int32_t cand_capacity,
                             int32_t* h_cand_nhits, uint8_t* h_cand_keep, int32_t* h_overflowed);
 
+/* Work-sizing tables, for inspection and tests (HOST only, no CUDA call; S19: these never change a result).
+ * Hits are grouped into radius classes; for (class c, d0 slice k) every column a hit of that class can vote in
+ * lies in the run of `steps[c*n_d0+k]` columns starting at ceil(u + lo_off[c*n_d0+k]) (cyclic), where
+ * u = phi * n_phi / 2pi - 0.5 is the hit's azimuth in column units.  The kernels evaluate the exact D3
+ * sequence at every column of the run, so a run may be too long but must never miss a voting column.
+ * edge_r2[c] = lower r^2 edge of class c (class = largest c with edge_r2[c] <= x*x + y*y; the last class is
+ * open-ended).  Output arrays may be NULL; capacities: edge_r2 256 floats, lo_off / steps 256 * n_d0 entries. */
+int hough_window_table(const hough_binning* binning, const hough_geometry* geometry, int32_t* n_class,
+                       float* edge_r2, float* lo_off, int32_t* steps);
+
 /* Measurement support (K6): peak-rate microbenchmarks for the roofline denominators that
  * MEASURED_PEAKS.json lacks.  Each runs `iters` launches on cuda_stream, synchronises, and writes the
  * average operations per second of the best launch to *ops_per_s.  kind:

@@ -4,7 +4,7 @@ The product is `libhough_b200.so` (CUDA, sm_100a; C ABI in include/hough.h).  Th
 binding: same names as the C calls, argument marshalling only, PyTorch for device memory and streams.
 """
 from .binding import (HoughPlan, HoughError, CAND_DTYPE, HOUGH_ACC_I32, HOUGH_ACC_U16, alloc_candidates,
-                      candidates_to_numpy, load_library, microbench, kernel_launches, version, LIB_PATH, EXPORTS)
+                      candidates_to_numpy, load_library, microbench, window_table, kernel_launches, version, LIB_PATH, EXPORTS)
 
 
 def hough_plan_create(binning, bz_tesla=3.8, layers=(), max_hits=1 << 20, max_events=1) -> HoughPlan:

@@ -39,7 +39,7 @@ class hough_geometry(C.Structure):
 
 EXPORTS = ["hough_plan_create", "hough_plan_destroy", "hough_accum_bytes", "hough_vote", "hough_find_peaks",
            "hough_assign_hits", "hough_plan_set_option", "hough_pipeline_create", "hough_pipeline_destroy",
-           "hough_pipeline_run_host", "hough_microbench", "hough_kernel_launches", "hough_status_string",
+           "hough_pipeline_run_host", "hough_window_table", "hough_microbench", "hough_kernel_launches", "hough_status_string",
            "hough_version"]
 
 _lib = None
@@ -75,6 +75,8 @@ def load_library() -> C.CDLL:
     lib.hough_pipeline_destroy.argtypes = [P]
     lib.hough_pipeline_run_host.restype = C.c_int
     lib.hough_pipeline_run_host.argtypes = [P, P, I, P, I, I, I, I, P, P, P, I, P, P, P]
+    lib.hough_window_table.restype = C.c_int
+    lib.hough_window_table.argtypes = [C.POINTER(hough_binning), C.POINTER(hough_geometry), C.POINTER(I), P, P, P]
     lib.hough_microbench.restype = C.c_int
     lib.hough_microbench.argtypes = [I, C.c_size_t, I, C.POINTER(C.c_double), P]
     lib.hough_kernel_launches.restype = C.c_int64
@@ -187,6 +189,21 @@ class HoughPlan:
                                           _dptr(cands), _dptr(cand_offsets), int(capacity), int(assoc_dj),
                                           int(min_hits), _dptr(hit_to_cand), _dptr(cand_nhits), _dptr(cand_keep),
                                           _stream_ptr(stream)), "hough_assign_hits")
+
+
+def window_table(n_phi, n_qpt, n_d0, qpt_min=-1.0, qpt_max=1.0, d0_min=-20.0, d0_max=20.0, bz_tesla=3.8, layers=()):
+    """hough_window_table (host only): (edge_r2 [n_class], lo_off [n_class, n_d0], steps [n_class, n_d0])."""
+    lib = load_library()
+    b, g, _keep = make_structs(n_phi, n_qpt, n_d0, qpt_min, qpt_max, d0_min, d0_max, HOUGH_ACC_I32, bz_tesla, layers)
+    n = C.c_int32(0)
+    edge = np.zeros(256, np.float32)
+    lo = np.zeros(256 * n_d0, np.float32)
+    steps = np.zeros(256 * n_d0, np.int32)
+    _check(lib.hough_window_table(C.byref(b), C.byref(g), C.byref(n), edge.ctypes.data_as(C.c_void_p),
+                                  lo.ctypes.data_as(C.c_void_p), steps.ctypes.data_as(C.c_void_p)),
+           "hough_window_table")
+    nc = int(n.value)
+    return edge[:nc].copy(), lo[:nc * n_d0].reshape(nc, n_d0).copy(), steps[:nc * n_d0].reshape(nc, n_d0).copy()
 
 
 def alloc_candidates(capacity: int, device="cuda") -> torch.Tensor:

@@ -4,6 +4,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <vector>
+
 #include "../../include/hough.h"
 
 #ifndef __CUDA_ARCH__
@@ -33,7 +35,24 @@ struct HoughConsts {
     float wq, wphi, wd, two_pi_f;
     const float2* cs;             // [n_phi] {cos, sin} of the column centres
     const float4* d0t;            // [n_d0]  {d0c, 2*d0c, d0c^2, 0}
+    // work sizing (windows.cu): never changes a result
+    int32_t n_class, n_sector, n_keys;   // radius classes, phi sectors, n_keys = n_class * n_sector (class-major)
+    float u_scale;                // n_phi / 2pi : column coordinate u = phi * u_scale - 0.5, phi in [0, 2pi)
+    float sector_scale;           // n_sector / 2pi
+    const float* edge2;           // [n_class] lower r^2 edge of each class (edge2[0] = 0; last class open-ended)
+    const int2* win;              // [n_class][n_d0] {bits(lo_off), steps}
 };
+
+constexpr int HOUGH_MAX_CLASSES = 255;
+constexpr int HOUGH_SECTORS = 32;
+
+struct HoughWindows {             // host copy of the class / window tables
+    int n_class = 0;
+    std::vector<float> edge2;     // [n_class]
+    std::vector<float> lo_off;    // [n_class * n_d0]
+    std::vector<int> steps;       // [n_class * n_d0]
+};
+int hough_build_windows(const hough_binning& b, float bz, int n_layers, const float* layer_r, HoughWindows& out);
 
 struct hough_plan {
     hough_binning b;
@@ -55,10 +74,18 @@ struct hough_plan {
     uint32_t* d_mask;                  // [max_events * words_per_event] peak bitmask (find_peaks) / candidate bitmask (assign)
     int32_t* d_word_rank;              // [max_events * words_per_event] rank of the first set bit of each word
     unsigned long long* d_best_key;    // [max_hits]
-    // workspace: staged hits (K1)
-    float4* d_staged;                  // [max_hits] {x, y, r2, bitcast(original index)}
-    int32_t* d_stage_cnt;              // histogram / offsets
-    size_t stage_cnt_len;
+    // device tables: radius classes and column windows (windows.cu)
+    float* d_edge2;                    // [n_class]
+    int2* d_win;                       // [n_class][n_d0] {bits(lo_off), steps}
+    // workspace: staged hits (K1, stage.cu)
+    float4* d_staged;                  // [max_hits] {x, y, u, bitcast(original index)} sorted by (event, class, sector)
+    int2* d_stage_tmp;                 // [max_hits] {key, rank within key}
+    int32_t* d_stage_cnt;              // [max_events][n_keys + 1] key counters -> exclusive key starts
+    // vote tile shape (vote.cu)
+    int32_t tile32;                    // 1: 32-bit bins in shared memory, 0: two 16-bit bins per word
+    int32_t tile_stride_words;         // shared-memory row stride (odd)
+    int32_t tile_max_cols;             // phi0 columns per tile that fit the shared-memory budget (0: no tiled path)
+    const int32_t* vote_offsets;       // event offsets of the call being enqueued (not kept after it returns)
 };
 
 constexpr int PEAK_BLOCK_BINS = 4096;  // bins per peak-scan block (multiple of 32)
@@ -86,7 +113,46 @@ __device__ __forceinline__ int d3_bin_from_w(float w, float r2, float d0c, float
 
 __device__ __forceinline__ float d3_r2(float x, float y) { return __fadd_rn(__fmul_rn(x, x), __fmul_rn(y, y)); }
 
+// exclusive scan of n ints in place by one CTA of 1024 threads; the total goes to *total_out.
+__device__ __forceinline__ void cta_exclusive_scan(int32_t* data, int n, int32_t* total_out) {
+    __shared__ int s_warp[32];
+    __shared__ int s_carry;
+    if (threadIdx.x == 0) s_carry = 0;
+    __syncthreads();
+    for (int base = 0; base < n; base += 1024) {
+        const int idx = base + threadIdx.x;
+        const int v = idx < n ? data[idx] : 0;
+        int x = v;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const int y = __shfl_up_sync(0xffffffffu, x, o);
+            if ((threadIdx.x & 31) >= o) x += y;
+        }
+        if ((threadIdx.x & 31) == 31) s_warp[threadIdx.x >> 5] = x;
+        __syncthreads();
+        if (threadIdx.x < 32) {
+            int ws = s_warp[threadIdx.x];
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) {
+                const int y = __shfl_up_sync(0xffffffffu, ws, o);
+                if (threadIdx.x >= o) ws += y;
+            }
+            s_warp[threadIdx.x] = ws;   // inclusive over warps
+        }
+        __syncthreads();
+        const int warp_prefix = (threadIdx.x >> 5) ? s_warp[(threadIdx.x >> 5) - 1] : 0;
+        const int carry = s_carry;
+        if (idx < n) data[idx] = carry + warp_prefix + x - v;
+        __syncthreads();
+        if (threadIdx.x == 0) s_carry = carry + s_warp[31];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) *total_out = s_carry;
+}
+
 // internal entry points (defined in the .cu files)
+int hough_stage_hits(hough_plan* p, const float* d_hits_xy, int32_t n_hits, const int32_t* d_event_offsets,
+                     int32_t n_events, cudaStream_t st);
 int hough_vote_fullscan(hough_plan* p, const float* d_hits_xy, int32_t n_hits, const int32_t* d_event_offsets,
                         int32_t n_events, void* d_accum, cudaStream_t st);
 int hough_vote_tiled(hough_plan* p, const float* d_hits_xy, int32_t n_hits, const int32_t* d_event_offsets,

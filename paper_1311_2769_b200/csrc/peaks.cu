@@ -81,43 +81,6 @@ __global__ void __launch_bounds__(256) peak_mask_kernel(HoughConsts c, const voi
     }
 }
 
-// exclusive scan of n ints in place by one CTA of 1024 threads; returns the total in *total.
-__device__ void cta_exclusive_scan(int32_t* data, int n, int32_t* total_out) {
-    __shared__ int s_warp[32];
-    __shared__ int s_carry;
-    if (threadIdx.x == 0) s_carry = 0;
-    __syncthreads();
-    for (int base = 0; base < n; base += 1024) {
-        const int idx = base + threadIdx.x;
-        const int v = idx < n ? data[idx] : 0;
-        int x = v;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int y = __shfl_up_sync(0xffffffffu, x, o);
-            if ((threadIdx.x & 31) >= o) x += y;
-        }
-        if ((threadIdx.x & 31) == 31) s_warp[threadIdx.x >> 5] = x;
-        __syncthreads();
-        if (threadIdx.x < 32) {
-            int ws = s_warp[threadIdx.x];
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                const int y = __shfl_up_sync(0xffffffffu, ws, o);
-                if (threadIdx.x >= o) ws += y;
-            }
-            s_warp[threadIdx.x] = ws;   // inclusive over warps
-        }
-        __syncthreads();
-        const int warp_prefix = (threadIdx.x >> 5) ? s_warp[(threadIdx.x >> 5) - 1] : 0;
-        const int carry = s_carry;
-        if (idx < n) data[idx] = carry + warp_prefix + x - v;
-        __syncthreads();
-        if (threadIdx.x == 0) s_carry = carry + s_warp[31];
-        __syncthreads();
-    }
-    if (threadIdx.x == 0) *total_out = s_carry;
-}
-
 __global__ void __launch_bounds__(1024) scan_blocks_kernel(int32_t* block_cnt, int blocks_per_event,
                                                            int32_t* event_cnt) {
     const int e = blockIdx.x;

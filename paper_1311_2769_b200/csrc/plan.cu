@@ -46,7 +46,10 @@ static void plan_free(hough_plan* p) {
     cudaFree(p->d_word_rank);
     cudaFree(p->d_best_key);
     cudaFree(p->d_staged);
+    cudaFree(p->d_stage_tmp);
     cudaFree(p->d_stage_cnt);
+    cudaFree(p->d_edge2);
+    cudaFree(p->d_win);
     delete p;
 }
 
@@ -120,9 +123,35 @@ extern "C" int hough_plan_create(const hough_binning* b, const hough_geometry* g
         d0t[k].w = 0.0f;
     }
 
+    // ---- work sizing: radius classes, column windows, tile shape (results never depend on these) ----
+    HoughWindows win;
+    if (hough_build_windows(*b, g->bz_tesla, g->n_layers, g->layer_radius_cm, win) != HOUGH_OK) { delete p; return HOUGH_ERR_INVALID_ARG; }
+    c.n_class = win.n_class;
+    c.n_sector = HOUGH_SECTORS;
+    c.n_keys = c.n_class * c.n_sector;
+    c.u_scale = (float)((double)b->n_phi / (2.0 * kPi));
+    c.sector_scale = (float)((double)c.n_sector / (2.0 * kPi));
+    std::vector<int2> winT((size_t)win.n_class * b->n_d0);
+    for (size_t t = 0; t < winT.size(); ++t) {
+        int lo_bits;
+        memcpy(&lo_bits, &win.lo_off[t], 4);
+        winT[t] = make_int2(lo_bits, win.steps[t]);
+    }
+    // packed 16-bit tiles are exact whenever no bin can exceed 65535: the U16 precondition, or at most 65535
+    // hits per call (a hit casts at most one vote per (phi0, d0) column, D3)
+    p->tile32 = (b->accum_dtype == HOUGH_ACC_I32 && max_hits > 65535) ? 1 : 0;
+    {
+        const long long row_words = p->tile32 ? (long long)b->n_qpt : ((long long)b->n_qpt + 1) / 2;
+        const long long stride = row_words | 1;
+        p->tile_stride_words = (int32_t)stride;
+        long long cols = (66LL * 1024) / (stride * 4);
+        if (cols < 8) cols = (200LL * 1024) / (stride * 4 + 8);          // wide rows: one big tile per SM
+        if (cols > b->n_phi) cols = b->n_phi;
+        p->tile_max_cols = (int32_t)cols;                                 // 0: no tiled path (fullscan fallback)
+    }
+
     p->peak_blocks_per_event = (int32_t)((bins + PEAK_BLOCK_BINS - 1) / PEAK_BLOCK_BINS);
     const size_t n_words = (size_t)max_events * c.words_per_event;
-    p->stage_cnt_len = (size_t)max_events * 64 * 64 + 1024;
 
     bool ok = true;
     auto A = [&](void** ptr, size_t bytes) {
@@ -137,9 +166,14 @@ extern "C" int hough_plan_create(const hough_binning* b, const hough_geometry* g
     A((void**)&p->d_word_rank, sizeof(int32_t) * n_words);
     A((void**)&p->d_best_key, sizeof(unsigned long long) * (size_t)max_hits);
     A((void**)&p->d_staged, sizeof(float4) * (size_t)max_hits);
-    A((void**)&p->d_stage_cnt, sizeof(int32_t) * p->stage_cnt_len);
+    A((void**)&p->d_stage_tmp, sizeof(int2) * (size_t)max_hits);
+    A((void**)&p->d_stage_cnt, sizeof(int32_t) * (size_t)max_events * ((size_t)c.n_keys + 1));
+    A((void**)&p->d_edge2, sizeof(float) * win.n_class);
+    A((void**)&p->d_win, sizeof(int2) * winT.size());
     if (!ok) { plan_free(p); return HOUGH_ERR_ALLOC; }
     if (cudaMemcpy(p->d_cs, cs.data(), sizeof(float2) * b->n_phi, cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(p->d_edge2, win.edge2.data(), sizeof(float) * win.n_class, cudaMemcpyHostToDevice) != cudaSuccess ||
+        cudaMemcpy(p->d_win, winT.data(), sizeof(int2) * winT.size(), cudaMemcpyHostToDevice) != cudaSuccess ||
         cudaMemcpy(p->d_d0t, d0t.data(), sizeof(float4) * b->n_d0, cudaMemcpyHostToDevice) != cudaSuccess) {
         hough_set_last_cuda_error(cudaGetLastError(), "table upload");
         plan_free(p);
@@ -147,6 +181,8 @@ extern "C" int hough_plan_create(const hough_binning* b, const hough_geometry* g
     }
     c.cs = p->d_cs;
     c.d0t = p->d_d0t;
+    c.edge2 = p->d_edge2;
+    c.win = p->d_win;
     *out = p;
     return HOUGH_OK;
 }

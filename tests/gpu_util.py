@@ -112,3 +112,27 @@ def assert_centroids_close(got, ref, binning):
         r = ref[name].astype(np.float64)
         tol = 1e-5 * np.maximum(np.abs(r), width)
         assert np.all(np.abs(g - r) <= tol), name
+
+
+def run_vote(binning, bz, layers, hits_xy, event_offsets, max_hits=None, misalign=False, fullscan=False):
+    """hough_vote alone -> accumulator as numpy.  misalign: the hit pointer is 8- but not 16-byte aligned."""
+    n_hits = int(hits_xy.shape[0])
+    n_events = int(event_offsets.shape[0] - 1)
+    plan = HoughPlan(binning.n_phi, binning.n_qpt, binning.n_d0, binning.qpt_min, binning.qpt_max, binning.d0_min,
+                     binning.d0_max, binning.accum_dtype, bz, layers, max_hits=max_hits or max(n_hits, 1),
+                     max_events=max(n_events, 1))
+    if fullscan:
+        plan.set_option("fullscan", 1)
+    buf = torch.zeros((n_hits + 2, 2), dtype=torch.float32, device="cuda")
+    assert buf.data_ptr() % 16 == 0
+    first = 1 if misalign else 0
+    d_hits = buf[first:first + n_hits]
+    d_hits.copy_(torch.from_numpy(np.ascontiguousarray(hits_xy, np.float32).reshape(-1, 2)))
+    d_off = torch.from_numpy(np.ascontiguousarray(event_offsets, np.int32)).cuda()
+    accum = plan.alloc_accum(n_events)
+    accum.fill_(3)
+    plan.vote(d_hits, d_off, accum)
+    torch.cuda.synchronize()
+    out = accum.cpu().numpy()
+    plan.close()
+    return out

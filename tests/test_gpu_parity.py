@@ -12,7 +12,7 @@ from workloads.configs import ACC_I32, ACC_U16
 
 pytestmark = pytest.mark.gpu
 
-from gpu_util import (assert_centroids_close, oracle_peaks_parallel, oracle_vote_parallel, run_cuda)  # noqa: E402
+from gpu_util import (assert_centroids_close, oracle_peaks_parallel, oracle_vote_parallel, run_cuda, run_vote)  # noqa: E402
 
 
 def _narrow(acc_i32, binning):
@@ -125,6 +125,50 @@ def test_config_4_full_size_sampled_columns_and_slab_peaks():
     kept_hits = np.bincount(got.hit_to_cand[got.hit_to_cand >= 0], minlength=got.total)
     assert np.array_equal(kept_hits, np.where(got.cand_keep[:got.total] > 0, got.cand_nhits[:got.total], 0))
     assert raw_assigned <= batch.n_hits
+
+
+# ----------------------------------------------------------------------------- every tile variant of the vote
+def _mixed_hits(seed, n, layers):
+    """Hits on the layers (as generated) and at arbitrary radii (generic radius classes), several events."""
+    rng = np.random.default_rng(seed)
+    r = np.concatenate([rng.choice(np.asarray(layers), n // 2), rng.uniform(0.0, 150.0, n - n // 2 - 3), [1e-3, 19.99, 500.0]])
+    ph = rng.uniform(0, 2 * np.pi, r.shape[0])
+    hits = np.stack([r * np.cos(ph), r * np.sin(ph)], 1).astype(np.float32)
+    cuts = np.sort(rng.integers(0, n, 2))
+    off = np.array([0, cuts[0], cuts[0], cuts[1], n], np.int32)         # 4 events, one empty
+    return hits, off
+
+
+@pytest.mark.parametrize("shape,dtype,max_hits,layers,misalign", [
+    ((256, 128, 4), ACC_U16, None, LAYERS_10, False),      # full-phi tile, packed, u16 out
+    ((256, 128, 4), ACC_I32, None, LAYERS_10, True),       # full-phi tile, packed, i32 out, 8-byte aligned hits
+    ((256, 128, 4), ACC_I32, 70000, LAYERS_10, False),     # 32-bit tile (a call may hold > 65535 hits)
+    ((512, 256, 3), ACC_I32, None, LAYERS_10, False),      # phi slabs, packed, i32 out
+    ((512, 256, 3), ACC_U16, None, (), True),              # phi slabs, u16 out, no geometry (uniform classes)
+    ((1024, 512, 2), ACC_U16, None, LAYERS_10, False),     # config-4 row length, 16+ slabs
+    ((100, 37, 3), ACC_U16, None, LAYERS_10, False),       # odd n_qpt: scalar flush, ragged last slab
+    ((100, 37, 3), ACC_I32, 70000, LAYERS_10, True),
+    ((64, 20000, 1), ACC_I32, None, LAYERS_10, False),     # a row larger than the small-tile budget
+    ((8, 300000, 1), ACC_I32, 70000, LAYERS_10, False),    # a row that fits no tile: full-scan fallback
+])
+def test_vote_tile_variants_bit_exact(shape, dtype, max_hits, layers, misalign):
+    bn = HoughBinning(*shape, accum_dtype=dtype)
+    hits, off = _mixed_hits(shape[0] + shape[1], 3000, LAYERS_10)
+    o = Oracle.from_binning(bn, 3.8)
+    acc, votes = oracle_vote_parallel(o, hits, off)
+    got = run_vote(bn, 3.8, layers, hits, off, max_hits=max_hits, misalign=misalign)
+    assert votes > 0 and np.array_equal(got.astype(np.int32), acc)
+
+
+def test_vote_half_circle_windows_and_negative_field():
+    """A r q > 1 on the outer layers (windows = the whole forward half, wrap-around in every tile) and Bz < 0."""
+    hits, off = _mixed_hits(9, 2000, LAYERS_10)
+    for bz, q in ((3.8, 3.0), (-3.8, 1.0), (0.0, 1.0)):
+        bn = HoughBinning(256, 64, 3, qpt_min=-q, qpt_max=q, d0_min=-1.0, d0_max=1.0)
+        o = Oracle.from_binning(bn, bz)
+        acc, votes = o.vote(hits, off)
+        got = run_vote(bn, bz, LAYERS_10, hits, off)
+        assert np.array_equal(got, acc), (bz, q)
 
 
 # ----------------------------------------------------------------------------- edge cases
