@@ -1,10 +1,14 @@
 // assign.cu -- A5: hit-to-candidate association and duplicate removal (D8/D9).
 //
-// K4-index : candidate list -> dense lookup (1 bit per bin + rank of the first set bit of each word)
-// K4a      : per hit, re-trace its vote columns (D3) and probe bins jh-dj..jh+dj; 64-bit best key
-// K4b      : decode best key -> hit_to_cand, count hits per candidate
-// K4c      : keep = nhits >= min_hits; hits of dropped candidates -> -1
-#include "common.cuh"
+// Tiled path (default):
+//   K1       : stage the hits (stage.cu), exactly as for the vote
+//   K4-slice : candidate range of every (event, d0 slice, phi0 slab) tile by binary search in the sorted list
+//   K4a      : the column walk of walk.cuh in WALK_ASSIGN mode -> 64-bit best key per hit (atomicMax)
+//   K4b      : decode best key (linear bin) -> candidate index by binary search; count hits per candidate
+//   K4c      : keep = nhits >= min_hits; hits of dropped candidates -> -1
+// Full-scan path (plan option "fullscan", or rows too long for a tile): a bitmask + rank index over all bins
+// and one thread per (hit, phi0 column), no windowing.
+#include "walk.cuh"
 
 namespace {
 
@@ -96,6 +100,61 @@ __global__ void __launch_bounds__(256) assign_decode_kernel(const unsigned long 
     hit_to_cand[h] = ci;
 }
 
+// {first, end} candidate of tile (event e, slice k, slab): lower bounds of the tile's first and last+1 linear
+// bins among the event's participating candidates (rank < capacity)
+__global__ void __launch_bounds__(256) cand_slice_kernel(HoughConsts c, const hough_candidate* __restrict__ cands,
+                                                         const int32_t* __restrict__ cand_offsets, int n_events,
+                                                         int capacity, int n_slabs, int slab_cols,
+                                                         int2* __restrict__ slice) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n_events * c.n_d0 * n_slabs) return;
+    const int slab = t % n_slabs;
+    const int k = (t / n_slabs) % c.n_d0;
+    const int e = t / (n_slabs * c.n_d0);
+    const int first = min(__ldg(cand_offsets + e), capacity), end = min(__ldg(cand_offsets + e + 1), capacity);
+    const int c0 = slab * slab_cols, c1 = min(c0 + slab_cols, c.n_phi);
+    int2 out;
+#pragma unroll
+    for (int s = 0; s < 2; ++s) {
+        const int ti = s ? c1 : c0;                 // lower bound of (k, ti, 0); (k, n_phi, 0) == (k + 1, 0, 0)
+        int lo = first, hi = end;
+        while (lo < hi) {
+            const int mid = (lo + hi) >> 1;
+            const int4 q = __ldg(reinterpret_cast<const int4*>(cands + mid));    // event, k, i, j
+            if (q.y < k || (q.y == k && q.z < ti)) lo = mid + 1; else hi = mid;
+        }
+        if (s) out.y = lo; else out.x = lo;
+    }
+    slice[t] = out;
+}
+
+// best key -> candidate index: the key's low word is ~(linear bin); the event's candidates are sorted by it
+__global__ void __launch_bounds__(256) assign_decode_bin_kernel(HoughConsts c, const unsigned long long* __restrict__ best_key,
+                                                                int n_hits, const int32_t* __restrict__ off, int n_events,
+                                                                const hough_candidate* __restrict__ cands,
+                                                                const int32_t* __restrict__ cand_offsets, int capacity,
+                                                                int32_t* __restrict__ hit_to_cand,
+                                                                int32_t* __restrict__ cand_nhits) {
+    const int h = blockIdx.x * blockDim.x + threadIdx.x;
+    if (h >= n_hits) return;
+    const unsigned long long key = best_key[h];
+    int ci = -1;
+    if (key) {
+        const unsigned lin = 0xFFFFFFFFu - (unsigned)(key & 0xFFFFFFFFull);
+        const int e = find_event_a(off, n_events, h);
+        int lo = min(__ldg(cand_offsets + e), capacity), hi = min(__ldg(cand_offsets + e + 1), capacity);
+        while (lo < hi) {
+            const int mid = (lo + hi) >> 1;
+            const int4 q = __ldg(reinterpret_cast<const int4*>(cands + mid));
+            const unsigned lm = (unsigned)(q.y * c.n_phi + q.z) * (unsigned)c.n_qpt + (unsigned)q.w;
+            if (lm < lin) lo = mid + 1; else hi = mid;
+        }
+        ci = lo;
+        atomicAdd(cand_nhits + ci, 1);
+    }
+    hit_to_cand[h] = ci;
+}
+
 __global__ void __launch_bounds__(256) cand_keep_kernel(const int32_t* __restrict__ cand_nhits, int capacity, int min_hits,
                                                         const int32_t* __restrict__ cand_offsets, int n_events,
                                                         uint8_t* __restrict__ cand_keep) {
@@ -127,31 +186,64 @@ extern "C" int hough_assign_hits(hough_plan* p, const float* d_hits_xy, int32_t 
         return HOUGH_ERR_INVALID_ARG;
     if (n_events == 0) return n_hits == 0 ? HOUGH_OK : HOUGH_ERR_INVALID_ARG;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
-    const size_t n_words = (size_t)n_events * p->c.words_per_event;
-    HOUGH_CUDA_TRY(cudaMemsetAsync(p->d_mask, 0, sizeof(uint32_t) * n_words, st));
+    const bool tiled = !p->fullscan && p->tile_max_cols >= 1;
     if (capacity > 0) HOUGH_CUDA_TRY(cudaMemsetAsync(d_cand_nhits, 0, sizeof(int32_t) * (size_t)capacity, st));
     if (n_hits > 0) HOUGH_CUDA_TRY(cudaMemsetAsync(p->d_best_key, 0, sizeof(unsigned long long) * (size_t)n_hits, st));
-    if (capacity > 0) {
-        const int blocks = min((capacity + 255) / 256, p->sm_count * 8);
-        cand_index_kernel<<<blocks, 256, 0, st>>>(p->c, d_cands, d_cand_offsets, n_events, capacity, p->d_mask,
-                                                  p->d_word_rank);
-        HOUGH_CUDA_TRY(cudaGetLastError());
-        hough_count_launches(1);
-    }
-    if (n_hits > 0) {
-        const float2* hits = reinterpret_cast<const float2*>(d_hits_xy);
-        const long long threads = (long long)n_hits * p->c.n_phi;
-        const long long blocks = (threads + 255) / 256;
-        if (blocks > 0x7fffffffLL) return HOUGH_ERR_UNSUPPORTED;
-        if (capacity > 0) {
-            assign_fullscan_kernel<<<(unsigned)blocks, 256, 0, st>>>(p->c, hits, n_hits, d_event_offsets, n_events, d_cands,
-                                                                     p->d_mask, p->d_word_rank, assoc_dj, p->d_best_key);
+    if (tiled) {
+        if (n_hits > 0 && capacity > 0) {
+            int rc = hough_stage_hits(p, d_hits_xy, n_hits, d_event_offsets, n_events, st);
+            if (rc != HOUGH_OK) return rc;
+            WalkArgs a{};
+            a.staged = p->d_staged;
+            a.off = d_event_offsets;
+            a.key_start = p->d_stage_cnt;
+            walk_shape(p, n_events, a.n_slabs, a.slab_cols);
+            a.stride = p->tile_stride_words;
+            a.cands = d_cands;
+            a.slice = p->d_slice;
+            a.assoc_dj = assoc_dj;
+            a.best_key = p->d_best_key;
+            const long long tiles = (long long)n_events * p->c.n_d0 * a.n_slabs;
+            if (tiles > (long long)p->slice_len) return HOUGH_ERR_UNSUPPORTED;
+            cand_slice_kernel<<<(unsigned)((tiles + 255) / 256), 256, 0, st>>>(p->c, d_cands, d_cand_offsets, n_events,
+                                                                                capacity, a.n_slabs, a.slab_cols, p->d_slice);
+            HOUGH_CUDA_TRY(cudaGetLastError());
+            hough_count_launches(1);
+            rc = walk_dispatch<WALK_ASSIGN>(p, n_events, a, p->tile32 != 0, false, st);
+            if (rc != HOUGH_OK) return rc;
+        }
+        if (n_hits > 0) {
+            assign_decode_bin_kernel<<<(n_hits + 255) / 256, 256, 0, st>>>(p->c, p->d_best_key, n_hits, d_event_offsets,
+                                                                           n_events, d_cands, d_cand_offsets, capacity,
+                                                                           d_hit_to_cand, d_cand_nhits);
             HOUGH_CUDA_TRY(cudaGetLastError());
             hough_count_launches(1);
         }
-        assign_decode_kernel<<<(n_hits + 255) / 256, 256, 0, st>>>(p->d_best_key, n_hits, d_hit_to_cand, d_cand_nhits);
-        HOUGH_CUDA_TRY(cudaGetLastError());
-        hough_count_launches(1);
+    } else {
+        const size_t n_words = (size_t)n_events * p->c.words_per_event;
+        HOUGH_CUDA_TRY(cudaMemsetAsync(p->d_mask, 0, sizeof(uint32_t) * n_words, st));
+        if (capacity > 0) {
+            const int blocks = min((capacity + 255) / 256, p->sm_count * 8);
+            cand_index_kernel<<<blocks, 256, 0, st>>>(p->c, d_cands, d_cand_offsets, n_events, capacity, p->d_mask,
+                                                      p->d_word_rank);
+            HOUGH_CUDA_TRY(cudaGetLastError());
+            hough_count_launches(1);
+        }
+        if (n_hits > 0) {
+            const float2* hits = reinterpret_cast<const float2*>(d_hits_xy);
+            const long long threads = (long long)n_hits * p->c.n_phi;
+            const long long blocks = (threads + 255) / 256;
+            if (blocks > 0x7fffffffLL) return HOUGH_ERR_UNSUPPORTED;
+            if (capacity > 0) {
+                assign_fullscan_kernel<<<(unsigned)blocks, 256, 0, st>>>(p->c, hits, n_hits, d_event_offsets, n_events, d_cands,
+                                                                         p->d_mask, p->d_word_rank, assoc_dj, p->d_best_key);
+                HOUGH_CUDA_TRY(cudaGetLastError());
+                hough_count_launches(1);
+            }
+            assign_decode_kernel<<<(n_hits + 255) / 256, 256, 0, st>>>(p->d_best_key, n_hits, d_hit_to_cand, d_cand_nhits);
+            HOUGH_CUDA_TRY(cudaGetLastError());
+            hough_count_launches(1);
+        }
     }
     if (capacity > 0) {
         const int blocks = min((capacity + 255) / 256, p->sm_count * 8);

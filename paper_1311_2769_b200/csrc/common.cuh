@@ -74,6 +74,8 @@ struct hough_plan {
     uint32_t* d_mask;                  // [max_events * words_per_event] peak bitmask (find_peaks) / candidate bitmask (assign)
     int32_t* d_word_rank;              // [max_events * words_per_event] rank of the first set bit of each word
     unsigned long long* d_best_key;    // [max_hits]
+    int2* d_slice;                     // [slice_len] candidate range of each assign tile
+    size_t slice_len;
     // device tables: radius classes and column windows (windows.cu)
     float* d_edge2;                    // [n_class]
     int2* d_win;                       // [n_class][n_d0] {bits(lo_off), steps}
@@ -85,7 +87,6 @@ struct hough_plan {
     int32_t tile32;                    // 1: 32-bit bins in shared memory, 0: two 16-bit bins per word
     int32_t tile_stride_words;         // shared-memory row stride (odd)
     int32_t tile_max_cols;             // phi0 columns per tile that fit the shared-memory budget (0: no tiled path)
-    const int32_t* vote_offsets;       // event offsets of the call being enqueued (not kept after it returns)
 };
 
 constexpr int PEAK_BLOCK_BINS = 4096;  // bins per peak-scan block (multiple of 32)

@@ -6,6 +6,7 @@
 #include <new>
 #include <atomic>
 #include <vector>
+#include <algorithm>
 
 #include "common.cuh"
 
@@ -48,6 +49,7 @@ static void plan_free(hough_plan* p) {
     cudaFree(p->d_staged);
     cudaFree(p->d_stage_tmp);
     cudaFree(p->d_stage_cnt);
+    cudaFree(p->d_slice);
     cudaFree(p->d_edge2);
     cudaFree(p->d_win);
     delete p;
@@ -168,6 +170,13 @@ extern "C" int hough_plan_create(const hough_binning* b, const hough_geometry* g
     A((void**)&p->d_staged, sizeof(float4) * (size_t)max_hits);
     A((void**)&p->d_stage_tmp, sizeof(int2) * (size_t)max_hits);
     A((void**)&p->d_stage_cnt, sizeof(int32_t) * (size_t)max_events * ((size_t)c.n_keys + 1));
+    // tiles per call: walk_shape() never uses more slabs than ceil(n_phi / 32) or than the budget needs
+    {
+        const long long slabs_budget = p->tile_max_cols >= 1 ? (b->n_phi + p->tile_max_cols - 1) / p->tile_max_cols : 1;
+        const long long slabs_max = std::max<long long>(2 * slabs_budget, (b->n_phi + 31) / 32 * 2);
+        p->slice_len = (size_t)max_events * (size_t)b->n_d0 * (size_t)slabs_max;
+    }
+    A((void**)&p->d_slice, sizeof(int2) * p->slice_len);
     A((void**)&p->d_edge2, sizeof(float) * win.n_class);
     A((void**)&p->d_win, sizeof(int2) * winT.size());
     if (!ok) { plan_free(p); return HOUGH_ERR_ALLOC; }

@@ -136,3 +136,30 @@ def run_vote(binning, bz, layers, hits_xy, event_offsets, max_hits=None, misalig
     out = accum.cpu().numpy()
     plan.close()
     return out
+
+
+def run_assign(binning, bz, layers, hits_xy, event_offsets, records, cand_offsets, capacity, assoc_dj, min_hits,
+               max_hits=None, fullscan=False):
+    """hough_assign_hits alone on a caller-made candidate list (CAND_DTYPE records, int32 offsets)."""
+    n_hits = int(hits_xy.shape[0])
+    n_events = int(event_offsets.shape[0] - 1)
+    plan = HoughPlan(binning.n_phi, binning.n_qpt, binning.n_d0, binning.qpt_min, binning.qpt_max, binning.d0_min,
+                     binning.d0_max, binning.accum_dtype, bz, layers, max_hits=max_hits or max(n_hits, 1),
+                     max_events=max(n_events, 1))
+    if fullscan:
+        plan.set_option("fullscan", 1)
+    d_hits = torch.from_numpy(np.ascontiguousarray(hits_xy, np.float32).reshape(-1, 2)).cuda()
+    d_off = torch.from_numpy(np.ascontiguousarray(event_offsets, np.int32)).cuda()
+    cands = alloc_candidates(capacity)
+    n_c = min(capacity, len(records))
+    if n_c:
+        cands[:n_c].copy_(torch.from_numpy(np.ascontiguousarray(records[:n_c]).view(np.uint8).reshape(n_c, 32)))
+    d_coff = torch.from_numpy(np.ascontiguousarray(cand_offsets, np.int32)).cuda()
+    h2c = torch.full((max(n_hits, 1),), -7, dtype=torch.int32, device="cuda")
+    nh = torch.full((max(capacity, 1),), -3, dtype=torch.int32, device="cuda")
+    keep = torch.full((max(capacity, 1),), 9, dtype=torch.uint8, device="cuda")
+    plan.assign_hits(d_hits, d_off, cands, d_coff, capacity, assoc_dj, min_hits, h2c, nh, keep)
+    torch.cuda.synchronize()
+    out = h2c[:n_hits].cpu().numpy(), nh[:capacity].cpu().numpy(), keep[:capacity].cpu().numpy()
+    plan.close()
+    return out

@@ -12,7 +12,7 @@ from workloads.configs import ACC_I32, ACC_U16
 
 pytestmark = pytest.mark.gpu
 
-from gpu_util import (assert_centroids_close, oracle_peaks_parallel, oracle_vote_parallel, run_cuda, run_vote)  # noqa: E402
+from gpu_util import (assert_centroids_close, oracle_peaks_parallel, oracle_vote_parallel, run_assign, run_cuda, run_vote)  # noqa: E402
 
 
 def _narrow(acc_i32, binning):
@@ -169,6 +169,50 @@ def test_vote_half_circle_windows_and_negative_field():
         acc, votes = o.vote(hits, off)
         got = run_vote(bn, bz, LAYERS_10, hits, off)
         assert np.array_equal(got, acc), (bz, q)
+
+
+@pytest.mark.parametrize("shape,dtype,max_hits,dj", [
+    ((256, 128, 4), ACC_U16, None, 1),        # full-phi tiles, 16-bit entries
+    ((256, 128, 4), ACC_I32, 70000, 2),       # 32-bit entries
+    ((512, 256, 3), ACC_I32, None, 0),        # phi slabs, exact-bin association only
+    ((512, 256, 3), ACC_U16, None, 3),        # phi slabs, wide association window
+    ((100, 37, 3), ACC_U16, None, 1),         # ragged last slab, odd n_qpt
+])
+def test_assign_tile_variants_bit_exact(shape, dtype, max_hits, dj):
+    """vote -> peaks -> assign through every tile variant of the association walk, vs the oracle's brute force."""
+    bn = HoughBinning(*shape, accum_dtype=dtype)
+    hits, off = _mixed_hits(shape[0] + dj, 3000, LAYERS_10)
+    o = Oracle.from_binning(bn, 3.8)
+    acc, _ = o.vote(hits, off)
+    thr = 3
+    ref = o.find_peaks(acc, thr)
+    assert ref.total > 50
+    h2c, nh, keep = o.assign_brute(hits, off, ref, dj, 2)
+    got = run_assign(bn, 3.8, LAYERS_10, hits, off, ref.records, ref.offsets, ref.total + 5, dj, 2, max_hits=max_hits)
+    assert np.array_equal(got[0], h2c)
+    assert np.array_equal(got[1][:ref.total], nh) and np.array_equal(got[2][:ref.total], keep)
+    assert (h2c >= 0).sum() > 100
+
+
+def test_assign_saturated_votes_and_truncated_list():
+    """Candidate votes at and beyond the 16-bit tile entry (exact through the record lookup) and capacity < total."""
+    w = get_workload(1)
+    bn = w.binning
+    batch = generate_events(w)
+    o = Oracle.from_binning(bn, w.bz_tesla)
+    acc, _ = o.vote(batch.hits_xy)
+    ref = o.find_peaks(acc, w.threshold)
+    rec = ref.records.copy()
+    rng = np.random.default_rng(1)
+    sel = rng.choice(len(rec), 40, replace=False)
+    rec["votes"][sel] = rng.choice([65533, 65534, 65535, 65536, 70000, 1 << 20], 40)
+    from oracle import OracleCandidates
+    mod = OracleCandidates(rec, ref.offsets, ref.total)
+    for cap in (ref.total, ref.total // 2):
+        h2c, nh, keep = o.assign_brute(batch.hits_xy, batch.event_offsets, mod, 1, 3, capacity=cap)
+        got = run_assign(bn, w.bz_tesla, w.layers, batch.hits_xy, batch.event_offsets, rec, ref.offsets, cap, 1, 3)
+        assert np.array_equal(got[0], h2c), cap
+        assert np.array_equal(got[1][:cap], nh) and np.array_equal(got[2][:cap], keep)
 
 
 # ----------------------------------------------------------------------------- edge cases
