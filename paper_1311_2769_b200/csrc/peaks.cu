@@ -1,9 +1,14 @@
 // peaks.cu -- A4: local-maximum search with ordered compaction ("local maxima"; D5-D7).
 //
-// K3a  peak_mask_kernel : per bin, threshold + 3x3(x3) test -> 1 bit per bin (warp ballot), per-block count
-// K3b  scan kernels     : per-event scan of block counts, then scan of event totals -> cand_offsets
-// K3c  peak_emit_kernel : per mask word, rank = offsets + popcounts; write records (centroid D7) in
-//                         ascending (event, k, i, j) order for rank < capacity
+// Tiled path (default): a CTA owns PEAK_BLOCK_BINS consecutive bins of one event (whole phi0 rows of one d0
+// slice) and stages those rows, their two phi0 neighbours and the same rows of slices k-1 and k+1 in shared
+// memory, so the accumulator is read from L2/HBM with coalesced row copies only.
+//   K3a  peak_tile_kernel<EMIT=false> : D5 test from the tile -> per-block count
+//   K3b  scan kernels                 : per-event scan of block counts, then scan of event totals -> cand_offsets
+//   K3c  peak_tile_kernel<EMIT=true>  : same test, ranks from the scans, records (centroid D7) written in
+//                                       ascending (event, k, i, j) order for rank < capacity
+// Generic path (a block that spans two d0 slices, or rows too long for the tile): per-bin global loads,
+//   peak_mask_kernel (1 bit per bin + per-block count) and peak_emit_kernel (per mask word).
 #include "common.cuh"
 
 namespace {
@@ -179,6 +184,258 @@ __global__ void __launch_bounds__(128) peak_emit_kernel(HoughConsts c, const voi
     }
 }
 
+
+// ---- tiled path ------------------------------------------------------------------------------------------
+template <bool U16> struct BinT { typedef int type; };
+template <> struct BinT<true> { typedef unsigned short type; };
+
+// shared-memory bytes of the halo tile of one block: 3 slices x (rows + 2) x n_qpt bins
+inline size_t peak_tile_bytes(const HoughConsts& c) {
+    const size_t rows = (size_t)(PEAK_BLOCK_BINS + c.n_qpt - 1) / c.n_qpt + 1;      // rows a block can touch
+    return 3 * (rows + 2) * (size_t)c.n_qpt * (c.is_u16 ? 2 : 4) + 16;
+}
+
+// D7 centroid from the integer moments: every fp32 operation individually rounded.
+__device__ __forceinline__ void write_candidate(const HoughConsts& c, hough_candidate* __restrict__ out, int e, int k, int i,
+                                                int j, int a, long long S, long long Sj, long long Si, long long Sk) {
+    const float fS = __ll2float_rn(S);
+    const float oj = __fdiv_rn(__ll2float_rn(Sj), fS);
+    const float oi = __fdiv_rn(__ll2float_rn(Si), fS);
+    const float ok = __fdiv_rn(__ll2float_rn(Sk), fS);
+    const float tj = __fadd_rn(__fadd_rn((float)j, 0.5f), oj);
+    const float qpt = __fadd_rn(c.qpt_min, __fmul_rn(tj, c.wq));
+    const float ti = __fadd_rn(__fadd_rn((float)i, 0.5f), oi);
+    float ph = __fmul_rn(ti, c.wphi);
+    if (ph < 0.0f) ph = __fadd_rn(ph, c.two_pi_f);
+    else if (ph >= c.two_pi_f) ph = __fsub_rn(ph, c.two_pi_f);
+    float d0 = 0.0f;
+    if (c.n_d0 > 1) {
+        const float tk = __fadd_rn(__fadd_rn((float)k, 0.5f), ok);
+        d0 = __fadd_rn(c.d0_min, __fmul_rn(tk, c.wd));
+    }
+    int4* o = reinterpret_cast<int4*>(out);
+    o[0] = make_int4(e, k, i, j);
+    o[1] = make_int4(a, __float_as_int(ph), __float_as_int(qpt), __float_as_int(d0));
+}
+
+// A block that spans two d0 slices (n_phi * n_qpt not a multiple of PEAK_BLOCK_BINS): per-bin global loads.
+template <bool U16, bool EMIT>
+__device__ void peak_block_generic(const HoughConsts& c, const void* __restrict__ acc, int threshold, int e, int blk,
+                                   int blocks_per_event, int32_t* __restrict__ block_cnt,
+                                   const int32_t* __restrict__ cand_offsets, hough_candidate* __restrict__ cands,
+                                   int capacity, int* s_warp_cnt) {
+    const int nphi = c.n_phi, nq = c.n_qpt, nd = c.n_d0;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const size_t ebase = (size_t)e * (size_t)c.bins_per_event;
+    int base = 0;
+    if (EMIT) base = cand_offsets[e] + block_cnt[(size_t)e * blocks_per_event + blk];
+    int cnt = 0;
+    for (int it = 0; it < PEAK_BLOCK_BINS / 256; ++it) {
+        const int b = blk * PEAK_BLOCK_BINS + it * 256 + tid;
+        bool pk = false;
+        int a = 0, k = 0, i = 0, j = 0;
+        if (b < c.bins_per_event) {
+            const int r = b / nq;
+            j = b - r * nq;
+            k = r / nphi;
+            i = r - k * nphi;
+            a = load_bin<U16>(acc, ebase + b);
+            if (a >= threshold) pk = is_peak<U16>(c, acc, ebase, k, i, j, a);
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, pk);
+        if (!EMIT) {
+            if (lane == 0) cnt += __popc(m);
+            continue;
+        }
+        if (lane == 0) s_warp_cnt[warp] = __popc(m);
+        __syncthreads();
+        int before_me = 0, total = 0;
+        for (int w = 0; w < 8; ++w) {
+            const int n = s_warp_cnt[w];
+            if (w < warp) before_me += n;
+            total += n;
+        }
+        const int rank = base + before_me + __popc(m & ((1u << lane) - 1u));
+        if (pk && rank < capacity) {
+            long long S = 0, Sj = 0, Si = 0, Sk = 0;
+            for (int dk = -1; dk <= 1; ++dk) {
+                const int kk = k + dk;
+                if (kk < 0 || kk >= nd) continue;
+                for (int di = -1; di <= 1; ++di) {
+                    int ii = i + di;
+                    ii = ii < 0 ? ii + nphi : (ii >= nphi ? ii - nphi : ii);
+                    for (int dj = -1; dj <= 1; ++dj) {
+                        const int jj = j + dj;
+                        if (jj < 0 || jj >= nq) continue;
+                        const int v = load_bin<U16>(acc, ebase + ((size_t)kk * nphi + ii) * nq + jj);
+                        S += v; Sj += (long long)v * dj; Si += (long long)v * di; Sk += (long long)v * dk;
+                    }
+                }
+            }
+            write_candidate(c, cands + rank, e, k, i, j, a, S, Sj, Si, Sk);
+        }
+        base += total;
+        __syncthreads();
+    }
+    if (!EMIT) {
+        if (lane == 0) s_warp_cnt[warp] = cnt;
+        __syncthreads();
+        if (tid == 0) {
+            int t = 0;
+            for (int w = 0; w < 8; ++w) t += s_warp_cnt[w];
+            block_cnt[(size_t)e * blocks_per_event + blk] = t;
+        }
+    }
+}
+
+constexpr int PEAK_WARP_BINS = PEAK_BLOCK_BINS / 8;     // consecutive bins owned by one warp of the block
+
+template <bool U16, bool EMIT>
+__global__ void __launch_bounds__(256) peak_tile_kernel(HoughConsts c, const void* __restrict__ acc, int threshold,
+                                                        int blocks_per_event, int32_t* __restrict__ block_cnt,
+                                                        const int32_t* __restrict__ cand_offsets,
+                                                        hough_candidate* __restrict__ cands, int capacity) {
+    typedef typename BinT<U16>::type bin_t;
+    extern __shared__ __align__(16) unsigned char peak_smem[];
+    __shared__ int s_warp_cnt[8];
+    __shared__ unsigned short s_list[8][PEAK_WARP_BINS];
+    bin_t* tile = reinterpret_cast<bin_t*>(peak_smem);
+    const int e = blockIdx.y, blk = blockIdx.x;
+    const int nphi = c.n_phi, nq = c.n_qpt, nd = c.n_d0;
+    const int b0 = blk * PEAK_BLOCK_BINS;
+    const int b1 = min(b0 + PEAK_BLOCK_BINS, c.bins_per_event);
+    const int r_a = b0 / nq, r_b = (b1 - 1) / nq;          // global rows (k * n_phi + i) touched by the block
+    const int k = r_a / nphi;
+    if ((r_b / nphi) != k) {
+        peak_block_generic<U16, EMIT>(c, acc, threshold, e, blk, blocks_per_event, block_cnt, cand_offsets, cands, capacity,
+                                      s_warp_cnt);
+        return;
+    }
+    const int i_a = r_a - k * nphi;
+    const int tr = (r_b - r_a + 1) + 2;                     // tile rows per slice: i_a - 1 .. i_a + n_rows
+    const bin_t* ev = reinterpret_cast<const bin_t*>(acc) + (size_t)e * (size_t)c.bins_per_event;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+
+    // ---- stage the halo tile: slices k-1, k, k+1 (rows of absent slices are never read) ----
+    {
+        const bool vec = ((nq * (int)sizeof(bin_t)) % 16 == 0) && ((reinterpret_cast<uintptr_t>(ev) & 15u) == 0);
+        for (int s = 0; s < 3; ++s) {
+            const int kk = k + s - 1;
+            if (kk < 0 || kk >= nd) continue;
+            if (vec) {
+                const int v_per_row = nq * (int)sizeof(bin_t) / 16;
+                for (int rr = warp; rr < tr; rr += 8) {
+                    int ii = i_a - 1 + rr;
+                    ii = ii < 0 ? ii + nphi : (ii >= nphi ? ii - nphi : ii);
+                    const uint4* src = reinterpret_cast<const uint4*>(ev + ((size_t)kk * nphi + ii) * nq);
+                    uint4* dst = reinterpret_cast<uint4*>(tile + ((size_t)s * tr + rr) * nq);
+                    for (int vv = lane; vv < v_per_row; vv += 32) dst[vv] = __ldg(src + vv);
+                }
+            } else {
+                for (int rr = warp; rr < tr; rr += 8) {
+                    int ii = i_a - 1 + rr;
+                    ii = ii < 0 ? ii + nphi : (ii >= nphi ? ii - nphi : ii);
+                    const bin_t* src = ev + ((size_t)kk * nphi + ii) * nq;
+                    bin_t* dst = tile + ((size_t)s * tr + rr) * nq;
+                    for (int jj = lane; jj < nq; jj += 32) dst[jj] = __ldg(src + jj);
+                }
+            }
+        }
+    }
+    __syncthreads();
+
+    // ---- phase A: each warp compacts the bins of its chunk that reach the threshold (order preserved) ----
+    // bin b of the block sits at tile[centre0 + (b - r_a * nq)] (the centre slice's rows are contiguous)
+    const int centre0 = (tr + 1) * nq - r_a * nq;
+    const int slice_stride = tr * nq;
+    const int wb0 = b0 + warp * PEAK_WARP_BINS;
+    unsigned short* list = s_list[warp];
+    int n = 0;
+#pragma unroll 4
+    for (int it = 0; it < PEAK_WARP_BINS / 32; ++it) {
+        const int off = it * 32 + lane;
+        const int b = wb0 + off;
+        const bool pass = b < b1 && (int)tile[centre0 + b] >= threshold;
+        const unsigned m = __ballot_sync(0xffffffffu, pass);
+        if (pass) list[n + __popc(m & ((1u << lane) - 1u))] = (unsigned short)off;
+        n += __popc(m);
+    }
+    __syncwarp();
+
+    // ---- phase B: D5 test of the compacted bins, 32 at a time; survivors are compacted in place ----
+    int np = 0;
+    for (int base = 0; base < n; base += 32) {
+        const int idx = base + lane;
+        const bool valid = idx < n;
+        const int off = valid ? (int)list[idx] : 0;
+        __syncwarp();
+        bool pk = false;
+        if (valid) {
+            const int b = wb0 + off;
+            const int ci = centre0 + b;
+            const int j = (b - r_a * nq) % nq;
+            const int a = (int)tile[ci];
+            const bool jlo = j > 0, jhi = j + 1 < nq;
+            pk = true;
+#pragma unroll
+            for (int dk = -1; dk <= 1; ++dk) {
+                if (k + dk < 0 || k + dk >= nd) continue;
+#pragma unroll
+                for (int di = -1; di <= 1; ++di) {
+                    const bin_t* row = tile + ci + dk * slice_stride + di * nq;
+                    const bool before_row = dk < 0 || (dk == 0 && di < 0);
+                    const bool after_row = dk > 0 || (dk == 0 && di > 0);
+                    if (jlo) { const int v = (int)row[-1]; pk = pk && ((before_row || !after_row) ? (a > v) : (a >= v)); }
+                    if (dk != 0 || di != 0) { const int v = (int)row[0]; pk = pk && (before_row ? (a > v) : (a >= v)); }
+                    if (jhi) { const int v = (int)row[1]; pk = pk && (before_row ? (a > v) : (a >= v)); }
+                }
+            }
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, pk);
+        if (pk) list[np + __popc(m & ((1u << lane) - 1u))] = (unsigned short)off;
+        np += __popc(m);
+    }
+    if (lane == 0) s_warp_cnt[warp] = np;
+    __syncthreads();
+    if (!EMIT) {
+        if (tid == 0) {
+            int t = 0;
+            for (int w = 0; w < 8; ++w) t += s_warp_cnt[w];
+            block_cnt[(size_t)e * blocks_per_event + blk] = t;
+        }
+        return;
+    }
+
+    // ---- phase C (EMIT): ranks in linear-bin order = warps in order, list order inside a warp ----
+    int rank0 = cand_offsets[e] + block_cnt[(size_t)e * blocks_per_event + blk];
+    for (int w = 0; w < warp; ++w) rank0 += s_warp_cnt[w];
+    for (int idx = lane; idx < np; idx += 32) {
+        const int rank = rank0 + idx;
+        if (rank >= capacity) break;
+        const int b = wb0 + (int)list[idx];
+        const int ci = centre0 + b;
+        const int r = b / nq;
+        const int j = b - r * nq;
+        const int i = r - k * nphi;
+        long long S = 0, Sj = 0, Si = 0, Sk = 0;
+#pragma unroll
+        for (int dk = -1; dk <= 1; ++dk) {
+            if (k + dk < 0 || k + dk >= nd) continue;
+#pragma unroll
+            for (int di = -1; di <= 1; ++di) {
+                const bin_t* row = tile + ci + dk * slice_stride + di * nq;
+#pragma unroll
+                for (int dj = -1; dj <= 1; ++dj) {
+                    if (j + dj < 0 || j + dj >= nq) continue;
+                    const int v = (int)row[dj];
+                    S += v; Sj += (long long)v * dj; Si += (long long)v * di; Sk += (long long)v * dk;
+                }
+            }
+        }
+        write_candidate(c, cands + rank, e, k, i, j, (int)tile[ci], S, Sj, Si, Sk);
+    }
+}
+
 }  // namespace
 
 extern "C" int hough_find_peaks(hough_plan* p, const void* d_accum, int32_t n_events, int32_t threshold,
@@ -196,7 +453,26 @@ extern "C" int hough_find_peaks(hough_plan* p, const void* d_accum, int32_t n_ev
     if (n_events > 65535) return HOUGH_ERR_UNSUPPORTED;
     const int bpe = p->peak_blocks_per_event;
     dim3 grid(bpe, n_events);
-    if (p->c.is_u16)
+    const size_t tile_bytes = peak_tile_bytes(p->c);
+    const bool tiled = !p->fullscan && tile_bytes <= 100 * 1024;
+    if (tiled) {
+        static bool smem_configured = false;        // the tiled path never needs more than 100 KB
+        if (!smem_configured) {
+            const int cap = 100 * 1024;
+            HOUGH_CUDA_TRY(cudaFuncSetAttribute(peak_tile_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap));
+            HOUGH_CUDA_TRY(cudaFuncSetAttribute(peak_tile_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap));
+            HOUGH_CUDA_TRY(cudaFuncSetAttribute(peak_tile_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap));
+            HOUGH_CUDA_TRY(cudaFuncSetAttribute(peak_tile_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap));
+            smem_configured = true;
+        }
+        if (p->c.is_u16) {
+            peak_tile_kernel<true, false><<<grid, 256, tile_bytes, st>>>(p->c, d_accum, threshold, bpe, p->d_peak_block_cnt,
+                                                                         nullptr, nullptr, 0);
+        } else {
+            peak_tile_kernel<false, false><<<grid, 256, tile_bytes, st>>>(p->c, d_accum, threshold, bpe, p->d_peak_block_cnt,
+                                                                          nullptr, nullptr, 0);
+        }
+    } else if (p->c.is_u16)
         peak_mask_kernel<true><<<grid, 256, 0, st>>>(p->c, d_accum, threshold, bpe, p->d_mask, p->d_peak_block_cnt);
     else
         peak_mask_kernel<false><<<grid, 256, 0, st>>>(p->c, d_accum, threshold, bpe, p->d_mask, p->d_peak_block_cnt);
@@ -205,7 +481,14 @@ extern "C" int hough_find_peaks(hough_plan* p, const void* d_accum, int32_t n_ev
     HOUGH_CUDA_TRY(cudaGetLastError());
     scan_events_kernel<<<1, 1024, 0, st>>>(p->d_event_cnt, n_events, d_cand_offsets);
     HOUGH_CUDA_TRY(cudaGetLastError());
-    if (p->c.is_u16)
+    if (tiled) {
+        if (p->c.is_u16)
+            peak_tile_kernel<true, true><<<grid, 256, tile_bytes, st>>>(p->c, d_accum, threshold, bpe, p->d_peak_block_cnt,
+                                                                        d_cand_offsets, d_cands, capacity);
+        else
+            peak_tile_kernel<false, true><<<grid, 256, tile_bytes, st>>>(p->c, d_accum, threshold, bpe, p->d_peak_block_cnt,
+                                                                         d_cand_offsets, d_cands, capacity);
+    } else if (p->c.is_u16)
         peak_emit_kernel<true><<<grid, 128, 0, st>>>(p->c, d_accum, bpe, p->d_mask, p->d_peak_block_cnt, d_cand_offsets,
                                                      d_cands, capacity, nullptr);
     else

@@ -298,7 +298,11 @@ template <int MODE, bool TILE32, bool OUT16, bool FULLPHI>
 int walk_launch(hough_plan* p, int n_events, WalkArgs a, cudaStream_t st) {
     const size_t smem = walk_smem_bytes(a.slab_cols, a.stride, p->c.n_class);
     auto kern = walk_kernel<MODE, TILE32, OUT16, FULLPHI>;
-    HOUGH_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    static size_t smem_configured = 0;              // per instantiation; raised only when a call needs more
+    if (smem > smem_configured) {
+        HOUGH_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+        smem_configured = smem;
+    }
     const long long grid = (long long)a.n_slabs * p->c.n_d0 * n_events;
     if (grid > 0x7fffffffLL) return HOUGH_ERR_UNSUPPORTED;
     kern<<<(unsigned)grid, WALK_THREADS, smem, st>>>(p->c, a);

@@ -194,6 +194,33 @@ def test_assign_tile_variants_bit_exact(shape, dtype, max_hits, dj):
     assert (h2c >= 0).sum() > 100
 
 
+@pytest.mark.parametrize("shape,dtype,fullscan", [
+    ((100, 37, 3), ACC_U16, False),      # peak blocks that span two d0 slices, unaligned rows
+    ((100, 37, 3), ACC_I32, True),       # generic per-bin path
+    ((64, 4096, 2), ACC_I32, False),     # one row per peak block
+    ((16, 20000, 2), ACC_U16, False),    # rows too long for the halo tile
+    ((512, 256, 3), ACC_I32, False),
+    ((256, 128, 1), ACC_U16, False),     # 2-D: no neighbour slices at all
+])
+def test_peaks_tile_variants_bit_exact(shape, dtype, fullscan):
+    bn = HoughBinning(*shape, accum_dtype=dtype)
+    hits, off = _mixed_hits(shape[1], 2500, LAYERS_10)
+    hits = np.concatenate([hits, hits[::3]])                      # duplicated hits -> plateaus
+    off = np.array([0, 700, 700, hits.shape[0]], np.int32)
+    o = Oracle.from_binning(bn, 3.8)
+    acc, _ = o.vote(hits, off)
+    thr = 2
+    ref = o.find_peaks(acc, thr)
+    assert ref.total > 20
+    for cap in (ref.total + 3, ref.total // 2):
+        got = run_cuda(bn, 3.8, LAYERS_10, hits, off, thr, 1, 2, cap, fullscan=fullscan)
+        assert got.total == ref.total and np.array_equal(got.offsets, ref.offsets)
+        n_c = min(cap, ref.total)
+        for f in ("event", "k", "i", "j", "votes"):
+            assert np.array_equal(got.records[f], ref.records[f][:n_c]), f
+        assert_centroids_close(got.records, ref.records[:n_c], bn)
+
+
 def test_assign_saturated_votes_and_truncated_list():
     """Candidate votes at and beyond the 16-bit tile entry (exact through the record lookup) and capacity < total."""
     w = get_workload(1)
