@@ -40,7 +40,7 @@ struct HoughConsts {
     float u_scale;                // n_phi / 2pi : column coordinate u = phi * u_scale - 0.5, phi in [0, 2pi)
     float sector_scale;           // n_sector / 2pi
     const float* edge2;           // [n_class] lower r^2 edge of each class (edge2[0] = 0; last class open-ended)
-    const int2* win;              // [n_class][n_d0] {bits(lo_off), steps}
+    const int2* win;              // [n_class][n_d0] {bits(lo_off), steps | fwd_safe << 30}
 };
 
 constexpr int HOUGH_MAX_CLASSES = 255;
@@ -51,6 +51,7 @@ struct HoughWindows {             // host copy of the class / window tables
     std::vector<float> edge2;     // [n_class]
     std::vector<float> lo_off;    // [n_class * n_d0]
     std::vector<int> steps;       // [n_class * n_d0]
+    std::vector<char> fwd_safe;   // [n_class * n_d0] 1: the D3 forward test passes at every column of the window
 };
 int hough_build_windows(const hough_binning& b, float bz, int n_layers, const float* layer_r, HoughWindows& out);
 
@@ -60,6 +61,7 @@ struct hough_plan {
     int32_t max_hits, max_events;
     int device, sm_count;
     int fullscan;
+    int exact_walk;                    // 1: the walks evaluate the D3 sequence at every column (no fast path)
     HoughConsts c;
     // geometry (work sizing only)
     int32_t n_layers;

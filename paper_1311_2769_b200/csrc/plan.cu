@@ -80,6 +80,8 @@ extern "C" int hough_plan_create(const hough_binning* b, const hough_geometry* g
     for (int l = 0; l < g->n_layers; ++l) p->layer_r[l] = g->layer_radius_cm[l];
     const char* env = getenv("HOUGH_DEBUG_FULLSCAN");
     p->fullscan = (env && env[0] == '1') ? 1 : 0;
+    env = getenv("HOUGH_DEBUG_EXACT_WALK");
+    p->exact_walk = (env && env[0] == '1') ? 1 : 0;
 
     cudaError_t ce = cudaGetDevice(&p->device);
     if (ce == cudaSuccess) ce = cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, p->device);
@@ -137,7 +139,7 @@ extern "C" int hough_plan_create(const hough_binning* b, const hough_geometry* g
     for (size_t t = 0; t < winT.size(); ++t) {
         int lo_bits;
         memcpy(&lo_bits, &win.lo_off[t], 4);
-        winT[t] = make_int2(lo_bits, win.steps[t]);
+        winT[t] = make_int2(lo_bits, win.steps[t] | (win.fwd_safe[t] ? (1 << 30) : 0));
     }
     // packed 16-bit tiles are exact whenever no bin can exceed 65535: the U16 precondition, or at most 65535
     // hits per call (a hit casts at most one vote per (phi0, d0) column, D3)
@@ -210,5 +212,6 @@ extern "C" size_t hough_accum_bytes(const hough_plan* p, int32_t n_events) {
 extern "C" int hough_plan_set_option(hough_plan* p, const char* key, int32_t value) {
     if (!p || !key) return HOUGH_ERR_INVALID_ARG;
     if (strcmp(key, "fullscan") == 0) { p->fullscan = value ? 1 : 0; return HOUGH_OK; }
+    if (strcmp(key, "exact_walk") == 0) { p->exact_walk = value ? 1 : 0; return HOUGH_OK; }
     return HOUGH_ERR_INVALID_ARG;
 }
