@@ -61,6 +61,7 @@ struct hough_plan {
     int32_t max_hits, max_events;
     int device, sm_count;
     int fullscan;
+    int peaks_tiled;                   // 1: find_peaks uses the shared-memory halo-tile kernels instead of the slice walk
     int exact_walk;                    // 1: the walks evaluate the D3 sequence at every column (no fast path)
     HoughConsts c;
     // geometry (work sizing only)

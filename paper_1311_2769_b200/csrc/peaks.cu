@@ -436,6 +436,133 @@ __global__ void __launch_bounds__(256) peak_tile_kernel(HoughConsts c, const voi
     }
 }
 
+
+// ---- slice-walk mask kernel (default when rows are 16-byte multiples) -------------------------------------------
+// One thread owns VEC consecutive q/pT bins of one phi0 row (one 16-byte load: 8 uint16 or 4 int32 bins) and walks
+// a run of d0 slices k0..k1-1, keeping in registers the rows i-1, i, i+1 of the centre slice, the same rows of the
+// next slice and the column maximum of the previous slice.  With
+//     V_s[j]  = max over di of slice s           (all of slice k-1 is "before" the centre, all of slice k+1 "after")
+//     B[j]    = max(V_{k-1}[j], R_k[i-1][j]),    A[j] = max(V_{k+1}[j], R_k[i+1][j])
+// the D5 predicate of bin (k, i, j) with value a is
+//     a >= threshold  &&  a > max(B[j-1], B[j], B[j+1], R_k[i][j-1])  &&  a >= max(A[j-1], A[j], A[j+1], R_k[i][j+1]).
+// Missing neighbours (q/pT and d0 faces) enter as MISSING = a value below every bin, which leaves both
+// comparisons true, i.e. skips them (D5).  The accumulator is read once from L2/HBM per slice run plus a
+// one-slice halo at each end of a run; neighbouring rows come from L1.
+// Output: the peak bitmask (1 bit per bin) and the per-block peak counts consumed by scan + peak_emit_kernel.
+template <bool U16> struct KW { static constexpr int VEC = 4; static constexpr int MISSING = (int)0x80000000; };
+template <> struct KW<true> { static constexpr int VEC = 8; static constexpr int MISSING = -1; };
+
+template <bool U16>
+__device__ __forceinline__ void kw_load_row(const void* __restrict__ acc, size_t row_bin0, int j0, int nq, bool present,
+                                            int (&v)[KW<U16>::VEC + 2]) {
+    constexpr int VEC = KW<U16>::VEC;
+    constexpr int MISSING = KW<U16>::MISSING;
+    if (!present) {
+#pragma unroll
+        for (int x = 0; x < VEC + 2; ++x) v[x] = MISSING;
+        return;
+    }
+    if (U16) {
+        const unsigned short* row = reinterpret_cast<const unsigned short*>(acc) + row_bin0;
+        const uint4 q = __ldg(reinterpret_cast<const uint4*>(row + j0));
+        v[1] = (int)(q.x & 0xffffu); v[2] = (int)(q.x >> 16);
+        v[3] = (int)(q.y & 0xffffu); v[4] = (int)(q.y >> 16);
+        v[5] = (int)(q.z & 0xffffu); v[6] = (int)(q.z >> 16);
+        v[7] = (int)(q.w & 0xffffu); v[8] = (int)(q.w >> 16);
+        v[0] = j0 > 0 ? (int)__ldg(row + j0 - 1) : MISSING;
+        v[VEC + 1] = j0 + VEC < nq ? (int)__ldg(row + j0 + VEC) : MISSING;
+    } else {
+        const int* row = reinterpret_cast<const int*>(acc) + row_bin0;
+        const int4 q = __ldg(reinterpret_cast<const int4*>(row + j0));
+        v[1] = q.x; v[2] = q.y; v[3] = q.z; v[4] = q.w;
+        v[0] = j0 > 0 ? __ldg(row + j0 - 1) : MISSING;
+        v[VEC + 1] = j0 + VEC < nq ? __ldg(row + j0 + VEC) : MISSING;
+    }
+}
+
+__device__ __forceinline__ int kw_max3(int a, int b, int c) { return max(max(a, b), c); }
+
+template <bool U16>
+__global__ void __launch_bounds__(256, 2) peak_kwalk_kernel(HoughConsts c, const void* __restrict__ acc, int threshold,
+                                                            int n_events, int kseg, int n_seg, int blocks_per_event,
+                                                            uint32_t* __restrict__ mask, int32_t* __restrict__ block_cnt) {
+    constexpr int VEC = KW<U16>::VEC;
+    constexpr int W = VEC + 2;
+    const int nphi = c.n_phi, nq = c.n_qpt, nd = c.n_d0;
+    const int cpr = nq / VEC;                                   // chunks per row
+    const long long strips_per_seg = (long long)nphi * cpr;
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long total = strips_per_seg * n_seg * n_events;
+    const bool live = gid < total;                              // (nphi * cpr) % 32 == 0: a warp is all live or all dead
+    if (!live) return;
+    const int chunk = (int)(gid % cpr);
+    const int i = (int)((gid / cpr) % nphi);
+    const int seg = (int)((gid / strips_per_seg) % n_seg);
+    const int e = (int)(gid / (strips_per_seg * n_seg));
+    const int j0 = chunk * VEC;
+    const int k0 = seg * kseg, k1 = min(k0 + kseg, nd);
+    const int im = i == 0 ? nphi - 1 : i - 1, ip = i == nphi - 1 ? 0 : i + 1;
+    const size_t ebin = (size_t)e * (size_t)c.bins_per_event;
+    const size_t slice_bins = (size_t)nphi * nq;
+    const size_t rm = ebin + (size_t)im * nq, r0 = ebin + (size_t)i * nq, rp = ebin + (size_t)ip * nq;
+    unsigned char* mask_bytes = reinterpret_cast<unsigned char*>(mask + (size_t)e * c.words_per_event);
+
+    int Vm[W], Rm[W], R0[W], Rp[W];
+    {
+        int a[W], b[W], d[W];
+        const bool has = k0 > 0;
+        const size_t so = (size_t)(has ? k0 - 1 : 0) * slice_bins;
+        kw_load_row<U16>(acc, rm + so, j0, nq, has, a);
+        kw_load_row<U16>(acc, r0 + so, j0, nq, has, b);
+        kw_load_row<U16>(acc, rp + so, j0, nq, has, d);
+#pragma unroll
+        for (int x = 0; x < W; ++x) Vm[x] = kw_max3(a[x], b[x], d[x]);
+        const size_t sc = (size_t)k0 * slice_bins;
+        kw_load_row<U16>(acc, rm + sc, j0, nq, true, Rm);
+        kw_load_row<U16>(acc, r0 + sc, j0, nq, true, R0);
+        kw_load_row<U16>(acc, rp + sc, j0, nq, true, Rp);
+    }
+    for (int k = k0; k < k1; ++k) {
+        int Nm[W], N0[W], Np[W];
+        const bool has = k + 1 < nd;
+        const size_t sn = (size_t)(has ? k + 1 : k) * slice_bins;
+        kw_load_row<U16>(acc, rm + sn, j0, nq, has, Nm);
+        kw_load_row<U16>(acc, r0 + sn, j0, nq, has, N0);
+        kw_load_row<U16>(acc, rp + sn, j0, nq, has, Np);
+        int B[W], A[W];
+#pragma unroll
+        for (int x = 0; x < W; ++x) {
+            B[x] = max(Vm[x], Rm[x]);
+            A[x] = max(kw_max3(Nm[x], N0[x], Np[x]), Rp[x]);
+        }
+        unsigned flags = 0u;
+#pragma unroll
+        for (int x = 1; x <= VEC; ++x) {
+            const int a = R0[x];
+            const int before = max(kw_max3(B[x - 1], B[x], B[x + 1]), R0[x - 1]);
+            const int after = max(kw_max3(A[x - 1], A[x], A[x + 1]), R0[x + 1]);
+            if (a >= threshold && a > before && a >= after) flags |= 1u << (x - 1);
+        }
+        // bitmask: bin b of the event -> bit (b & 7) of byte (b >> 3)
+        const size_t bin0 = ((size_t)k * nphi + i) * nq + j0;
+        if (U16) {
+            mask_bytes[bin0 >> 3] = (unsigned char)flags;
+        } else {
+            const unsigned other = __shfl_xor_sync(0xffffffffu, flags, 1);
+            if ((threadIdx.x & 1) == 0) mask_bytes[bin0 >> 3] = (unsigned char)(flags | (other << 4));
+        }
+        // a warp covers 32 * VEC consecutive bins of one slice, i.e. one peak block
+        const int cnt = __reduce_add_sync(0xffffffffu, __popc(flags));
+        if ((threadIdx.x & 31) == 0 && cnt)
+            atomicAdd(block_cnt + (size_t)e * blocks_per_event + (int)(bin0 / PEAK_BLOCK_BINS), cnt);
+#pragma unroll
+        for (int x = 0; x < W; ++x) {
+            Vm[x] = kw_max3(Rm[x], R0[x], Rp[x]);
+            Rm[x] = Nm[x]; R0[x] = N0[x]; Rp[x] = Np[x];
+        }
+    }
+}
+
 }  // namespace
 
 extern "C" int hough_find_peaks(hough_plan* p, const void* d_accum, int32_t n_events, int32_t threshold,
@@ -454,8 +581,29 @@ extern "C" int hough_find_peaks(hough_plan* p, const void* d_accum, int32_t n_ev
     const int bpe = p->peak_blocks_per_event;
     dim3 grid(bpe, n_events);
     const size_t tile_bytes = peak_tile_bytes(p->c);
-    const bool tiled = !p->fullscan && tile_bytes <= 100 * 1024;
-    if (tiled) {
+    const int kw_vec = p->c.is_u16 ? 8 : 4;
+    const bool kwalk = !p->fullscan && !p->peaks_tiled && p->c.n_qpt % 8 == 0 &&
+                       ((long long)p->c.n_phi * (p->c.n_qpt / kw_vec)) % 32 == 0 && PEAK_BLOCK_BINS % (32 * kw_vec) == 0 &&
+                       (reinterpret_cast<uintptr_t>(d_accum) & 15u) == 0;
+    const bool tiled = !kwalk && !p->fullscan && tile_bytes <= 100 * 1024;
+    if (kwalk) {
+        // enough slice runs to fill the GPU, each at least 8 slices long (a run re-reads one halo slice per end)
+        const long long strips = (long long)p->c.n_phi * (p->c.n_qpt / kw_vec) * n_events;
+        int n_seg = 1;
+        while (strips * n_seg < 256LL * 2 * p->sm_count * 2 && (p->c.n_d0 + n_seg) / (n_seg + 1) >= 8) ++n_seg;
+        const int kseg = (p->c.n_d0 + n_seg - 1) / n_seg;
+        n_seg = (p->c.n_d0 + kseg - 1) / kseg;
+        const long long threads = strips * n_seg;
+        const long long nblk = (threads + 255) / 256;
+        if (nblk > 0x7fffffffLL) return HOUGH_ERR_UNSUPPORTED;
+        HOUGH_CUDA_TRY(cudaMemsetAsync(p->d_peak_block_cnt, 0, sizeof(int32_t) * (size_t)n_events * bpe, st));
+        if (p->c.is_u16)
+            peak_kwalk_kernel<true><<<(unsigned)nblk, 256, 0, st>>>(p->c, d_accum, threshold, n_events, kseg, n_seg, bpe,
+                                                                    p->d_mask, p->d_peak_block_cnt);
+        else
+            peak_kwalk_kernel<false><<<(unsigned)nblk, 256, 0, st>>>(p->c, d_accum, threshold, n_events, kseg, n_seg, bpe,
+                                                                     p->d_mask, p->d_peak_block_cnt);
+    } else if (tiled) {
         static bool smem_configured = false;        // the tiled path never needs more than 100 KB
         if (!smem_configured) {
             const int cap = 100 * 1024;

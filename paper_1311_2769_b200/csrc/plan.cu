@@ -212,6 +212,7 @@ extern "C" size_t hough_accum_bytes(const hough_plan* p, int32_t n_events) {
 extern "C" int hough_plan_set_option(hough_plan* p, const char* key, int32_t value) {
     if (!p || !key) return HOUGH_ERR_INVALID_ARG;
     if (strcmp(key, "fullscan") == 0) { p->fullscan = value ? 1 : 0; return HOUGH_OK; }
+    if (strcmp(key, "peaks_tiled") == 0) { p->peaks_tiled = value ? 1 : 0; return HOUGH_OK; }
     if (strcmp(key, "exact_walk") == 0) { p->exact_walk = value ? 1 : 0; return HOUGH_OK; }
     return HOUGH_ERR_INVALID_ARG;
 }

@@ -24,7 +24,7 @@ class CudaResult:
 
 
 def run_cuda(binning, bz, layers, hits_xy, event_offsets, threshold, assoc_dj, min_hits, capacity,
-             fullscan=False, want_accum=True, plan=None) -> CudaResult:
+             fullscan=False, want_accum=True, plan=None, options=()) -> CudaResult:
     n_hits = int(hits_xy.shape[0])
     n_events = int(event_offsets.shape[0] - 1)
     own = plan is None
@@ -34,6 +34,8 @@ def run_cuda(binning, bz, layers, hits_xy, event_offsets, threshold, assoc_dj, m
                          max_events=max(n_events, 1))
     if fullscan:
         plan.set_option("fullscan", 1)
+    for key in options:
+        plan.set_option(key, 1)
     dev = "cuda"
     d_hits = torch.from_numpy(np.ascontiguousarray(hits_xy, np.float32).reshape(-1, 2)).to(dev)
     if n_hits == 0:
@@ -114,7 +116,7 @@ def assert_centroids_close(got, ref, binning):
         assert np.all(np.abs(g - r) <= tol), name
 
 
-def run_vote(binning, bz, layers, hits_xy, event_offsets, max_hits=None, misalign=False, fullscan=False):
+def run_vote(binning, bz, layers, hits_xy, event_offsets, max_hits=None, misalign=False, fullscan=False, options=()):
     """hough_vote alone -> accumulator as numpy.  misalign: the hit pointer is 8- but not 16-byte aligned."""
     n_hits = int(hits_xy.shape[0])
     n_events = int(event_offsets.shape[0] - 1)
@@ -123,6 +125,8 @@ def run_vote(binning, bz, layers, hits_xy, event_offsets, max_hits=None, misalig
                      max_events=max(n_events, 1))
     if fullscan:
         plan.set_option("fullscan", 1)
+    for key in options:
+        plan.set_option(key, 1)
     buf = torch.zeros((n_hits + 2, 2), dtype=torch.float32, device="cuda")
     assert buf.data_ptr() % 16 == 0
     first = 1 if misalign else 0
@@ -139,7 +143,7 @@ def run_vote(binning, bz, layers, hits_xy, event_offsets, max_hits=None, misalig
 
 
 def run_assign(binning, bz, layers, hits_xy, event_offsets, records, cand_offsets, capacity, assoc_dj, min_hits,
-               max_hits=None, fullscan=False):
+               max_hits=None, fullscan=False, options=()):
     """hough_assign_hits alone on a caller-made candidate list (CAND_DTYPE records, int32 offsets)."""
     n_hits = int(hits_xy.shape[0])
     n_events = int(event_offsets.shape[0] - 1)
@@ -148,6 +152,8 @@ def run_assign(binning, bz, layers, hits_xy, event_offsets, records, cand_offset
                      max_events=max(n_events, 1))
     if fullscan:
         plan.set_option("fullscan", 1)
+    for key in options:
+        plan.set_option(key, 1)
     d_hits = torch.from_numpy(np.ascontiguousarray(hits_xy, np.float32).reshape(-1, 2)).cuda()
     d_off = torch.from_numpy(np.ascontiguousarray(event_offsets, np.int32)).cuda()
     cands = alloc_candidates(capacity)

@@ -22,7 +22,7 @@ def _narrow(acc_i32, binning):
     return acc_i32
 
 
-def _compare_all(w, batch, binning=None, capacity=None, fullscan=False, oracle_parallel=False):
+def _compare_all(w, batch, binning=None, capacity=None, fullscan=False, oracle_parallel=False, options=()):
     bn = binning or w.binning
     o = Oracle.from_binning(bn, w.bz_tesla)
     if oracle_parallel:
@@ -33,7 +33,7 @@ def _compare_all(w, batch, binning=None, capacity=None, fullscan=False, oracle_p
         ref = o.find_peaks(acc, w.threshold)
     cap = ref.total + 7 if capacity is None else capacity
     got = run_cuda(bn, w.bz_tesla, w.layers, batch.hits_xy, batch.event_offsets, w.threshold, w.assoc_dj, w.min_hits,
-                   cap, fullscan=fullscan)
+                   cap, fullscan=fullscan, options=options)
     assert np.array_equal(got.accum, _narrow(acc, bn)), "accumulator differs"
     assert int(got.accum.astype(np.int64).sum()) == votes
     assert got.total == ref.total and np.array_equal(got.offsets, ref.offsets)
@@ -55,6 +55,13 @@ def test_config_0_1_bit_exact(cfg, fullscan):
     w = get_workload(cfg)
     got, ref = _compare_all(w, generate_events(w), fullscan=fullscan)
     assert ref.total > 0
+
+
+@pytest.mark.parametrize("cfg", [0, 1])
+def test_config_0_1_exact_walk_and_tiled_peaks(cfg):
+    """The bisecting options: D3 at every window column (no fast path) and the halo-tile peak kernels."""
+    w = get_workload(cfg)
+    _compare_all(w, generate_events(w), options=("exact_walk", "peaks_tiled"))
 
 
 def test_config_2_bit_exact():
@@ -158,6 +165,8 @@ def test_vote_tile_variants_bit_exact(shape, dtype, max_hits, layers, misalign):
     acc, votes = oracle_vote_parallel(o, hits, off)
     got = run_vote(bn, 3.8, layers, hits, off, max_hits=max_hits, misalign=misalign)
     assert votes > 0 and np.array_equal(got.astype(np.int32), acc)
+    got = run_vote(bn, 3.8, layers, hits, off, max_hits=max_hits, misalign=misalign, options=("exact_walk",))
+    assert np.array_equal(got.astype(np.int32), acc)
 
 
 def test_vote_half_circle_windows_and_negative_field():
@@ -194,15 +203,21 @@ def test_assign_tile_variants_bit_exact(shape, dtype, max_hits, dj):
     assert (h2c >= 0).sum() > 100
 
 
-@pytest.mark.parametrize("shape,dtype,fullscan", [
-    ((100, 37, 3), ACC_U16, False),      # peak blocks that span two d0 slices, unaligned rows
-    ((100, 37, 3), ACC_I32, True),       # generic per-bin path
-    ((64, 4096, 2), ACC_I32, False),     # one row per peak block
-    ((16, 20000, 2), ACC_U16, False),    # rows too long for the halo tile
-    ((512, 256, 3), ACC_I32, False),
-    ((256, 128, 1), ACC_U16, False),     # 2-D: no neighbour slices at all
+@pytest.mark.parametrize("shape,dtype,fullscan,tiled", [
+    ((100, 37, 3), ACC_U16, False, False),      # odd rows: halo tiles; peak blocks that span two d0 slices
+    ((100, 37, 3), ACC_I32, True, False),       # generic per-bin path
+    ((64, 4096, 2), ACC_I32, False, False),     # slice walk, one row per peak block
+    ((64, 4096, 2), ACC_I32, False, True),      # halo tiles, one row per peak block
+    ((16, 20000, 2), ACC_U16, False, False),    # slice walk, long rows
+    ((16, 20000, 2), ACC_U16, False, True),     # rows too long for the halo tile
+    ((512, 256, 3), ACC_I32, False, False),
+    ((512, 256, 3), ACC_I32, False, True),
+    ((256, 128, 1), ACC_U16, False, False),     # 2-D: no neighbour slices at all
+    ((256, 128, 1), ACC_U16, False, True),
+    ((64, 64, 40), ACC_U16, False, False),      # slice walk cut into several slice runs
+    ((32, 8, 5), ACC_I32, False, False),        # slice walk, one 16-byte chunk pair per row
 ])
-def test_peaks_tile_variants_bit_exact(shape, dtype, fullscan):
+def test_peaks_tile_variants_bit_exact(shape, dtype, fullscan, tiled):
     bn = HoughBinning(*shape, accum_dtype=dtype)
     hits, off = _mixed_hits(shape[1], 2500, LAYERS_10)
     hits = np.concatenate([hits, hits[::3]])                      # duplicated hits -> plateaus
@@ -213,7 +228,8 @@ def test_peaks_tile_variants_bit_exact(shape, dtype, fullscan):
     ref = o.find_peaks(acc, thr)
     assert ref.total > 20
     for cap in (ref.total + 3, ref.total // 2):
-        got = run_cuda(bn, 3.8, LAYERS_10, hits, off, thr, 1, 2, cap, fullscan=fullscan)
+        got = run_cuda(bn, 3.8, LAYERS_10, hits, off, thr, 1, 2, cap, fullscan=fullscan,
+                       options=("peaks_tiled",) if tiled else ())
         assert got.total == ref.total and np.array_equal(got.offsets, ref.offsets)
         n_c = min(cap, ref.total)
         for f in ("event", "k", "i", "j", "votes"):
