@@ -47,7 +47,8 @@ __host__ __device__ inline size_t walk_smem_bytes(int cols, int stride, int n_cl
     b += (size_t)cols * 8;                                              // cos/sin of the tile's columns
     b += (size_t)n_class * 8;                                           // lo_off, steps
     b += (size_t)n_class * 2 * 8 + ((size_t)n_class * 2 + 1) * 4;       // segments
-    return (b + 15) & ~(size_t)15;
+    b = (b + 15) & ~(size_t)15;
+    return b + 128;                                                     // one scratch word per lane (walk_kernel: s_trash)
 }
 
 // D8 key with the candidate's linear bin in place of its index: inside one event the candidate list is sorted
@@ -83,10 +84,15 @@ __device__ __forceinline__ float rcp_approx(float g) {
     return r;
 }
 
-// atomicAdd on shared memory under a predicate, without a branch in the instruction stream
-__device__ __forceinline__ void red_shared_if(bool p, unsigned saddr, unsigned val) {
-    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.u32 q, %2, 0;\n\t@q red.shared.add.u32 [%0], %1;\n\t}"
-                 :: "r"(saddr), "r"(val), "r"((unsigned)p) : "memory");
+__device__ __forceinline__ float rsqrt_approx(float g) {
+    float r;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(r) : "f"(g));
+    return r;
+}
+
+// atomicAdd on shared memory by shared-window address (no generic-address conversion in the hot loop)
+__device__ __forceinline__ void red_shared(unsigned saddr, unsigned val) {
+    asm volatile("red.shared.add.u32 [%0], %1;" :: "r"(saddr), "r"(val) : "memory");
 }
 
 // Per-tile constants of the fast path (uniform over the CTA).  DESIGN.md "Fast path":
@@ -159,6 +165,9 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
         s_seg_cnt = reinterpret_cast<int*>(q);    q += (size_t)nc * 2 * 4;
         s_seg_pref = reinterpret_cast<int*>(q);
     }
+    // one scratch word per lane at the end of the block: where the branch-free vote sends the lanes that do not vote
+    const unsigned trash_saddr = (unsigned)__cvta_generic_to_shared(
+        smem_raw + walk_smem_bytes(slab_cols, stride, nc) - 128 + 4 * lane);
     unsigned short* s_tile16 = reinterpret_cast<unsigned short*>(s_tile);
     const unsigned tile_saddr = (unsigned)__cvta_generic_to_shared(s_tile);
 
@@ -285,13 +294,9 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
     const FastK fk = make_fastk(c, d);
     const bool exact_only = a.exact_only != 0 || nq > (1 << 20);      // the rint trick needs |t| < 2^22
     const unsigned row_lin0 = (unsigned)(k * nphi + c0) * (unsigned)nq;   // linear bin of (k, c0, 0) inside the event
+    int seg = 0;                                        // batches ascend per warp: a running segment pointer
     for (int bt = warp; bt < n_batches; bt += WALK_WARPS) {
-        int lo_i = 0, hi_i = 2 * nc;                    // largest segment with seg_pref[seg] <= bt
-        while (hi_i - lo_i > 1) {
-            const int mid = (lo_i + hi_i) >> 1;
-            if (s_seg_pref[mid] <= bt) lo_i = mid; else hi_i = mid;
-        }
-        const int seg = lo_i;
+        while (s_seg_pref[seg + 1] <= bt) ++seg;         // largest segment with seg_pref[seg] <= bt (seg_pref[2nc] = n_batches > bt)
         const int in_seg = (bt - s_seg_pref[seg]) * 32 + lane;
         const bool active = in_seg < s_seg_cnt[seg];
         const int cl = seg >> 1;
@@ -309,8 +314,10 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
         float arel_h;
         {
             const float S = __fmaf_rn(8.0f * fk.d0abs, L, r2 + fk.d0sq);
-            const float dr = sqrtf(r2) - fk.d0abs;                        // den >= (r - |d0|)^2
-            arel_h = WALK_U * __fmaf_rn(6.0f, __fdividef(S, dr * dr), 24.0f);
+            // den >= (r - |d0|)^2; r from the approximate reciprocal square root (2 ulp), shrunk by 2^-20 r
+            const float rr = r2 * rsqrt_approx(r2);
+            const float dr = fmaxf(fabsf(rr - fk.d0abs) - 9.5367432e-7f * rr, 0.0f);
+            arel_h = WALK_U * __fmaf_rn(6.0f, S * rcp_approx(dr * dr), 24.0f);
             if (!(arel_h < 1.0f)) arel_h = 1.0f;                          // r ~ |d0| (or NaN): every evaluation goes exact
         }
         int i_lo = (int)ceilf(hv.z + s_lo[cl]);
@@ -372,13 +379,13 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
             }                                                                                                   \
         } while (0)
 
-// the same under predicate P, branch-free for the vote (J may be anything when P is false)
+// the same under predicate P; the vote is branch-free: lanes with P false add to their scratch word (J arbitrary)
 #define WALK_AT_IF(P, COL, J)                                                                                   \
         do {                                                                                                    \
             if (MODE == WALK_VOTE) {                                                                            \
-                if (TILE32) red_shared_if((P), tile_saddr + (unsigned)(((COL) * stride + (J)) << 2), 1u);       \
-                else red_shared_if((P), tile_saddr + (unsigned)(((COL) * stride + ((J) >> 1)) << 2),            \
-                                   __funnelshift_l(0u, 1u, (unsigned)(J) << 4));                                \
+                if (TILE32) red_shared((P) ? tile_saddr + (unsigned)(((COL) * stride + (J)) << 2) : trash_saddr, 1u); \
+                else red_shared((P) ? tile_saddr + (unsigned)(((COL) * stride + ((J) >> 1)) << 2) : trash_saddr, \
+                                __funnelshift_l(0u, 1u, (unsigned)(J) << 4));                                   \
             } else {                                                                                            \
                 if (P) WALK_AT(COL, J);                                                                         \
             }                                                                                                   \
@@ -403,23 +410,26 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
             for (int tb0 = 0; tb0 < t_cnt; tb0 += 32) {
                 const int n_it = min(32, t_cnt - tb0);
                 const int col_chunk = col;
+                // inactive lanes (tail of a batch): range test never passes, bin decision always "sure"
+                const unsigned nq_l = active ? (unsigned)nq : 0u;
+                const float hm0_l = active ? fk.hm0 : 3.0e38f;
                 unsigned slowmask = 0u;                  // bit (n_it - 1 - i): column i of the chunk needs the exact path
                 if (fwd_safe) {
 #pragma unroll 2
                     for (int t = tb0; t < tb0 + n_it; ++t) {
                         const bool in_tile = FULLPHI ? true : (col < cols);
-                        const bool mine = FULLPHI ? active : (in_tile && (unsigned)(t - my_b) < (unsigned)my_n);
+                        const bool mine = FULLPHI ? true : (in_tile && (unsigned)(t - my_b) < (unsigned)my_n);
                         const float2 cs = s_cs[in_tile ? col : 0];
                         const float w = __fmaf_rn(y, cs.x, -__fmul_rn(x, cs.y));
                         const float numq = __fmaf_rn(-w, fk.inv_wq, fk.d0cq);
                         const float rinv = rcp_approx(__fmaf_rn(fk.ntd0A, w, r2Ak));
                         const float th = __fmaf_rn(numq, rinv, fk.c0h);                        // t~ - 1/2
-                        const float hm = __fmaf_rn(__fmaf_rn(arel_h, fabsf(numq), elin_h), -fabsf(rinv), fk.hm0);
+                        const float hm = __fmaf_rn(__fmaf_rn(arel_h, fabsf(numq), elin_h), -fabsf(rinv), hm0_l);
                         const float yb = __fadd_rn(th, WALK_MAGIC);
                         const float dlt = __fsub_rn(th, __fsub_rn(yb, WALK_MAGIC));             // (t~ - 1/2) - J
                         const int jf = __float_as_int(yb) - __float_as_int(WALK_MAGIC);         // J = rint(t~ - 1/2)
                         const bool sure = fabsf(dlt) < hm;                                      // J <= t_D3 < J + 1
-                        WALK_AT_IF(mine && sure && (unsigned)jf < (unsigned)nq, col, jf);
+                        WALK_AT_IF(mine && sure && (unsigned)jf < nq_l, col, jf);
                         slowmask = (slowmask << 1) | ((mine && !sure) ? 1u : 0u);
                         ++col;
                         if (col == nphi) col = 0;
@@ -428,24 +438,25 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
 #pragma unroll 2
                     for (int t = tb0; t < tb0 + n_it; ++t) {
                         const bool in_tile = FULLPHI ? true : (col < cols);
-                        const bool mine = FULLPHI ? active : (in_tile && (unsigned)(t - my_b) < (unsigned)my_n);
+                        const bool mine = FULLPHI ? true : (in_tile && (unsigned)(t - my_b) < (unsigned)my_n);
                         const float2 cs = s_cs[in_tile ? col : 0];
                         const float w = __fmaf_rn(y, cs.x, -__fmul_rn(x, cs.y));
                         const bool fwd = __fadd_rn(__fmul_rn(x, cs.x), __fmul_rn(y, cs.y)) > 0.0f;   // the exact D3 forward test
                         const float numq = __fmaf_rn(-w, fk.inv_wq, fk.d0cq);
                         const float rinv = rcp_approx(__fmaf_rn(fk.ntd0A, w, r2Ak));
                         const float th = __fmaf_rn(numq, rinv, fk.c0h);
-                        const float hm = __fmaf_rn(__fmaf_rn(arel_h, fabsf(numq), elin_h), -fabsf(rinv), fk.hm0);
+                        const float hm = __fmaf_rn(__fmaf_rn(arel_h, fabsf(numq), elin_h), -fabsf(rinv), hm0_l);
                         const float yb = __fadd_rn(th, WALK_MAGIC);
                         const float dlt = __fsub_rn(th, __fsub_rn(yb, WALK_MAGIC));
                         const int jf = __float_as_int(yb) - __float_as_int(WALK_MAGIC);
                         const bool sure = fabsf(dlt) < hm;
-                        WALK_AT_IF(mine && fwd && sure && (unsigned)jf < (unsigned)nq, col, jf);
+                        WALK_AT_IF(mine && fwd && sure && (unsigned)jf < nq_l, col, jf);
                         slowmask = (slowmask << 1) | ((mine && fwd && !sure) ? 1u : 0u);
                         ++col;
                         if (col == nphi) col = 0;
                     }
                 }
+                if (!active) slowmask = 0u;
                 if (__any_sync(0xffffffffu, slowmask != 0u)) {
                     while (slowmask) {
                         const int bpos = __ffs(slowmask) - 1;
