@@ -8,7 +8,7 @@
 #include <vector>
 #include <algorithm>
 
-#include "common.cuh"
+#include "walk.cuh"
 
 namespace {
 thread_local char g_last_cuda[256] = "";
@@ -145,12 +145,14 @@ extern "C" int hough_plan_create(const hough_binning* b, const hough_geometry* g
     // hits per call (a hit casts at most one vote per (phi0, d0) column, D3)
     p->tile32 = (b->accum_dtype == HOUGH_ACC_I32 && max_hits > 65535) ? 1 : 0;
     {
-        const long long row_words = p->tile32 ? (long long)b->n_qpt : ((long long)b->n_qpt + 1) / 2;
-        const long long stride = row_words | 1;
+        // walk.cuh "Tile layout": a row (32-bit bins) or a row of column PAIRS (16-bit bins) has nq + 2 words
+        const long long stride = (long long)walk_row_stride(b->n_qpt);
         p->tile_stride_words = (int32_t)stride;
-        long long cols = (66LL * 1024) / (stride * 4);
-        if (cols < 8) cols = (200LL * 1024) / (stride * 4 + 8);          // wide rows: one big tile per SM
+        const long long col_bytes = (p->tile32 ? stride * 4 : stride * 2) + 8;     // tile + column-pair table
+        long long cols = (68LL * 1024) / col_bytes;
+        if (cols < 8) cols = (200LL * 1024) / col_bytes;                  // wide rows: one big tile per SM
         if (cols > b->n_phi) cols = b->n_phi;
+        cols &= ~1LL;                                                     // column pairs
         p->tile_max_cols = (int32_t)cols;                                 // 0: no tiled path (fullscan fallback)
     }
 

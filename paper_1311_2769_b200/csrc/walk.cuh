@@ -1,23 +1,30 @@
 // walk.cuh -- the column walk shared by the vote (A2/A3, vote.cu) and the hit association (A5, assign.cu).
 //
 // One CTA owns the tile (event e, d0 slice k, phi0 columns [c0, c0 + cols)) in shared memory:
-//   WALK_VOTE   : the tile is that part of the accumulator (two 16-bit bins per word, or 32-bit bins); votes
-//                 are shared-memory atomics, the tile is written to HBM exactly once (no global atomic; this
-//                 also implements "overwrite", S8).
+//   WALK_VOTE   : the tile is that part of the accumulator; votes are shared-memory atomics, the tile is written
+//                 to HBM exactly once (no global atomic; this also implements "overwrite", S8).
 //   WALK_ASSIGN : the tile holds, per bin, the best candidate of the event within assoc_dj bins of it along
 //                 q/pT ("dilated" entries, built from the candidate list in the prologue); every vote position
 //                 of a hit needs ONE probe; the best D8 key per (hit, tile) is published with one atomicMax.
 //
-// Work mapping: lane = hit.  A warp takes 32 consecutive staged hits of one radius class (same window length,
-// neighbouring azimuth thanks to the (class, sector) sort of stage.cu); every lane walks the `steps` columns of
-// its own window.  Lanes stay converged because `steps` is a property of (class, k).
+// Tile layout.  A row has nq + 2 slots h = J + 1: the q/pT bins J = 0..nq-1 and one
+// GUARD slot at each end (J = -1 and J = nq) that absorbs the fast path's "one bin outside" results and is never
+// flushed.  Packed tiles (16-bit bins) store the two columns of an even/odd column PAIR in one 32-bit word per
+// slot (low half = even column, high half = odd column), so the increment is the constant 1 or 65536 and the
+// address is pair_row + 4 h.  32-bit tiles store one word per (column, slot).
 //
-// Bin index per (hit, column): DESIGN.md "Fast path".  The prescribed D3 sequence costs ~30 issue slots
-// (IEEE reciprocal, unfused multiplies).  The walk first evaluates the same real-valued function with FMAs and
-// MUFU.RCP (t~) together with a bound m on |t~ - t_D3| (first-order rounding analysis of BOTH sequences, x3
-// safety); if floor(t~ - m) == floor(t~ + m) the D3 bin is that integer (or certainly out of range) without
-// running D3.  Otherwise (about 0.1 % of the evaluations: t within m of a bin edge, NaN/inf, |t| huge) the lane
-// runs the exact D3 sequence (d3_exact_bin).  The result is therefore the D3 bin in every case.
+// Work mapping: lane = hit.  A warp takes 32 consecutive staged hits of one radius class (same window length,
+// neighbouring azimuth thanks to the (class, sector) sort of stage.cu); every lane walks the columns of its own
+// window TWO AT A TIME with packed fp32x2 arithmetic (FFMA2 / FADD2 on sm_100a).
+//
+// Bin index per (hit, column): DESIGN.md "Fast path".  The prescribed D3 sequence costs ~30 issue slots (IEEE
+// reciprocal, unfused multiplies).  The walk evaluates the same real-valued function with FMAs and MUFU.RCP (t~)
+// and owns, per (hit, d0 slice), a bound m on |t~ - t_D3| (first-order rounding analysis of BOTH sequences with a
+// safety factor); if t~ is further than m from a bin edge the D3 bin is floor(t~) (or certainly out of range)
+// without running D3.  Otherwise (about 0.1 % of the evaluations) the (hit, column) goes to a small shared-memory
+// queue and is redone with the exact D3 sequence (d3_exact_bin) by the whole CTA at the end.  Hits whose bound is
+// useless (r ~ |d0|, non-finite coordinates), classes whose window is not certainly forward, and the plan option
+// "exact_walk" take the exact sequence at every column.  The result is therefore the D3 bin in every case.
 #pragma once
 
 #include "common.cuh"
@@ -26,12 +33,14 @@ constexpr int WALK_VOTE = 0;
 constexpr int WALK_ASSIGN = 1;
 constexpr int WALK_THREADS = 256;
 constexpr int WALK_WARPS = WALK_THREADS / 32;
+constexpr int WALK_CHUNK_PAIRS = 16;             // column pairs per chunk: 32 columns = the bits of the redo mask
+constexpr int WALK_QCAP = 192;                   // entries of the exact-redo queue (overflow: redone on the spot)
 
 struct WalkArgs {
     const float4* staged;            // [n_hits] staged hits (stage.cu)
     const int32_t* off;              // [n_events + 1] event offsets
     const int32_t* key_start;        // [n_events][n_keys + 1] exclusive key starts
-    int n_slabs, slab_cols, stride;  // tile shape
+    int n_slabs, slab_cols, stride;  // tile shape (slab_cols even; stride = words per row / pair row, odd)
     int exact_only;                  // 1: never take the fast path (plan option "exact_walk", for bisecting)
     // WALK_VOTE
     void* accum;
@@ -42,13 +51,20 @@ struct WalkArgs {
     unsigned long long* best_key;    // [n_hits] by original hit index
 };
 
-__host__ __device__ inline size_t walk_smem_bytes(int cols, int stride, int n_class) {
-    size_t b = ((size_t)cols * stride * 4 + 15) & ~(size_t)15;
-    b += (size_t)cols * 8;                                              // cos/sin of the tile's columns
+__host__ __device__ inline int walk_row_stride(int nq) { return (nq + 2) | 1; }
+
+__host__ __device__ inline size_t walk_tile_words(int cols, int stride, bool tile32) {
+    return tile32 ? (size_t)cols * stride : (size_t)((cols + 1) / 2) * stride;
+}
+
+__host__ __device__ inline size_t walk_smem_bytes(int cols, int stride, bool tile32, int n_class) {
+    size_t b = (walk_tile_words(cols, stride, tile32) * 4 + 15) & ~(size_t)15;
+    b += (size_t)(cols / 2 + WALK_CHUNK_PAIRS + 1) * 16;               // column pairs {cosA, cosB, sinA, sinB}
+    b += (size_t)WALK_QCAP * 8;                                         // exact-redo queue
     b += (size_t)n_class * 8;                                           // lo_off, steps
     b += (size_t)n_class * 2 * 8 + ((size_t)n_class * 2 + 1) * 4;       // segments
     b = (b + 15) & ~(size_t)15;
-    return b + 128;                                                     // one scratch word per lane (walk_kernel: s_trash)
+    return b + 128;                                                     // one scratch word per lane (walk_kernel: trash_saddr)
 }
 
 // D8 key with the candidate's linear bin in place of its index: inside one event the candidate list is sorted
@@ -90,20 +106,64 @@ __device__ __forceinline__ float rsqrt_approx(float g) {
     return r;
 }
 
-// atomicAdd on shared memory by shared-window address (no generic-address conversion in the hot loop)
+// ---- packed fp32x2 arithmetic (sm_100a: FFMA2 / FADD2, two fp32 lanes per issue slot) ----
+typedef unsigned long long f32x2;
+__device__ __forceinline__ f32x2 pk2(float lo, float hi) {
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void upk2(f32x2 v, float& lo, float& hi) {
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 fma2(f32x2 a, f32x2 b, f32x2 c) {
+    f32x2 r;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+    return r;
+}
+__device__ __forceinline__ f32x2 add2(f32x2 a, f32x2 b) {
+    f32x2 r;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+__device__ __forceinline__ f32x2 sub2(f32x2 a, f32x2 b) {
+    f32x2 r;
+    asm("sub.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+    return r;
+}
+
+// shared-memory accesses by shared-window address (no generic-address conversion in the hot loop)
 __device__ __forceinline__ void red_shared(unsigned saddr, unsigned val) {
     asm volatile("red.shared.add.u32 [%0], %1;" :: "r"(saddr), "r"(val) : "memory");
 }
-
-// Per-tile constants of the fast path (uniform over the CTA).  DESIGN.md "Fast path":
-//   t~ - 1/2 = numq * rinv + c0h,   numq = (d0c - w) * inv_wq,   rinv ~ 1 / (A * den),
-//   |t~ - t_D3| < m = |rinv| * (elin_h + arel_h * |numq|) + a0,   hm = 1/2 - m.
-struct FastK {
-    float inv_wq, d0cq, ntd0A, d0sqA, c0h, hm0, e_lin, d0abs, d0sq, A_f;
-};
+__device__ __forceinline__ unsigned lds_u16(unsigned saddr) {
+    unsigned short v;
+    asm volatile("ld.shared.u16 %0, [%1];" : "=h"(v) : "r"(saddr));
+    return (unsigned)v;
+}
+__device__ __forceinline__ unsigned lds_u32(unsigned saddr) {
+    unsigned v;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(saddr));
+    return v;
+}
+// base + 4 * idx as one IMAD (keeps the compiler from re-associating the address into three instructions)
+__device__ __forceinline__ unsigned addr_w(unsigned base, unsigned idx) {
+    unsigned r;
+    asm("mad.lo.u32 %0, %1, 4, %2;" : "=r"(r) : "r"(idx), "r"(base));
+    return r;
+}
 
 constexpr float WALK_U = 5.9604645e-8f;                 // 2^-24, unit roundoff of fp32
 constexpr float WALK_MAGIC = 12582912.0f;               // 1.5 * 2^23: x + MAGIC has rint(x) in its low mantissa bits
+constexpr int WALK_MAGIC_BITS = 0x4B400000;
+
+// Per-tile constants of the fast path (uniform over the CTA).  DESIGN.md "Fast path":
+//   t~ - 1/2 = numq * rinv + c0h,   numq = ny c + nx s + d0cq = (d0c - w) inv_wq,   rinv ~ 1 / (gy c + gx s + r2Ak) = 1 / (A den)
+//   |t~ - t_D3| < m_h = rmax_h * elin_h + arel_h * Tmax + a0   for every column whose t~ lies in [-1, nq + 1]
+struct FastK {
+    float inv_wq, d0cq, ntd0A, d0sqA, c0h, a0, e_lin, d0abs, d0sq, A_f, inv_A_abs, t_max;
+    bool usable;
+};
 
 __device__ __forceinline__ FastK make_fastk(const HoughConsts& c, float4 d) {
     FastK k;
@@ -114,10 +174,14 @@ __device__ __forceinline__ FastK make_fastk(const HoughConsts& c, float4 d) {
     k.d0sqA = d.z * c.A_f;
     const float c0 = -(c.qmin * c.inv_wq);
     k.c0h = c0 - 0.5f;
-    k.hm0 = 0.5f - 8.0f * WALK_U * (fabsf(c0) + 1.0f);
+    k.a0 = 8.0f * WALK_U * (fabsf(c0) + 1.0f);
     k.e_lin = 12.0f * WALK_U * fabsf(c.inv_wq);
     k.d0abs = fabsf(d.x);
     k.d0sq = d.z;
+    k.inv_A_abs = 1.0f / fabsf(c.A_f);
+    k.t_max = fmaxf(fabsf(c0), fabsf(c.nq_f - c0)) + 2.0f;
+    // the rint trick needs |t| < 2^22; a zero / non-finite field constant or range has no usable bound
+    k.usable = c.n_qpt < (1 << 20) && k.inv_A_abs < 3.0e38f && k.t_max < 4.0e6f && k.e_lin < 3.0e38f;
     return k;
 }
 
@@ -140,9 +204,52 @@ template <> struct EntryT<true> {                    // 32-bit entries: 27 bits 
     static __device__ __forceinline__ unsigned ent_hi(pkey_t p) { return (unsigned)(p >> 32); }
 };
 
+// ---- tile accessors by (tile column, q/pT bin J in [0, nq)) ----
+template <bool TILE32>
+__device__ __forceinline__ void tile_vote(uint32_t* s_tile, int stride, int col, int J) {
+    if (TILE32) atomicAdd(s_tile + col * stride + J + 1, 1u);
+    else atomicAdd(s_tile + (col >> 1) * stride + J + 1, 1u << (16 * (col & 1)));
+}
+template <bool TILE32>
+__device__ __forceinline__ unsigned tile_entry(const uint32_t* s_tile, int stride, int col, int J) {
+    if (TILE32) return s_tile[col * stride + J + 1];
+    return (unsigned)reinterpret_cast<const unsigned short*>(s_tile)[(((col >> 1) * stride + J + 1) << 1) + (col & 1)];
+}
+
+// What one exact vote position (tile column col, q/pT bin J in [0, nq)) does.  Association: the D8 key of the best
+// candidate serving the position is folded into `best`.
+template <int MODE, bool TILE32>
+__device__ __forceinline__ void walk_apply(uint32_t* s_tile, int stride, int nq, int col, int J, bool legacy, int assoc_dj,
+                                           const hough_candidate* __restrict__ cands, int cand_first, int cand_end, int c0,
+                                           unsigned row_lin0, unsigned long long& best) {
+    if (MODE == WALK_VOTE) {
+        tile_vote<TILE32>(s_tile, stride, col, J);
+    } else if (!legacy) {
+        const unsigned ent = tile_entry<TILE32>(s_tile, stride, col, J);
+        if (ent) {
+            const int adj = 15 - (int)((ent >> 1) & 15u);
+            const int jc = J + ((ent & 1u) ? -adj : adj);
+            const unsigned long long key = walk_key((ent >> 5) - 1u, adj, row_lin0 + (unsigned)(col * nq + jc));
+            best = key > best ? key : best;
+        }
+    } else {
+        const int j0 = max(J - assoc_dj, 0), j1 = min(J + assoc_dj, nq - 1);
+        for (int jj = j0; jj <= j1; ++jj) {
+            unsigned v = tile_entry<TILE32>(s_tile, stride, col, jj);
+            if (v) {
+                if (!TILE32 && v == 65535u)                       // saturated 16-bit entry: votes from the record
+                    v = walk_lookup_votes(cands, cand_first, cand_end, c0 + col, jj) + 1u;
+                const unsigned long long key = walk_key(v - 1u, abs(jj - J), row_lin0 + (unsigned)(col * nq + jj));
+                best = key > best ? key : best;
+            }
+        }
+    }
+}
+
 template <int MODE, bool TILE32, bool OUT16, bool FULLPHI>
 __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, WalkArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ int s_qn;
     const int n_slabs = a.n_slabs, slab_cols = a.slab_cols, stride = a.stride;
     const int slab = blockIdx.x % n_slabs;
     const int k = (blockIdx.x / n_slabs) % c.n_d0;
@@ -153,23 +260,26 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
     const int nq = c.n_qpt;
     const int nc = c.n_class;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int n_pair_tab = slab_cols / 2 + WALK_CHUNK_PAIRS + 1;
 
-    uint32_t* s_tile; float2* s_cs; float* s_lo; int* s_steps; int* s_seg_start; int* s_seg_cnt; int* s_seg_pref;
+    uint32_t* s_tile; float4* s_pair; int2* s_q; float* s_lo; int* s_steps; int* s_seg_start; int* s_seg_cnt; int* s_seg_pref;
     {
         unsigned char* q = smem_raw;
-        s_tile = reinterpret_cast<uint32_t*>(q);  q += ((size_t)slab_cols * stride * 4 + 15) & ~(size_t)15;
-        s_cs = reinterpret_cast<float2*>(q);      q += (size_t)slab_cols * 8;
+        s_tile = reinterpret_cast<uint32_t*>(q);  q += (walk_tile_words(slab_cols, stride, TILE32) * 4 + 15) & ~(size_t)15;
+        s_pair = reinterpret_cast<float4*>(q);    q += (size_t)n_pair_tab * 16;
+        s_q = reinterpret_cast<int2*>(q);         q += (size_t)WALK_QCAP * 8;
         s_lo = reinterpret_cast<float*>(q);       q += (size_t)nc * 4;
         s_steps = reinterpret_cast<int*>(q);      q += (size_t)nc * 4;
         s_seg_start = reinterpret_cast<int*>(q);  q += (size_t)nc * 2 * 4;
         s_seg_cnt = reinterpret_cast<int*>(q);    q += (size_t)nc * 2 * 4;
         s_seg_pref = reinterpret_cast<int*>(q);
     }
-    // one scratch word per lane at the end of the block: where the branch-free vote sends the lanes that do not vote
-    const unsigned trash_saddr = (unsigned)__cvta_generic_to_shared(
-        smem_raw + walk_smem_bytes(slab_cols, stride, nc) - 128 + 4 * lane);
     unsigned short* s_tile16 = reinterpret_cast<unsigned short*>(s_tile);
     const unsigned tile_saddr = (unsigned)__cvta_generic_to_shared(s_tile);
+    const unsigned stride4 = (unsigned)stride * 4u;
+    // one scratch word per lane at the end of the block: where the branch-free vote sends the lanes that do not vote
+    const unsigned trash_saddr = (unsigned)__cvta_generic_to_shared(
+        smem_raw + walk_smem_bytes(slab_cols, stride, TILE32, nc) - 128 + 4 * lane);
 
     int cand_first = 0, cand_end = 0;
     if (MODE == WALK_ASSIGN) {
@@ -181,9 +291,15 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
     // ---- prologue: zero the tile, load tables, list the segments of staged hits that can reach the tile ----
     {
         uint4* t4 = reinterpret_cast<uint4*>(s_tile);
-        const int n4 = (cols * stride + 3) >> 2;
+        const int n4 = (int)((walk_tile_words(cols, stride, TILE32) + 3) >> 2);
         for (int x = tid; x < n4; x += WALK_THREADS) t4[x] = make_uint4(0u, 0u, 0u, 0u);
-        for (int x = tid; x < cols; x += WALK_THREADS) s_cs[x] = __ldg(c.cs + c0 + x);
+        for (int p = tid; p < n_pair_tab; p += WALK_THREADS) {
+            int ca = c0 + 2 * p;                         // the table runs past the tile / wraps: never an out-of-range read
+            while (ca >= nphi) ca -= nphi;
+            const float2 A = __ldg(c.cs + ca), B = __ldg(c.cs + ca + 1);
+            s_pair[p] = make_float4(A.x, B.x, A.y, B.y);
+        }
+        if (tid == 0) s_qn = 0;
     }
     const int ev_begin = __ldg(a.off + e);
     const int32_t* ks = a.key_start + (size_t)e * (c.n_keys + 1);
@@ -192,7 +308,7 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
         const float lo = __int_as_float(w.x);
         const int steps = w.y & 0x3fffffff;
         s_lo[cl] = lo;
-        s_steps[cl] = w.y;                               // bit 30: every column of the window is forward (f > 0)
+        s_steps[cl] = w.y;                               // bit 30: every column of the window (+-2) is forward (f > 0)
         int a0 = 0, n0 = 0, a1 = 0, n1 = 0;
         if (steps > 0) {
             const int NS = c.n_sector;
@@ -256,8 +372,8 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
                 const int4 q = __ldg(reinterpret_cast<const int4*>(a.cands + ci));          // event, k, i, j
                 const unsigned v = (unsigned)__ldg(&a.cands[ci].votes) + 1u;
                 const int col = q.z - c0;
-                if (TILE32) s_tile[col * stride + q.w] = v;
-                else s_tile16[col * stride * 2 + q.w] = (unsigned short)min(v, 65535u);
+                if (TILE32) s_tile[col * stride + q.w + 1] = v;
+                else s_tile16[(((col >> 1) * stride + q.w + 1) << 1) + (col & 1)] = (unsigned short)min(v, 65535u);
             }
         } else {                                        // dilated entries: max over the candidates within assoc_dj
             const int dj = a.assoc_dj;
@@ -269,11 +385,10 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
                     const int d = q.w - jb;                                                  // j_cand - j_bin
                     const unsigned ent = v | (unsigned)((15 - abs(d)) * 2 + (d < 0 ? 1 : 0));
                     if (TILE32) {
-                        atomicMax(s_tile + col * stride + jb, ent);
+                        atomicMax(s_tile + col * stride + jb + 1, ent);
                     } else {
-                        const int h = col * stride * 2 + jb;
-                        uint32_t* wp = s_tile + (h >> 1);
-                        const int sh = (h & 1) * 16;
+                        uint32_t* wp = s_tile + (col >> 1) * stride + jb + 1;
+                        const int sh = (col & 1) * 16;
                         uint32_t old = *wp;
                         while (((old >> sh) & 0xffffu) < ent) {
                             const uint32_t nw = (old & ~(0xffffu << sh)) | (ent << sh);
@@ -292,8 +407,12 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
     const int n_batches = s_seg_pref[2 * nc];
     const float4 d = __ldg(c.d0t + k);
     const FastK fk = make_fastk(c, d);
-    const bool exact_only = a.exact_only != 0 || nq > (1 << 20);      // the rint trick needs |t| < 2^22
+    const bool exact_mode = a.exact_only != 0 || !fk.usable || (MODE == WALK_ASSIGN && legacy);
     const unsigned row_lin0 = (unsigned)(k * nphi + c0) * (unsigned)nq;   // linear bin of (k, c0, 0) inside the event
+    const unsigned tile_bytes = (unsigned)(walk_tile_words(cols, stride, TILE32) * 4);   // FULLPHI: the wrap distance
+    const unsigned nqg = (unsigned)nq + 2u;
+    const f32x2 d0cq2 = pk2(fk.d0cq, fk.d0cq), c0h2 = pk2(fk.c0h, fk.c0h);
+    const f32x2 magic2 = pk2(WALK_MAGIC, WALK_MAGIC), nmagic2 = pk2(-WALK_MAGIC, -WALK_MAGIC);
     int seg = 0;                                        // batches ascend per warp: a running segment pointer
     for (int bt = warp; bt < n_batches; bt += WALK_WARPS) {
         while (s_seg_pref[seg + 1] <= bt) ++seg;         // largest segment with seg_pref[seg] <= bt (seg_pref[2nc] = n_batches > bt)
@@ -303,240 +422,239 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
         const int steps_w = s_steps[cl];
         const int steps = steps_w & 0x3fffffff;
         const bool fwd_safe = (steps_w >> 30) & 1;
+        const int sidx = ev_begin + s_seg_start[seg] + in_seg;      // index of the lane's staged hit
         float4 hv = make_float4(1.f, 0.f, 0.f, 0.f);
-        if (active) hv = __ldg(a.staged + ev_begin + s_seg_start[seg] + in_seg);
+        if (active) hv = __ldg(a.staged + sidx);
         const float x = hv.x, y = hv.y;
         const float r2 = d3_r2(x, y);
-        // fast-path per-hit terms
-        const float r2Ak = __fmaf_rn(r2, fk.A_f, fk.d0sqA);              // g~ = ntd0A * w + r2Ak
-        const float L = fabsf(x) + fabsf(y);
-        const float elin_h = fk.e_lin * (L + fk.d0abs);
-        float arel_h;
-        {
-            const float S = __fmaf_rn(8.0f * fk.d0abs, L, r2 + fk.d0sq);
-            // den >= (r - |d0|)^2; r from the approximate reciprocal square root (2 ulp), shrunk by 2^-20 r
-            const float rr = r2 * rsqrt_approx(r2);
-            const float dr = fmaxf(fabsf(rr - fk.d0abs) - 9.5367432e-7f * rr, 0.0f);
-            arel_h = WALK_U * __fmaf_rn(6.0f, S * rcp_approx(dr * dr), 24.0f);
-            if (!(arel_h < 1.0f)) arel_h = 1.0f;                          // r ~ |d0| (or NaN): every evaluation goes exact
-        }
         int i_lo = (int)ceilf(hv.z + s_lo[cl]);
         if (i_lo < 0) i_lo += nphi;
         if (i_lo >= nphi) i_lo -= nphi;
         if (!(i_lo >= 0 && i_lo < nphi)) i_lo = 0;
-        int col, t_cnt, my_b = 0, my_n;
-        if (FULLPHI) {
-            col = i_lo;
-            t_cnt = steps;
-            my_n = 0;
-        } else {
-            int dd = i_lo - c0;                          // column relative to the tile, cyclic
-            if (dd < 0) dd += nphi;
-            const bool inside = dd < cols;
-            int t_begin = inside ? 0 : nphi - dd;
-            int t_end = inside ? min(steps, cols - dd) : min(steps, nphi - dd + cols);
-            if (steps + cols > nphi) { t_begin = 0; t_end = steps; }       // a window could re-enter the tile
-            if (!active || t_begin >= t_end) { t_begin = 0x3fffffff; t_end = 0; }
-            const int tb = __reduce_min_sync(0xffffffffu, t_begin);
-            const int te = __reduce_max_sync(0xffffffffu, t_end);
-            if (tb >= te) continue;
-            col = dd + tb;
-            if (col >= nphi) col -= nphi;
-            t_cnt = te - tb;
-            my_b = t_begin - tb;                         // this lane's own part of the warp's column range
-            my_n = t_end > t_begin ? t_end - t_begin : 0;
-        }
 
-        unsigned long long best = 0ull;                  // legacy association: full D8 key
+        unsigned long long best = 0ull;                  // association: full D8 key from the exact paths
         // dilated association: (entry >> 1) above ~column (equal votes and |dj| in two columns: the smaller linear
         // bin wins, D8); the entry's sign bit travels with the q/pT bin in bestj
         typename EntryT<TILE32>::pkey_t bestp = 0;
         int bestj = 0;
 
-// what one vote position (tile column `col`, q/pT bin J >= 0) does
-#define WALK_AT(COL, J)                                                                                              \
-        do {                                                                                                    \
-            if (MODE == WALK_VOTE) {                                                                            \
-                if (TILE32) atomicAdd(s_tile + (COL) * stride + (J), 1u);                                         \
-                else atomicAdd(s_tile + (COL) * stride + ((J) >> 1), (unsigned)((J) & 1) * 0xffffu + 1u);         \
-            } else if (!legacy) {                                                                               \
-                const unsigned ent_ = TILE32 ? s_tile[(COL) * stride + (J)] : (unsigned)s_tile16[(COL) * stride * 2 + (J)]; \
-                const typename EntryT<TILE32>::pkey_t p_ = EntryT<TILE32>::pkey(ent_, (COL));                    \
-                if (p_ > bestp) { bestp = p_; bestj = ((J) << 1) | (int)(ent_ & 1u); }                          \
-            } else {                                                                                            \
-                const int j0_ = max((J) - a.assoc_dj, 0), j1_ = min((J) + a.assoc_dj, nq - 1);                  \
-                for (int jj = j0_; jj <= j1_; ++jj) {                                                           \
-                    unsigned v_;                                                                                \
-                    if (TILE32) v_ = s_tile[(COL) * stride + jj];                                                 \
-                    else v_ = s_tile16[(COL) * stride * 2 + jj];                                                  \
-                    if (v_) {                                                                                   \
-                        if (!TILE32 && v_ == 65535u) /* saturated 16-bit entry: votes from the record */        \
-                            v_ = walk_lookup_votes(a.cands, cand_first, cand_end, c0 + (COL), jj) + 1u;           \
-                        const unsigned long long key_ = walk_key(v_ - 1u, abs(jj - (J)), row_lin0 + (unsigned)((COL) * nq + jj)); \
-                        best = key_ > best ? key_ : best;                                                       \
-                    }                                                                                           \
-                }                                                                                               \
-            }                                                                                                   \
-        } while (0)
+        // ---- fast-path per-hit terms ----
+        const bool fast_batch = !exact_mode && fwd_safe && steps > 0 && (FULLPHI || steps + cols + 2 <= nphi);
+        float gy = 0.f, gx = 0.f, ny = 0.f, nx = 0.f, r2Ak = 1.f, hm_h = 0.f;
+        bool good = false;
+        if (fast_batch) {
+            gy = fk.ntd0A * y;  gx = -(fk.ntd0A * x);                     // A den ~ gy c + gx s + r2Ak
+            ny = -(fk.inv_wq * y);  nx = fk.inv_wq * x;                   // numq  ~ ny c + nx s + d0cq
+            r2Ak = __fmaf_rn(r2, fk.A_f, fk.d0sqA);
+            const float L = fabsf(x) + fabsf(y);
+            const float S = __fmaf_rn(8.0f * fk.d0abs, L, r2 + fk.d0sq);
+            // den >= (r - |d0|)^2; r from the approximate reciprocal square root (2 ulp), shrunk by 2^-20 r
+            const float rr = r2 * rsqrt_approx(r2);
+            const float dr = fmaxf(fabsf(rr - fk.d0abs) - 9.5367432e-7f * rr, 0.0f);
+            const float inv_dr2 = rcp_approx(dr * dr) * 1.000001f;
+            const float arel_h = WALK_U * __fmaf_rn(6.0f * S, inv_dr2, 24.0f);
+            const float elin_h = fk.e_lin * (L + fk.d0abs);
+            const float m_h = __fmaf_rn(fk.inv_A_abs * inv_dr2, elin_h, __fmaf_rn(arel_h, fk.t_max, fk.a0));
+            good = active && (m_h < 0.45f);                               // false for NaN / r ~ |d0| / huge coordinates
+            hm_h = 0.5f - m_h;
+        }
 
-// the same under predicate P; the vote is branch-free: lanes with P false add to their scratch word (J arbitrary)
-#define WALK_AT_IF(P, COL, J)                                                                                   \
-        do {                                                                                                    \
-            if (MODE == WALK_VOTE) {                                                                            \
-                if (TILE32) red_shared((P) ? tile_saddr + (unsigned)(((COL) * stride + (J)) << 2) : trash_saddr, 1u); \
-                else red_shared((P) ? tile_saddr + (unsigned)(((COL) * stride + ((J) >> 1)) << 2) : trash_saddr, \
-                                __funnelshift_l(0u, 1u, (unsigned)(J) << 4));                                   \
-            } else {                                                                                            \
-                if (P) WALK_AT(COL, J);                                                                         \
-            }                                                                                                   \
-        } while (0)
-
-        if (exact_only || (MODE == WALK_ASSIGN && legacy)) {
-            // the D3 sequence at every column of the window (bisecting option / saturated association tiles)
-            for (int t = 0; t < t_cnt; ++t) {
-                const bool in_tile = FULLPHI ? true : (col < cols);
-                const bool mine = FULLPHI ? active : (in_tile && (unsigned)(t - my_b) < (unsigned)my_n);
-                if (mine) {
-                    const float2 cs = s_cs[col];
-                    const int j = d3_exact_bin(x, y, r2, cs.x, cs.y, d.x, d.y, d.z, c.A_f, c.qmin, c.inv_wq, c.nq_f);
-                    if (j >= 0) WALK_AT(col, j);
+        // ---- exact D3 sequence at every column of the window: lanes (or whole batches) without a usable bound ----
+        if (__any_sync(0xffffffffu, active && !good)) {
+            if (active && !good) {
+                int col = i_lo - c0;                     // column relative to the tile, cyclic
+                if (col < 0) col += nphi;
+                for (int t = 0; t < steps; ++t) {
+                    if (col < cols) {
+                        const float4 T = s_pair[col >> 1];
+                        const int j = d3_exact_bin(x, y, r2, (col & 1) ? T.y : T.x, (col & 1) ? T.w : T.z, d.x, d.y, d.z, c.A_f,
+                                                   c.qmin, c.inv_wq, c.nq_f);
+                        if (j >= 0)
+                            walk_apply<MODE, TILE32>(s_tile, stride, nq, col, j, legacy, a.assoc_dj, a.cands, cand_first, cand_end,
+                                                     c0, row_lin0, best);
+                    }
+                    ++col;
+                    if (col == nphi) col = 0;
                 }
-                ++col;
-                if (col == nphi) col = 0;
             }
-        } else {
-            // Fast path.  Lanes whose t~ lies within m of a bin edge (or is NaN) are recorded in `slowmask` and
-            // redone with the exact D3 sequence after each chunk of 32 columns, so the hot loop has no branch.
-            for (int tb0 = 0; tb0 < t_cnt; tb0 += 32) {
-                const int n_it = min(32, t_cnt - tb0);
+        }
+
+        // ---- fast path: the lane's window, two columns at a time ----
+        if (__any_sync(0xffffffffu, good)) {
+            // first column (even, tile-relative) and number of columns of the lane's part of the tile
+            int start, my_n;
+            if (FULLPHI) {
+                start = i_lo & ~1;                       // one column early when i_lo is odd; never past the window + 2
+                my_n = good ? ((steps + 2) & ~1) : 0;
+            } else {
+                int rel = i_lo - c0;
+                if (rel < 0) rel += nphi;
+                int n;
+                if (rel < cols) { start = rel; n = min(steps, cols - rel); }
+                else { const int over = rel + steps - nphi; start = 0; n = over > 0 ? min(over, cols) : 0; }
+                if (!good) { start = 0; n = 0; }
+                const int se = start & ~1;
+                my_n = n > 0 ? n + (start - se) : 0;
+                start = se;
+            }
+            const int np_total = __reduce_max_sync(0xffffffffu, (my_n + 1) >> 1);
+            const unsigned nqg_l = good ? nqg : 0u;      // lanes without work: the range test never passes
+            const f32x2 r2Ak2 = pk2(r2Ak, r2Ak);
+            const f32x2 gy2 = pk2(gy, gy), gx2 = pk2(gx, gx), ny2 = pk2(ny, ny), nx2 = pk2(nx, nx);
+            int col = start;
+            int rem = my_n;                              // columns left in the lane's part (slab tiles)
+            for (int p0 = 0; p0 < np_total; p0 += WALK_CHUNK_PAIRS) {
+                const int np = min(WALK_CHUNK_PAIRS, np_total - p0);
+                if (FULLPHI && col >= nphi) col -= nphi;
+                if (!FULLPHI && rem <= 0) col = 0;       // a finished lane idles at the first pair (table bounds)
                 const int col_chunk = col;
-                // inactive lanes (tail of a batch): range test never passes, bin decision always "sure"
-                const unsigned nq_l = active ? (unsigned)nq : 0u;
-                const float hm0_l = active ? fk.hm0 : 3.0e38f;
-                unsigned slowmask = 0u;                  // bit (n_it - 1 - i): column i of the chunk needs the exact path
-                if (fwd_safe) {
+                const float4* pp = s_pair + (col >> 1);
+                unsigned rowaddr = tile_saddr + (TILE32 ? (unsigned)col * stride4 : (unsigned)(col >> 1) * stride4);
+                int wrap_t = FULLPHI ? ((nphi - col) >> 1) : 0x7fffffff;   // pair of the chunk at which the lane wraps
+                unsigned slowmask = 0u, bit = 1u;
 #pragma unroll 2
-                    for (int t = tb0; t < tb0 + n_it; ++t) {
-                        const bool in_tile = FULLPHI ? true : (col < cols);
-                        const bool mine = FULLPHI ? true : (in_tile && (unsigned)(t - my_b) < (unsigned)my_n);
-                        const float2 cs = s_cs[in_tile ? col : 0];
-                        const float w = __fmaf_rn(y, cs.x, -__fmul_rn(x, cs.y));
-                        const float numq = __fmaf_rn(-w, fk.inv_wq, fk.d0cq);
-                        const float rinv = rcp_approx(__fmaf_rn(fk.ntd0A, w, r2Ak));
-                        const float th = __fmaf_rn(numq, rinv, fk.c0h);                        // t~ - 1/2
-                        const float hm = __fmaf_rn(__fmaf_rn(arel_h, fabsf(numq), elin_h), -fabsf(rinv), hm0_l);
-                        const float yb = __fadd_rn(th, WALK_MAGIC);
-                        const float dlt = __fsub_rn(th, __fsub_rn(yb, WALK_MAGIC));             // (t~ - 1/2) - J
-                        const int jf = __float_as_int(yb) - __float_as_int(WALK_MAGIC);         // J = rint(t~ - 1/2)
-                        const bool sure = fabsf(dlt) < hm;                                      // J <= t_D3 < J + 1
-                        WALK_AT_IF(mine && sure && (unsigned)jf < nq_l, col, jf);
-                        slowmask = (slowmask << 1) | ((mine && !sure) ? 1u : 0u);
-                        ++col;
-                        if (col == nphi) col = 0;
+                for (int t = 0; t < np; ++t) {
+                    if (FULLPHI && t == wrap_t) { rowaddr -= tile_bytes; col -= nphi; }
+                    const float4 T = *pp++;              // {cosA, cosB, sinA, sinB}
+                    const f32x2 C2 = pk2(T.x, T.y), S2 = pk2(T.z, T.w);
+                    const f32x2 g2 = fma2(gx2, S2, fma2(gy2, C2, r2Ak2));
+                    const f32x2 n2 = fma2(nx2, S2, fma2(ny2, C2, d0cq2));
+                    float gA, gB;
+                    upk2(g2, gA, gB);
+                    const f32x2 th2 = fma2(n2, pk2(rcp_approx(gA), rcp_approx(gB)), c0h2);   // t~ - 1/2
+                    const f32x2 yb2 = add2(th2, magic2);
+                    const f32x2 dl2 = sub2(th2, add2(yb2, nmagic2));                          // (t~ - 1/2) - J
+                    float ybA, ybB, dA, dB;
+                    upk2(yb2, ybA, ybB);
+                    upk2(dl2, dA, dB);
+                    const unsigned hA = (unsigned)(__float_as_int(ybA) - (WALK_MAGIC_BITS - 1));   // slot J + 1
+                    const unsigned hB = (unsigned)(__float_as_int(ybB) - (WALK_MAGIC_BITS - 1));
+                    bool inA = hA < nqg_l, inB = hB < nqg_l;                                  // J in [-1, nq]
+                    if (!FULLPHI) { inA = inA && rem > 0; inB = inB && rem > 1; rem -= 2; }
+                    const bool sureA = fabsf(dA) < hm_h, sureB = fabsf(dB) < hm_h;           // J <= t_D3 < J + 1
+                    if (MODE == WALK_VOTE) {
+                        // branch-free vote: lanes that do not vote add to their scratch word
+                        const bool vA = inA && sureA, vB = inB && sureB;
+                        red_shared(vA ? addr_w(rowaddr, hA) : trash_saddr, 1u);
+                        if (TILE32) red_shared(vB ? addr_w(rowaddr + stride4, hB) : trash_saddr, 1u);
+                        else red_shared(vB ? addr_w(rowaddr, hB) : trash_saddr, 65536u);
+                    } else {
+                        if (inA && sureA) {
+                            const unsigned ent = TILE32 ? lds_u32(addr_w(rowaddr, hA)) : lds_u16(addr_w(rowaddr, hA));
+                            const typename EntryT<TILE32>::pkey_t p_ = EntryT<TILE32>::pkey(ent, col);
+                            if (p_ > bestp) { bestp = p_; bestj = ((int)(hA - 1u) << 1) | (int)(ent & 1u); }
+                        }
+                        if (inB && sureB) {
+                            const unsigned ent = TILE32 ? lds_u32(addr_w(rowaddr + stride4, hB)) : lds_u16(addr_w(rowaddr, hB) + 2u);
+                            const typename EntryT<TILE32>::pkey_t p_ = EntryT<TILE32>::pkey(ent, col + 1);
+                            if (p_ > bestp) { bestp = p_; bestj = ((int)(hB - 1u) << 1) | (int)(ent & 1u); }
+                        }
                     }
-                } else {
-#pragma unroll 2
-                    for (int t = tb0; t < tb0 + n_it; ++t) {
-                        const bool in_tile = FULLPHI ? true : (col < cols);
-                        const bool mine = FULLPHI ? true : (in_tile && (unsigned)(t - my_b) < (unsigned)my_n);
-                        const float2 cs = s_cs[in_tile ? col : 0];
-                        const float w = __fmaf_rn(y, cs.x, -__fmul_rn(x, cs.y));
-                        const bool fwd = __fadd_rn(__fmul_rn(x, cs.x), __fmul_rn(y, cs.y)) > 0.0f;   // the exact D3 forward test
-                        const float numq = __fmaf_rn(-w, fk.inv_wq, fk.d0cq);
-                        const float rinv = rcp_approx(__fmaf_rn(fk.ntd0A, w, r2Ak));
-                        const float th = __fmaf_rn(numq, rinv, fk.c0h);
-                        const float hm = __fmaf_rn(__fmaf_rn(arel_h, fabsf(numq), elin_h), -fabsf(rinv), hm0_l);
-                        const float yb = __fadd_rn(th, WALK_MAGIC);
-                        const float dlt = __fsub_rn(th, __fsub_rn(yb, WALK_MAGIC));
-                        const int jf = __float_as_int(yb) - __float_as_int(WALK_MAGIC);
-                        const bool sure = fabsf(dlt) < hm;
-                        WALK_AT_IF(mine && fwd && sure && (unsigned)jf < nq_l, col, jf);
-                        slowmask = (slowmask << 1) | ((mine && fwd && !sure) ? 1u : 0u);
-                        ++col;
-                        if (col == nphi) col = 0;
-                    }
+                    if (inA && !sureA) slowmask |= bit;
+                    if (inB && !sureB) slowmask |= bit << 1;
+                    bit <<= 2;
+                    rowaddr += TILE32 ? 2u * stride4 : stride4;
+                    col += 2;
                 }
-                if (!active) slowmask = 0u;
-                if (__any_sync(0xffffffffu, slowmask != 0u)) {
-                    while (slowmask) {
-                        const int bpos = __ffs(slowmask) - 1;
-                        slowmask &= slowmask - 1u;
-                        int cc = col_chunk + (n_it - 1 - bpos);
-                        if (cc >= nphi) cc -= nphi;
-                        const float2 cs = s_cs[cc];
-                        const int j = d3_exact_bin(x, y, r2, cs.x, cs.y, d.x, d.y, d.z, c.A_f, c.qmin, c.inv_wq, c.nq_f);
-                        if (j >= 0) WALK_AT(cc, j);
+                // uncertain (hit, column) evaluations of the chunk -> the CTA's exact-redo queue
+                while (slowmask) {
+                    const int b = __ffs(slowmask) - 1;
+                    slowmask &= slowmask - 1u;
+                    int cc = col_chunk + b;
+                    if (FULLPHI && cc >= nphi) cc -= nphi;
+                    const int slot = atomicAdd(&s_qn, 1);
+                    if (slot < WALK_QCAP) {
+                        s_q[slot] = make_int2(sidx, cc);
+                    } else {                             // queue full: redo on the spot
+                        const float4 T = s_pair[cc >> 1];
+                        const int j = d3_exact_bin(x, y, r2, (cc & 1) ? T.y : T.x, (cc & 1) ? T.w : T.z, d.x, d.y, d.z, c.A_f,
+                                                   c.qmin, c.inv_wq, c.nq_f);
+                        if (j >= 0)
+                            walk_apply<MODE, TILE32>(s_tile, stride, nq, cc, j, legacy, a.assoc_dj, a.cands, cand_first, cand_end,
+                                                     c0, row_lin0, best);
                     }
                 }
             }
         }
-#undef WALK_AT_IF
-#undef WALK_AT
         if (MODE == WALK_ASSIGN) {
-            if (!legacy) {
-                const unsigned eh = EntryT<TILE32>::ent_hi(bestp);      // entry >> 1: votes + 1 above (15 - |dj|)
-                if (eh) {
-                    const int bcol = EntryT<TILE32>::col_of(bestp);
-                    const int adj = 15 - (int)(eh & 15u);
-                    const int jc = (bestj >> 1) + ((bestj & 1) ? -adj : adj);
-                    best = walk_key((eh >> 4) - 1u, adj, row_lin0 + (unsigned)(bcol * nq + jc));
-                }
+            const unsigned eh = EntryT<TILE32>::ent_hi(bestp);          // entry >> 1: votes + 1 above (15 - |dj|)
+            if (eh >> 4) {
+                const int bcol = EntryT<TILE32>::col_of(bestp);
+                const int adj = 15 - (int)(eh & 15u);
+                const int jc = (bestj >> 1) + ((bestj & 1) ? -adj : adj);
+                const unsigned long long key = walk_key((eh >> 4) - 1u, adj, row_lin0 + (unsigned)(bcol * nq + jc));
+                best = key > best ? key : best;
             }
             if (best) atomicMax(a.best_key + __float_as_int(hv.w), best);
+        }
+    }
+    __syncthreads();
+
+    // ---- exact redo of the queued (hit, column) evaluations, by the whole CTA ----
+    {
+        const int nqd = min(s_qn, WALK_QCAP);
+        for (int q = tid; q < nqd; q += WALK_THREADS) {
+            const int2 en = s_q[q];
+            const float4 hv = __ldg(a.staged + en.x);
+            const float4 T = s_pair[en.y >> 1];
+            const int j = d3_exact_bin(hv.x, hv.y, d3_r2(hv.x, hv.y), (en.y & 1) ? T.y : T.x, (en.y & 1) ? T.w : T.z, d.x, d.y, d.z,
+                                       c.A_f, c.qmin, c.inv_wq, c.nq_f);
+            if (j >= 0) {
+                unsigned long long best = 0ull;
+                walk_apply<MODE, TILE32>(s_tile, stride, nq, en.y, j, legacy, a.assoc_dj, a.cands, cand_first, cand_end, c0,
+                                         row_lin0, best);
+                if (MODE == WALK_ASSIGN && best) atomicMax(a.best_key + __float_as_int(hv.w), best);
+            }
         }
     }
     if (MODE == WALK_ASSIGN) return;
     __syncthreads();
 
-    // ---- flush: the tile is written to the global accumulator exactly once (A3) ----
+    // ---- flush: the tile is written to the global accumulator exactly once (A3); guard slots are dropped ----
     const size_t row0 = ((size_t)e * c.n_d0 + k) * (size_t)nphi + c0;      // first global row of the tile
     if (TILE32) {
         int* g = reinterpret_cast<int*>(a.accum) + row0 * nq;
         for (int ci = warp; ci < cols; ci += WALK_WARPS)
-            for (int j = lane; j < nq; j += 32) g[(size_t)ci * nq + j] = (int)s_tile[ci * stride + j];
+            for (int j = lane; j < nq; j += 32) g[(size_t)ci * nq + j] = (int)s_tile[ci * stride + j + 1];
     } else if (OUT16) {
-        if ((nq & 1) == 0) {
+        if ((nq & 1) == 0) {                             // two bins per 32-bit store
             uint32_t* g = reinterpret_cast<uint32_t*>(reinterpret_cast<unsigned short*>(a.accum) + row0 * nq);
             const int rw = nq >> 1;
-            for (int ci = warp; ci < cols; ci += WALK_WARPS)
-                for (int jw = lane; jw < rw; jw += 32) g[(size_t)ci * rw + jw] = s_tile[ci * stride + jw];
+            for (int ci = warp; ci < cols; ci += WALK_WARPS) {
+                const uint32_t* trow = s_tile + (ci >> 1) * stride + 1;
+                const unsigned sel = (ci & 1) ? 0x7632u : 0x5410u;
+                for (int jw = lane; jw < rw; jw += 32)
+                    g[(size_t)ci * rw + jw] = __byte_perm(trow[2 * jw], trow[2 * jw + 1], sel);
+            }
         } else {
             unsigned short* g = reinterpret_cast<unsigned short*>(a.accum) + row0 * nq;
             for (int ci = warp; ci < cols; ci += WALK_WARPS)
                 for (int j = lane; j < nq; j += 32)
-                    g[(size_t)ci * nq + j] = (unsigned short)((s_tile[ci * stride + (j >> 1)] >> (16 * (j & 1))) & 0xffffu);
+                    g[(size_t)ci * nq + j] = (unsigned short)((s_tile[(ci >> 1) * stride + j + 1] >> (16 * (ci & 1))) & 0xffffu);
         }
     } else {
         int* g = reinterpret_cast<int*>(a.accum) + row0 * nq;
-        if ((nq & 1) == 0) {
-            const int rw = nq >> 1;
-            for (int ci = warp; ci < cols; ci += WALK_WARPS)
-                for (int jw = lane; jw < rw; jw += 32) {
-                    const uint32_t v = s_tile[ci * stride + jw];
-                    *reinterpret_cast<int2*>(g + (size_t)ci * nq + 2 * jw) = make_int2((int)(v & 0xffffu), (int)(v >> 16));
-                }
-        } else {
-            for (int ci = warp; ci < cols; ci += WALK_WARPS)
-                for (int j = lane; j < nq; j += 32)
-                    g[(size_t)ci * nq + j] = (int)((s_tile[ci * stride + (j >> 1)] >> (16 * (j & 1))) & 0xffffu);
-        }
+        for (int ci = warp; ci < cols; ci += WALK_WARPS)
+            for (int j = lane; j < nq; j += 32)
+                g[(size_t)ci * nq + j] = (int)((s_tile[(ci >> 1) * stride + j + 1] >> (16 * (ci & 1))) & 0xffffu);
     }
 }
 
 // tile shape of a call: as many columns as fit the shared-memory budget, then split further until the grid
-// fills the GPU
+// fills the GPU; slab widths are even (column pairs)
 inline void walk_shape(const hough_plan* p, int n_events, int& n_slabs, int& slab_cols) {
     const int nphi = p->c.n_phi;
     n_slabs = (nphi + p->tile_max_cols - 1) / p->tile_max_cols;
     const long long want = 3LL * p->sm_count;
     while ((long long)n_slabs * p->c.n_d0 * n_events < want && (nphi + n_slabs - 1) / n_slabs > 32) n_slabs *= 2;
     slab_cols = (nphi + n_slabs - 1) / n_slabs;
+    slab_cols += slab_cols & 1;
     n_slabs = (nphi + slab_cols - 1) / slab_cols;
 }
 
 template <int MODE, bool TILE32, bool OUT16, bool FULLPHI>
 int walk_launch(hough_plan* p, int n_events, WalkArgs a, cudaStream_t st) {
-    const size_t smem = walk_smem_bytes(a.slab_cols, a.stride, p->c.n_class);
+    const size_t smem = walk_smem_bytes(a.slab_cols, a.stride, TILE32, p->c.n_class);
     auto kern = walk_kernel<MODE, TILE32, OUT16, FULLPHI>;
     static size_t smem_configured = 0;              // per instantiation; raised only when a call needs more
     if (smem > smem_configured) {

@@ -118,11 +118,12 @@ int hough_build_windows(const hough_binning& b, float bz, int n_layers, const fl
             lo = (float)lo_c;
             if ((double)lo > lo_c) lo = std::nextafterf(lo, -1.0e30f);
             st = steps + 1;                           // +1: the float rounding of u + lo_off on the device
-            // Every column of the window is within 89 degrees of the hit's azimuth and the class excludes r = 0:
+            // Every column of the window, one before it and two after it (the walk visits even/odd column pairs) is
+            // within 89 degrees of the hit's azimuth and the class excludes r = 0:
             // f = r cos(phi0 - phi) >= 0.017 r exceeds its fp32 rounding error (2^-23 r) by far, so the D3 forward
             // test passes at every column of the window and the walk's fast path may skip it.
             const double lim = 89.0 / 360.0 * (double)nphi;
-            if (c > 0 && ra > 0.0 && (double)lo - 1.0 >= -lim && (double)lo + (double)st + 1.0 <= lim)
+            if (c > 0 && ra > 0.0 && (double)lo - 2.0 >= -lim && (double)lo + (double)st + 3.0 <= lim)
                 out.fwd_safe[(size_t)c * nd + k] = 1;
         }
     }
