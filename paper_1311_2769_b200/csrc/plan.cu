@@ -145,15 +145,22 @@ extern "C" int hough_plan_create(const hough_binning* b, const hough_geometry* g
     // hits per call (a hit casts at most one vote per (phi0, d0) column, D3)
     p->tile32 = (b->accum_dtype == HOUGH_ACC_I32 && max_hits > 65535) ? 1 : 0;
     {
-        // walk.cuh "Tile layout": a row (32-bit bins) or a row of column PAIRS (16-bit bins) has nq + 2 words
-        const long long stride = (long long)walk_row_stride(b->n_qpt);
-        p->tile_stride_words = (int32_t)stride;
-        const long long col_bytes = (p->tile32 ? stride * 4 : stride * 2) + 8;     // tile + column-pair table
-        long long cols = (68LL * 1024) / col_bytes;
-        if (cols < 8) cols = (200LL * 1024) / col_bytes;                  // wide rows: one big tile per SM
-        if (cols > b->n_phi) cols = b->n_phi;
-        cols &= ~1LL;                                                     // column pairs
-        p->tile_max_cols = (int32_t)cols;                                 // 0: no tiled path (fullscan fallback)
+        // walk.cuh "Tile layout": a row (32-bit bins) or a row of column PAIRS (16-bit bins) has `stride` words.
+        // Largest even column count whose whole shared-memory block lets 3 CTAs share an SM (228 KB, 1 KB reserved per
+        // CTA); rows too wide for that get one big tile per SM.
+        const int stride = walk_row_stride(b->n_qpt);
+        p->tile_stride_words = stride;
+        auto fit = [&](size_t budget) {
+            int lo = 0, hi = b->n_phi / 2;                                // pairs of columns
+            while (lo < hi) {
+                const int mid = (lo + hi + 1) / 2;
+                if (walk_smem_bytes(2 * mid, stride, p->tile32 != 0, win.n_class) <= budget) lo = mid; else hi = mid - 1;
+            }
+            return 2 * lo;
+        };
+        int cols = fit((size_t)(233472 / 3 - 1024 - 64));
+        if (cols < 8) cols = fit((size_t)(200 * 1024));
+        p->tile_max_cols = cols;                                          // 0: no tiled path (fullscan fallback)
     }
 
     p->peak_blocks_per_event = (int32_t)((bins + PEAK_BLOCK_BINS - 1) / PEAK_BLOCK_BINS);

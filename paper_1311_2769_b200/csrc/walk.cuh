@@ -8,8 +8,8 @@
 //                 of a hit needs ONE probe; the best D8 key per (hit, tile) is published with one atomicMax.
 //
 // Tile layout.  A row has nq + 2 slots h = J + 1: the q/pT bins J = 0..nq-1 and one
-// GUARD slot at each end (J = -1 and J = nq) that absorbs the fast path's "one bin outside" results and is never
-// flushed.  Packed tiles (16-bit bins) store the two columns of an even/odd column PAIR in one 32-bit word per
+// GUARD slot at each end (J = -1 and J = nq) that absorbs the fast path's "one bin outside" results, followed by
+// WALK_DUMP dump slots for everything further out; guard and dump slots are never flushed.  Packed tiles (16-bit bins) store the two columns of an even/odd column PAIR in one 32-bit word per
 // slot (low half = even column, high half = odd column), so the increment is the constant 1 or 65536 and the
 // address is pair_row + 4 h.  32-bit tiles store one word per (column, slot).
 //
@@ -26,6 +26,8 @@
 // useless (r ~ |d0|, non-finite coordinates), classes whose window is not certainly forward, and the plan option
 // "exact_walk" take the exact sequence at every column.  The result is therefore the D3 bin in every case.
 #pragma once
+
+#include <type_traits>
 
 #include "common.cuh"
 
@@ -51,7 +53,8 @@ struct WalkArgs {
     unsigned long long* best_key;    // [n_hits] by original hit index
 };
 
-__host__ __device__ inline int walk_row_stride(int nq) { return (nq + 2) | 1; }
+constexpr int WALK_DUMP = 4;                     // dump slots per row: where results outside [-1, nq] are added (by lane & 3)
+__host__ __device__ inline int walk_row_stride(int nq) { return (nq + 2 + WALK_DUMP) | 1; }
 
 __host__ __device__ inline size_t walk_tile_words(int cols, int stride, bool tile32) {
     return tile32 ? (size_t)cols * stride : (size_t)((cols + 1) / 2) * stride;
@@ -185,6 +188,25 @@ __device__ __forceinline__ FastK make_fastk(const HoughConsts& c, float4 d) {
     return k;
 }
 
+// Per-hit terms of the fast path.  Used by the hot loop (packed) and by the redo of queued pairs, which must
+// reproduce the hot loop's slot bit for bit: explicit intrinsics, no contraction, one definition.
+struct FastHit { float gy, gx, ny, nx, r2Ak; };
+__device__ __forceinline__ FastHit make_fasthit(const FastK& fk, float x, float y, float r2) {
+    FastHit h;
+    h.gy = __fmul_rn(fk.ntd0A, y);  h.gx = -__fmul_rn(fk.ntd0A, x);       // A den ~ gy c + gx s + r2Ak
+    h.ny = -__fmul_rn(fk.inv_wq, y);  h.nx = __fmul_rn(fk.inv_wq, x);      // numq  ~ ny c + nx s + d0cq
+    h.r2Ak = __fmaf_rn(r2, fk.A_f, fk.d0sqA);
+    return h;
+}
+// slot h = J + 1 of one column, scalar form of the packed sequence of the hot loop (same operations, same rounding)
+__device__ __forceinline__ unsigned fast_slot(const FastK& fk, const FastHit& h, float cs_c, float cs_s) {
+    const float g = __fmaf_rn(h.gx, cs_s, __fmaf_rn(h.gy, cs_c, h.r2Ak));
+    const float n = __fmaf_rn(h.nx, cs_s, __fmaf_rn(h.ny, cs_c, fk.d0cq));
+    const float th = __fmaf_rn(n, rcp_approx(g), fk.c0h);
+    const float yb = __fadd_rn(th, WALK_MAGIC);
+    return (unsigned)(__float_as_int(yb) - (WALK_MAGIC_BITS - 1));
+}
+
 // Entry of an association tile: (min(votes, VCAP) + 1) << 5 | p,  p = (15 - |dj|) * 2 + (dj < 0), dj = j_cand - j_bin.
 // Integer order of entries == D8 order among the candidates of one row that can serve bin j_bin.
 template <bool TILE32> struct EntryT {               // 16-bit entries: 11 bits of votes + 1
@@ -209,6 +231,12 @@ template <bool TILE32>
 __device__ __forceinline__ void tile_vote(uint32_t* s_tile, int stride, int col, int J) {
     if (TILE32) atomicAdd(s_tile + col * stride + J + 1, 1u);
     else atomicAdd(s_tile + (col >> 1) * stride + J + 1, 1u << (16 * (col & 1)));
+}
+// +1 / -1 at slot `slot` (guard slots included) of tile column col
+template <bool TILE32>
+__device__ __forceinline__ void tile_add_slot(uint32_t* s_tile, int stride, int col, unsigned slot, int delta) {
+    if (TILE32) atomicAdd(s_tile + col * stride + slot, (unsigned)delta);
+    else atomicAdd(s_tile + (col >> 1) * stride + slot, (unsigned)delta << (16 * (col & 1)));
 }
 template <bool TILE32>
 __device__ __forceinline__ unsigned tile_entry(const uint32_t* s_tile, int stride, int col, int J) {
@@ -244,6 +272,37 @@ __device__ __forceinline__ void walk_apply(uint32_t* s_tile, int stride, int nq,
             }
         }
     }
+}
+
+// Redo of one flagged column pair {staged hit, pair column | dump slot << 28 | live flags << 30} with the exact D3
+// sequence.
+// Vote: the hot loop has already cast the pair's fast votes at slots min(fast_slot, nq + 1); they are taken back
+// (integer adds commute, also across a transient 16-bit wrap) and the exact votes are cast.  Association: the
+// hot loop skipped the pair; its exact positions are probed and published here.
+template <int MODE, bool TILE32>
+__device__ __noinline__ void walk_redo_pair(const HoughConsts& c, const FastK& fk, float4 d, const WalkArgs& a, int2 entry,
+                                            uint32_t* s_tile, const float4* s_pair, int stride, bool legacy, int cand_first,
+                                            int cand_end, int c0, unsigned row_lin0) {
+    const float4 hv = __ldg(a.staged + entry.x);
+    const int cc = entry.y & 0x0fffffff;
+    const unsigned live = (unsigned)entry.y >> 30;
+    const unsigned hmax = (unsigned)c.n_qpt + 2u + (((unsigned)entry.y >> 28) & 3u);    // the lane's dump slot
+    const float r2 = d3_r2(hv.x, hv.y);
+    const FastHit fh = make_fasthit(fk, hv.x, hv.y, r2);
+    const float4 T = s_pair[cc >> 1];
+    unsigned long long best = 0ull;
+#pragma unroll
+    for (int w = 0; w < 2; ++w) {
+        if (!((live >> w) & 1u)) continue;
+        const float cs_c = w ? T.y : T.x, cs_s = w ? T.w : T.z;
+        if (MODE == WALK_VOTE)
+            tile_add_slot<TILE32>(s_tile, stride, cc + w, min(fast_slot(fk, fh, cs_c, cs_s), hmax), -1);
+        const int j = d3_exact_bin(hv.x, hv.y, r2, cs_c, cs_s, d.x, d.y, d.z, c.A_f, c.qmin, c.inv_wq, c.nq_f);
+        if (j >= 0)
+            walk_apply<MODE, TILE32>(s_tile, stride, c.n_qpt, cc + w, j, legacy, a.assoc_dj, a.cands, cand_first, cand_end, c0,
+                                     row_lin0, best);
+    }
+    if (MODE == WALK_ASSIGN && best) atomicMax(a.best_key + __float_as_int(hv.w), best);
 }
 
 template <int MODE, bool TILE32, bool OUT16, bool FULLPHI>
@@ -300,6 +359,8 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
             s_pair[p] = make_float4(A.x, B.x, A.y, B.y);
         }
         if (tid == 0) s_qn = 0;
+        if (tid < 32)                                    // scratch words: read (as empty entries) by the association probes
+            reinterpret_cast<uint32_t*>(smem_raw + walk_smem_bytes(slab_cols, stride, TILE32, nc) - 128)[tid] = 0u;
     }
     const int ev_begin = __ldg(a.off + e);
     const int32_t* ks = a.key_start + (size_t)e * (c.n_keys + 1);
@@ -443,9 +504,8 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
         float gy = 0.f, gx = 0.f, ny = 0.f, nx = 0.f, r2Ak = 1.f, hm_h = 0.f;
         bool good = false;
         if (fast_batch) {
-            gy = fk.ntd0A * y;  gx = -(fk.ntd0A * x);                     // A den ~ gy c + gx s + r2Ak
-            ny = -(fk.inv_wq * y);  nx = fk.inv_wq * x;                   // numq  ~ ny c + nx s + d0cq
-            r2Ak = __fmaf_rn(r2, fk.A_f, fk.d0sqA);
+            const FastHit fh = make_fasthit(fk, x, y, r2);
+            gy = fh.gy; gx = fh.gx; ny = fh.ny; nx = fh.nx; r2Ak = fh.r2Ak;
             const float L = fabsf(x) + fabsf(y);
             const float S = __fmaf_rn(8.0f * fk.d0abs, L, r2 + fk.d0sq);
             // den >= (r - |d0|)^2; r from the approximate reciprocal square root (2 ulp), shrunk by 2^-20 r
@@ -485,6 +545,7 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
             int start, my_n;
             if (FULLPHI) {
                 start = i_lo & ~1;                       // one column early when i_lo is odd; never past the window + 2
+                if (!good) start = (2 * lane) % nphi;    // lanes without work walk rows of their own (no same-word adds)
                 my_n = good ? ((steps + 2) & ~1) : 0;
             } else {
                 int rel = i_lo - c0;
@@ -498,7 +559,9 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
                 start = se;
             }
             const int np_total = __reduce_max_sync(0xffffffffu, (my_n + 1) >> 1);
-            const unsigned nqg_l = good ? nqg : 0u;      // lanes without work: the range test never passes
+            // lanes without work: every evaluation lands in guard slot 0 and none is ever "uncertain"
+            const unsigned hmax_l = good ? (unsigned)nq + 2u + (unsigned)(lane & (WALK_DUMP - 1)) : 0u;
+            const float hm_l = good ? hm_h : __int_as_float(0x7f800000);
             const f32x2 r2Ak2 = pk2(r2Ak, r2Ak);
             const f32x2 gy2 = pk2(gy, gy), gx2 = pk2(gx, gx), ny2 = pk2(ny, ny), nx2 = pk2(nx, nx);
             int col = start;
@@ -507,72 +570,81 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
                 const int np = min(WALK_CHUNK_PAIRS, np_total - p0);
                 if (FULLPHI && col >= nphi) col -= nphi;
                 if (!FULLPHI && rem <= 0) col = 0;       // a finished lane idles at the first pair (table bounds)
-                const int col_chunk = col;
+                const int col_chunk = col, rem_chunk = rem;
                 const float4* pp = s_pair + (col >> 1);
                 unsigned rowaddr = tile_saddr + (TILE32 ? (unsigned)col * stride4 : (unsigned)(col >> 1) * stride4);
-                int wrap_t = FULLPHI ? ((nphi - col) >> 1) : 0x7fffffff;   // pair of the chunk at which the lane wraps
-                unsigned slowmask = 0u, bit = 1u;
+                const int wrap_t = FULLPHI ? ((nphi - col) >> 1) : 0x7fffffff;   // pair of the chunk at which the lane wraps
+                int colp = col;                          // association: running tile column of the pair
+                unsigned slowmask = 0u;                  // bit (np - 1 - t): pair t of the chunk is uncertain
+                // One chunk of column pairs; WRAP: some lane of the warp passes column n_phi - 1 inside the chunk.
+                // The vote is unconditional: slot min(h, nq + 1) of the column's row (results outside [-1, nq] land in
+                // a guard slot).  A pair with an uncertain column is flagged; the redo takes the pair's two fast votes
+                // back (fast_slot reproduces them) and casts the exact ones.
+                auto run_chunk = [&](auto wrap_c) {
+                    constexpr bool WRAP = decltype(wrap_c)::value;
 #pragma unroll 2
-                for (int t = 0; t < np; ++t) {
-                    if (FULLPHI && t == wrap_t) { rowaddr -= tile_bytes; col -= nphi; }
-                    const float4 T = *pp++;              // {cosA, cosB, sinA, sinB}
-                    const f32x2 C2 = pk2(T.x, T.y), S2 = pk2(T.z, T.w);
-                    const f32x2 g2 = fma2(gx2, S2, fma2(gy2, C2, r2Ak2));
-                    const f32x2 n2 = fma2(nx2, S2, fma2(ny2, C2, d0cq2));
-                    float gA, gB;
-                    upk2(g2, gA, gB);
-                    const f32x2 th2 = fma2(n2, pk2(rcp_approx(gA), rcp_approx(gB)), c0h2);   // t~ - 1/2
-                    const f32x2 yb2 = add2(th2, magic2);
-                    const f32x2 dl2 = sub2(th2, add2(yb2, nmagic2));                          // (t~ - 1/2) - J
-                    float ybA, ybB, dA, dB;
-                    upk2(yb2, ybA, ybB);
-                    upk2(dl2, dA, dB);
-                    const unsigned hA = (unsigned)(__float_as_int(ybA) - (WALK_MAGIC_BITS - 1));   // slot J + 1
-                    const unsigned hB = (unsigned)(__float_as_int(ybB) - (WALK_MAGIC_BITS - 1));
-                    bool inA = hA < nqg_l, inB = hB < nqg_l;                                  // J in [-1, nq]
-                    if (!FULLPHI) { inA = inA && rem > 0; inB = inB && rem > 1; rem -= 2; }
-                    const bool sureA = fabsf(dA) < hm_h, sureB = fabsf(dB) < hm_h;           // J <= t_D3 < J + 1
-                    if (MODE == WALK_VOTE) {
-                        // branch-free vote: lanes that do not vote add to their scratch word
-                        const bool vA = inA && sureA, vB = inB && sureB;
-                        red_shared(vA ? addr_w(rowaddr, hA) : trash_saddr, 1u);
-                        if (TILE32) red_shared(vB ? addr_w(rowaddr + stride4, hB) : trash_saddr, 1u);
-                        else red_shared(vB ? addr_w(rowaddr, hB) : trash_saddr, 65536u);
-                    } else {
-                        if (inA && sureA) {
-                            const unsigned ent = TILE32 ? lds_u32(addr_w(rowaddr, hA)) : lds_u16(addr_w(rowaddr, hA));
-                            const typename EntryT<TILE32>::pkey_t p_ = EntryT<TILE32>::pkey(ent, col);
-                            if (p_ > bestp) { bestp = p_; bestj = ((int)(hA - 1u) << 1) | (int)(ent & 1u); }
+                    for (int t = 0; t < np; ++t) {
+                        if (WRAP && t == wrap_t) { rowaddr -= tile_bytes; colp -= nphi; }
+                        const float4 T = *pp++;          // {cosA, cosB, sinA, sinB}
+                        const f32x2 C2 = pk2(T.x, T.y), S2 = pk2(T.z, T.w);
+                        const f32x2 g2 = fma2(gx2, S2, fma2(gy2, C2, r2Ak2));
+                        const f32x2 n2 = fma2(nx2, S2, fma2(ny2, C2, d0cq2));
+                        float gA, gB;
+                        upk2(g2, gA, gB);
+                        const f32x2 th2 = fma2(n2, pk2(rcp_approx(gA), rcp_approx(gB)), c0h2);   // t~ - 1/2
+                        const f32x2 yb2 = add2(th2, magic2);
+                        const f32x2 dl2 = sub2(th2, add2(yb2, nmagic2));                          // (t~ - 1/2) - J
+                        float ybA, ybB, dA, dB;
+                        upk2(yb2, ybA, ybB);
+                        upk2(dl2, dA, dB);
+                        unsigned hA = min((unsigned)(__float_as_int(ybA) - (WALK_MAGIC_BITS - 1)), hmax_l);   // slot J + 1
+                        unsigned hB = min((unsigned)(__float_as_int(ybB) - (WALK_MAGIC_BITS - 1)), hmax_l);
+                        // uncertain: t~ within m of a bin edge, J <= t_D3 < J + 1 not proven (NaN never compares true)
+                        bool unsA = fabsf(dA) >= hm_l, unsB = fabsf(dB) >= hm_l;
+                        unsigned adA = addr_w(rowaddr, hA), adB = addr_w(TILE32 ? rowaddr + stride4 : rowaddr, hB);
+                        if (!FULLPHI) {                  // slab tiles: the lane's own part of the tile only
+                            const bool liveA = rem > 0, liveB = rem > 1;
+                            adA = liveA ? adA : trash_saddr;  adB = liveB ? adB : trash_saddr;   // rows past the tile: scratch word
+                            unsA = unsA && liveA;  unsB = unsB && liveB;
+                            rem -= 2;
                         }
-                        if (inB && sureB) {
-                            const unsigned ent = TILE32 ? lds_u32(addr_w(rowaddr + stride4, hB)) : lds_u16(addr_w(rowaddr, hB) + 2u);
-                            const typename EntryT<TILE32>::pkey_t p_ = EntryT<TILE32>::pkey(ent, col + 1);
-                            if (p_ > bestp) { bestp = p_; bestj = ((int)(hB - 1u) << 1) | (int)(ent & 1u); }
+                        const bool uns = unsA || unsB;
+                        if (MODE == WALK_VOTE) {
+                            red_shared(adA, 1u);
+                            red_shared(adB, TILE32 ? 1u : 65536u);
+                        } else {
+                            const unsigned entA = TILE32 ? lds_u32(adA) : lds_u16(adA);
+                            const unsigned entB = TILE32 ? lds_u32(adB) : lds_u16(adB + 2u);
+                            const typename EntryT<TILE32>::pkey_t pA = EntryT<TILE32>::pkey(entA, colp);
+                            const typename EntryT<TILE32>::pkey_t pB = EntryT<TILE32>::pkey(entB, colp + 1);
+                            if (!uns) {                  // flagged pairs are probed by the redo
+                                if (pA > bestp) { bestp = pA; bestj = ((int)(hA - 1u) << 1) | (int)(entA & 1u); }
+                                if (pB > bestp) { bestp = pB; bestj = ((int)(hB - 1u) << 1) | (int)(entB & 1u); }
+                            }
+                            colp += 2;
                         }
+                        slowmask = slowmask * 2u + (uns ? 1u : 0u);
+                        rowaddr += TILE32 ? 2u * stride4 : stride4;
                     }
-                    if (inA && !sureA) slowmask |= bit;
-                    if (inB && !sureB) slowmask |= bit << 1;
-                    bit <<= 2;
-                    rowaddr += TILE32 ? 2u * stride4 : stride4;
-                    col += 2;
-                }
-                // uncertain (hit, column) evaluations of the chunk -> the CTA's exact-redo queue
+                };
+                if (FULLPHI && __any_sync(0xffffffffu, wrap_t < np)) run_chunk(std::true_type{});
+                else run_chunk(std::false_type{});
+                col += 2 * np;                           // FULLPHI: reduced modulo n_phi at the top of the next chunk
+                // uncertain pairs of the chunk -> the CTA's exact-redo queue {staged hit, pair column | live flags << 30}
                 while (slowmask) {
                     const int b = __ffs(slowmask) - 1;
                     slowmask &= slowmask - 1u;
-                    int cc = col_chunk + b;
+                    const int t = np - 1 - b;
+                    int cc = col_chunk + 2 * t;
                     if (FULLPHI && cc >= nphi) cc -= nphi;
+                    unsigned live = 3u;
+                    if (!FULLPHI) live = (rem_chunk - 2 * t > 0 ? 1u : 0u) | (rem_chunk - 2 * t > 1 ? 2u : 0u);
+                    const int2 entry = make_int2(sidx, (int)((unsigned)cc | ((unsigned)(lane & (WALK_DUMP - 1)) << 28) | (live << 30)));
                     const int slot = atomicAdd(&s_qn, 1);
-                    if (slot < WALK_QCAP) {
-                        s_q[slot] = make_int2(sidx, cc);
-                    } else {                             // queue full: redo on the spot
-                        const float4 T = s_pair[cc >> 1];
-                        const int j = d3_exact_bin(x, y, r2, (cc & 1) ? T.y : T.x, (cc & 1) ? T.w : T.z, d.x, d.y, d.z, c.A_f,
-                                                   c.qmin, c.inv_wq, c.nq_f);
-                        if (j >= 0)
-                            walk_apply<MODE, TILE32>(s_tile, stride, nq, cc, j, legacy, a.assoc_dj, a.cands, cand_first, cand_end,
-                                                     c0, row_lin0, best);
-                    }
+                    if (slot < WALK_QCAP) s_q[slot] = entry;
+                    else                                 // queue full: redo on the spot
+                        walk_redo_pair<MODE, TILE32>(c, fk, d, a, entry, s_tile, s_pair, stride, legacy, cand_first, cand_end, c0,
+                                                     row_lin0);
                 }
             }
         }
@@ -590,22 +662,11 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
     }
     __syncthreads();
 
-    // ---- exact redo of the queued (hit, column) evaluations, by the whole CTA ----
+    // ---- exact redo of the queued pairs, by the whole CTA ----
     {
         const int nqd = min(s_qn, WALK_QCAP);
-        for (int q = tid; q < nqd; q += WALK_THREADS) {
-            const int2 en = s_q[q];
-            const float4 hv = __ldg(a.staged + en.x);
-            const float4 T = s_pair[en.y >> 1];
-            const int j = d3_exact_bin(hv.x, hv.y, d3_r2(hv.x, hv.y), (en.y & 1) ? T.y : T.x, (en.y & 1) ? T.w : T.z, d.x, d.y, d.z,
-                                       c.A_f, c.qmin, c.inv_wq, c.nq_f);
-            if (j >= 0) {
-                unsigned long long best = 0ull;
-                walk_apply<MODE, TILE32>(s_tile, stride, nq, en.y, j, legacy, a.assoc_dj, a.cands, cand_first, cand_end, c0,
-                                         row_lin0, best);
-                if (MODE == WALK_ASSIGN && best) atomicMax(a.best_key + __float_as_int(hv.w), best);
-            }
-        }
+        for (int q = tid; q < nqd; q += WALK_THREADS)
+            walk_redo_pair<MODE, TILE32>(c, fk, d, a, s_q[q], s_tile, s_pair, stride, legacy, cand_first, cand_end, c0, row_lin0);
     }
     if (MODE == WALK_ASSIGN) return;
     __syncthreads();
