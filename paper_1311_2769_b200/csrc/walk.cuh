@@ -36,7 +36,7 @@ constexpr int WALK_ASSIGN = 1;
 constexpr int WALK_THREADS = 256;
 constexpr int WALK_WARPS = WALK_THREADS / 32;
 constexpr int WALK_CHUNK_PAIRS = 16;             // column pairs per chunk: 32 columns = the bits of the redo mask
-constexpr int WALK_QCAP = 192;                   // entries of the exact-redo queue (overflow: redone on the spot)
+constexpr int WALK_WQ_CAP = 48;                  // entries of a warp's exact-redo queue (drained by the whole warp)
 
 struct WalkArgs {
     const float4* staged;            // [n_hits] staged hits (stage.cu)
@@ -63,10 +63,9 @@ __host__ __device__ inline size_t walk_tile_words(int cols, int stride, bool til
 __host__ __device__ inline size_t walk_smem_bytes(int cols, int stride, bool tile32, int n_class) {
     size_t b = (walk_tile_words(cols, stride, tile32) * 4 + 15) & ~(size_t)15;
     b += (size_t)(cols / 2 + WALK_CHUNK_PAIRS + 1) * 16;               // column pairs {cosA, cosB, sinA, sinB}
-    b += (size_t)WALK_QCAP * 8;                                         // exact-redo queue
-    b += (size_t)n_class * 8;                                           // lo_off, steps
-    b += (size_t)n_class * 2 * 8 + ((size_t)n_class * 2 + 1) * 4;       // segments
-    b = (b + 15) & ~(size_t)15;
+    b += (size_t)n_class * 16;                                          // per class: window, error bound
+    b += ((size_t)n_class * 2 + 1) * 16;                                // segments
+    b += (size_t)WALK_WARPS * WALK_WQ_CAP * 4;                          // redo queues
     return b + 128;                                                     // one scratch word per lane (walk_kernel: trash_saddr)
 }
 
@@ -274,41 +273,63 @@ __device__ __forceinline__ void walk_apply(uint32_t* s_tile, int stride, int nq,
     }
 }
 
-// Redo of one flagged column pair {staged hit, pair column | dump slot << 28 | live flags << 30} with the exact D3
-// sequence.
-// Vote: the hot loop has already cast the pair's fast votes at slots min(fast_slot, nq + 1); they are taken back
-// (integer adds commute, also across a transient 16-bit wrap) and the exact votes are cast.  Association: the
+// Redo of one flagged column pair with the exact D3 sequence.  `sidx` = staged hit, `cc` = tile column of the
+// pair, `dump` = the lane's dump slot, `live` = which columns of the pair belonged to the lane's part of the tile.
+// Vote: the hot loop has already cast the pair's fast votes at slots min(fast_slot, nq + 2 + dump); they are taken
+// back (integer adds commute, also across a transient 16-bit wrap) and the exact votes are cast.  Association: the
 // hot loop skipped the pair; its exact positions are probed and published here.
+struct WalkTile {
+    uint32_t* s_tile;
+    const float4* s_pair;
+    int stride, c0, cand_first, cand_end;
+    unsigned row_lin0;
+    bool legacy;
+};
+
 template <int MODE, bool TILE32>
-__device__ __noinline__ void walk_redo_pair(const HoughConsts& c, const FastK& fk, float4 d, const WalkArgs& a, int2 entry,
-                                            uint32_t* s_tile, const float4* s_pair, int stride, bool legacy, int cand_first,
-                                            int cand_end, int c0, unsigned row_lin0) {
-    const float4 hv = __ldg(a.staged + entry.x);
-    const int cc = entry.y & 0x0fffffff;
-    const unsigned live = (unsigned)entry.y >> 30;
-    const unsigned hmax = (unsigned)c.n_qpt + 2u + (((unsigned)entry.y >> 28) & 3u);    // the lane's dump slot
+__device__ __noinline__ void walk_redo_pair(const HoughConsts& c, const FastK& fk, float4 d, const WalkArgs& a, const WalkTile& tl,
+                                            int sidx, int cc, unsigned dump, unsigned live) {
+    const float4 hv = __ldg(a.staged + sidx);
+    const unsigned hmax = (unsigned)c.n_qpt + 2u + dump;
     const float r2 = d3_r2(hv.x, hv.y);
     const FastHit fh = make_fasthit(fk, hv.x, hv.y, r2);
-    const float4 T = s_pair[cc >> 1];
+    const float4 T = tl.s_pair[cc >> 1];
     unsigned long long best = 0ull;
 #pragma unroll
     for (int w = 0; w < 2; ++w) {
         if (!((live >> w) & 1u)) continue;
         const float cs_c = w ? T.y : T.x, cs_s = w ? T.w : T.z;
         if (MODE == WALK_VOTE)
-            tile_add_slot<TILE32>(s_tile, stride, cc + w, min(fast_slot(fk, fh, cs_c, cs_s), hmax), -1);
+            tile_add_slot<TILE32>(tl.s_tile, tl.stride, cc + w, min(fast_slot(fk, fh, cs_c, cs_s), hmax), -1);
         const int j = d3_exact_bin(hv.x, hv.y, r2, cs_c, cs_s, d.x, d.y, d.z, c.A_f, c.qmin, c.inv_wq, c.nq_f);
         if (j >= 0)
-            walk_apply<MODE, TILE32>(s_tile, stride, c.n_qpt, cc + w, j, legacy, a.assoc_dj, a.cands, cand_first, cand_end, c0,
-                                     row_lin0, best);
+            walk_apply<MODE, TILE32>(tl.s_tile, tl.stride, c.n_qpt, cc + w, j, tl.legacy, a.assoc_dj, a.cands, tl.cand_first,
+                                     tl.cand_end, tl.c0, tl.row_lin0, best);
     }
     if (MODE == WALK_ASSIGN && best) atomicMax(a.best_key + __float_as_int(hv.w), best);
+}
+
+// Redo queue entry (32 bits): staged index inside the event (18 bits) | pair index inside the tile (10) | dump (2) | live (2)
+__device__ __forceinline__ unsigned wq_pack(int in_event, int cc, unsigned dump, unsigned live) {
+    return (unsigned)in_event | ((unsigned)(cc >> 1) << 18) | (dump << 28) | (live << 30);
+}
+
+template <int MODE, bool TILE32>
+__device__ __forceinline__ void walk_drain(const HoughConsts& c, const FastK& fk, float4 d, const WalkArgs& a, const WalkTile& tl,
+                                           const unsigned* wq, int n, int ev_begin, int lane) {
+    __syncwarp();
+    for (int q = lane; q < n; q += 32) {
+        const unsigned en = wq[q];
+        walk_redo_pair<MODE, TILE32>(c, fk, d, a, tl, ev_begin + (int)(en & 0x3ffffu), (int)((en >> 18) & 0x3ffu) * 2, (en >> 28) & 3u,
+                                     en >> 30);
+    }
+    __syncwarp();
 }
 
 template <int MODE, bool TILE32, bool OUT16, bool FULLPHI>
 __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, WalkArgs a) {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ int s_qn;
+    __shared__ int s_meta[2];                           // number of batches of the tile
     const int n_slabs = a.n_slabs, slab_cols = a.slab_cols, stride = a.stride;
     const int slab = blockIdx.x % n_slabs;
     const int k = (blockIdx.x / n_slabs) % c.n_d0;
@@ -321,24 +342,21 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int n_pair_tab = slab_cols / 2 + WALK_CHUNK_PAIRS + 1;
 
-    uint32_t* s_tile; float4* s_pair; int2* s_q; float* s_lo; int* s_steps; int* s_seg_start; int* s_seg_cnt; int* s_seg_pref;
+    uint32_t* s_tile; float4* s_pair; unsigned* s_wq; float4* s_cls; int4* s_seg;
     {
         unsigned char* q = smem_raw;
         s_tile = reinterpret_cast<uint32_t*>(q);  q += (walk_tile_words(slab_cols, stride, TILE32) * 4 + 15) & ~(size_t)15;
         s_pair = reinterpret_cast<float4*>(q);    q += (size_t)n_pair_tab * 16;
-        s_q = reinterpret_cast<int2*>(q);         q += (size_t)WALK_QCAP * 8;
-        s_lo = reinterpret_cast<float*>(q);       q += (size_t)nc * 4;
-        s_steps = reinterpret_cast<int*>(q);      q += (size_t)nc * 4;
-        s_seg_start = reinterpret_cast<int*>(q);  q += (size_t)nc * 2 * 4;
-        s_seg_cnt = reinterpret_cast<int*>(q);    q += (size_t)nc * 2 * 4;
-        s_seg_pref = reinterpret_cast<int*>(q);
+        s_cls = reinterpret_cast<float4*>(q);     q += (size_t)nc * 16;              // {lo_off, bits(steps | flags), hm, -}
+        s_seg = reinterpret_cast<int4*>(q);       q += ((size_t)nc * 2 + 1) * 16;    // {first staged hit, hits, class, first batch}
+        s_wq = reinterpret_cast<unsigned*>(q);                                        // [WALK_WARPS][WALK_WQ_CAP]
     }
     unsigned short* s_tile16 = reinterpret_cast<unsigned short*>(s_tile);
     const unsigned tile_saddr = (unsigned)__cvta_generic_to_shared(s_tile);
     const unsigned stride4 = (unsigned)stride * 4u;
-    // one scratch word per lane at the end of the block: where the branch-free vote sends the lanes that do not vote
-    const unsigned trash_saddr = (unsigned)__cvta_generic_to_shared(
-        smem_raw + walk_smem_bytes(slab_cols, stride, TILE32, nc) - 128 + 4 * lane);
+    // one scratch word per lane at the end of the block: where slab tiles send the lanes that are past their part
+    unsigned char* trash_ptr = smem_raw + walk_smem_bytes(slab_cols, stride, TILE32, nc) - 128;
+    const unsigned trash_saddr = (unsigned)__cvta_generic_to_shared(trash_ptr + 4 * lane);
 
     int cand_first = 0, cand_end = 0;
     if (MODE == WALK_ASSIGN) {
@@ -346,8 +364,22 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
         cand_first = sl.x; cand_end = sl.y;
         if (cand_first >= cand_end) return;              // no candidate in this tile: nothing to associate
     }
+    const float4 d = __ldg(c.d0t + k);
+    const FastK fk = make_fastk(c, d);
+    const int ev_begin = __ldg(a.off + e);
+    const int ev_hits = __ldg(a.off + e + 1) - ev_begin;
+    const int32_t* ks = a.key_start + (size_t)e * (c.n_keys + 1);
 
     // ---- prologue: zero the tile, load tables, list the segments of staged hits that can reach the tile ----
+    // association: does any candidate of the tile exceed the entry's vote field?  (then: exact probing, below)
+    bool legacy = false;
+    if (MODE == WALK_ASSIGN) {
+        int sat = 0;
+        for (int ci = cand_first + tid; ci < cand_end; ci += WALK_THREADS)
+            sat |= ((unsigned)__ldg(&a.cands[ci].votes) + 1u >= EntryT<TILE32>::VSAT) ? 1 : 0;
+        legacy = __syncthreads_or(sat) != 0 || a.exact_only != 0;
+    }
+    const bool exact_mode = a.exact_only != 0 || !fk.usable || (MODE == WALK_ASSIGN && legacy);
     {
         uint4* t4 = reinterpret_cast<uint4*>(s_tile);
         const int n4 = (int)((walk_tile_words(cols, stride, TILE32) + 3) >> 2);
@@ -358,76 +390,89 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
             const float2 A = __ldg(c.cs + ca), B = __ldg(c.cs + ca + 1);
             s_pair[p] = make_float4(A.x, B.x, A.y, B.y);
         }
-        if (tid == 0) s_qn = 0;
-        if (tid < 32)                                    // scratch words: read (as empty entries) by the association probes
-            reinterpret_cast<uint32_t*>(smem_raw + walk_smem_bytes(slab_cols, stride, TILE32, nc) - 128)[tid] = 0u;
+        if (tid < 32) reinterpret_cast<uint32_t*>(trash_ptr)[tid] = 0u;   // read (as empty entries) by association probes
     }
-    const int ev_begin = __ldg(a.off + e);
-    const int32_t* ks = a.key_start + (size_t)e * (c.n_keys + 1);
+    // per class: column window and the fast path's error bound over the class's radius interval (DESIGN.md "Fast
+    // path"): hm = 1/2 - m, or 0 when the class takes the exact sequence at every column
     for (int cl = tid; cl < nc; cl += WALK_THREADS) {
         const int2 w = __ldg(c.win + (size_t)cl * c.n_d0 + k);
-        const float lo = __int_as_float(w.x);
         const int steps = w.y & 0x3fffffff;
-        s_lo[cl] = lo;
-        s_steps[cl] = w.y;                               // bit 30: every column of the window (+-2) is forward (f > 0)
-        int a0 = 0, n0 = 0, a1 = 0, n1 = 0;
-        if (steps > 0) {
-            const int NS = c.n_sector;
-            int sa = 0, ns = NS;
-            if (!FULLPHI) {
-                // hits whose window [ceil(u + lo), +steps) meets [c0, c0 + cols): u in (c0 - steps - lo, c0 + cols - lo)
-                const float W = (float)nphi / (float)NS;
-                const float ua = (float)(c0 - steps) - lo - 2.0f;
-                const float ub = (float)(c0 + cols) - lo + 2.0f;
-                const int s0 = (int)floorf((ua + 0.5f) / W);
-                const int s1 = (int)floorf((ub + 0.5f) / W);
-                ns = s1 - s0 + 1;
-                if (ns >= NS) { sa = 0; ns = NS; }
-                else { sa = s0 % NS; if (sa < 0) sa += NS; }
-            }
-            const int base = cl * NS;
-            if (sa + ns <= NS) {
-                a0 = __ldg(ks + base + sa);
-                n0 = __ldg(ks + base + sa + ns) - a0;
-            } else {
-                a0 = __ldg(ks + base + sa);
-                n0 = __ldg(ks + base + NS) - a0;
-                a1 = __ldg(ks + base);
-                n1 = __ldg(ks + base + (sa + ns - NS)) - a1;
-            }
+        const bool fwd_safe = (w.y >> 30) & 1;           // every column of the window (+-2) is forward (f > 0)
+        float hm = 0.0f;
+        if (!exact_mode && fwd_safe && steps > 0 && cl > 0 && cl + 1 < nc && (FULLPHI || steps + cols + 2 <= nphi)) {
+            const float ra = sqrtf(__ldg(c.edge2 + cl)) * 0.999998f, rb = sqrtf(__ldg(c.edge2 + cl + 1)) * 1.000002f;
+            const float L = 1.4142137f * rb;                                  // |x| + |y| <= sqrt(2) r
+            float dr = (fk.d0abs >= ra && fk.d0abs <= rb) ? 0.0f : fminf(fabsf(ra - fk.d0abs), fabsf(rb - fk.d0abs));
+            dr = fmaxf(dr - 1.0e-6f * rb, 0.0f);                              // den >= (r - |d0|)^2 >= dr^2
+            const float S = 8.0f * fk.d0abs * L + rb * rb + fk.d0sq;
+            const float inv_dr2 = 1.000001f / (dr * dr);
+            const float arel = WALK_U * (6.0f * S * inv_dr2 + 24.0f);
+            const float elin = fk.e_lin * (L + fk.d0abs);
+            const float m = fk.inv_A_abs * inv_dr2 * elin + arel * fk.t_max + fk.a0;
+            if (m < 0.45f) hm = 0.5f - m;                                     // false for NaN / inf
         }
-        s_seg_start[2 * cl] = a0;     s_seg_cnt[2 * cl] = n0;
-        s_seg_start[2 * cl + 1] = a1; s_seg_cnt[2 * cl + 1] = n1;
+        s_cls[cl] = make_float4(__int_as_float(w.x), __int_as_float(steps), hm, 0.0f);
     }
-    // association: does any candidate of the tile exceed the entry's vote field?  (then: exact probing, below)
-    bool legacy = false;
-    if (MODE == WALK_ASSIGN) {
-        int sat = 0;
-        for (int ci = cand_first + tid; ci < cand_end; ci += WALK_THREADS)
-            sat |= ((unsigned)__ldg(&a.cands[ci].votes) + 1u >= EntryT<TILE32>::VSAT) ? 1 : 0;
-        legacy = __syncthreads_or(sat) != 0 || a.exact_only != 0;
-    } else {
-        __syncthreads();
-    }
-    if (warp == 0) {                                    // exclusive prefix of batch counts over 2*nc segments
-        const int nseg = 2 * nc;
-        const int per = (nseg + 31) / 32;
-        int sum = 0;
-        for (int x = lane * per; x < min(nseg, (lane + 1) * per); ++x) sum += (s_seg_cnt[x] + 31) >> 5;
-        int incl = sum;
+    // segments (class, sector run) of staged hits whose window can meet the tile: non-empty ones, compacted, with
+    // the exclusive prefix of their 32-hit batch counts
+    if (warp == 0) {
+        int n_out = 0, run = 0;
+        const unsigned lt = (1u << lane) - 1u;
+        for (int cl0 = 0; cl0 < nc; cl0 += 32) {
+            const int cl = cl0 + lane;
+            int a0 = 0, n0 = 0, a1 = 0, n1 = 0;
+            if (cl < nc) {
+                const int2 w = __ldg(c.win + (size_t)cl * c.n_d0 + k);
+                const float lo = __int_as_float(w.x);
+                const int steps = w.y & 0x3fffffff;
+                if (steps > 0) {
+                    const int NS = c.n_sector;
+                    int sa = 0, ns = NS;
+                    if (!FULLPHI) {
+                        // hits whose window [ceil(u + lo), +steps) meets [c0, c0 + cols): u in (c0 - steps - lo, c0 + cols - lo)
+                        const float W = (float)nphi / (float)NS;
+                        const float ua = (float)(c0 - steps) - lo - 2.0f;
+                        const float ub = (float)(c0 + cols) - lo + 2.0f;
+                        const int s0 = (int)floorf((ua + 0.5f) / W);
+                        const int s1 = (int)floorf((ub + 0.5f) / W);
+                        ns = s1 - s0 + 1;
+                        if (ns >= NS) { sa = 0; ns = NS; }
+                        else { sa = s0 % NS; if (sa < 0) sa += NS; }
+                    }
+                    const int base = cl * NS;
+                    if (sa + ns <= NS) {
+                        a0 = __ldg(ks + base + sa);
+                        n0 = __ldg(ks + base + sa + ns) - a0;
+                    } else {
+                        a0 = __ldg(ks + base + sa);
+                        n0 = __ldg(ks + base + NS) - a0;
+                        a1 = __ldg(ks + base);
+                        n1 = __ldg(ks + base + (sa + ns - NS)) - a1;
+                    }
+                }
+            }
+            const int b0 = (n0 + 31) >> 5, b1 = (n1 + 31) >> 5;
+            const unsigned m0 = __ballot_sync(0xffffffffu, n0 > 0), m1 = __ballot_sync(0xffffffffu, n1 > 0);
+            int incl = b0 + b1;
 #pragma unroll
-        for (int o = 1; o < 32; o <<= 1) {
-            const int y = __shfl_up_sync(0xffffffffu, incl, o);
-            if (lane >= o) incl += y;
+            for (int o = 1; o < 32; o <<= 1) {
+                const int y = __shfl_up_sync(0xffffffffu, incl, o);
+                if (lane >= o) incl += y;
+            }
+            const int excl = run + incl - (b0 + b1);
+            const int o0 = n_out + __popc(m0 & lt) + __popc(m1 & lt);
+            if (n0 > 0) s_seg[o0] = make_int4(a0, n0, cl, excl);
+            if (n1 > 0) s_seg[o0 + (n0 > 0 ? 1 : 0)] = make_int4(a1, n1, cl, excl + b0);
+            n_out += __popc(m0) + __popc(m1);
+            run += __shfl_sync(0xffffffffu, incl, 31);
         }
-        int run = incl - sum;
-        for (int x = lane * per; x < min(nseg, (lane + 1) * per); ++x) {
-            s_seg_pref[x] = run;
-            run += (s_seg_cnt[x] + 31) >> 5;
+        if (lane == 0) {
+            s_seg[n_out] = make_int4(0, 0, 0, run);      // sentinel: first batch past the end
+            s_meta[0] = run;
         }
-        if (lane == 31) s_seg_pref[nseg] = incl;
     }
     if (MODE == WALK_ASSIGN) {
+        __syncthreads();                                // the tile is zero
         if (legacy) {                                   // votes + 1 at the candidates' own bins
             for (int ci = cand_first + tid; ci < cand_end; ci += WALK_THREADS) {
                 const int4 q = __ldg(reinterpret_cast<const int4*>(a.cands + ci));          // event, k, i, j
@@ -443,8 +488,8 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
                 const unsigned v = ((unsigned)__ldg(&a.cands[ci].votes) + 1u) << 5;
                 const int col = q.z - c0;
                 for (int jb = max(q.w - dj, 0); jb <= min(q.w + dj, nq - 1); ++jb) {
-                    const int d = q.w - jb;                                                  // j_cand - j_bin
-                    const unsigned ent = v | (unsigned)((15 - abs(d)) * 2 + (d < 0 ? 1 : 0));
+                    const int dd = q.w - jb;                                                 // j_cand - j_bin
+                    const unsigned ent = v | (unsigned)((15 - abs(dd)) * 2 + (dd < 0 ? 1 : 0));
                     if (TILE32) {
                         atomicMax(s_tile + col * stride + jb + 1, ent);
                     } else {
@@ -465,63 +510,45 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
     __syncthreads();
 
     // ---- main loop: 32-hit batches, static round-robin over the CTA's warps ----
-    const int n_batches = s_seg_pref[2 * nc];
-    const float4 d = __ldg(c.d0t + k);
-    const FastK fk = make_fastk(c, d);
-    const bool exact_mode = a.exact_only != 0 || !fk.usable || (MODE == WALK_ASSIGN && legacy);
+    const int n_batches = s_meta[0];
     const unsigned row_lin0 = (unsigned)(k * nphi + c0) * (unsigned)nq;   // linear bin of (k, c0, 0) inside the event
     const unsigned tile_bytes = (unsigned)(walk_tile_words(cols, stride, TILE32) * 4);   // FULLPHI: the wrap distance
-    const unsigned nqg = (unsigned)nq + 2u;
     const f32x2 d0cq2 = pk2(fk.d0cq, fk.d0cq), c0h2 = pk2(fk.c0h, fk.c0h);
     const f32x2 magic2 = pk2(WALK_MAGIC, WALK_MAGIC), nmagic2 = pk2(-WALK_MAGIC, -WALK_MAGIC);
+    WalkTile tl;
+    tl.s_tile = s_tile; tl.s_pair = s_pair; tl.stride = stride; tl.c0 = c0; tl.cand_first = cand_first; tl.cand_end = cand_end;
+    tl.row_lin0 = row_lin0; tl.legacy = legacy;
+    unsigned* wq = s_wq + warp * WALK_WQ_CAP;           // the warp's redo queue
+    int wq_n = 0;
+    const bool wq_ok = ev_hits < (1 << 18) && slab_cols <= 2048;          // entries fit 32 bits (else: redo on the spot)
     int seg = 0;                                        // batches ascend per warp: a running segment pointer
     for (int bt = warp; bt < n_batches; bt += WALK_WARPS) {
-        while (s_seg_pref[seg + 1] <= bt) ++seg;         // largest segment with seg_pref[seg] <= bt (seg_pref[2nc] = n_batches > bt)
-        const int in_seg = (bt - s_seg_pref[seg]) * 32 + lane;
-        const bool active = in_seg < s_seg_cnt[seg];
-        const int cl = seg >> 1;
-        const int steps_w = s_steps[cl];
-        const int steps = steps_w & 0x3fffffff;
-        const bool fwd_safe = (steps_w >> 30) & 1;
-        const int sidx = ev_begin + s_seg_start[seg] + in_seg;      // index of the lane's staged hit
+        while (s_seg[seg + 1].w <= bt) ++seg;            // last segment with first batch <= bt (the sentinel ends the search)
+        const int4 sg = s_seg[seg];
+        const int in_seg = (bt - sg.w) * 32 + lane;
+        const bool active = in_seg < sg.y;
+        const float4 cw = s_cls[sg.z];
+        const int steps = __float_as_int(cw.y);
+        const float hm_c = cw.z;
+        const int sidx = ev_begin + sg.x + in_seg;       // index of the lane's staged hit
         float4 hv = make_float4(1.f, 0.f, 0.f, 0.f);
         if (active) hv = __ldg(a.staged + sidx);
         const float x = hv.x, y = hv.y;
         const float r2 = d3_r2(x, y);
-        int i_lo = (int)ceilf(hv.z + s_lo[cl]);
+        int i_lo = (int)ceilf(hv.z + cw.x);
         if (i_lo < 0) i_lo += nphi;
         if (i_lo >= nphi) i_lo -= nphi;
         if (!(i_lo >= 0 && i_lo < nphi)) i_lo = 0;
 
-        unsigned long long best = 0ull;                  // association: full D8 key from the exact paths
+        unsigned long long best = 0ull;                  // association: full D8 key from the exact path
         // dilated association: (entry >> 1) above ~column (equal votes and |dj| in two columns: the smaller linear
         // bin wins, D8); the entry's sign bit travels with the q/pT bin in bestj
         typename EntryT<TILE32>::pkey_t bestp = 0;
         int bestj = 0;
 
-        // ---- fast-path per-hit terms ----
-        const bool fast_batch = !exact_mode && fwd_safe && steps > 0 && (FULLPHI || steps + cols + 2 <= nphi);
-        float gy = 0.f, gx = 0.f, ny = 0.f, nx = 0.f, r2Ak = 1.f, hm_h = 0.f;
-        bool good = false;
-        if (fast_batch) {
-            const FastHit fh = make_fasthit(fk, x, y, r2);
-            gy = fh.gy; gx = fh.gx; ny = fh.ny; nx = fh.nx; r2Ak = fh.r2Ak;
-            const float L = fabsf(x) + fabsf(y);
-            const float S = __fmaf_rn(8.0f * fk.d0abs, L, r2 + fk.d0sq);
-            // den >= (r - |d0|)^2; r from the approximate reciprocal square root (2 ulp), shrunk by 2^-20 r
-            const float rr = r2 * rsqrt_approx(r2);
-            const float dr = fmaxf(fabsf(rr - fk.d0abs) - 9.5367432e-7f * rr, 0.0f);
-            const float inv_dr2 = rcp_approx(dr * dr) * 1.000001f;
-            const float arel_h = WALK_U * __fmaf_rn(6.0f * S, inv_dr2, 24.0f);
-            const float elin_h = fk.e_lin * (L + fk.d0abs);
-            const float m_h = __fmaf_rn(fk.inv_A_abs * inv_dr2, elin_h, __fmaf_rn(arel_h, fk.t_max, fk.a0));
-            good = active && (m_h < 0.45f);                               // false for NaN / r ~ |d0| / huge coordinates
-            hm_h = 0.5f - m_h;
-        }
-
-        // ---- exact D3 sequence at every column of the window: lanes (or whole batches) without a usable bound ----
-        if (__any_sync(0xffffffffu, active && !good)) {
-            if (active && !good) {
+        if (!(hm_c > 0.0f)) {
+            // ---- exact D3 sequence at every column of the window: classes without a usable bound ----
+            if (active) {
                 int col = i_lo - c0;                     // column relative to the tile, cyclic
                 if (col < 0) col += nphi;
                 for (int t = 0; t < steps; ++t) {
@@ -537,33 +564,33 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
                     if (col == nphi) col = 0;
                 }
             }
-        }
-
-        // ---- fast path: the lane's window, two columns at a time ----
-        if (__any_sync(0xffffffffu, good)) {
+        } else {
+            // ---- fast path: the lane's window, two columns at a time ----
+            const FastHit fh = make_fasthit(fk, x, y, r2);
             // first column (even, tile-relative) and number of columns of the lane's part of the tile
             int start, my_n;
             if (FULLPHI) {
                 start = i_lo & ~1;                       // one column early when i_lo is odd; never past the window + 2
-                if (!good) start = (2 * lane) % nphi;    // lanes without work walk rows of their own (no same-word adds)
-                my_n = good ? ((steps + 2) & ~1) : 0;
+                if (!active) start = (2 * lane) % nphi;  // lanes without work walk rows of their own (no same-word adds)
+                my_n = active ? ((steps + 2) & ~1) : 0;
             } else {
                 int rel = i_lo - c0;
                 if (rel < 0) rel += nphi;
                 int n;
                 if (rel < cols) { start = rel; n = min(steps, cols - rel); }
                 else { const int over = rel + steps - nphi; start = 0; n = over > 0 ? min(over, cols) : 0; }
-                if (!good) { start = 0; n = 0; }
+                if (!active) { start = 0; n = 0; }
                 const int se = start & ~1;
                 my_n = n > 0 ? n + (start - se) : 0;
                 start = se;
             }
             const int np_total = __reduce_max_sync(0xffffffffu, (my_n + 1) >> 1);
             // lanes without work: every evaluation lands in guard slot 0 and none is ever "uncertain"
-            const unsigned hmax_l = good ? (unsigned)nq + 2u + (unsigned)(lane & (WALK_DUMP - 1)) : 0u;
-            const float hm_l = good ? hm_h : __int_as_float(0x7f800000);
-            const f32x2 r2Ak2 = pk2(r2Ak, r2Ak);
-            const f32x2 gy2 = pk2(gy, gy), gx2 = pk2(gx, gx), ny2 = pk2(ny, ny), nx2 = pk2(nx, nx);
+            const unsigned dump = (unsigned)(lane & (WALK_DUMP - 1));
+            const unsigned hmax_l = active ? (unsigned)nq + 2u + dump : 0u;
+            const float hm_l = active ? hm_c : __int_as_float(0x7f800000);
+            const f32x2 r2Ak2 = pk2(fh.r2Ak, fh.r2Ak);
+            const f32x2 gy2 = pk2(fh.gy, fh.gy), gx2 = pk2(fh.gx, fh.gx), ny2 = pk2(fh.ny, fh.ny), nx2 = pk2(fh.nx, fh.nx);
             int col = start;
             int rem = my_n;                              // columns left in the lane's part (slab tiles)
             for (int p0 = 0; p0 < np_total; p0 += WALK_CHUNK_PAIRS) {
@@ -577,9 +604,9 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
                 int colp = col;                          // association: running tile column of the pair
                 unsigned slowmask = 0u;                  // bit (np - 1 - t): pair t of the chunk is uncertain
                 // One chunk of column pairs; WRAP: some lane of the warp passes column n_phi - 1 inside the chunk.
-                // The vote is unconditional: slot min(h, nq + 1) of the column's row (results outside [-1, nq] land in
-                // a guard slot).  A pair with an uncertain column is flagged; the redo takes the pair's two fast votes
-                // back (fast_slot reproduces them) and casts the exact ones.
+                // The vote is unconditional: slot min(h, nq + 2 + dump) of the column's row (results outside [-1, nq]
+                // land in a dump slot).  A pair with an uncertain column is flagged; the redo takes the pair's two fast
+                // votes back (fast_slot reproduces them) and casts the exact ones.
                 auto run_chunk = [&](auto wrap_c) {
                     constexpr bool WRAP = decltype(wrap_c)::value;
 #pragma unroll 2
@@ -597,8 +624,8 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
                         float ybA, ybB, dA, dB;
                         upk2(yb2, ybA, ybB);
                         upk2(dl2, dA, dB);
-                        unsigned hA = min((unsigned)(__float_as_int(ybA) - (WALK_MAGIC_BITS - 1)), hmax_l);   // slot J + 1
-                        unsigned hB = min((unsigned)(__float_as_int(ybB) - (WALK_MAGIC_BITS - 1)), hmax_l);
+                        const unsigned hA = min((unsigned)(__float_as_int(ybA) - (WALK_MAGIC_BITS - 1)), hmax_l);   // slot J + 1
+                        const unsigned hB = min((unsigned)(__float_as_int(ybB) - (WALK_MAGIC_BITS - 1)), hmax_l);
                         // uncertain: t~ within m of a bin edge, J <= t_D3 < J + 1 not proven (NaN never compares true)
                         bool unsA = fabsf(dA) >= hm_l, unsB = fabsf(dB) >= hm_l;
                         unsigned adA = addr_w(rowaddr, hA), adB = addr_w(TILE32 ? rowaddr + stride4 : rowaddr, hB);
@@ -630,21 +657,26 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
                 if (FULLPHI && __any_sync(0xffffffffu, wrap_t < np)) run_chunk(std::true_type{});
                 else run_chunk(std::false_type{});
                 col += 2 * np;                           // FULLPHI: reduced modulo n_phi at the top of the next chunk
-                // uncertain pairs of the chunk -> the CTA's exact-redo queue {staged hit, pair column | live flags << 30}
-                while (slowmask) {
-                    const int b = __ffs(slowmask) - 1;
-                    slowmask &= slowmask - 1u;
-                    const int t = np - 1 - b;
-                    int cc = col_chunk + 2 * t;
-                    if (FULLPHI && cc >= nphi) cc -= nphi;
-                    unsigned live = 3u;
-                    if (!FULLPHI) live = (rem_chunk - 2 * t > 0 ? 1u : 0u) | (rem_chunk - 2 * t > 1 ? 2u : 0u);
-                    const int2 entry = make_int2(sidx, (int)((unsigned)cc | ((unsigned)(lane & (WALK_DUMP - 1)) << 28) | (live << 30)));
-                    const int slot = atomicAdd(&s_qn, 1);
-                    if (slot < WALK_QCAP) s_q[slot] = entry;
-                    else                                 // queue full: redo on the spot
-                        walk_redo_pair<MODE, TILE32>(c, fk, d, a, entry, s_tile, s_pair, stride, legacy, cand_first, cand_end, c0,
-                                                     row_lin0);
+                // uncertain pairs of the chunk -> the warp's redo queue, drained 32 at a time by the whole warp
+                while (__any_sync(0xffffffffu, slowmask != 0u)) {
+                    if (wq_n > WALK_WQ_CAP - 32) {
+                        walk_drain<MODE, TILE32>(c, fk, d, a, tl, wq, wq_n, ev_begin, lane);
+                        wq_n = 0;
+                    }
+                    const bool has = slowmask != 0u;
+                    const unsigned bal = __ballot_sync(0xffffffffu, has);
+                    if (has) {
+                        const int b = __ffs(slowmask) - 1;
+                        slowmask &= slowmask - 1u;
+                        const int t = np - 1 - b;
+                        int cc = col_chunk + 2 * t;
+                        if (FULLPHI && cc >= nphi) cc -= nphi;
+                        unsigned live = 3u;
+                        if (!FULLPHI) live = (rem_chunk - 2 * t > 0 ? 1u : 0u) | (rem_chunk - 2 * t > 1 ? 2u : 0u);
+                        if (wq_ok) wq[wq_n + __popc(bal & ((1u << lane) - 1u))] = wq_pack(sidx - ev_begin, cc, dump, live);
+                        else walk_redo_pair<MODE, TILE32>(c, fk, d, a, tl, sidx, cc, dump, live);
+                    }
+                    if (wq_ok) wq_n += __popc(bal);
                 }
             }
         }
@@ -660,14 +692,7 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
             if (best) atomicMax(a.best_key + __float_as_int(hv.w), best);
         }
     }
-    __syncthreads();
-
-    // ---- exact redo of the queued pairs, by the whole CTA ----
-    {
-        const int nqd = min(s_qn, WALK_QCAP);
-        for (int q = tid; q < nqd; q += WALK_THREADS)
-            walk_redo_pair<MODE, TILE32>(c, fk, d, a, s_q[q], s_tile, s_pair, stride, legacy, cand_first, cand_end, c0, row_lin0);
-    }
+    if (wq_n > 0) walk_drain<MODE, TILE32>(c, fk, d, a, tl, wq, wq_n, ev_begin, lane);
     if (MODE == WALK_ASSIGN) return;
     __syncthreads();
 
