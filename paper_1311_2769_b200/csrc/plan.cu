@@ -154,7 +154,7 @@ extern "C" int hough_plan_create(const hough_binning* b, const hough_geometry* g
             int lo = 0, hi = b->n_phi / 2;                                // pairs of columns
             while (lo < hi) {
                 const int mid = (lo + hi + 1) / 2;
-                if (walk_smem_bytes(2 * mid, stride, p->tile32 != 0, win.n_class) <= budget) lo = mid; else hi = mid - 1;
+                if (walk_smem_bytes(2 * mid, stride, p->tile32 != 0, win.n_class, 2 * mid == b->n_phi) <= budget) lo = mid; else hi = mid - 1;
             }
             return 2 * lo;
         };

@@ -33,7 +33,7 @@
 
 constexpr int WALK_VOTE = 0;
 constexpr int WALK_ASSIGN = 1;
-constexpr int WALK_THREADS = 256;
+constexpr int WALK_THREADS = 320;
 constexpr int WALK_WARPS = WALK_THREADS / 32;
 constexpr int WALK_CHUNK_PAIRS = 16;             // column pairs per chunk: 32 columns = the bits of the redo mask
 constexpr int WALK_WQ_CAP = 48;                  // entries of a warp's exact-redo queue (drained by the whole warp)
@@ -60,11 +60,11 @@ __host__ __device__ inline size_t walk_tile_words(int cols, int stride, bool til
     return tile32 ? (size_t)cols * stride : (size_t)((cols + 1) / 2) * stride;
 }
 
-__host__ __device__ inline size_t walk_smem_bytes(int cols, int stride, bool tile32, int n_class) {
+__host__ __device__ inline size_t walk_smem_bytes(int cols, int stride, bool tile32, int n_class, bool fullphi) {
     size_t b = (walk_tile_words(cols, stride, tile32) * 4 + 15) & ~(size_t)15;
     b += (size_t)(cols / 2 + WALK_CHUNK_PAIRS + 1) * 16;               // column pairs {cosA, cosB, sinA, sinB}
     b += (size_t)n_class * 16;                                          // per class: window, error bound
-    b += ((size_t)n_class * 2 + 1) * 16;                                // segments
+    b += ((size_t)n_class * (fullphi ? 1 : 2) + 1) * 16;                // segments (a full-phi tile has one per class)
     b += (size_t)WALK_WARPS * WALK_WQ_CAP * 4;                          // redo queues
     return b + 128;                                                     // one scratch word per lane (walk_kernel: trash_saddr)
 }
@@ -348,14 +348,14 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
         s_tile = reinterpret_cast<uint32_t*>(q);  q += (walk_tile_words(slab_cols, stride, TILE32) * 4 + 15) & ~(size_t)15;
         s_pair = reinterpret_cast<float4*>(q);    q += (size_t)n_pair_tab * 16;
         s_cls = reinterpret_cast<float4*>(q);     q += (size_t)nc * 16;              // {lo_off, bits(steps | flags), hm, -}
-        s_seg = reinterpret_cast<int4*>(q);       q += ((size_t)nc * 2 + 1) * 16;    // {first staged hit, hits, class, first batch}
+        s_seg = reinterpret_cast<int4*>(q);       q += ((size_t)nc * (FULLPHI ? 1 : 2) + 1) * 16;   // {first staged hit, hits, class, first batch}
         s_wq = reinterpret_cast<unsigned*>(q);                                        // [WALK_WARPS][WALK_WQ_CAP]
     }
     unsigned short* s_tile16 = reinterpret_cast<unsigned short*>(s_tile);
     const unsigned tile_saddr = (unsigned)__cvta_generic_to_shared(s_tile);
     const unsigned stride4 = (unsigned)stride * 4u;
     // one scratch word per lane at the end of the block: where slab tiles send the lanes that are past their part
-    unsigned char* trash_ptr = smem_raw + walk_smem_bytes(slab_cols, stride, TILE32, nc) - 128;
+    unsigned char* trash_ptr = smem_raw + walk_smem_bytes(slab_cols, stride, TILE32, nc, FULLPHI) - 128;
     const unsigned trash_saddr = (unsigned)__cvta_generic_to_shared(trash_ptr + 4 * lane);
 
     int cand_first = 0, cand_end = 0;
@@ -740,7 +740,7 @@ inline void walk_shape(const hough_plan* p, int n_events, int& n_slabs, int& sla
 
 template <int MODE, bool TILE32, bool OUT16, bool FULLPHI>
 int walk_launch(hough_plan* p, int n_events, WalkArgs a, cudaStream_t st) {
-    const size_t smem = walk_smem_bytes(a.slab_cols, a.stride, TILE32, p->c.n_class);
+    const size_t smem = walk_smem_bytes(a.slab_cols, a.stride, TILE32, p->c.n_class, FULLPHI);
     auto kern = walk_kernel<MODE, TILE32, OUT16, FULLPHI>;
     static size_t smem_configured = 0;              // per instantiation; raised only when a call needs more
     if (smem > smem_configured) {
