@@ -131,13 +131,31 @@ def load_peaks():
 
 
 # ----------------------------------------------------------------------------------------------
+def shard_event_range(rank: int, events_per_rank: int) -> range:
+    """events are independent units, so rank r owns events [r * n, (r + 1) * n) of the workload's
+    event sequence (weak scaling: n is fixed per GPU); no data-path collective follows."""
+    return range(rank * events_per_rank, (rank + 1) * events_per_rank)
+
+
+def reduce_job(ms_total: float, votes: float, events: float, hits: float, world: int, device):
+    """Whole-job figures from per-rank ones: time = MAX over ranks, work = SUM over ranks (the only collectives
+    of the bench; the data path has none)."""
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms_total], dtype=torch.float64, device=device)
+    v = torch.tensor([float(votes), float(events), float(hits)], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dist.all_reduce(v, op=dist.ReduceOp.SUM)
+    return float(t.item()), tuple(float(x) for x in v.tolist())
+
+
 def make_batch(cfg: int, n_events: int, rank: int):
     from workloads import generate_events, get_workload
     w = get_workload(cfg)
     if w.n_events > 1 or n_events != w.n_events:
         w = w.scaled(n_events)
-    first = rank * n_events
-    batch = generate_events(w, events=range(first, first + n_events))
+    batch = generate_events(w, events=shard_event_range(rank, n_events))
     return w, batch
 
 
@@ -262,56 +280,42 @@ class DeviceRun:
         return total
 
 
-def e2e_python(run: DeviceRun, steps: int, warmup: int):
-    """End-to-end through the public Python API with HOST buffers: per tile, pinned hits/offsets -> device,
-    the three calls, results -> pinned host (cand_offsets, hit_to_cand, candidate records, nhits, keep)."""
+def e2e_pipeline(run: DeviceRun, steps: int, warmup: int, n_streams: int):
+    """End-to-end through the library's batched path (hough_pipeline_run_host): pinned HOST buffers in (hits, offsets)
+    and out (hit_to_cand, cand_offsets, candidate records, nhits, keep); every host<->device copy is inside the
+    timed region.  Wall-clock around the blocking call (it returns when the results are in the host buffers)."""
     torch = run.torch
+    from paper_1311_2769_b200 import HoughPipeline
     w, batch = run.w, run.batch
-    h_hits = torch.from_numpy(batch.hits_xy).pin_memory()
-    off = batch.event_offsets.astype(np.int64)
-    h_offs = [torch.from_numpy((off[e0:e1 + 1] - h0).astype(np.int32)).pin_memory() for (e0, e1, h0, _) in run.tiles]
     max_hits = run.h2c.numel()
-    d_hits = torch.empty((max_hits, 2), dtype=torch.float32, device="cuda")
-    d_off = torch.empty(run.tile_events + 1, dtype=torch.int32, device="cuda")
-    out_h2c = torch.empty(batch.n_hits, dtype=torch.int32).pin_memory()
-    out_off = torch.empty((len(run.tiles), run.tile_events + 1), dtype=torch.int32).pin_memory()
-    out_cands = torch.empty((run.cap, 32), dtype=torch.uint8).pin_memory()
-    out_nh = torch.empty(run.cap, dtype=torch.int32).pin_memory()
-    out_keep = torch.empty(run.cap, dtype=torch.uint8).pin_memory()
-    h2d = d2h = 0
+    pipe = HoughPipeline.from_workload(w, run.tile_events, max_hits, run.cap, n_streams)
+    total_cap = int(sum(min(int(t), run.cap) for t in run.totals.tolist())) + 1024
+    h_hits = torch.from_numpy(batch.hits_xy).pin_memory()
+    h_off = torch.from_numpy(batch.event_offsets.astype(np.int32)).pin_memory()
+    out_h2c = torch.empty(max(batch.n_hits, 1), dtype=torch.int32).pin_memory()
+    out_off = torch.empty(batch.n_events + 1, dtype=torch.int32).pin_memory()
+    out_cands = torch.empty((total_cap, 32), dtype=torch.uint8).pin_memory()
+    out_nh = torch.empty(total_cap, dtype=torch.int32).pin_memory()
+    out_keep = torch.empty(total_cap, dtype=torch.uint8).pin_memory()
 
-    def one_step(count: bool):
-        nonlocal h2d, d2h
-        for t, (e0, e1, h0, h1) in enumerate(run.tiles):
-            n_ev, n_h = e1 - e0, h1 - h0
-            d_hits[:n_h].copy_(h_hits[h0:h1], non_blocking=True)
-            d_off[:n_ev + 1].copy_(h_offs[t], non_blocking=True)
-            run.plan.vote(d_hits[:n_h], d_off[:n_ev + 1], run.accum)
-            run.plan.find_peaks(run.accum, n_ev, w.threshold, run.cands, run.cap, run.cand_off)
-            run.plan.assign_hits(d_hits[:n_h], d_off[:n_ev + 1], run.cands, run.cand_off, run.cap, w.assoc_dj,
-                                 w.min_hits, run.h2c[:max(n_h, 1)], run.nh, run.keep)
-            out_off[t, :n_ev + 1].copy_(run.cand_off[:n_ev + 1], non_blocking=True)
-            torch.cuda.current_stream().synchronize()           # the candidate count decides the copy sizes
-            n_c = min(int(out_off[t, n_ev]), run.cap)
-            out_h2c[h0:h1].copy_(run.h2c[:n_h], non_blocking=True)
-            out_cands[:n_c].copy_(run.cands[:n_c], non_blocking=True)
-            out_nh[:n_c].copy_(run.nh[:n_c], non_blocking=True)
-            out_keep[:n_c].copy_(run.keep[:n_c], non_blocking=True)
-            if count:
-                h2d += n_h * 8 + (n_ev + 1) * 4
-                d2h += (n_ev + 1) * 4 + n_h * 4 + n_c * (32 + 4 + 1)
-        torch.cuda.current_stream().synchronize()
+    def one_step():
+        return pipe.run_host(h_hits, h_off, w.threshold, w.assoc_dj, w.min_hits, out_h2c[:batch.n_hits], out_off, out_cands,
+                             total_cap, out_nh, out_keep)
 
-    for _ in range(warmup):
-        one_step(False)
+    for _ in range(max(warmup, 1)):
+        one_step()
     torch.cuda.synchronize()
-    a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
-    a.record()
+    t0 = time.perf_counter()
+    over = False
     for _ in range(steps):
-        one_step(True)
-    b.record()
+        over = one_step() or over
     torch.cuda.synchronize()
-    return a.elapsed_time(b) / steps, h2d // max(steps, 1), d2h // max(steps, 1)
+    ms = 1e3 * (time.perf_counter() - t0) / steps
+    n_c = int(out_off[batch.n_events])
+    h2d = batch.n_hits * 8 + (batch.n_events + len(run.tiles)) * 4
+    d2h = (batch.n_events + len(run.tiles)) * 4 + batch.n_hits * 4 + min(n_c, total_cap) * (32 + 4 + 1)
+    pipe.close()
+    return ms, h2d, d2h, over
 
 
 def run_ours(args, rank, world, local_rank):
@@ -365,17 +369,11 @@ def run_ours(args, rank, world, local_rank):
     peaks_overflow = bool((run.totals > run.cap).any().item())
 
     # max over ranks (device time), whole-job totals
-    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-    v = torch.tensor([float(votes_per_step), float(batch.n_events), float(batch.n_hits)], dtype=torch.float64,
-                     device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        dist.all_reduce(v, op=dist.ReduceOp.SUM)
-    ms_step = float(t.item()) / args.steps
-    job_votes, job_events, job_hits = (float(x) for x in v.tolist())
+    ms_job, (job_votes, job_events, job_hits) = reduce_job(ms_total, votes_per_step, batch.n_events, batch.n_hits, world, "cuda")
+    ms_step = ms_job / args.steps
 
     # e2e leg (host buffers in and out), same workload
-    e2e_ms, h2d, d2h = e2e_python(run, max(1, min(args.steps, args.e2e_steps)), 1)
+    e2e_ms, h2d, d2h, e2e_over = e2e_pipeline(run, max(1, min(args.steps, args.e2e_steps)), 1, args.streams)
     te = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
     if world > 1:
         dist.all_reduce(te, op=dist.ReduceOp.MAX)
@@ -430,7 +428,9 @@ def run_ours(args, rank, world, local_rank):
             "events_per_s": job_events / (ms_step * 1e-3), "hits_per_s": job_hits / (ms_step * 1e-3),
             "e2e": {"value": job_votes / (e2e_ms * 1e-3), "unit": UNIT, "events_per_s": job_events / (e2e_ms * 1e-3),
                     "ms_per_step": e2e_ms, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-                    "api": "HoughPlan.vote/find_peaks/assign_hits per event tile, pinned host buffers in and out"},
+                    "api": f"hough_pipeline_run_host: {run.tile_events}-event tiles on {args.streams} streams, CUDA graph per "
+                           "lane, pinned host buffers in and out; wall clock around the blocking call",
+                    "candidate_overflow": bool(e2e_over)},
             "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks,
             "candidate_overflow": peaks_overflow}
     print(json.dumps(line), flush=True)
@@ -449,6 +449,7 @@ def main():
     ap.add_argument("--tile-events", type=int, default=64)
     ap.add_argument("--cand-per-bin", type=float, default=1.0 / 16.0, help="candidate capacity per accumulator bin")
     ap.add_argument("--e2e-steps", type=int, default=2)
+    ap.add_argument("--streams", type=int, default=4, help="CUDA streams of the batched pipeline (B:L10: 4)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target oracle time of the cpu_baseline sample")
     ap.add_argument("--ref-seconds-per-step", type=float, default=10.0)
     ap.add_argument("--smem-atomic-gops", type=float, default=7593.0,

@@ -191,6 +191,60 @@ class HoughPlan:
                                           _stream_ptr(stream)), "hough_assign_hits")
 
 
+class HoughPipeline:
+    """hough_pipeline_create / hough_pipeline_run_host: the batched multi-event path over HOST buffers (pinned
+    torch CPU tensors in and out; event tiles on n_streams CUDA streams, each tile's sequence replayed as a CUDA graph)."""
+
+    def __init__(self, n_phi, n_qpt, n_d0, qpt_min=-1.0, qpt_max=1.0, d0_min=-20.0, d0_max=20.0,
+                 accum_dtype=HOUGH_ACC_I32, bz_tesla=3.8, layers=(), tile_events=64, max_hits_per_tile=1 << 20,
+                 tile_cand_capacity=1 << 20, n_streams=4):
+        self.lib = load_library()
+        if not torch.cuda.is_available():
+            raise HoughError("no CUDA device: libhough_b200 has no CPU fallback")
+        b, g, self._keep = make_structs(n_phi, n_qpt, n_d0, qpt_min, qpt_max, d0_min, d0_max, accum_dtype,
+                                        bz_tesla, layers)
+        h = C.c_void_p()
+        _check(self.lib.hough_pipeline_create(C.byref(b), C.byref(g), int(tile_events), int(max_hits_per_tile),
+                                              int(tile_cand_capacity), int(n_streams), C.byref(h)),
+               "hough_pipeline_create")
+        self._h = h
+
+    @classmethod
+    def from_workload(cls, w, tile_events, max_hits_per_tile, tile_cand_capacity, n_streams=4):
+        bn = w.binning
+        return cls(bn.n_phi, bn.n_qpt, bn.n_d0, bn.qpt_min, bn.qpt_max, bn.d0_min, bn.d0_max, bn.accum_dtype,
+                   w.bz_tesla, w.layers, tile_events, max_hits_per_tile, tile_cand_capacity, n_streams)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self.lib.hough_pipeline_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def run_host(self, hits_xy, event_offsets, threshold, assoc_dj, min_hits, hit_to_cand, cand_offsets, cands,
+                 cand_capacity, cand_nhits, cand_keep) -> bool:
+        """All tensors are HOST (CPU, ideally pinned) and contiguous: hits_xy float32 [n_hits, 2], event_offsets int32
+        [n_events + 1]; outputs hit_to_cand int32 [n_hits], cand_offsets int32 [n_events + 1], cands uint8
+        [cand_capacity, 32], cand_nhits int32 [cand_capacity], cand_keep uint8 [cand_capacity].  Blocks until the
+        results are in the host buffers.  Returns True if a candidate capacity was exceeded."""
+        for t in (hits_xy, event_offsets, hit_to_cand, cand_offsets, cands, cand_nhits, cand_keep):
+            assert (not t.is_cuda) and t.is_contiguous(), "host-resident contiguous tensor required"
+        assert hits_xy.dtype == torch.float32 and event_offsets.dtype == torch.int32
+        n_hits, n_events = int(hits_xy.shape[0]), int(event_offsets.shape[0]) - 1
+        over = C.c_int32(0)
+        _check(self.lib.hough_pipeline_run_host(self._h, hits_xy.data_ptr(), n_hits, event_offsets.data_ptr(), n_events,
+                                                int(threshold), int(assoc_dj), int(min_hits), hit_to_cand.data_ptr(),
+                                                cand_offsets.data_ptr(), cands.data_ptr(), int(cand_capacity),
+                                                cand_nhits.data_ptr(), cand_keep.data_ptr(), C.byref(over)),
+               "hough_pipeline_run_host")
+        return bool(over.value)
+
+
 def window_table(n_phi, n_qpt, n_d0, qpt_min=-1.0, qpt_max=1.0, d0_min=-20.0, d0_max=20.0, bz_tesla=3.8, layers=()):
     """hough_window_table (host only): (edge_r2 [n_class], lo_off [n_class, n_d0], steps [n_class, n_d0])."""
     lib = load_library()

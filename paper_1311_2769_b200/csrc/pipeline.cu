@@ -1,12 +1,263 @@
-// pipeline.cu -- A6: batched multi-event path (streams + CUDA graphs).  Placeholder until the tiled
-// kernels land: the entry points exist and report HOUGH_ERR_UNSUPPORTED.
+// pipeline.cu -- A6: batched multi-event path (B:L5 "a batched multi-event path using CUDA streams and graphs";
+// B:L10 "one accumulator per event, reused across event tiles on 4 CUDA streams").
+//
+// hough_pipeline_run_host cuts the events into tiles of `tile_events`, deals the tiles round-robin to `n_streams`
+// lanes (stream + plan + accumulator + device buffers of ONE tile) and, per tile, runs
+//     H2D hits, offsets -> hough_vote -> hough_find_peaks -> hough_assign_hits -> D2H per-event counts      (part A)
+//     [host: the tile's candidate base is the sum of the totals of all earlier tiles]
+//     rebase kernel (tile-local -> global event and candidate indices) -> D2H hit_to_cand, records, nhits, keep   (part B)
+// Part A of a lane is captured as a CUDA graph the first time and re-captured + cudaGraphExecUpdate'd for the
+// following tiles of that lane (same topology, other sizes), then launched with one cudaGraphLaunch.  Part B of tile
+// t is issued when tile t + n_streams is about to reuse the lane, so n_streams - 1 tiles are always in flight while
+// the host waits for a count.  Host buffers should be pinned (copies are cudaMemcpyAsync).
+#include <algorithm>
+#include <new>
+#include <vector>
+
 #include "common.cuh"
 
-struct hough_pipeline { int unused; };
+namespace {
 
-extern "C" int hough_pipeline_create(const hough_binning*, const hough_geometry*, int32_t, int32_t, int32_t, int32_t,
-                                     hough_pipeline**) { return HOUGH_ERR_UNSUPPORTED; }
-extern "C" int hough_pipeline_destroy(hough_pipeline*) { return HOUGH_ERR_UNSUPPORTED; }
-extern "C" int hough_pipeline_run_host(hough_pipeline*, const float*, int32_t, const int32_t*, int32_t, int32_t, int32_t,
-                                       int32_t, int32_t*, int32_t*, hough_candidate*, int32_t, int32_t*, uint8_t*,
-                                       int32_t*) { return HOUGH_ERR_UNSUPPORTED; }
+__global__ void __launch_bounds__(256) rebase_kernel(int32_t* __restrict__ hit_to_cand, int n_hits, int cand_base,
+                                                     hough_candidate* __restrict__ cands, int n_cands, int event_base) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t < n_hits) {
+        const int c = hit_to_cand[t];
+        if (c >= 0) hit_to_cand[t] = c + cand_base;
+    }
+    if (t < n_cands) cands[t].event += event_base;
+}
+
+struct Lane {
+    cudaStream_t st = nullptr;
+    hough_plan* plan = nullptr;
+    void* d_accum = nullptr;
+    float* d_hits = nullptr;
+    int32_t* d_off = nullptr;
+    hough_candidate* d_cands = nullptr;
+    int32_t* d_cand_off = nullptr;
+    int32_t* d_h2c = nullptr;
+    int32_t* d_nh = nullptr;
+    uint8_t* d_keep = nullptr;
+    int32_t* h_off = nullptr;        // pinned: tile-relative event offsets
+    int32_t* h_cand_off = nullptr;   // pinned: the tile's exclusive per-event candidate offsets
+    cudaEvent_t counted = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    bool warmed = false;             // first tile of a lane runs un-captured (lazy kernel attributes)
+    // tile in flight
+    int tile = -1, e0 = 0, e1 = 0, h0 = 0, h1 = 0;
+};
+
+}  // namespace
+
+struct hough_pipeline {
+    hough_binning b;
+    int32_t tile_events, max_hits, tile_cap, n_streams;
+    std::vector<Lane> lanes;
+    int use_graphs;
+};
+
+static void pipeline_free(hough_pipeline* p) {
+    if (!p) return;
+    for (Lane& l : p->lanes) {
+        if (l.exec) cudaGraphExecDestroy(l.exec);
+        if (l.counted) cudaEventDestroy(l.counted);
+        if (l.plan) hough_plan_destroy(l.plan);
+        cudaFree(l.d_accum); cudaFree(l.d_hits); cudaFree(l.d_off); cudaFree(l.d_cands); cudaFree(l.d_cand_off);
+        cudaFree(l.d_h2c); cudaFree(l.d_nh); cudaFree(l.d_keep);
+        if (l.h_off) cudaFreeHost(l.h_off);
+        if (l.h_cand_off) cudaFreeHost(l.h_cand_off);
+        if (l.st) cudaStreamDestroy(l.st);
+    }
+    delete p;
+}
+
+extern "C" int hough_pipeline_create(const hough_binning* b, const hough_geometry* g, int32_t tile_events,
+                                     int32_t max_hits_per_tile, int32_t tile_cand_capacity, int32_t n_streams,
+                                     hough_pipeline** out) {
+    if (!b || !g || !out) return HOUGH_ERR_INVALID_ARG;
+    if (tile_events <= 0 || max_hits_per_tile <= 0 || tile_cand_capacity < 0 || n_streams <= 0 || n_streams > 64)
+        return HOUGH_ERR_INVALID_ARG;
+    hough_pipeline* p = new (std::nothrow) hough_pipeline();
+    if (!p) return HOUGH_ERR_ALLOC;
+    p->b = *b;
+    p->tile_events = tile_events;
+    p->max_hits = max_hits_per_tile;
+    p->tile_cap = tile_cand_capacity;
+    p->n_streams = n_streams;
+    const char* env = getenv("HOUGH_PIPELINE_NO_GRAPHS");
+    p->use_graphs = (env && env[0] == '1') ? 0 : 1;
+    p->lanes.resize(n_streams);
+    int rc = HOUGH_OK;
+    for (Lane& l : p->lanes) {
+        rc = hough_plan_create(b, g, max_hits_per_tile, tile_events, &l.plan);
+        if (rc != HOUGH_OK) break;
+        bool ok = cudaStreamCreateWithFlags(&l.st, cudaStreamNonBlocking) == cudaSuccess;
+        ok = ok && cudaEventCreateWithFlags(&l.counted, cudaEventDisableTiming) == cudaSuccess;
+        const size_t cap = (size_t)std::max(tile_cand_capacity, 1);
+        ok = ok && cudaMalloc(&l.d_accum, hough_accum_bytes(l.plan, tile_events)) == cudaSuccess;
+        ok = ok && cudaMalloc((void**)&l.d_hits, sizeof(float) * 2 * (size_t)max_hits_per_tile) == cudaSuccess;
+        ok = ok && cudaMalloc((void**)&l.d_off, sizeof(int32_t) * ((size_t)tile_events + 1)) == cudaSuccess;
+        ok = ok && cudaMalloc((void**)&l.d_cands, sizeof(hough_candidate) * cap) == cudaSuccess;
+        ok = ok && cudaMalloc((void**)&l.d_cand_off, sizeof(int32_t) * ((size_t)tile_events + 1)) == cudaSuccess;
+        ok = ok && cudaMalloc((void**)&l.d_h2c, sizeof(int32_t) * (size_t)max_hits_per_tile) == cudaSuccess;
+        ok = ok && cudaMalloc((void**)&l.d_nh, sizeof(int32_t) * cap) == cudaSuccess;
+        ok = ok && cudaMalloc((void**)&l.d_keep, cap) == cudaSuccess;
+        ok = ok && cudaMallocHost((void**)&l.h_off, sizeof(int32_t) * ((size_t)tile_events + 1)) == cudaSuccess;
+        ok = ok && cudaMallocHost((void**)&l.h_cand_off, sizeof(int32_t) * ((size_t)tile_events + 1)) == cudaSuccess;
+        if (!ok) { (void)cudaGetLastError(); rc = HOUGH_ERR_ALLOC; break; }
+    }
+    if (rc != HOUGH_OK) { pipeline_free(p); return rc; }
+    *out = p;
+    return HOUGH_OK;
+}
+
+extern "C" int hough_pipeline_destroy(hough_pipeline* p) {
+    if (!p) return HOUGH_ERR_INVALID_ARG;
+    pipeline_free(p);
+    return HOUGH_OK;
+}
+
+// part A of one tile on its lane's stream: copies in, the three calls, counts out
+static int enqueue_part_a(hough_pipeline* p, Lane& l, const float* h_hits_xy, int32_t threshold, int32_t assoc_dj,
+                          int32_t min_hits) {
+    const int n_ev = l.e1 - l.e0, n_h = l.h1 - l.h0;
+    if (n_h > 0)
+        HOUGH_CUDA_TRY(cudaMemcpyAsync(l.d_hits, h_hits_xy + 2 * (size_t)l.h0, sizeof(float) * 2 * (size_t)n_h,
+                                       cudaMemcpyHostToDevice, l.st));
+    HOUGH_CUDA_TRY(cudaMemcpyAsync(l.d_off, l.h_off, sizeof(int32_t) * ((size_t)n_ev + 1), cudaMemcpyHostToDevice, l.st));
+    int rc = hough_vote(l.plan, l.d_hits, n_h, l.d_off, n_ev, l.d_accum, l.st);
+    if (rc != HOUGH_OK) return rc;
+    rc = hough_find_peaks(l.plan, l.d_accum, n_ev, threshold, p->tile_cap > 0 ? l.d_cands : nullptr, p->tile_cap, l.d_cand_off,
+                          l.st);
+    if (rc != HOUGH_OK) return rc;
+    rc = hough_assign_hits(l.plan, l.d_hits, n_h, l.d_off, n_ev, l.d_cands, l.d_cand_off, p->tile_cap, assoc_dj, min_hits,
+                           l.d_h2c, l.d_nh, l.d_keep, l.st);
+    if (rc != HOUGH_OK) return rc;
+    HOUGH_CUDA_TRY(cudaMemcpyAsync(l.h_cand_off, l.d_cand_off, sizeof(int32_t) * ((size_t)n_ev + 1), cudaMemcpyDeviceToHost,
+                                   l.st));
+    return HOUGH_OK;
+}
+
+static int launch_part_a(hough_pipeline* p, Lane& l, const float* h_hits_xy, int32_t threshold, int32_t assoc_dj,
+                         int32_t min_hits) {
+    if (!p->use_graphs || !l.warmed) {
+        l.warmed = true;
+        return enqueue_part_a(p, l, h_hits_xy, threshold, assoc_dj, min_hits);
+    }
+    // capture the tile's sequence, then update the lane's executable graph in place (same topology, other sizes)
+    HOUGH_CUDA_TRY(cudaStreamBeginCapture(l.st, cudaStreamCaptureModeThreadLocal));
+    const int rc = enqueue_part_a(p, l, h_hits_xy, threshold, assoc_dj, min_hits);
+    cudaGraph_t graph = nullptr;
+    const cudaError_t ce = cudaStreamEndCapture(l.st, &graph);
+    if (rc != HOUGH_OK || ce != cudaSuccess || !graph) {
+        if (graph) cudaGraphDestroy(graph);
+        (void)cudaGetLastError();
+        if (rc != HOUGH_OK) return rc;
+        p->use_graphs = 0;                               // capture not possible here: plain launches from now on
+        return enqueue_part_a(p, l, h_hits_xy, threshold, assoc_dj, min_hits);
+    }
+    bool ready = false;
+    if (l.exec) {
+        cudaGraphExecUpdateResultInfo info;
+        if (cudaGraphExecUpdate(l.exec, graph, &info) == cudaSuccess) ready = true;
+        else { (void)cudaGetLastError(); cudaGraphExecDestroy(l.exec); l.exec = nullptr; }
+    }
+    if (!ready) {
+        if (cudaGraphInstantiate(&l.exec, graph, 0) != cudaSuccess) {
+            hough_set_last_cuda_error(cudaGetLastError(), "cudaGraphInstantiate");
+            cudaGraphDestroy(graph);
+            return HOUGH_ERR_CUDA;
+        }
+    }
+    cudaGraphDestroy(graph);
+    HOUGH_CUDA_TRY(cudaGraphLaunch(l.exec, l.st));
+    return HOUGH_OK;
+}
+
+extern "C" int hough_pipeline_run_host(hough_pipeline* p, const float* h_hits_xy, int32_t n_hits,
+                                       const int32_t* h_event_offsets, int32_t n_events, int32_t threshold,
+                                       int32_t assoc_dj, int32_t min_hits, int32_t* h_hit_to_cand,
+                                       int32_t* h_cand_offsets, hough_candidate* h_cands, int32_t cand_capacity,
+                                       int32_t* h_cand_nhits, uint8_t* h_cand_keep, int32_t* h_overflowed) {
+    if (!p || !h_event_offsets || !h_cand_offsets) return HOUGH_ERR_INVALID_ARG;
+    if (n_hits < 0 || n_events < 0 || cand_capacity < 0 || assoc_dj < 0 || assoc_dj > 15) return HOUGH_ERR_INVALID_ARG;
+    if (n_hits > 0 && (!h_hits_xy || !h_hit_to_cand)) return HOUGH_ERR_INVALID_ARG;
+    if (cand_capacity > 0 && (!h_cands || !h_cand_nhits || !h_cand_keep)) return HOUGH_ERR_INVALID_ARG;
+    if (h_event_offsets[0] != 0 || h_event_offsets[n_events] != n_hits) return HOUGH_ERR_INVALID_ARG;
+    if (h_overflowed) *h_overflowed = 0;
+    h_cand_offsets[0] = 0;
+    const int n_tiles = (n_events + p->tile_events - 1) / p->tile_events;
+    const int S = p->n_streams;
+    long long cand_base = 0;                             // global rank of the first candidate of the tile being finished
+    int status = HOUGH_OK;
+
+    // part B of the tile that lane `l` carries: wait for its counts, rebase on the device, copy the results out
+    auto finish = [&](Lane& l) -> int {
+        if (l.tile < 0) return HOUGH_OK;
+        HOUGH_CUDA_TRY(cudaEventSynchronize(l.counted));
+        const int n_ev = l.e1 - l.e0, n_h = l.h1 - l.h0;
+        const int total = l.h_cand_off[n_ev];
+        const int n_c = std::min(total, p->tile_cap);
+        if (total > p->tile_cap && h_overflowed) *h_overflowed = 1;
+        for (int i = 1; i <= n_ev; ++i)
+            h_cand_offsets[l.e0 + i] = (int32_t)std::min<long long>(cand_base + l.h_cand_off[i], 0x7fffffffLL);
+        // records that fit the caller's capacity
+        const long long room = std::max<long long>(0, (long long)cand_capacity - cand_base);
+        const int n_out = (int)std::min<long long>(n_c, room);
+        if (n_c > n_out && h_overflowed) *h_overflowed = 1;
+        const int n_thr = std::max(n_h, n_c);
+        if (n_thr > 0) {
+            rebase_kernel<<<(n_thr + 255) / 256, 256, 0, l.st>>>(l.d_h2c, n_h, (int)std::min<long long>(cand_base, 0x7fffffffLL),
+                                                                l.d_cands, n_c, l.e0);
+            HOUGH_CUDA_TRY(cudaGetLastError());
+            hough_count_launches(1);
+        }
+        if (n_h > 0)
+            HOUGH_CUDA_TRY(cudaMemcpyAsync(h_hit_to_cand + l.h0, l.d_h2c, sizeof(int32_t) * (size_t)n_h, cudaMemcpyDeviceToHost, l.st));
+        if (n_out > 0) {
+            HOUGH_CUDA_TRY(cudaMemcpyAsync(h_cands + cand_base, l.d_cands, sizeof(hough_candidate) * (size_t)n_out,
+                                           cudaMemcpyDeviceToHost, l.st));
+            HOUGH_CUDA_TRY(cudaMemcpyAsync(h_cand_nhits + cand_base, l.d_nh, sizeof(int32_t) * (size_t)n_out, cudaMemcpyDeviceToHost, l.st));
+            HOUGH_CUDA_TRY(cudaMemcpyAsync(h_cand_keep + cand_base, l.d_keep, (size_t)n_out, cudaMemcpyDeviceToHost, l.st));
+        }
+        cand_base += total;
+        l.tile = -1;
+        return HOUGH_OK;
+    };
+
+    for (int t = 0; t < n_tiles && status == HOUGH_OK; ++t) {
+        Lane& l = p->lanes[t % S];
+        status = finish(l);                              // the lane's previous tile (t - S)
+        if (status != HOUGH_OK) break;
+        l.tile = t;
+        l.e0 = t * p->tile_events;
+        l.e1 = std::min(n_events, l.e0 + p->tile_events);
+        l.h0 = h_event_offsets[l.e0];
+        l.h1 = h_event_offsets[l.e1];
+        if (l.h1 - l.h0 > p->max_hits || l.h1 < l.h0) { status = HOUGH_ERR_INVALID_ARG; l.tile = -1; break; }
+        // the lane's pinned offset buffer is free: the previous H2D from it completed before `counted`
+        for (int i = 0; i <= l.e1 - l.e0; ++i) l.h_off[i] = h_event_offsets[l.e0 + i] - l.h0;
+        status = launch_part_a(p, l, h_hits_xy, threshold, assoc_dj, min_hits);
+        if (status != HOUGH_OK) break;
+        if (cudaEventRecord(l.counted, l.st) != cudaSuccess) { status = HOUGH_ERR_CUDA; break; }
+    }
+    // drain: tiles still in flight, in tile order
+    if (status == HOUGH_OK) {
+        std::vector<Lane*> order;
+        for (Lane& l : p->lanes) if (l.tile >= 0) order.push_back(&l);
+        std::sort(order.begin(), order.end(), [](const Lane* a, const Lane* b) { return a->tile < b->tile; });
+        for (Lane* l : order) {
+            status = finish(*l);
+            if (status != HOUGH_OK) break;
+        }
+    }
+    for (Lane& l : p->lanes) {
+        if (cudaStreamSynchronize(l.st) != cudaSuccess && status == HOUGH_OK) {
+            hough_set_last_cuda_error(cudaGetLastError(), "cudaStreamSynchronize");
+            status = HOUGH_ERR_CUDA;
+        }
+        l.tile = -1;
+    }
+    return status;
+}
