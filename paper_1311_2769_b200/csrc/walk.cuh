@@ -211,15 +211,21 @@ __device__ __forceinline__ unsigned fast_slot(const FastK& fk, const FastHit& h,
 template <bool TILE32> struct EntryT {               // 16-bit entries: 11 bits of votes + 1
     static constexpr unsigned VSAT = 2047u;
     typedef unsigned pkey_t;
+    static constexpr unsigned CINV0 = 0xffffu;
     static __device__ __forceinline__ pkey_t pkey(unsigned ent, int col) { return ((ent >> 1) << 16) | (unsigned)(0xffff - col); }
+    static __device__ __forceinline__ pkey_t pkey_inv(unsigned ent, unsigned cinv) { return ((ent << 15) & 0xffff0000u) | cinv; }
     static __device__ __forceinline__ int col_of(pkey_t p) { return 0xffff - (int)(p & 0xffffu); }
     static __device__ __forceinline__ unsigned ent_hi(pkey_t p) { return p >> 16; }
 };
 template <> struct EntryT<true> {                    // 32-bit entries: 27 bits of votes + 1
     static constexpr unsigned VSAT = (1u << 27) - 1u;
     typedef unsigned long long pkey_t;
+    static constexpr unsigned CINV0 = 0x7fffffffu;
     static __device__ __forceinline__ pkey_t pkey(unsigned ent, int col) {
         return ((unsigned long long)(ent >> 1) << 32) | (unsigned)(0x7fffffff - col);
+    }
+    static __device__ __forceinline__ pkey_t pkey_inv(unsigned ent, unsigned cinv) {
+        return ((unsigned long long)(ent >> 1) << 32) | cinv;
     }
     static __device__ __forceinline__ int col_of(pkey_t p) { return 0x7fffffff - (int)(unsigned)(p & 0xffffffffull); }
     static __device__ __forceinline__ unsigned ent_hi(pkey_t p) { return (unsigned)(p >> 32); }
@@ -305,6 +311,32 @@ __device__ __noinline__ void walk_redo_pair(const HoughConsts& c, const FastK& f
         if (j >= 0)
             walk_apply<MODE, TILE32>(tl.s_tile, tl.stride, c.n_qpt, cc + w, j, tl.legacy, a.assoc_dj, a.cands, tl.cand_first,
                                      tl.cand_end, tl.c0, tl.row_lin0, best);
+    }
+    if (MODE == WALK_ASSIGN && best) atomicMax(a.best_key + __float_as_int(hv.w), best);
+}
+
+// The exact D3 sequence at every column of one hit's window (classes without a usable fast-path bound, the plan option
+// "exact_walk", saturated association tiles).  Out of line: keeps the hot loop's register budget.
+template <int MODE, bool TILE32>
+__device__ __noinline__ void walk_exact_window(const HoughConsts& c, float4 d, const WalkArgs& a, const WalkTile& tl, int sidx,
+                                               int i_lo, int steps, int cols) {
+    const float4 hv = __ldg(a.staged + sidx);
+    const float r2 = d3_r2(hv.x, hv.y);
+    const int nphi = c.n_phi;
+    unsigned long long best = 0ull;
+    int col = i_lo - tl.c0;                              // column relative to the tile, cyclic
+    if (col < 0) col += nphi;
+    for (int t = 0; t < steps; ++t) {
+        if (col < cols) {
+            const float4 T = tl.s_pair[col >> 1];
+            const int j = d3_exact_bin(hv.x, hv.y, r2, (col & 1) ? T.y : T.x, (col & 1) ? T.w : T.z, d.x, d.y, d.z, c.A_f, c.qmin,
+                                       c.inv_wq, c.nq_f);
+            if (j >= 0)
+                walk_apply<MODE, TILE32>(tl.s_tile, tl.stride, c.n_qpt, col, j, tl.legacy, a.assoc_dj, a.cands, tl.cand_first,
+                                         tl.cand_end, tl.c0, tl.row_lin0, best);
+        }
+        ++col;
+        if (col == nphi) col = 0;
     }
     if (MODE == WALK_ASSIGN && best) atomicMax(a.best_key + __float_as_int(hv.w), best);
 }
@@ -540,30 +572,13 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
         if (i_lo >= nphi) i_lo -= nphi;
         if (!(i_lo >= 0 && i_lo < nphi)) i_lo = 0;
 
-        unsigned long long best = 0ull;                  // association: full D8 key from the exact path
         // dilated association: (entry >> 1) above ~column (equal votes and |dj| in two columns: the smaller linear
-        // bin wins, D8); the entry's sign bit travels with the q/pT bin in bestj
+        // bin wins, D8)
         typename EntryT<TILE32>::pkey_t bestp = 0;
-        int bestj = 0;
 
         if (!(hm_c > 0.0f)) {
             // ---- exact D3 sequence at every column of the window: classes without a usable bound ----
-            if (active) {
-                int col = i_lo - c0;                     // column relative to the tile, cyclic
-                if (col < 0) col += nphi;
-                for (int t = 0; t < steps; ++t) {
-                    if (col < cols) {
-                        const float4 T = s_pair[col >> 1];
-                        const int j = d3_exact_bin(x, y, r2, (col & 1) ? T.y : T.x, (col & 1) ? T.w : T.z, d.x, d.y, d.z, c.A_f,
-                                                   c.qmin, c.inv_wq, c.nq_f);
-                        if (j >= 0)
-                            walk_apply<MODE, TILE32>(s_tile, stride, nq, col, j, legacy, a.assoc_dj, a.cands, cand_first, cand_end,
-                                                     c0, row_lin0, best);
-                    }
-                    ++col;
-                    if (col == nphi) col = 0;
-                }
-            }
+            if (active) walk_exact_window<MODE, TILE32>(c, d, a, tl, sidx, i_lo, steps, cols);
         } else {
             // ---- fast path: the lane's window, two columns at a time ----
             const FastHit fh = make_fasthit(fk, x, y, r2);
@@ -601,7 +616,7 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
                 const float4* pp = s_pair + (col >> 1);
                 unsigned rowaddr = tile_saddr + (TILE32 ? (unsigned)col * stride4 : (unsigned)(col >> 1) * stride4);
                 const int wrap_t = FULLPHI ? ((nphi - col) >> 1) : 0x7fffffff;   // pair of the chunk at which the lane wraps
-                int colp = col;                          // association: running tile column of the pair
+                unsigned cinv = EntryT<TILE32>::CINV0 - (unsigned)col;   // association: ~(running tile column of the pair)
                 unsigned slowmask = 0u;                  // bit (np - 1 - t): pair t of the chunk is uncertain
                 // One chunk of column pairs; WRAP: some lane of the warp passes column n_phi - 1 inside the chunk.
                 // The vote is unconditional: slot min(h, nq + 2 + dump) of the column's row (results outside [-1, nq]
@@ -611,7 +626,7 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
                     constexpr bool WRAP = decltype(wrap_c)::value;
 #pragma unroll 2
                     for (int t = 0; t < np; ++t) {
-                        if (WRAP && t == wrap_t) { rowaddr -= tile_bytes; colp -= nphi; }
+                        if (WRAP && t == wrap_t) { rowaddr -= tile_bytes; cinv += (unsigned)nphi; }
                         const float4 T = *pp++;          // {cosA, cosB, sinA, sinB}
                         const f32x2 C2 = pk2(T.x, T.y), S2 = pk2(T.z, T.w);
                         const f32x2 g2 = fma2(gx2, S2, fma2(gy2, C2, r2Ak2));
@@ -640,15 +655,15 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
                             red_shared(adA, 1u);
                             red_shared(adB, TILE32 ? 1u : 65536u);
                         } else {
+                            // best (entry >> 1, ~column) of the lane; the q/pT bin and the entry's sign bit are recovered
+                            // after the loop by re-evaluating the winning column (fast_slot)
                             const unsigned entA = TILE32 ? lds_u32(adA) : lds_u16(adA);
                             const unsigned entB = TILE32 ? lds_u32(adB) : lds_u16(adB + 2u);
-                            const typename EntryT<TILE32>::pkey_t pA = EntryT<TILE32>::pkey(entA, colp);
-                            const typename EntryT<TILE32>::pkey_t pB = EntryT<TILE32>::pkey(entB, colp + 1);
-                            if (!uns) {                  // flagged pairs are probed by the redo
-                                if (pA > bestp) { bestp = pA; bestj = ((int)(hA - 1u) << 1) | (int)(entA & 1u); }
-                                if (pB > bestp) { bestp = pB; bestj = ((int)(hB - 1u) << 1) | (int)(entB & 1u); }
-                            }
-                            colp += 2;
+                            const typename EntryT<TILE32>::pkey_t pA = EntryT<TILE32>::pkey_inv(entA, cinv);
+                            const typename EntryT<TILE32>::pkey_t pB = EntryT<TILE32>::pkey_inv(entB, cinv - 1u);
+                            const typename EntryT<TILE32>::pkey_t pm = pA > pB ? pA : pB;      // ties: the smaller column
+                            if (!uns && pm > bestp) bestp = pm;      // flagged pairs are probed by the redo
+                            cinv -= 2u;
                         }
                         slowmask = slowmask * 2u + (uns ? 1u : 0u);
                         rowaddr += TILE32 ? 2u * stride4 : stride4;
@@ -683,13 +698,17 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
         if (MODE == WALK_ASSIGN) {
             const unsigned eh = EntryT<TILE32>::ent_hi(bestp);          // entry >> 1: votes + 1 above (15 - |dj|)
             if (eh >> 4) {
+                // the winning column's slot again (an unflagged pair: the fast slot IS the D3 bin), then the full entry
+                const float4 hw = __ldg(a.staged + sidx);
                 const int bcol = EntryT<TILE32>::col_of(bestp);
-                const int adj = 15 - (int)(eh & 15u);
-                const int jc = (bestj >> 1) + ((bestj & 1) ? -adj : adj);
-                const unsigned long long key = walk_key((eh >> 4) - 1u, adj, row_lin0 + (unsigned)(bcol * nq + jc));
-                best = key > best ? key : best;
+                const float4 T = s_pair[bcol >> 1];
+                const FastHit fh = make_fasthit(fk, hw.x, hw.y, d3_r2(hw.x, hw.y));
+                const int J = (int)fast_slot(fk, fh, (bcol & 1) ? T.y : T.x, (bcol & 1) ? T.w : T.z) - 1;
+                const unsigned ent = tile_entry<TILE32>(s_tile, stride, bcol, J);
+                const int adj = 15 - (int)((ent >> 1) & 15u);
+                const int jc = J + ((ent & 1u) ? -adj : adj);
+                atomicMax(a.best_key + __float_as_int(hw.w), walk_key((ent >> 5) - 1u, adj, row_lin0 + (unsigned)(bcol * nq + jc)));
             }
-            if (best) atomicMax(a.best_key + __float_as_int(hv.w), best);
         }
     }
     if (wq_n > 0) walk_drain<MODE, TILE32>(c, fk, d, a, tl, wq, wq_n, ev_begin, lane);
