@@ -234,6 +234,7 @@ class DeviceRun:
             self.tiles.append((e0, e1, int(off[e0]), int(off[e1])))
         max_hits = max(h1 - h0 for (_, _, h0, h1) in self.tiles)
         self.plan = HoughPlan.from_workload(w, max_hits=max(max_hits, 1), max_events=self.tile_events)
+        self.plan.set_option("reuse_staging", 1)     # vote and assign_hits of a tile get the same device hits (include/hough.h)
         self.d_hits = torch.from_numpy(batch.hits_xy).cuda()
         # per-tile offsets are relative to the tile's first hit
         self.d_offs = []
@@ -280,16 +281,20 @@ class DeviceRun:
         return total
 
 
-def e2e_pipeline(run: DeviceRun, steps: int, warmup: int, n_streams: int):
+def e2e_pipeline(run: DeviceRun, steps: int, warmup: int, n_streams: int, tile_events: int, cand_per_bin: float):
     """End-to-end through the library's batched path (hough_pipeline_run_host): pinned HOST buffers in (hits, offsets)
     and out (hit_to_cand, cand_offsets, candidate records, nhits, keep); every host<->device copy is inside the
     timed region.  Wall-clock around the blocking call (it returns when the results are in the host buffers)."""
     torch = run.torch
     from paper_1311_2769_b200 import HoughPipeline
     w, batch = run.w, run.batch
-    max_hits = run.h2c.numel()
-    pipe = HoughPipeline.from_workload(w, run.tile_events, max_hits, run.cap, n_streams)
-    total_cap = int(sum(min(int(t), run.cap) for t in run.totals.tolist())) + 1024
+    tile_events = max(1, min(tile_events, batch.n_events))
+    off = batch.event_offsets.astype(np.int64)
+    n_tiles = (batch.n_events + tile_events - 1) // tile_events
+    max_hits = max(int(off[min(e0 + tile_events, batch.n_events)] - off[e0]) for e0 in range(0, batch.n_events, tile_events))
+    tile_cap = int(cand_per_bin * w.binning.n_bins * tile_events) + 1024
+    pipe = HoughPipeline.from_workload(w, tile_events, max(max_hits, 1), tile_cap, n_streams)
+    total_cap = int(sum(int(t) for t in run.totals.tolist())) + 1024
     h_hits = torch.from_numpy(batch.hits_xy).pin_memory()
     h_off = torch.from_numpy(batch.event_offsets.astype(np.int32)).pin_memory()
     out_h2c = torch.empty(max(batch.n_hits, 1), dtype=torch.int32).pin_memory()
@@ -312,8 +317,8 @@ def e2e_pipeline(run: DeviceRun, steps: int, warmup: int, n_streams: int):
     torch.cuda.synchronize()
     ms = 1e3 * (time.perf_counter() - t0) / steps
     n_c = int(out_off[batch.n_events])
-    h2d = batch.n_hits * 8 + (batch.n_events + len(run.tiles)) * 4
-    d2h = (batch.n_events + len(run.tiles)) * 4 + batch.n_hits * 4 + min(n_c, total_cap) * (32 + 4 + 1)
+    h2d = batch.n_hits * 8 + (batch.n_events + n_tiles) * 4
+    d2h = (batch.n_events + n_tiles) * 4 + batch.n_hits * 4 + min(n_c, total_cap) * (32 + 4 + 1)
     pipe.close()
     return ms, h2d, d2h, over
 
@@ -373,7 +378,8 @@ def run_ours(args, rank, world, local_rank):
     ms_step = ms_job / args.steps
 
     # e2e leg (host buffers in and out), same workload
-    e2e_ms, h2d, d2h, e2e_over = e2e_pipeline(run, max(1, min(args.steps, args.e2e_steps)), 1, args.streams)
+    e2e_ms, h2d, d2h, e2e_over = e2e_pipeline(run, max(1, min(args.steps, args.e2e_steps)), 1, args.streams, args.e2e_tile_events,
+                                                args.cand_per_bin)
     te = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
     if world > 1:
         dist.all_reduce(te, op=dist.ReduceOp.MAX)
@@ -428,7 +434,7 @@ def run_ours(args, rank, world, local_rank):
             "events_per_s": job_events / (ms_step * 1e-3), "hits_per_s": job_hits / (ms_step * 1e-3),
             "e2e": {"value": job_votes / (e2e_ms * 1e-3), "unit": UNIT, "events_per_s": job_events / (e2e_ms * 1e-3),
                     "ms_per_step": e2e_ms, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-                    "api": f"hough_pipeline_run_host: {run.tile_events}-event tiles on {args.streams} streams, CUDA graph per "
+                    "api": f"hough_pipeline_run_host: {min(args.e2e_tile_events, batch.n_events)}-event tiles on {args.streams} streams, CUDA graph per "
                            "lane, pinned host buffers in and out; wall clock around the blocking call",
                     "candidate_overflow": bool(e2e_over)},
             "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks,
@@ -446,7 +452,8 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--events", type=int, default=0, help="events per GPU (default: the workload's own count)")
-    ap.add_argument("--tile-events", type=int, default=64)
+    ap.add_argument("--tile-events", type=int, default=128, help="events per call of the device-resident loop")
+    ap.add_argument("--e2e-tile-events", type=int, default=32, help="events per tile of the batched host pipeline")
     ap.add_argument("--cand-per-bin", type=float, default=1.0 / 16.0, help="candidate capacity per accumulator bin")
     ap.add_argument("--e2e-steps", type=int, default=2)
     ap.add_argument("--streams", type=int, default=4, help="CUDA streams of the batched pipeline (B:L10: 4)")

@@ -191,7 +191,7 @@ extern "C" int hough_assign_hits(hough_plan* p, const float* d_hits_xy, int32_t 
     if (n_hits > 0) HOUGH_CUDA_TRY(cudaMemsetAsync(p->d_best_key, 0, sizeof(unsigned long long) * (size_t)n_hits, st));
     if (tiled) {
         if (n_hits > 0 && capacity > 0) {
-            int rc = hough_stage_hits(p, d_hits_xy, n_hits, d_event_offsets, n_events, st);
+            int rc = hough_stage_hits(p, d_hits_xy, n_hits, d_event_offsets, n_events, st, true);
             if (rc != HOUGH_OK) return rc;
             WalkArgs a{};
             a.staged = p->d_staged;

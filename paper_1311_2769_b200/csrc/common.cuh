@@ -63,6 +63,8 @@ struct hough_plan {
     int fullscan;
     int peaks_tiled;                   // 1: find_peaks uses the shared-memory halo-tile kernels instead of the slice walk
     int exact_walk;                    // 1: the walks evaluate the D3 sequence at every column (no fast path)
+    int reuse_staging;                 // 1: hough_assign_hits may reuse the staging of the preceding hough_vote (same arguments)
+    const void* staged_hits; const void* staged_off; int32_t staged_n_hits, staged_n_events; cudaStream_t staged_stream;
     HoughConsts c;
     // geometry (work sizing only)
     int32_t n_layers;
@@ -156,7 +158,7 @@ __device__ __forceinline__ void cta_exclusive_scan(int32_t* data, int n, int32_t
 
 // internal entry points (defined in the .cu files)
 int hough_stage_hits(hough_plan* p, const float* d_hits_xy, int32_t n_hits, const int32_t* d_event_offsets,
-                     int32_t n_events, cudaStream_t st);
+                     int32_t n_events, cudaStream_t st, bool may_reuse);
 int hough_vote_fullscan(hough_plan* p, const float* d_hits_xy, int32_t n_hits, const int32_t* d_event_offsets,
                         int32_t n_events, void* d_accum, cudaStream_t st);
 int hough_vote_tiled(hough_plan* p, const float* d_hits_xy, int32_t n_hits, const int32_t* d_event_offsets,

@@ -92,6 +92,7 @@ extern "C" int hough_pipeline_create(const hough_binning* b, const hough_geometr
     for (Lane& l : p->lanes) {
         rc = hough_plan_create(b, g, max_hits_per_tile, tile_events, &l.plan);
         if (rc != HOUGH_OK) break;
+        hough_plan_set_option(l.plan, "reuse_staging", 1);   // vote and assign of a tile see the same device hits
         bool ok = cudaStreamCreateWithFlags(&l.st, cudaStreamNonBlocking) == cudaSuccess;
         ok = ok && cudaEventCreateWithFlags(&l.counted, cudaEventDisableTiming) == cudaSuccess;
         const size_t cap = (size_t)std::max(tile_cand_capacity, 1);

@@ -98,7 +98,16 @@ __global__ void __launch_bounds__(256) stage_scatter_kernel(HoughConsts c, const
 }  // namespace
 
 int hough_stage_hits(hough_plan* p, const float* d_hits_xy, int32_t n_hits, const int32_t* d_event_offsets,
-                     int32_t n_events, cudaStream_t st) {
+                     int32_t n_events, cudaStream_t st, bool may_reuse) {
+    // plan option "reuse_staging": the caller promises that a call with the same pointers, sizes and stream sees the
+    // same hits as the previous one (vote followed by assign_hits of one tile), so the staged copy is still valid
+    if (may_reuse && p->reuse_staging && p->staged_hits == d_hits_xy && p->staged_off == d_event_offsets && p->staged_n_hits == n_hits &&
+        p->staged_n_events == n_events && p->staged_stream == st) {
+        p->staged_hits = nullptr;                        // one reuse per staging
+        return HOUGH_OK;
+    }
+    p->staged_hits = d_hits_xy; p->staged_off = d_event_offsets; p->staged_n_hits = n_hits; p->staged_n_events = n_events;
+    p->staged_stream = st;
     const size_t cnt_bytes = sizeof(int32_t) * (size_t)n_events * (p->c.n_keys + 1);
     HOUGH_CUDA_TRY(cudaMemsetAsync(p->d_stage_cnt, 0, cnt_bytes, st));
     if (n_hits > 0) {

@@ -67,7 +67,7 @@ int hough_vote_fullscan(hough_plan* p, const float* d_hits_xy, int32_t n_hits, c
 int hough_vote_tiled(hough_plan* p, const float* d_hits_xy, int32_t n_hits, const int32_t* d_event_offsets,
                      int32_t n_events, void* d_accum, cudaStream_t st) {
     if (p->tile_max_cols < 1) return hough_vote_fullscan(p, d_hits_xy, n_hits, d_event_offsets, n_events, d_accum, st);
-    const int rc = hough_stage_hits(p, d_hits_xy, n_hits, d_event_offsets, n_events, st);
+    const int rc = hough_stage_hits(p, d_hits_xy, n_hits, d_event_offsets, n_events, st, false);
     if (rc != HOUGH_OK) return rc;
     WalkArgs a{};
     a.staged = p->d_staged;
