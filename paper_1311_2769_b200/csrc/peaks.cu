@@ -9,6 +9,8 @@
 //                                       ascending (event, k, i, j) order for rank < capacity
 // Generic path (a block that spans two d0 slices, or rows too long for the tile): per-bin global loads,
 //   peak_mask_kernel (1 bit per bin + per-block count) and peak_emit_kernel (per mask word).
+#include <type_traits>
+
 #include "common.cuh"
 
 namespace {
@@ -101,100 +103,6 @@ __global__ void __launch_bounds__(1024) scan_events_kernel(int32_t* event_cnt, i
     if (threadIdx.x == 0) cand_offsets[n_events] = total;
 }
 
-template <bool U16>
-__global__ void __launch_bounds__(128) peak_emit_kernel(HoughConsts c, const void* __restrict__ acc,
-                                                        int blocks_per_event, const uint32_t* __restrict__ mask,
-                                                        const int32_t* __restrict__ block_off,
-                                                        const int32_t* __restrict__ cand_offsets,
-                                                        hough_candidate* __restrict__ cands, int capacity,
-                                                        int32_t* __restrict__ word_rank) {
-    const int e = blockIdx.y, blk = blockIdx.x;
-    const int word = blk * (PEAK_BLOCK_BINS / 32) + threadIdx.x;
-    const bool valid = word < c.words_per_event;
-    const uint32_t m = valid ? mask[(size_t)e * c.words_per_event + word] : 0u;
-    // CTA exclusive scan of popc(m) over 128 threads
-    const int v = __popc(m);
-    int x = v;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-        const int y = __shfl_up_sync(0xffffffffu, x, o);
-        if ((threadIdx.x & 31) >= o) x += y;
-    }
-    __shared__ int s_w[4];
-    if ((threadIdx.x & 31) == 31) s_w[threadIdx.x >> 5] = x;
-    __syncthreads();
-    int prefix = x - v;
-    for (int w = 0; w < (int)(threadIdx.x >> 5); ++w) prefix += s_w[w];
-    const int rank0 = cand_offsets[e] + block_off[(size_t)e * blocks_per_event + blk] + prefix;
-    if (valid && word_rank) word_rank[(size_t)e * c.words_per_event + word] = rank0;
-    if (m == 0u) return;
-
-    const size_t ebase = (size_t)e * (size_t)c.bins_per_event;
-    const int nphi = c.n_phi, nq = c.n_qpt, nd = c.n_d0;
-    const int row_bins = nphi * nq;
-    uint32_t mm = m;
-    int rank = rank0;
-    while (mm) {
-        const int bit = __ffs(mm) - 1;
-        mm &= mm - 1;
-        if (rank >= capacity) break;
-        const int b = word * 32 + bit;
-        const int k = b / row_bins;
-        const int r = b - k * row_bins;
-        const int i = r / nq;
-        const int j = r - i * nq;
-        long long S = 0, Sj = 0, Si = 0, Sk = 0;
-        int a = 0;
-        for (int dk = -1; dk <= 1; ++dk) {
-            const int kk = k + dk;
-            if (kk < 0 || kk >= nd) continue;
-            for (int di = -1; di <= 1; ++di) {
-                int ii = i + di;
-                ii = ii < 0 ? ii + nphi : (ii >= nphi ? ii - nphi : ii);
-                const size_t row = ebase + ((size_t)kk * nphi + ii) * nq;
-                for (int dj = -1; dj <= 1; ++dj) {
-                    const int jj = j + dj;
-                    if (jj < 0 || jj >= nq) continue;
-                    const int val = load_bin<U16>(acc, row + jj);
-                    S += val; Sj += (long long)val * dj; Si += (long long)val * di; Sk += (long long)val * dk;
-                    if (dk == 0 && di == 0 && dj == 0) a = val;
-                }
-            }
-        }
-        // D7 centroid: every fp32 operation individually rounded
-        const float fS = __ll2float_rn(S);
-        const float oj = __fdiv_rn(__ll2float_rn(Sj), fS);
-        const float oi = __fdiv_rn(__ll2float_rn(Si), fS);
-        const float ok = __fdiv_rn(__ll2float_rn(Sk), fS);
-        const float tj = __fadd_rn(__fadd_rn((float)j, 0.5f), oj);
-        const float qpt = __fadd_rn(c.qpt_min, __fmul_rn(tj, c.wq));
-        const float ti = __fadd_rn(__fadd_rn((float)i, 0.5f), oi);
-        float ph = __fmul_rn(ti, c.wphi);
-        if (ph < 0.0f) ph = __fadd_rn(ph, c.two_pi_f);
-        else if (ph >= c.two_pi_f) ph = __fsub_rn(ph, c.two_pi_f);
-        float d0 = 0.0f;
-        if (nd > 1) {
-            const float tk = __fadd_rn(__fadd_rn((float)k, 0.5f), ok);
-            d0 = __fadd_rn(c.d0_min, __fmul_rn(tk, c.wd));
-        }
-        int4* out = reinterpret_cast<int4*>(cands + rank);
-        out[0] = make_int4(e, k, i, j);
-        out[1] = make_int4(a, __float_as_int(ph), __float_as_int(qpt), __float_as_int(d0));
-        ++rank;
-    }
-}
-
-
-// ---- tiled path ------------------------------------------------------------------------------------------
-template <bool U16> struct BinT { typedef int type; };
-template <> struct BinT<true> { typedef unsigned short type; };
-
-// shared-memory bytes of the halo tile of one block: 3 slices x (rows + 2) x n_qpt bins
-inline size_t peak_tile_bytes(const HoughConsts& c) {
-    const size_t rows = (size_t)(PEAK_BLOCK_BINS + c.n_qpt - 1) / c.n_qpt + 1;      // rows a block can touch
-    return 3 * (rows + 2) * (size_t)c.n_qpt * (c.is_u16 ? 2 : 4) + 16;
-}
-
 // D7 centroid from the integer moments: every fp32 operation individually rounded.
 __device__ __forceinline__ void write_candidate(const HoughConsts& c, hough_candidate* __restrict__ out, int e, int k, int i,
                                                 int j, int a, long long S, long long Sj, long long Si, long long Sk) {
@@ -216,6 +124,97 @@ __device__ __forceinline__ void write_candidate(const HoughConsts& c, hough_cand
     int4* o = reinterpret_cast<int4*>(out);
     o[0] = make_int4(e, k, i, j);
     o[1] = make_int4(a, __float_as_int(ph), __float_as_int(qpt), __float_as_int(d0));
+}
+
+// One CTA = one peak block (PEAK_BLOCK_BINS bins = 128 mask words).  The block's candidates are dealt to the threads
+// by rank (thread t takes candidates t, t + 128, ...), so the lanes of a warp stay busy however the peaks cluster.
+template <bool U16>
+__global__ void __launch_bounds__(128) peak_emit_kernel(HoughConsts c, const void* __restrict__ acc,
+                                                        int blocks_per_event, const uint32_t* __restrict__ mask,
+                                                        const int32_t* __restrict__ block_off,
+                                                        const int32_t* __restrict__ cand_offsets,
+                                                        hough_candidate* __restrict__ cands, int capacity,
+                                                        int32_t* __restrict__ word_rank) {
+    typedef typename std::conditional<U16, int, long long>::type mom_t;     // 27 * 65535 fits an int
+    __shared__ uint32_t s_mask[PEAK_BLOCK_BINS / 32];
+    __shared__ int s_pref[PEAK_BLOCK_BINS / 32 + 1];
+    __shared__ int s_w[4];
+    const int e = blockIdx.y, blk = blockIdx.x;
+    const int word = blk * (PEAK_BLOCK_BINS / 32) + threadIdx.x;
+    const bool valid = word < c.words_per_event;
+    const uint32_t m = valid ? mask[(size_t)e * c.words_per_event + word] : 0u;
+    // CTA exclusive scan of popc(m) over 128 threads
+    const int v = __popc(m);
+    int x = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int y = __shfl_up_sync(0xffffffffu, x, o);
+        if ((threadIdx.x & 31) >= o) x += y;
+    }
+    if ((threadIdx.x & 31) == 31) s_w[threadIdx.x >> 5] = x;
+    __syncthreads();
+    int prefix = x - v;
+    for (int w = 0; w < (int)(threadIdx.x >> 5); ++w) prefix += s_w[w];
+    const int base = cand_offsets[e] + block_off[(size_t)e * blocks_per_event + blk];
+    if (valid && word_rank) word_rank[(size_t)e * c.words_per_event + word] = base + prefix;
+    s_mask[threadIdx.x] = m;
+    s_pref[threadIdx.x] = prefix;
+    const int total = s_w[0] + s_w[1] + s_w[2] + s_w[3];
+    if (threadIdx.x == 0) s_pref[PEAK_BLOCK_BINS / 32] = total;
+    __syncthreads();
+
+    const size_t ebase = (size_t)e * (size_t)c.bins_per_event;
+    const int nphi = c.n_phi, nq = c.n_qpt, nd = c.n_d0;
+    const int row_bins = nphi * nq;
+    for (int ci = threadIdx.x; ci < total; ci += 128) {
+        const int rank = base + ci;
+        if (rank >= capacity) break;                     // ranks ascend with ci
+        int lo = 0, hi = PEAK_BLOCK_BINS / 32;           // last word with s_pref[word] <= ci
+        while (hi - lo > 1) {
+            const int mid = (lo + hi) >> 1;
+            if (s_pref[mid] <= ci) lo = mid; else hi = mid;
+        }
+        uint32_t mm = s_mask[lo];
+        for (int skip = ci - s_pref[lo]; skip > 0; --skip) mm &= mm - 1;
+        const int b = (blk * (PEAK_BLOCK_BINS / 32) + lo) * 32 + (__ffs(mm) - 1);
+        const int k = b / row_bins;
+        const int r = b - k * row_bins;
+        const int i = r / nq;
+        const int j = r - i * nq;
+        mom_t S = 0, Sj = 0, Si = 0, Sk = 0;
+        int a = 0;
+#pragma unroll
+        for (int dk = -1; dk <= 1; ++dk) {
+            const int kk = k + dk;
+            if (kk < 0 || kk >= nd) continue;
+#pragma unroll
+            for (int di = -1; di <= 1; ++di) {
+                int ii = i + di;
+                ii = ii < 0 ? ii + nphi : (ii >= nphi ? ii - nphi : ii);
+                const size_t row = ebase + ((size_t)kk * nphi + ii) * nq;
+#pragma unroll
+                for (int dj = -1; dj <= 1; ++dj) {
+                    const int jj = j + dj;
+                    if (jj < 0 || jj >= nq) continue;
+                    const int val = load_bin<U16>(acc, row + jj);
+                    S += val; Sj += (mom_t)val * dj; Si += (mom_t)val * di; Sk += (mom_t)val * dk;
+                    if (dk == 0 && di == 0 && dj == 0) a = val;
+                }
+            }
+        }
+        write_candidate(c, cands + rank, e, k, i, j, a, (long long)S, (long long)Sj, (long long)Si, (long long)Sk);
+    }
+}
+
+
+// ---- tiled path ------------------------------------------------------------------------------------------
+template <bool U16> struct BinT { typedef int type; };
+template <> struct BinT<true> { typedef unsigned short type; };
+
+// shared-memory bytes of the halo tile of one block: 3 slices x (rows + 2) x n_qpt bins
+inline size_t peak_tile_bytes(const HoughConsts& c) {
+    const size_t rows = (size_t)(PEAK_BLOCK_BINS + c.n_qpt - 1) / c.n_qpt + 1;      // rows a block can touch
+    return 3 * (rows + 2) * (size_t)c.n_qpt * (c.is_u16 ? 2 : 4) + 16;
 }
 
 // A block that spans two d0 slices (n_phi * n_qpt not a multiple of PEAK_BLOCK_BINS): per-bin global loads.

@@ -722,14 +722,17 @@ __global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, Wa
         for (int ci = warp; ci < cols; ci += WALK_WARPS)
             for (int j = lane; j < nq; j += 32) g[(size_t)ci * nq + j] = (int)s_tile[ci * stride + j + 1];
     } else if (OUT16) {
-        if ((nq & 1) == 0) {                             // two bins per 32-bit store
+        if ((nq & 1) == 0) {                             // two bins per 32-bit store; a pair row feeds both of its columns
             uint32_t* g = reinterpret_cast<uint32_t*>(reinterpret_cast<unsigned short*>(a.accum) + row0 * nq);
             const int rw = nq >> 1;
-            for (int ci = warp; ci < cols; ci += WALK_WARPS) {
-                const uint32_t* trow = s_tile + (ci >> 1) * stride + 1;
-                const unsigned sel = (ci & 1) ? 0x7632u : 0x5410u;
-                for (int jw = lane; jw < rw; jw += 32)
-                    g[(size_t)ci * rw + jw] = __byte_perm(trow[2 * jw], trow[2 * jw + 1], sel);
+            for (int pr = warp; pr < (cols >> 1); pr += WALK_WARPS) {
+                const uint32_t* trow = s_tile + pr * stride + 1;
+                uint32_t* gA = g + (size_t)(2 * pr) * rw;
+                for (int jw = lane; jw < rw; jw += 32) {
+                    const uint32_t w0 = trow[2 * jw], w1 = trow[2 * jw + 1];
+                    gA[jw] = __byte_perm(w0, w1, 0x5410u);
+                    gA[rw + jw] = __byte_perm(w0, w1, 0x7632u);
+                }
             }
         } else {
             unsigned short* g = reinterpret_cast<unsigned short*>(a.accum) + row0 * nq;
