@@ -562,6 +562,116 @@ __global__ void __launch_bounds__(256, 2) peak_kwalk_kernel(HoughConsts c, const
     }
 }
 
+// ---- packed slice walk for 16-bit bins (threshold in [1, 65535]) ---------------------------------------------------
+// Same walk and the same D5 algebra as peak_kwalk_kernel, but the 8 bins of a thread stay packed two per register and
+// the maxima / comparisons are the DPX instructions VIMNMX3.U16x2 and VIMNMX.U16x2 (with predicate outputs).  A row is
+// 6 words X[0..5]: X[1..4] = the 8 bins, X[0].hi = bin j0 - 1, X[5].lo = bin j0 + 8.  Missing neighbours (q/pT and d0
+// faces) enter as 0: with a >= threshold >= 1 both "a > 0" and "a >= 0" hold, i.e. the comparison is skipped (D5).
+struct Row6 { unsigned x[6]; };
+
+__device__ __forceinline__ Row6 k16_load_row(const unsigned short* __restrict__ row, int j0, int nq, bool present) {
+    Row6 r;
+    if (!present) {
+#pragma unroll
+        for (int w = 0; w < 6; ++w) r.x[w] = 0u;
+        return r;
+    }
+    const uint4 q = __ldg(reinterpret_cast<const uint4*>(row + j0));
+    r.x[1] = q.x; r.x[2] = q.y; r.x[3] = q.z; r.x[4] = q.w;
+    r.x[0] = j0 > 0 ? ((unsigned)__ldg(row + j0 - 1) << 16) : 0u;
+    r.x[5] = j0 + 8 < nq ? (unsigned)__ldg(row + j0 + 8) : 0u;
+    return r;
+}
+
+__device__ __forceinline__ Row6 k16_max3(const Row6& a, const Row6& b, const Row6& c) {
+    Row6 r;
+#pragma unroll
+    for (int w = 0; w < 6; ++w) r.x[w] = __vimax3_u16x2(a.x[w], b.x[w], c.x[w]);
+    return r;
+}
+
+__device__ __forceinline__ Row6 k16_max2(const Row6& a, const Row6& b) {
+    Row6 r;
+#pragma unroll
+    for (int w = 0; w < 6; ++w) r.x[w] = __vmaxu2(a.x[w], b.x[w]);
+    return r;
+}
+
+__global__ void __launch_bounds__(256, 3) peak_kwalk16_kernel(HoughConsts c, const unsigned short* __restrict__ acc,
+                                                              int threshold, int n_events, int kseg, int n_seg,
+                                                              int blocks_per_event, uint32_t* __restrict__ mask,
+                                                              int32_t* __restrict__ block_cnt) {
+    const int nphi = c.n_phi, nq = c.n_qpt, nd = c.n_d0;
+    const int cpr = nq / 8;                                     // chunks per row
+    const long long strips_per_seg = (long long)nphi * cpr;
+    const long long gid = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    const long long total = strips_per_seg * n_seg * n_events;
+    if (gid >= total) return;                                   // (nphi * cpr) % 32 == 0: a warp is all live or all dead
+    const int chunk = (int)(gid % cpr);
+    const int i = (int)((gid / cpr) % nphi);
+    const int seg = (int)((gid / strips_per_seg) % n_seg);
+    const int e = (int)(gid / (strips_per_seg * n_seg));
+    const int j0 = chunk * 8;
+    const int k0 = seg * kseg, k1 = min(k0 + kseg, nd);
+    const int im = i == 0 ? nphi - 1 : i - 1, ip = i == nphi - 1 ? 0 : i + 1;
+    const size_t slice_bins = (size_t)nphi * nq;
+    const unsigned short* ev = acc + (size_t)e * (size_t)c.bins_per_event;
+    const unsigned short* pm = ev + (size_t)im * nq;
+    const unsigned short* p0 = ev + (size_t)i * nq;
+    const unsigned short* pp = ev + (size_t)ip * nq;
+    unsigned char* mask_bytes = reinterpret_cast<unsigned char*>(mask + (size_t)e * c.words_per_event);
+    const unsigned thr2 = (unsigned)threshold * 0x00010001u;
+
+    Row6 Vm, Rm, R0, Rp;
+    {
+        const bool has = k0 > 0;
+        const size_t so = (size_t)(has ? k0 - 1 : 0) * slice_bins;
+        Vm = k16_max3(k16_load_row(pm + so, j0, nq, has), k16_load_row(p0 + so, j0, nq, has), k16_load_row(pp + so, j0, nq, has));
+        const size_t sc = (size_t)k0 * slice_bins;
+        Rm = k16_load_row(pm + sc, j0, nq, true);
+        R0 = k16_load_row(p0 + sc, j0, nq, true);
+        Rp = k16_load_row(pp + sc, j0, nq, true);
+    }
+    for (int k = k0; k < k1; ++k) {
+        const bool has = k + 1 < nd;
+        const size_t sn = (size_t)(has ? k + 1 : k) * slice_bins;
+        const Row6 Nm = k16_load_row(pm + sn, j0, nq, has);
+        const Row6 N0 = k16_load_row(p0 + sn, j0, nq, has);
+        const Row6 Np = k16_load_row(pp + sn, j0, nq, has);
+        const Row6 B = k16_max2(Vm, Rm);                        // everything "before" the centre row, per q/pT bin
+        const Row6 A = k16_max2(k16_max3(Nm, N0, Np), Rp);      // everything "after" it
+        // shifted views: s[w] = {hi of x[w], lo of x[w + 1]} = the left neighbours of word w + 1 = the right ones of word w
+        unsigned sB[5], sA[5], sR[5];
+#pragma unroll
+        for (int w = 0; w < 5; ++w) {
+            sB[w] = __byte_perm(B.x[w], B.x[w + 1], 0x5432u);
+            sA[w] = __byte_perm(A.x[w], A.x[w + 1], 0x5432u);
+            sR[w] = __byte_perm(R0.x[w], R0.x[w + 1], 0x5432u);
+        }
+        unsigned flags = 0u;
+#pragma unroll
+        for (int w = 1; w <= 4; ++w) {
+            const unsigned a = R0.x[w];
+            const unsigned before = __vmaxu2(__vimax3_u16x2(sB[w - 1], B.x[w], sB[w]), sR[w - 1]);
+            const unsigned after = __vimax3_u16x2(__vimax3_u16x2(sA[w - 1], A.x[w], sA[w]), sR[w], thr2);
+            bool ge_hi, ge_lo, le_hi, le_lo;
+            (void)__vibmax_u16x2(a, after, &ge_hi, &ge_lo);     // a >= max(after, threshold)
+            (void)__vibmax_u16x2(before, a, &le_hi, &le_lo);    // before >= a  (then a is not a strict maximum)
+            flags |= (ge_lo && !le_lo ? 1u : 0u) << (2 * (w - 1));
+            flags |= (ge_hi && !le_hi ? 1u : 0u) << (2 * (w - 1) + 1);
+        }
+        // bitmask: bin b of the event -> bit (b & 7) of byte (b >> 3)
+        const size_t bin0 = ((size_t)k * nphi + i) * nq + j0;
+        mask_bytes[bin0 >> 3] = (unsigned char)flags;
+        // a warp covers 256 consecutive bins of one slice, i.e. one peak block
+        const int cnt = __reduce_add_sync(0xffffffffu, __popc(flags));
+        if ((threadIdx.x & 31) == 0 && cnt)
+            atomicAdd(block_cnt + (size_t)e * blocks_per_event + (int)(bin0 / PEAK_BLOCK_BINS), cnt);
+        Vm = k16_max3(Rm, R0, Rp);
+        Rm = Nm; R0 = N0; Rp = Np;
+    }
+}
+
 }  // namespace
 
 extern "C" int hough_find_peaks(hough_plan* p, const void* d_accum, int32_t n_events, int32_t threshold,
@@ -596,7 +706,10 @@ extern "C" int hough_find_peaks(hough_plan* p, const void* d_accum, int32_t n_ev
         const long long nblk = (threads + 255) / 256;
         if (nblk > 0x7fffffffLL) return HOUGH_ERR_UNSUPPORTED;
         HOUGH_CUDA_TRY(cudaMemsetAsync(p->d_peak_block_cnt, 0, sizeof(int32_t) * (size_t)n_events * bpe, st));
-        if (p->c.is_u16)
+        if (p->c.is_u16 && threshold >= 1 && threshold <= 65535 && !p->peaks_scalar)
+            peak_kwalk16_kernel<<<(unsigned)nblk, 256, 0, st>>>(p->c, reinterpret_cast<const unsigned short*>(d_accum), threshold,
+                                                                n_events, kseg, n_seg, bpe, p->d_mask, p->d_peak_block_cnt);
+        else if (p->c.is_u16)
             peak_kwalk_kernel<true><<<(unsigned)nblk, 256, 0, st>>>(p->c, d_accum, threshold, n_events, kseg, n_seg, bpe,
                                                                     p->d_mask, p->d_peak_block_cnt);
         else
