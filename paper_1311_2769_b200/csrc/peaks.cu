@@ -597,7 +597,7 @@ __device__ __forceinline__ Row6 k16_max2(const Row6& a, const Row6& b) {
     return r;
 }
 
-__global__ void __launch_bounds__(256, 3) peak_kwalk16_kernel(HoughConsts c, const unsigned short* __restrict__ acc,
+__global__ void __launch_bounds__(256, 2) peak_kwalk16_kernel(HoughConsts c, const unsigned short* __restrict__ acc,
                                                               int threshold, int n_events, int kseg, int n_seg,
                                                               int blocks_per_event, uint32_t* __restrict__ mask,
                                                               int32_t* __restrict__ block_cnt) {
@@ -622,7 +622,8 @@ __global__ void __launch_bounds__(256, 3) peak_kwalk16_kernel(HoughConsts c, con
     unsigned char* mask_bytes = reinterpret_cast<unsigned char*>(mask + (size_t)e * c.words_per_event);
     const unsigned thr2 = (unsigned)threshold * 0x00010001u;
 
-    Row6 Vm, Rm, R0, Rp;
+    // the rows of slice k + 1 are in registers and those of slice k + 2 are in flight while slice k is evaluated
+    Row6 Vm, Rm, R0, Rp, Nm, N0, Np;
     {
         const bool has = k0 > 0;
         const size_t so = (size_t)(has ? k0 - 1 : 0) * slice_bins;
@@ -631,13 +632,19 @@ __global__ void __launch_bounds__(256, 3) peak_kwalk16_kernel(HoughConsts c, con
         Rm = k16_load_row(pm + sc, j0, nq, true);
         R0 = k16_load_row(p0 + sc, j0, nq, true);
         Rp = k16_load_row(pp + sc, j0, nq, true);
+        const bool has1 = k0 + 1 < nd;
+        const size_t s1 = (size_t)(has1 ? k0 + 1 : k0) * slice_bins;
+        Nm = k16_load_row(pm + s1, j0, nq, has1);
+        N0 = k16_load_row(p0 + s1, j0, nq, has1);
+        Np = k16_load_row(pp + s1, j0, nq, has1);
     }
+#pragma unroll 3
     for (int k = k0; k < k1; ++k) {
-        const bool has = k + 1 < nd;
-        const size_t sn = (size_t)(has ? k + 1 : k) * slice_bins;
-        const Row6 Nm = k16_load_row(pm + sn, j0, nq, has);
-        const Row6 N0 = k16_load_row(p0 + sn, j0, nq, has);
-        const Row6 Np = k16_load_row(pp + sn, j0, nq, has);
+        const bool has2 = k + 2 < nd && k + 1 < k1;              // slice k + 2 is needed only if slice k + 1 is evaluated
+        const size_t s2 = (size_t)(has2 ? k + 2 : k) * slice_bins;
+        const Row6 Pm = k16_load_row(pm + s2, j0, nq, has2);
+        const Row6 P0 = k16_load_row(p0 + s2, j0, nq, has2);
+        const Row6 Pp = k16_load_row(pp + s2, j0, nq, has2);
         const Row6 B = k16_max2(Vm, Rm);                        // everything "before" the centre row, per q/pT bin
         const Row6 A = k16_max2(k16_max3(Nm, N0, Np), Rp);      // everything "after" it
         // shifted views: s[w] = {hi of x[w], lo of x[w + 1]} = the left neighbours of word w + 1 = the right ones of word w
@@ -669,6 +676,7 @@ __global__ void __launch_bounds__(256, 3) peak_kwalk16_kernel(HoughConsts c, con
             atomicAdd(block_cnt + (size_t)e * blocks_per_event + (int)(bin0 / PEAK_BLOCK_BINS), cnt);
         Vm = k16_max3(Rm, R0, Rp);
         Rm = Nm; R0 = N0; Rp = Np;
+        Nm = Pm; N0 = P0; Np = Pp;
     }
 }
 
