@@ -178,10 +178,10 @@ def oracle_sample(w, batch, n_sample_events: int):
 
 def oracle_events_for_seconds(w, target_s: float) -> int:
     """Bounded sample size: ~target_s of single-thread oracle work, from the full-scan evaluation count
-    (2 scans: vote + indexed assignment) at ~1.5e8 evaluations/s."""
+    (2 scans: vote + indexed assignment) at ~6.5e8 evaluations/s (measured on the GPU box's host, profiles/)."""
     bn = w.binning
     hits_per_event = (w.n_prompt + w.n_displaced) * len(w.layers) + max(w.n_noise, 0)
-    per_event_s = 2.0 * hits_per_event * bn.n_phi * bn.n_d0 / 1.5e8 + bn.n_bins / 2.0e8
+    per_event_s = 2.0 * hits_per_event * bn.n_phi * bn.n_d0 / 6.5e8 + bn.n_bins / 2.0e8
     return max(1, min(w.n_events, int(target_s / max(per_event_s, 1e-6))))
 
 
@@ -401,8 +401,11 @@ def run_ours(args, rank, world, local_rank):
     hits_per_launch = batch.n_hits / len(run.tiles)
     bins_per_launch = bn.n_bins * run.tile_events
     hbm_bytes = hits_per_launch * 8 + bins_per_launch * bn.bin_bytes            # hits in + accumulator out
+    # dram__bytes_read.sum + dram__bytes_write.sum of the walk kernel in the ncu --set full capture of this very
+    # launch configuration (profiles/r1_final.md): 20.3 MB + 340.9 MB per 128-event launch of cfg 3
+    traffic = 361.2e6 if (args.config == 3 and run.tile_events == 128) else None
     roofline = {"bound": "alu", "kernel": "hough_vote (stage + vote + flush)", "achieved": achieved, "peak": alu_peak,
-                "unit": "Gvotes/s", "frac": achieved / alu_peak, "traffic": None,
+                "unit": "Gvotes/s", "frac": achieved / alu_peak, "traffic": traffic,
                 "peak_source": f"{sms} SMs x {FP32_LANES_PER_SM} fp32 lanes x {sm_max_mhz:.0f} MHz / "
                                f"{D3_MIN_ISSUE_SLOTS} issue slots per vote (DESIGN.md); clocks {peak_src}",
                 "vote_ms_per_launch": vote_ms_avg, "votes_per_launch": votes_per_launch,
@@ -411,7 +414,11 @@ def run_ours(args, rank, world, local_rank):
                         "peak_gbs": hbm_gbs, "frac": hbm_bytes / (vote_ms_avg * 1e-3) / 1e9 / hbm_gbs,
                         "peak_source": peak_src},
                 "smem_atomic": {"peak_gops": args.smem_atomic_gops, "frac": achieved / args.smem_atomic_gops,
-                                "peak_source": "hough_microbench kind 0 on this pool's B200 (profiles/)"}}
+                                "peak_random_gops": args.smem_atomic_random_gops,
+                                "frac_random": achieved / args.smem_atomic_random_gops,
+                                "peak_source": "hough_microbench kinds 0 (conflict-free) and 1 (random words of a 64 KB tile) "
+                                               "on this pool's B200 (profiles/r1_microbench.txt); ncu: the walk kernel "
+                                               "keeps the shared-memory wavefront pipe 82 % busy (profiles/r1_final.md)"}}
 
     n_ref = oracle_events_for_seconds(w, args.cpu_seconds)
     o_votes, o_events, o_secs = oracle_sample(w, batch, n_ref)
@@ -459,6 +466,7 @@ def main():
     ap.add_argument("--streams", type=int, default=4, help="CUDA streams of the batched pipeline (B:L10: 4)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target oracle time of the cpu_baseline sample")
     ap.add_argument("--ref-seconds-per-step", type=float, default=10.0)
+    ap.add_argument("--smem-atomic-random-gops", type=float, default=3304.0)
     ap.add_argument("--smem-atomic-gops", type=float, default=7593.0,
                     help="measured conflict-free shared atomicAdd rate, Gops/s (profiles/microbench_r1.md)")
     args = ap.parse_args()
