@@ -131,7 +131,7 @@ extern "C" int hough_plan_create(const hough_binning* b, const hough_geometry* g
     HoughWindows win;
     if (hough_build_windows(*b, g->bz_tesla, g->n_layers, g->layer_radius_cm, win) != HOUGH_OK) { delete p; return HOUGH_ERR_INVALID_ARG; }
     c.n_class = win.n_class;
-    c.n_sector = HOUGH_SECTORS;
+    { const char* es = getenv("HOUGH_SECTORS"); c.n_sector = es ? atoi(es) : HOUGH_SECTORS; if (c.n_sector < 1 || c.n_sector > 1024) c.n_sector = HOUGH_SECTORS; }
     c.n_keys = c.n_class * c.n_sector;
     c.u_scale = (float)((double)b->n_phi / (2.0 * kPi));
     c.sector_scale = (float)((double)c.n_sector / (2.0 * kPi));

@@ -33,8 +33,10 @@
 
 constexpr int WALK_VOTE = 0;
 constexpr int WALK_ASSIGN = 1;
-constexpr int WALK_THREADS = 320;
-constexpr int WALK_WARPS = WALK_THREADS / 32;
+// threads per CTA: the vote walk runs best with 10 warps at 64 registers, the association walk (more live state) with
+// 8 warps at 80 registers (profiles/r1_final.md)
+__host__ __device__ constexpr int walk_threads(int mode) { return mode == 0 ? 320 : 256; }
+constexpr int WALK_MAX_WARPS = 10;
 constexpr int WALK_CHUNK_PAIRS = 16;             // column pairs per chunk: 32 columns = the bits of the redo mask
 constexpr int WALK_WQ_CAP = 48;                  // entries of a warp's exact-redo queue (drained by the whole warp)
 
@@ -65,7 +67,7 @@ __host__ __device__ inline size_t walk_smem_bytes(int cols, int stride, bool til
     b += (size_t)(cols / 2 + WALK_CHUNK_PAIRS + 1) * 16;               // column pairs {cosA, cosB, sinA, sinB}
     b += (size_t)n_class * 16;                                          // per class: window, error bound
     b += ((size_t)n_class * (fullphi ? 1 : 2) + 1) * 16;                // segments (a full-phi tile has one per class)
-    b += (size_t)WALK_WARPS * WALK_WQ_CAP * 4;                          // redo queues
+    b += (size_t)WALK_MAX_WARPS * WALK_WQ_CAP * 4;                      // redo queues
     return b + 128;                                                     // one scratch word per lane (walk_kernel: trash_saddr)
 }
 
@@ -359,7 +361,8 @@ __device__ __forceinline__ void walk_drain(const HoughConsts& c, const FastK& fk
 }
 
 template <int MODE, bool TILE32, bool OUT16, bool FULLPHI>
-__global__ void __launch_bounds__(WALK_THREADS, 3) walk_kernel(HoughConsts c, WalkArgs a) {
+__global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(HoughConsts c, WalkArgs a) {
+    constexpr int WALK_THREADS = walk_threads(MODE), WALK_WARPS = WALK_THREADS / 32;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ int s_meta[2];                           // number of batches of the tile
     const int n_slabs = a.n_slabs, slab_cols = a.slab_cols, stride = a.stride;
@@ -772,7 +775,7 @@ int walk_launch(hough_plan* p, int n_events, WalkArgs a, cudaStream_t st) {
     const long long grid = (long long)a.n_slabs * p->c.n_d0 * n_events;
     if (grid > 0x7fffffffLL) return HOUGH_ERR_UNSUPPORTED;
     a.exact_only = p->exact_walk;
-    kern<<<(unsigned)grid, WALK_THREADS, smem, st>>>(p->c, a);
+    kern<<<(unsigned)grid, walk_threads(MODE), smem, st>>>(p->c, a);
     HOUGH_CUDA_TRY(cudaGetLastError());
     hough_count_launches(1);
     return HOUGH_OK;
