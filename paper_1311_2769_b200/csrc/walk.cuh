@@ -702,10 +702,10 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(HoughConsts
             const unsigned eh = EntryT<TILE32>::ent_hi(bestp);          // entry >> 1: votes + 1 above (15 - |dj|)
             if (eh >> 4) {
                 // the winning column's slot again (an unflagged pair: the fast slot IS the D3 bin), then the full entry
-                const float4 hw = __ldg(a.staged + sidx);
+                const float4 hw = hv;
                 const int bcol = EntryT<TILE32>::col_of(bestp);
                 const float4 T = s_pair[bcol >> 1];
-                const FastHit fh = make_fasthit(fk, hw.x, hw.y, d3_r2(hw.x, hw.y));
+                const FastHit fh = make_fasthit(fk, hw.x, hw.y, r2);
                 const int J = (int)fast_slot(fk, fh, (bcol & 1) ? T.y : T.x, (bcol & 1) ? T.w : T.z) - 1;
                 const unsigned ent = tile_entry<TILE32>(s_tile, stride, bcol, J);
                 const int adj = 15 - (int)((ent >> 1) & 15u);
