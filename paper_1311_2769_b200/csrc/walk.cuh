@@ -556,18 +556,45 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(HoughConsts
     unsigned* wq = s_wq + warp * WALK_WQ_CAP;           // the warp's redo queue
     int wq_n = 0;
     const bool wq_ok = ev_hits < (1 << 18) && slab_cols <= 2048;          // entries fit 32 bits (else: redo on the spot)
-    int seg = 0;                                        // batches ascend per warp: a running segment pointer
+    // batches ascend per warp (a running segment pointer).  PREFETCH (association walk, which has the registers): the
+    // staged hit of the warp's NEXT batch is loaded while the current one is walked.
+    constexpr bool PREFETCH = MODE == WALK_ASSIGN;
+    int seg = 0;
+    int4 sg_n = make_int4(0, 0, 0, 0);
+    float4 hv_n = make_float4(1.f, 0.f, 0.f, 0.f);
+    if (PREFETCH && warp < n_batches) {
+        while (s_seg[seg + 1].w <= warp) ++seg;          // last segment with first batch <= bt (the sentinel ends the search)
+        sg_n = s_seg[seg];
+        const int in_n = (warp - sg_n.w) * 32 + lane;
+        if (in_n < sg_n.y) hv_n = __ldg(a.staged + ev_begin + sg_n.x + in_n);
+    }
     for (int bt = warp; bt < n_batches; bt += WALK_WARPS) {
-        while (s_seg[seg + 1].w <= bt) ++seg;            // last segment with first batch <= bt (the sentinel ends the search)
-        const int4 sg = s_seg[seg];
+        int4 sg;
+        float4 hv;
+        if (PREFETCH) {
+            sg = sg_n;
+            hv = hv_n;
+        } else {
+            while (s_seg[seg + 1].w <= bt) ++seg;
+            sg = s_seg[seg];
+        }
         const int in_seg = (bt - sg.w) * 32 + lane;
         const bool active = in_seg < sg.y;
         const float4 cw = s_cls[sg.z];
         const int steps = __float_as_int(cw.y);
         const float hm_c = cw.z;
         const int sidx = ev_begin + sg.x + in_seg;       // index of the lane's staged hit
-        float4 hv = make_float4(1.f, 0.f, 0.f, 0.f);
-        if (active) hv = __ldg(a.staged + sidx);
+        if (!PREFETCH) {
+            hv = make_float4(1.f, 0.f, 0.f, 0.f);
+            if (active) hv = __ldg(a.staged + sidx);
+        } else if (bt + WALK_WARPS < n_batches) {
+            const int bn = bt + WALK_WARPS;
+            while (s_seg[seg + 1].w <= bn) ++seg;
+            sg_n = s_seg[seg];
+            const int in_n = (bn - sg_n.w) * 32 + lane;
+            hv_n = make_float4(1.f, 0.f, 0.f, 0.f);
+            if (in_n < sg_n.y) hv_n = __ldg(a.staged + ev_begin + sg_n.x + in_n);
+        }
         const float x = hv.x, y = hv.y;
         const float r2 = d3_r2(x, y);
         int i_lo = (int)ceilf(hv.z + cw.x);
