@@ -2,6 +2,7 @@
 """bench.py -- the round-end measurement of the Hough track-finding hot path.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config C] [--tile-events T]
+                    [--e2e-tile-events T2] [--streams S]
     python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P \
         bench.py --gpus N --steps K --warmup W
 
@@ -13,8 +14,8 @@ the metric's "events/s" is quoted on; `--config` selects another one (0, 1, 2, 4
 One JSON line goes to stdout (rank 0):
   value            whole-job Hough votes/s, inputs resident in HBM before the timed region, all ranks
   events_per_s     the same step expressed in events/s (the metric's second figure)
-  e2e              the same metric through hough_pipeline_run_host: pinned HOST buffers in, HOST results out,
-                   host<->device copies inside the timed region
+  e2e              the same metric through hough_pipeline_run_host (T2-event tiles on S streams, CUDA graphs): pinned
+                   HOST buffers in, HOST results out, host<->device copies inside the timed region
   roofline         dominant kernel (vote): algorithmic votes per launch / average launch duration (CUDA events
                    on the launching stream, inside the timed region) against the ALU issue bound derived in
                    DESIGN.md; the atomic and HBM ceilings of SURVEY 8(d) are quoted beside it

@@ -116,14 +116,20 @@ int hough_assign_hits(hough_plan* plan, const float* d_hits_xy, int32_t n_hits, 
  * prescribed D3 sequence at every column (no fast path; HOUGH_DEBUG_EXACT_WALK=1).  "peaks_tiled": 1 = halo-tile
  * peak kernels; "peaks_scalar": 1 = the unpacked slice-walk peak kernel also for 16-bit bins.  "reuse_staging": 1 = the caller promises that a hough_assign_hits call whose hit pointer, offsets
  * pointer, sizes and stream equal those of the preceding hough_vote sees unchanged hits, so the staged (sorted)
- * copy of that vote is reused instead of rebuilt. */
+ * copy of that vote is reused instead of rebuilt.
+ * Environment (read at plan creation, work sizing only): HOUGH_SECTORS=n phi sectors of the staging sort (default 32). */
 int hough_plan_set_option(hough_plan* plan, const char* key, int32_t value);
 
 /* Batched multi-event pipeline (B:L5 "a batched multi-event path using CUDA streams and graphs"; B:L10).
  * Runs vote -> find_peaks -> assign_hits over HOST buffers: events are cut into tiles of tile_events, tiles
- * are dealt round-robin to n_streams streams, each with its own plan, accumulator and staging buffers; each
- * stream's tile sequence (H2D hits, kernels, D2H results) is captured once as a CUDA graph and replayed.
- * h_hits_xy / h_event_offsets and the outputs should be pinned for copies to overlap.
+ * are dealt round-robin to n_streams streams, each with its own plan, accumulator and staging buffers; a
+ * stream's per-tile sequence (H2D hits, the three calls, D2H of the counts) is stream-captured, the stream's
+ * executable CUDA graph is updated in place (cudaGraphExecUpdate: same topology, other sizes) and launched once per
+ * tile; a device kernel rebases tile-local event / candidate indices to global ones before the results are copied
+ * into the caller's buffers.  The call blocks until all results are in the host buffers.
+ * h_hits_xy and the outputs should be pinned (cudaHostAlloc / cudaHostRegister) for the copies to overlap with the
+ * kernels; pageable memory works (plain launches, no graphs) but serialises.
+ * Environment: HOUGH_PIPELINE_NO_GRAPHS=1 disables graph capture.
  * Outputs (host): h_hit_to_cand[n_hits] (indices are GLOBAL candidate ranks, events concatenated, -1 = none),
  * h_cand_offsets[n_events + 1], h_cands[cand_capacity] (records of rank < cand_capacity),
  * h_cand_nhits / h_cand_keep [cand_capacity].  Per-tile candidate capacity is tile_cand_capacity; a tile

@@ -9,9 +9,10 @@
 //
 // Tile layout.  A row has nq + 2 slots h = J + 1: the q/pT bins J = 0..nq-1 and one
 // GUARD slot at each end (J = -1 and J = nq) that absorbs the fast path's "one bin outside" results, followed by
-// WALK_DUMP dump slots for everything further out; guard and dump slots are never flushed.  Packed tiles (16-bit bins) store the two columns of an even/odd column PAIR in one 32-bit word per
-// slot (low half = even column, high half = odd column), so the increment is the constant 1 or 65536 and the
-// address is pair_row + 4 h.  32-bit tiles store one word per (column, slot).
+// WALK_DUMP dump slots for everything further out; guard and dump slots are never flushed.  Packed tiles (16-bit
+// bins) store the two columns of an even/odd column PAIR in one 32-bit word per slot (low half = even column, high
+// half = odd column), so the increment is the constant 1 or 65536 and the address is pair_row + 4 h.  32-bit tiles
+// store one word per (column, slot).
 //
 // Work mapping: lane = hit.  A warp takes 32 consecutive staged hits of one radius class (same window length,
 // neighbouring azimuth thanks to the (class, sector) sort of stage.cu); every lane walks the columns of its own
@@ -19,11 +20,13 @@
 //
 // Bin index per (hit, column): DESIGN.md "Fast path".  The prescribed D3 sequence costs ~30 issue slots (IEEE
 // reciprocal, unfused multiplies).  The walk evaluates the same real-valued function with FMAs and MUFU.RCP (t~)
-// and owns, per (hit, d0 slice), a bound m on |t~ - t_D3| (first-order rounding analysis of BOTH sequences with a
-// safety factor); if t~ is further than m from a bin edge the D3 bin is floor(t~) (or certainly out of range)
-// without running D3.  Otherwise (about 0.1 % of the evaluations) the (hit, column) goes to a small shared-memory
-// queue and is redone with the exact D3 sequence (d3_exact_bin) by the whole CTA at the end.  Hits whose bound is
-// useless (r ~ |d0|, non-finite coordinates), classes whose window is not certainly forward, and the plan option
+// and owns, per (radius class, d0 slice), a bound m on |t~ - t_D3| (first-order rounding analysis of BOTH sequences
+// with a safety factor); if t~ is further than m from a bin edge the D3 bin is floor(t~) (or certainly out of range)
+// without running D3.  The hot loop casts the fast vote of every evaluation unconditionally; a column pair with an
+// uncertain evaluation (about 0.15 % of the pairs) goes to the warp's small shared-memory queue and is redone 32 at a
+// time by the whole warp: the pair's two fast votes are taken back (fast_slot reproduces them bit for bit) and the
+// votes of the exact D3 sequence (d3_exact_bin) are cast.  Classes whose bound is useless (r ~ |d0|, the open-ended
+// last class where non-finite coordinates land), classes whose window is not certainly forward, and the plan option
 // "exact_walk" take the exact sequence at every column.  The result is therefore the D3 bin in every case.
 #pragma once
 
