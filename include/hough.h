@@ -114,7 +114,8 @@ int hough_assign_hits(hough_plan* plan, const float* d_hits_xy, int32_t n_hits, 
  * no windowing and vote straight into global memory (the bisecting path of SURVEY section 5; also read once at
  * plan creation from the environment: HOUGH_DEBUG_FULLSCAN=1).  "exact_walk": 1 = the windowed walk runs the
  * prescribed D3 sequence at every column (no fast path; HOUGH_DEBUG_EXACT_WALK=1).  "peaks_tiled": 1 = halo-tile
- * peak kernels; "peaks_scalar": 1 = the unpacked slice-walk peak kernel also for 16-bit bins.  "reuse_staging": 1 = the caller promises that a hough_assign_hits call whose hit pointer, offsets
+ * peak kernels; "peaks_scalar": 1 = the unpacked slice-walk peak kernel also for 16-bit bins, "peaks_regs": 1 = the packed
+ * 16-bit walk with rows held in registers instead of the cp.async shared-memory ring.  "reuse_staging": 1 = the caller promises that a hough_assign_hits call whose hit pointer, offsets
  * pointer, sizes and stream equal those of the preceding hough_vote sees unchanged hits, so the staged (sorted)
  * copy of that vote is reused instead of rebuilt.
  * Environment (read at plan creation, work sizing only): HOUGH_SECTORS=n phi sectors of the staging sort (default 32). */

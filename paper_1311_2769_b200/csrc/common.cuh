@@ -62,6 +62,7 @@ struct hough_plan {
     int device, sm_count;
     int fullscan;
     int peaks_tiled;                   // 1: find_peaks uses the shared-memory halo-tile kernels instead of the slice walk
+    int peaks_regs;                    // 1: 16-bit packed peak walk with register-held rows instead of the cp.async ring
     int peaks_scalar;                  // 1: 16-bit accumulators use the unpacked slice-walk peak kernel (bisecting)
     int exact_walk;                    // 1: the walks evaluate the D3 sequence at every column (no fast path)
     int reuse_staging;                 // 1: hough_assign_hits may reuse the staging of the preceding hough_vote (same arguments)

@@ -680,6 +680,123 @@ __global__ void __launch_bounds__(256, 2) peak_kwalk16_kernel(HoughConsts c, con
     }
 }
 
+// ---- streamed packed slice walk (16-bit bins): cp.async ring in shared memory ---------------------------------------
+// The walk of peak_kwalk16_kernel with the loads decoupled from the registers: a CTA of 256 threads owns R = 256 /
+// (n_qpt / 8) consecutive phi0 rows of one event and one run of d0 slices; slice after slice, the R + 2 rows it needs
+// (one halo row each side, cyclic) are copied into a ring of PS_STAGES shared-memory stages with cp.async (16 bytes per
+// request, whole rows, coalesced), so PS_STAGES - 1 slices are in flight per CTA while one is evaluated.  Bytes in
+// flight are bounded by shared memory instead of registers: the accumulator streams in at HBM speed.
+constexpr int PS_STAGES = 6;
+
+__device__ __forceinline__ void ps_cp_async16(unsigned saddr, const void* gptr) {
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(saddr), "l"(gptr) : "memory");
+}
+__device__ __forceinline__ void ps_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void ps_wait() { asm volatile("cp.async.wait_group %0;" :: "n"(N) : "memory"); }
+
+__device__ __forceinline__ Row6 ps_load_row(const unsigned short* __restrict__ srow, int j0, int nq) {
+    Row6 r;
+    const uint4 q = *reinterpret_cast<const uint4*>(srow + j0);
+    r.x[1] = q.x; r.x[2] = q.y; r.x[3] = q.z; r.x[4] = q.w;
+    r.x[0] = j0 > 0 ? ((unsigned)srow[j0 - 1] << 16) : 0u;
+    r.x[5] = j0 + 8 < nq ? (unsigned)srow[j0 + 8] : 0u;
+    return r;
+}
+
+__global__ void __launch_bounds__(256, 3) peak_stream16_kernel(HoughConsts c, const unsigned short* __restrict__ acc,
+                                                               int threshold, int kseg, int n_seg, int blocks_per_event,
+                                                               uint32_t* __restrict__ mask, int32_t* __restrict__ block_cnt) {
+    extern __shared__ __align__(16) unsigned char ps_smem[];
+    const int nphi = c.n_phi, nq = c.n_qpt, nd = c.n_d0;
+    const int cpr = nq / 8;                                     // 16-byte chunks per row
+    const int R = 256 / cpr;                                    // rows per CTA
+    const int rb_per_ev = nphi / R;
+    const int rb = blockIdx.x % rb_per_ev;
+    const int seg = (blockIdx.x / rb_per_ev) % n_seg;
+    const int e = blockIdx.x / (rb_per_ev * n_seg);
+    const int tid = threadIdx.x;
+    const int rl = tid / cpr, chunk = tid - rl * cpr;
+    const int j0 = chunk * 8;
+    const int i0 = rb * R, i = i0 + rl;
+    const int k0 = seg * kseg, k1 = min(k0 + kseg, nd);
+    const int stage_halfwords = (R + 2) * nq;
+    const int n_chunks = (R + 2) * cpr;                         // 16-byte chunks per stage (<= 512)
+    const unsigned short* ev = acc + (size_t)e * (size_t)c.bins_per_event;
+    unsigned short* s_base = reinterpret_cast<unsigned short*>(ps_smem);
+    unsigned char* mask_bytes = reinterpret_cast<unsigned char*>(mask + (size_t)e * c.words_per_event);
+    const unsigned thr2 = (unsigned)threshold * 0x00010001u;
+
+    // fill stage `stage` with slice v (rows i0 - 1 .. i0 + R, cyclic); slices outside [0, nd) are all "missing" = 0
+    auto issue = [&](int v, int stage) {
+        unsigned short* st = s_base + (size_t)stage * stage_halfwords;
+        for (int idx = tid; idx < n_chunks; idx += 256) {
+            const int sr = idx / cpr, ch = idx - sr * cpr;
+            unsigned short* dst = st + sr * nq + ch * 8;
+            if (v < 0 || v >= nd) {
+                *reinterpret_cast<uint4*>(dst) = make_uint4(0u, 0u, 0u, 0u);
+            } else {
+                int gi = i0 - 1 + sr;
+                gi = gi < 0 ? gi + nphi : (gi >= nphi ? gi - nphi : gi);
+                ps_cp_async16((unsigned)__cvta_generic_to_shared(dst), ev + ((size_t)v * nphi + gi) * nq + ch * 8);
+            }
+        }
+        ps_commit();
+    };
+
+    const int v_first = k0 - 1, v_last = k1;                    // virtual slices the run needs
+    for (int s = 0; s < PS_STAGES; ++s) {
+        if (v_first + s <= v_last) issue(v_first + s, s);
+        else ps_commit();
+    }
+    Row6 Vm, Rm, R0, Rp;
+#pragma unroll
+    for (int w = 0; w < 6; ++w) Vm.x[w] = Rm.x[w] = R0.x[w] = Rp.x[w] = 0u;
+    for (int it = 0, v = v_first; v <= v_last; ++it, ++v) {
+        ps_wait<PS_STAGES - 2>();                               // group `it` (slice v) has landed
+        __syncthreads();                                        // ... for every thread; the previous stage is free
+        if (it >= 1) {
+            const int vn = v - 1 + PS_STAGES;
+            if (vn <= v_last) issue(vn, (it - 1) % PS_STAGES);
+            else ps_commit();
+        }
+        const unsigned short* st = s_base + (size_t)(it % PS_STAGES) * stage_halfwords + rl * nq;
+        const Row6 Nm = ps_load_row(st, j0, nq);
+        const Row6 N0 = ps_load_row(st + nq, j0, nq);
+        const Row6 Np = ps_load_row(st + 2 * nq, j0, nq);
+        if (it == 0) { Vm = k16_max3(Nm, N0, Np); continue; }
+        if (it == 1) { Rm = Nm; R0 = N0; Rp = Np; continue; }
+        const int k = v - 1;                                    // centre slice, k0 <= k < k1
+        const Row6 B = k16_max2(Vm, Rm);                        // everything "before" the centre row, per q/pT bin
+        const Row6 A = k16_max2(k16_max3(Nm, N0, Np), Rp);      // everything "after" it
+        unsigned sB[5], sA[5], sR[5];
+#pragma unroll
+        for (int w = 0; w < 5; ++w) {
+            sB[w] = __byte_perm(B.x[w], B.x[w + 1], 0x5432u);
+            sA[w] = __byte_perm(A.x[w], A.x[w + 1], 0x5432u);
+            sR[w] = __byte_perm(R0.x[w], R0.x[w + 1], 0x5432u);
+        }
+        unsigned flags = 0u;
+#pragma unroll
+        for (int w = 1; w <= 4; ++w) {
+            const unsigned a = R0.x[w];
+            const unsigned before = __vmaxu2(__vimax3_u16x2(sB[w - 1], B.x[w], sB[w]), sR[w - 1]);
+            const unsigned after = __vimax3_u16x2(__vimax3_u16x2(sA[w - 1], A.x[w], sA[w]), sR[w], thr2);
+            bool ge_hi, ge_lo, le_hi, le_lo;
+            (void)__vibmax_u16x2(a, after, &ge_hi, &ge_lo);     // a >= max(after, threshold)
+            (void)__vibmax_u16x2(before, a, &le_hi, &le_lo);    // before >= a  (then a is not a strict maximum)
+            flags |= (ge_lo && !le_lo ? 1u : 0u) << (2 * (w - 1));
+            flags |= (ge_hi && !le_hi ? 1u : 0u) << (2 * (w - 1) + 1);
+        }
+        const size_t bin0 = ((size_t)k * nphi + i) * nq + j0;
+        mask_bytes[bin0 >> 3] = (unsigned char)flags;
+        const int cnt = __reduce_add_sync(0xffffffffu, __popc(flags));     // a warp = 256 consecutive bins of one peak block
+        if ((tid & 31) == 0 && cnt)
+            atomicAdd(block_cnt + (size_t)e * blocks_per_event + (int)(bin0 / PEAK_BLOCK_BINS), cnt);
+        Vm = k16_max3(Rm, R0, Rp);
+        Rm = Nm; R0 = N0; Rp = Np;
+    }
+}
+
 }  // namespace
 
 extern "C" int hough_find_peaks(hough_plan* p, const void* d_accum, int32_t n_events, int32_t threshold,
@@ -714,7 +831,23 @@ extern "C" int hough_find_peaks(hough_plan* p, const void* d_accum, int32_t n_ev
         const long long nblk = (threads + 255) / 256;
         if (nblk > 0x7fffffffLL) return HOUGH_ERR_UNSUPPORTED;
         HOUGH_CUDA_TRY(cudaMemsetAsync(p->d_peak_block_cnt, 0, sizeof(int32_t) * (size_t)n_events * bpe, st));
-        if (p->c.is_u16 && threshold >= 1 && threshold <= 65535 && !p->peaks_scalar)
+        const int cpr16 = p->c.n_qpt / 8;
+        const bool stream16 = p->c.is_u16 && threshold >= 1 && threshold <= 65535 && !p->peaks_scalar && !p->peaks_regs &&
+                              cpr16 <= 256 && 256 % cpr16 == 0 && p->c.n_phi % (256 / cpr16) == 0 &&
+                              (size_t)PS_STAGES * (256 / cpr16 + 2) * p->c.n_qpt * 2 <= 64 * 1024;
+        if (stream16) {
+            const int R = 256 / cpr16;
+            const size_t smem = (size_t)PS_STAGES * (R + 2) * p->c.n_qpt * 2;
+            static bool configured = false;
+            if (!configured) {
+                HOUGH_CUDA_TRY(cudaFuncSetAttribute(peak_stream16_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024));
+                configured = true;
+            }
+            const long long nb = (long long)(p->c.n_phi / R) * n_seg * n_events;
+            if (nb > 0x7fffffffLL) return HOUGH_ERR_UNSUPPORTED;
+            peak_stream16_kernel<<<(unsigned)nb, 256, smem, st>>>(p->c, reinterpret_cast<const unsigned short*>(d_accum), threshold,
+                                                                  kseg, n_seg, bpe, p->d_mask, p->d_peak_block_cnt);
+        } else if (p->c.is_u16 && threshold >= 1 && threshold <= 65535 && !p->peaks_scalar)
             peak_kwalk16_kernel<<<(unsigned)nblk, 256, 0, st>>>(p->c, reinterpret_cast<const unsigned short*>(d_accum), threshold,
                                                                 n_events, kseg, n_seg, bpe, p->d_mask, p->d_peak_block_cnt);
         else if (p->c.is_u16)

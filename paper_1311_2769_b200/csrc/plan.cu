@@ -222,6 +222,7 @@ extern "C" int hough_plan_set_option(hough_plan* p, const char* key, int32_t val
     if (!p || !key) return HOUGH_ERR_INVALID_ARG;
     if (strcmp(key, "fullscan") == 0) { p->fullscan = value ? 1 : 0; return HOUGH_OK; }
     if (strcmp(key, "peaks_tiled") == 0) { p->peaks_tiled = value ? 1 : 0; return HOUGH_OK; }
+    if (strcmp(key, "peaks_regs") == 0) { p->peaks_regs = value ? 1 : 0; return HOUGH_OK; }
     if (strcmp(key, "peaks_scalar") == 0) { p->peaks_scalar = value ? 1 : 0; return HOUGH_OK; }
     if (strcmp(key, "exact_walk") == 0) { p->exact_walk = value ? 1 : 0; return HOUGH_OK; }
     if (strcmp(key, "reuse_staging") == 0) { p->reuse_staging = value ? 1 : 0; p->staged_hits = nullptr; return HOUGH_OK; }

@@ -217,6 +217,9 @@ def test_assign_tile_variants_bit_exact(shape, dtype, max_hits, dj):
     ((64, 64, 40), ACC_U16, False, False),      # slice walk cut into several slice runs
     ((32, 8, 5), ACC_I32, False, False),        # slice walk, one 16-byte chunk pair per row
     ((64, 64, 40), ACC_U16, False, "scalar"),   # 16-bit bins through the unpacked slice walk
+    ((64, 64, 40), ACC_U16, False, "regs"),     # packed walk with register-held rows (no cp.async ring)
+    ((256, 128, 1), ACC_U16, False, "regs"),
+    ((512, 2048, 3), ACC_U16, False, False),    # cp.async ring: one row per CTA (256 chunks per row)
     ((32, 8, 5), ACC_U16, False, False),        # packed slice walk, one chunk per row (both q/pT faces in one thread)
 ])
 def test_peaks_tile_variants_bit_exact(shape, dtype, fullscan, tiled):
@@ -231,7 +234,8 @@ def test_peaks_tile_variants_bit_exact(shape, dtype, fullscan, tiled):
     assert ref.total > 20
     for cap in (ref.total + 3, ref.total // 2):
         got = run_cuda(bn, 3.8, LAYERS_10, hits, off, thr, 1, 2, cap, fullscan=fullscan,
-                       options=("peaks_scalar",) if tiled == "scalar" else (("peaks_tiled",) if tiled else ()))
+                       options=("peaks_scalar",) if tiled == "scalar" else (("peaks_regs",) if tiled == "regs" else
+                                                                              (("peaks_tiled",) if tiled else ())))
         assert got.total == ref.total and np.array_equal(got.offsets, ref.offsets)
         n_c = min(cap, ref.total)
         for f in ("event", "k", "i", "j", "votes"):
