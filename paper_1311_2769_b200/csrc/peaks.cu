@@ -720,25 +720,33 @@ __global__ void __launch_bounds__(256, 3) peak_stream16_kernel(HoughConsts c, co
     const int i0 = rb * R, i = i0 + rl;
     const int k0 = seg * kseg, k1 = min(k0 + kseg, nd);
     const int stage_halfwords = (R + 2) * nq;
-    const int n_chunks = (R + 2) * cpr;                         // 16-byte chunks per stage (<= 512)
     const unsigned short* ev = acc + (size_t)e * (size_t)c.bins_per_event;
     unsigned short* s_base = reinterpret_cast<unsigned short*>(ps_smem);
     unsigned char* mask_bytes = reinterpret_cast<unsigned char*>(mask + (size_t)e * c.words_per_event);
     const unsigned thr2 = (unsigned)threshold * 0x00010001u;
 
-    // fill stage `stage` with slice v (rows i0 - 1 .. i0 + R, cyclic); slices outside [0, nd) are all "missing" = 0
+    // fill stage `stage` with slice v (rows i0 - 1 .. i0 + R, cyclic); slices outside [0, nd) are all "missing" = 0.
+    // A thread copies chunk tid and, for tid < 2 * cpr, chunk 256 + tid (the last two rows): offsets fixed per thread.
+    const size_t slice_bins = (size_t)nphi * nq;
+    int gi_a = i0 - 1 + rl;
+    gi_a = gi_a < 0 ? gi_a + nphi : gi_a;
+    const unsigned short* src_a = ev + (size_t)gi_a * nq + j0;              // stage row rl
+    const int dst_a = rl * nq + j0;
+    const bool has_b = tid < 2 * cpr;
+    int gi_b = i0 - 1 + R + rl;                                             // stage rows R, R + 1 (rl = 0, 1 here)
+    gi_b = gi_b >= nphi ? gi_b - nphi : gi_b;
+    const unsigned short* src_b = ev + (size_t)gi_b * nq + j0;
+    const int dst_b = (R + rl) * nq + j0;
+    const unsigned s_base_saddr = (unsigned)__cvta_generic_to_shared(s_base);
     auto issue = [&](int v, int stage) {
-        unsigned short* st = s_base + (size_t)stage * stage_halfwords;
-        for (int idx = tid; idx < n_chunks; idx += 256) {
-            const int sr = idx / cpr, ch = idx - sr * cpr;
-            unsigned short* dst = st + sr * nq + ch * 8;
-            if (v < 0 || v >= nd) {
-                *reinterpret_cast<uint4*>(dst) = make_uint4(0u, 0u, 0u, 0u);
-            } else {
-                int gi = i0 - 1 + sr;
-                gi = gi < 0 ? gi + nphi : (gi >= nphi ? gi - nphi : gi);
-                ps_cp_async16((unsigned)__cvta_generic_to_shared(dst), ev + ((size_t)v * nphi + gi) * nq + ch * 8);
-            }
+        const int so = stage * stage_halfwords;
+        if (v < 0 || v >= nd) {
+            *reinterpret_cast<uint4*>(s_base + so + dst_a) = make_uint4(0u, 0u, 0u, 0u);
+            if (has_b) *reinterpret_cast<uint4*>(s_base + so + dst_b) = make_uint4(0u, 0u, 0u, 0u);
+        } else {
+            const size_t go = (size_t)v * slice_bins;
+            ps_cp_async16(s_base_saddr + 2u * (unsigned)(so + dst_a), src_a + go);
+            if (has_b) ps_cp_async16(s_base_saddr + 2u * (unsigned)(so + dst_b), src_b + go);
         }
         ps_commit();
     };
@@ -833,7 +841,7 @@ extern "C" int hough_find_peaks(hough_plan* p, const void* d_accum, int32_t n_ev
         HOUGH_CUDA_TRY(cudaMemsetAsync(p->d_peak_block_cnt, 0, sizeof(int32_t) * (size_t)n_events * bpe, st));
         const int cpr16 = p->c.n_qpt / 8;
         const bool stream16 = p->c.is_u16 && threshold >= 1 && threshold <= 65535 && !p->peaks_scalar && !p->peaks_regs &&
-                              cpr16 <= 256 && 256 % cpr16 == 0 && p->c.n_phi % (256 / cpr16) == 0 &&
+                              cpr16 <= 128 && 256 % cpr16 == 0 && p->c.n_phi % (256 / cpr16) == 0 &&
                               (size_t)PS_STAGES * (256 / cpr16 + 2) * p->c.n_qpt * 2 <= 64 * 1024;
         if (stream16) {
             const int R = 256 / cpr16;
