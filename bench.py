@@ -452,6 +452,52 @@ def run_ours(args, rank, world, local_rank):
         dist.destroy_process_group()
 
 
+def run_sweep(args):
+    """Fig. 2-style sweep ("time performance, as a function of number of tracks") on the
+    paper's toy detector (workload 5): one event of n tracks, vote + peaks + assign, median device time of `reps` runs.
+    Prints one JSON line per n (not the driver's bench line)."""
+    import torch
+    from paper_1311_2769_b200 import HoughPlan, alloc_candidates, load_library
+    from workloads import generate_events, get_workload
+    load_library()
+    torch.cuda.set_device(0)
+    base = get_workload(5)
+    for n in (50, 100, 200, 500, 1000, 2000, 5000, 10000, 20000):
+        w = base.with_tracks(n)
+        batch = generate_events(w)
+        plan = HoughPlan.from_workload(w, max_hits=max(batch.n_hits, 1), max_events=1)
+        plan.set_option("reuse_staging", 1)
+        d_hits = torch.from_numpy(batch.hits_xy).cuda()
+        d_off = torch.from_numpy(batch.event_offsets).cuda()
+        accum = plan.alloc_accum(1)
+        cap = w.binning.n_bins // 8 + 1024
+        cands = alloc_candidates(cap)
+        coff = torch.zeros(2, dtype=torch.int32, device="cuda")
+        h2c = torch.empty(max(batch.n_hits, 1), dtype=torch.int32, device="cuda")
+        nh = torch.empty(cap, dtype=torch.int32, device="cuda")
+        keep = torch.empty(cap, dtype=torch.uint8, device="cuda")
+
+        def once():
+            plan.vote(d_hits, d_off, accum)
+            plan.find_peaks(accum, 1, w.threshold, cands, cap, coff)
+            plan.assign_hits(d_hits, d_off, cands, coff, cap, w.assoc_dj, w.min_hits, h2c, nh, keep)
+        for _ in range(5):
+            once()
+        torch.cuda.synchronize()
+        times = []
+        for _ in range(args.sweep_reps):
+            a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+            a.record(); once(); b.record(); b.synchronize()
+            times.append(a.elapsed_time(b))
+        votes = int(accum.to(torch.int64).sum().item())
+        n_c = int(coff[1].item())
+        kept = int(keep[:min(n_c, cap)].sum().item())
+        print(json.dumps({"sweep": "paper_toy_2d", "cite": "P:L39, P:L55", "n_tracks": n, "hits": batch.n_hits, "votes": votes,
+                          "peaks": n_c, "kept": kept, "ms_median": statistics.median(times), "ms_min": min(times),
+                          "reps": args.sweep_reps}), flush=True)
+        plan.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -470,7 +516,12 @@ def main():
     ap.add_argument("--smem-atomic-random-gops", type=float, default=3304.0)
     ap.add_argument("--smem-atomic-gops", type=float, default=7593.0,
                     help="measured conflict-free shared atomicAdd rate, Gops/s (profiles/microbench_r1.md)")
+    ap.add_argument("--sweep-tracks", action="store_true", help="Fig. 2-style sweep on the paper's toy detector (workload 5)")
+    ap.add_argument("--sweep-reps", type=int, default=30)
     args = ap.parse_args()
+    if args.sweep_tracks:
+        run_sweep(args)
+        return
     rank, world, local_rank = _env_int("RANK", 0), _env_int("WORLD_SIZE", 1), _env_int("LOCAL_RANK", 0)
     if args.impl == "reference":
         run_reference(args, rank, world)

@@ -64,6 +64,15 @@ def test_config_0_1_exact_walk_and_tiled_peaks(cfg):
     _compare_all(w, generate_events(w), options=("exact_walk", "peaks_tiled"))
 
 
+def test_paper_toy_workload_bit_exact():
+    """the paper's own scenario (10 evenly spaced layers 3 -> 110 cm, 0.4 mm, 500 tracks)."""
+    w = get_workload(5)
+    got, ref = _compare_all(w, generate_events(w))
+    assert ref.total > 100
+    w2 = w.with_tracks(3000)                              # Fig. 2-style: more tracks, same detector
+    _compare_all(w2, generate_events(w2))
+
+
 def test_config_2_bit_exact():
     w = get_workload(2)
     _compare_all(w, generate_events(w), oracle_parallel=True)

@@ -451,3 +451,31 @@ def test_workload_shapes_match_baseline():
     # event e is the same whether generated alone or in a batch (per-event Philox key)
     assert np.array_equal(generate_events(w3, events=[2]).hits_xy, b3.event(2))
     assert len(LAYERS_14) == 14
+
+
+def test_paper_toy_workload_shape_and_physics_sanity():
+    """PAPER.md:39 (Fig. 1): beampipe 3.0 cm, ten evenly spaced layers out to 110.0 cm, 500 curved prompt tracks.
+    Not a parity pin: the found-track fraction depends on the (unstated) binning; it only has to be sane."""
+    import math
+    from workloads import LAYERS_PAPER_TOY
+    w = get_workload(5)
+    assert len(w.layers) == 10 and abs(w.layers[-1] - 110.0) < 1e-9 and abs(w.layers[0] - 13.7) < 1e-9
+    assert np.allclose(np.diff((3.0,) + tuple(LAYERS_PAPER_TOY)), 10.7)
+    assert w.n_prompt == 500 and w.n_displaced == 0 and w.binning.n_d0 == 1 and abs(w.sigma_rphi_cm - 0.04) < 1e-12
+    batch = generate_events(w, want_truth=True)
+    r = np.hypot(batch.hits_xy[:, 0], batch.hits_xy[:, 1])
+    assert batch.n_hits == 5000 and np.allclose(np.sort(np.unique(np.round(r, 3))), np.round(LAYERS_PAPER_TOY, 3), atol=2e-3)
+    o = Oracle.from_binning(w.binning, w.bz_tesla)
+    acc, votes = o.vote(batch.hits_xy, batch.event_offsets)
+    ref = o.find_peaks(acc, w.threshold)
+    h2c, nh, keep = o.assign_indexed(batch.hits_xy, batch.event_offsets, ref, w.assoc_dj, w.min_hits)
+    rec = ref.records[keep.astype(bool)]
+    t = batch.truth[0]
+    bn = w.binning
+    ti = np.floor(np.mod(t["direction"], 2 * math.pi) / (2 * math.pi) * bn.n_phi).astype(int)
+    tj = np.floor((t["charge"] / t["pt"] - bn.qpt_min) / (bn.qpt_max - bn.qpt_min) * bn.n_qpt).astype(int)
+    found = 0
+    for a, c in zip(ti, tj):
+        d = np.abs(((rec["i"] - a + bn.n_phi // 2) % bn.n_phi) - bn.n_phi // 2)
+        found += bool(np.any((d <= 1) & (np.abs(rec["j"] - c) <= 2)))
+    assert 0.25 < found / 500 < 1.0 and len(rec) < 500

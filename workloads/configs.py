@@ -15,6 +15,9 @@ ACC_U16 = 1
 
 # B:L7 -- 10 cylindrical barrel layers [cm]
 LAYERS_10: Tuple[float, ...] = (4.0, 7.0, 11.0, 25.0, 34.0, 43.0, 52.0, 61.0, 70.0, 110.0)
+# PAPER.md:39 (section 3, Fig. 1): "a beampipe with radius of 3.0 cm, surrounded by ten concentric, evenly-spaced
+# tracking layers with an outer radius of 110.0 cm" -- reading: spacing (110 - 3) / 10, first layer one spacing out
+LAYERS_PAPER_TOY: Tuple[float, ...] = tuple(3.0 + 10.7 * l for l in range(1, 11))
 # B:L9 "14 barrel layers from 4 to 110 cm"; radii per SURVEY S15 (config-0 radii plus 16, 80, 90, 100)
 LAYERS_14: Tuple[float, ...] = (4.0, 7.0, 11.0, 16.0, 25.0, 34.0, 43.0, 52.0, 61.0, 70.0, 80.0, 90.0, 100.0, 110.0)
 
@@ -69,6 +72,10 @@ class HoughWorkload:
         """Same generation law, different number of events (event e is identical in both)."""
         return replace(self, n_events=n_events)
 
+    def with_tracks(self, n_prompt: int) -> "HoughWorkload":
+        """Same detector and binning, another number of prompt tracks (Fig. 2-style sweeps)."""
+        return replace(self, n_prompt=n_prompt, name=f"{self.name}_{n_prompt}trk")
+
 
 WORKLOADS = {
     0: HoughWorkload(name="cfg0_single_prompt_2d", seed=1, n_events=1, layers=LAYERS_10,
@@ -86,6 +93,14 @@ WORKLOADS = {
     4: HoughWorkload(name="cfg4_fine_binned", seed=5, n_events=1, layers=LAYERS_14,
                      n_prompt=10000, n_displaced=200, n_noise=20000, pt_law="exp", pt_min=0.9, pt_max=0.0,
                      binning=HoughBinning(1024, 512, 128, accum_dtype=ACC_U16), threshold=11, cite="B:L11"),
+    # the paper's own toy scenario (Fig. 1): transverse plane, 10 evenly spaced layers
+    # 3 -> 110 cm, 0.4 mm hit resolution, 500 curved prompt tracks, two-parameter space.  The paper states
+    # neither field, pT spectrum, binning nor threshold: 3.8 T, pT = 1 GeV + Exp(2 GeV), 512 x 256 bins and threshold 8
+    # (of 10 layers) are this build's choices.
+    5: HoughWorkload(name="paper_toy_2d", seed=6, n_events=1, layers=LAYERS_PAPER_TOY,
+                     n_prompt=500, n_displaced=0, n_noise=0, pt_law="exp", pt_min=1.0, pt_max=0.0,
+                     binning=HoughBinning(512, 256, 1, accum_dtype=ACC_I32), threshold=8,
+                     sigma_rphi_cm=0.04, cite="P:L39"),
 }
 
 
