@@ -489,11 +489,32 @@ def run_sweep(args):
             a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
             a.record(); once(); b.record(); b.synchronize()
             times.append(a.elapsed_time(b))
+        # the same three calls captured once in a CUDA graph and replayed (the calls only enqueue: include/hough.h)
+        gtimes = []
+        try:
+            side = torch.cuda.Stream()
+            side.wait_stream(torch.cuda.current_stream())
+            with torch.cuda.stream(side):
+                once()
+            torch.cuda.current_stream().wait_stream(side)
+            graph = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(graph):
+                once()
+            for _ in range(5):
+                graph.replay()
+            torch.cuda.synchronize()
+            for _ in range(args.sweep_reps):
+                a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+                a.record(); graph.replay(); b.record(); b.synchronize()
+                gtimes.append(a.elapsed_time(b))
+        except Exception as exc:                          # noqa: BLE001 -- report, do not hide
+            print(f"bench.py: graph capture failed: {exc}", file=sys.stderr)
         votes = int(accum.to(torch.int64).sum().item())
         n_c = int(coff[1].item())
         kept = int(keep[:min(n_c, cap)].sum().item())
         print(json.dumps({"sweep": "paper_toy_2d", "cite": "P:L39, P:L55", "n_tracks": n, "hits": batch.n_hits, "votes": votes,
                           "peaks": n_c, "kept": kept, "ms_median": statistics.median(times), "ms_min": min(times),
+                          "ms_graph_median": statistics.median(gtimes) if gtimes else None,
                           "reps": args.sweep_reps}), flush=True)
         plan.close()
 
