@@ -178,6 +178,47 @@ def test_vote_tile_variants_bit_exact(shape, dtype, max_hits, layers, misalign):
     assert np.array_equal(got.astype(np.int32), acc)
 
 
+@pytest.mark.parametrize("seed", list(range(40)))
+def test_random_configurations_bit_exact(seed):
+    """Differential test over randomly drawn binnings (asymmetric and one-sided q/pT ranges, off-centre d0 ranges,
+    odd sizes, both dtypes, several fields, with and without layer geometry): the fast path's error bound, windows and
+    tile variants must never change a result."""
+    rng = np.random.default_rng(1000 + seed)
+    n_phi = 4 * int(rng.integers(2, 160))
+    n_qpt = int(rng.choice([8, 24, 37, 64, 128, 200, 256, 333]))
+    n_d0 = int(rng.choice([1, 2, 3, 5, 8]))
+    qa, qb = sorted(rng.uniform(-1.5, 1.5, 2))
+    if seed % 4 == 0:
+        qa = 0.0                                           # one-sided range: c0 = 0
+    if qb - qa < 0.2:
+        qb = qa + 0.2
+    da, db = sorted(rng.uniform(-25.0, 25.0, 2))
+    if db - da < 2.0:
+        db = da + 2.0
+    dtype = ACC_U16 if seed % 2 else ACC_I32
+    bz = float(rng.choice([3.8, 2.0, -3.8, 1.0]))
+    layers = LAYERS_10 if seed % 3 else ()
+    bn = HoughBinning(n_phi, n_qpt, n_d0, float(np.float32(qa)), float(np.float32(qb)), float(np.float32(da)),
+                      float(np.float32(db)), dtype)
+    hits, off = _mixed_hits(5000 + seed, 2500, LAYERS_10)
+    o = Oracle.from_binning(bn, bz)
+    acc, votes = o.vote(hits, off)
+    thr = 3
+    dj = int(rng.integers(0, 4))
+    ref = o.find_peaks(acc, thr)
+    cap = ref.total + 5
+    got = run_cuda(bn, bz, layers, hits, off, thr, dj, 2, cap)
+    assert np.array_equal(got.accum.astype(np.int32), acc), "accumulator differs"
+    assert got.total == ref.total and np.array_equal(got.offsets, ref.offsets)
+    for f in ("event", "k", "i", "j", "votes"):
+        assert np.array_equal(got.records[f], ref.records[f]), f
+    assert_centroids_close(got.records, ref.records, bn)
+    h2c, nh, keep = o.assign_indexed(hits, off, ref, dj, 2, capacity=cap)
+    assert np.array_equal(got.hit_to_cand, h2c), "hit_to_cand differs"
+    assert np.array_equal(got.cand_nhits[:ref.total], nh) and np.array_equal(got.cand_keep[:ref.total], keep)
+    assert votes > 0 or seed % 4 != 1
+
+
 def test_vote_half_circle_windows_and_negative_field():
     """A r q > 1 on the outer layers (windows = the whole forward half, wrap-around in every tile) and Bz < 0."""
     hits, off = _mixed_hits(9, 2000, LAYERS_10)
