@@ -282,7 +282,8 @@ class DeviceRun:
         return total
 
 
-def e2e_pipeline(run: DeviceRun, steps: int, warmup: int, n_streams: int, tile_events: int, cand_per_bin: float):
+def e2e_pipeline(run: DeviceRun, steps: int, warmup: int, n_streams: int, tile_events: int, cand_per_bin: float,
+                 kept_only: bool = False):
     """End-to-end through the library's batched path (hough_pipeline_run_host): pinned HOST buffers in (hits, offsets)
     and out (hit_to_cand, cand_offsets, candidate records, nhits, keep); every host<->device copy is inside the
     timed region.  Wall-clock around the blocking call (it returns when the results are in the host buffers)."""
@@ -295,6 +296,8 @@ def e2e_pipeline(run: DeviceRun, steps: int, warmup: int, n_streams: int, tile_e
     max_hits = max(int(off[min(e0 + tile_events, batch.n_events)] - off[e0]) for e0 in range(0, batch.n_events, tile_events))
     tile_cap = int(cand_per_bin * w.binning.n_bins * tile_events) + 1024
     pipe = HoughPipeline.from_workload(w, tile_events, max(max_hits, 1), tile_cap, n_streams)
+    if kept_only:
+        pipe.set_option("kept_only", 1)
     total_cap = int(sum(int(t) for t in run.totals.tolist())) + 1024
     h_hits = torch.from_numpy(batch.hits_xy).pin_memory()
     h_off = torch.from_numpy(batch.event_offsets.astype(np.int32)).pin_memory()
@@ -320,6 +323,8 @@ def e2e_pipeline(run: DeviceRun, steps: int, warmup: int, n_streams: int, tile_e
     n_c = int(out_off[batch.n_events])
     h2d = batch.n_hits * 8 + (batch.n_events + n_tiles) * 4
     d2h = (batch.n_events + n_tiles) * 4 + batch.n_hits * 4 + min(n_c, total_cap) * (32 + 4 + 1)
+    if kept_only:                                        # two offset arrays per tile; keep flags are not copied
+        d2h = 2 * (batch.n_events + n_tiles) * 4 + batch.n_hits * 4 + min(n_c, total_cap) * (32 + 4)
     pipe.close()
     return ms, h2d, d2h, over
 
@@ -381,10 +386,12 @@ def run_ours(args, rank, world, local_rank):
     # e2e leg (host buffers in and out), same workload
     e2e_ms, h2d, d2h, e2e_over = e2e_pipeline(run, max(1, min(args.steps, args.e2e_steps)), 1, args.streams, args.e2e_tile_events,
                                                 args.cand_per_bin)
-    te = torch.tensor([e2e_ms], dtype=torch.float64, device="cuda")
+    k_ms, k_h2d, k_d2h, k_over = e2e_pipeline(run, max(1, min(args.steps, args.e2e_steps)), 1, args.streams,
+                                              args.e2e_tile_events, args.cand_per_bin, kept_only=True)
+    te = torch.tensor([e2e_ms, k_ms], dtype=torch.float64, device="cuda")
     if world > 1:
         dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_ms = float(te.item())
+    e2e_ms, k_ms = (float(x) for x in te.tolist())
 
     if rank != 0:
         if world > 1:
@@ -445,6 +452,11 @@ def run_ours(args, rank, world, local_rank):
                     "api": f"hough_pipeline_run_host: {min(args.e2e_tile_events, batch.n_events)}-event tiles on {args.streams} streams, CUDA graph per "
                            "lane, pinned host buffers in and out; wall clock around the blocking call",
                     "candidate_overflow": bool(e2e_over)},
+            "e2e_kept_only": {"value": job_votes / (k_ms * 1e-3), "unit": UNIT, "events_per_s": job_events / (k_ms * 1e-3),
+                              "ms_per_step": k_ms, "h2d_bytes_per_step": int(k_h2d), "d2h_bytes_per_step": int(k_d2h),
+                              "api": "the same pipeline with option kept_only: identical work, only the candidates that "
+                                     "survive duplicate removal are compacted on the device and copied back",
+                              "candidate_overflow": bool(k_over)},
             "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks,
             "candidate_overflow": peaks_overflow}
     print(json.dumps(line), flush=True)

@@ -140,6 +140,13 @@ int hough_pipeline_create(const hough_binning* binning, const hough_geometry* ge
                           int32_t max_hits_per_tile, int32_t tile_cand_capacity, int32_t n_streams,
                           hough_pipeline** out);
 int hough_pipeline_destroy(hough_pipeline* p);
+/* Pipeline options.  "kept_only" = 1: only the candidates that survive duplicate removal (D9, cand_keep = 1) are
+ * returned -- the tile's kept records are compacted on the device before the copy, h_cand_offsets are the offsets of
+ * the KEPT list, h_hit_to_cand indexes it (hits of dropped candidates are -1 as always), h_cand_nhits follows it and
+ * h_cand_keep is 1 for every returned candidate; cand_capacity then bounds the kept list.  All the work (vote, peaks,
+ * association) is unchanged; only the result transfer shrinks (config 3: 1.0 GB -> 45 MB per 1024 events).
+ * "graphs" = 0 / 1: CUDA graph capture off / on.  INVALID_ARG for unknown keys. */
+int hough_pipeline_set_option(hough_pipeline* p, const char* key, int32_t value);
 int hough_pipeline_run_host(hough_pipeline* p, const float* h_hits_xy, int32_t n_hits,
                             const int32_t* h_event_offsets, int32_t n_events, int32_t threshold,
                             int32_t assoc_dj, int32_t min_hits, int32_t* h_hit_to_cand,

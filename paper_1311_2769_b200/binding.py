@@ -39,7 +39,7 @@ class hough_geometry(C.Structure):
 
 EXPORTS = ["hough_plan_create", "hough_plan_destroy", "hough_accum_bytes", "hough_vote", "hough_find_peaks",
            "hough_assign_hits", "hough_plan_set_option", "hough_pipeline_create", "hough_pipeline_destroy",
-           "hough_pipeline_run_host", "hough_window_table", "hough_microbench", "hough_kernel_launches", "hough_status_string",
+           "hough_pipeline_run_host", "hough_pipeline_set_option", "hough_window_table", "hough_microbench", "hough_kernel_launches", "hough_status_string",
            "hough_version"]
 
 _lib = None
@@ -73,6 +73,8 @@ def load_library() -> C.CDLL:
     lib.hough_pipeline_create.argtypes = [C.POINTER(hough_binning), C.POINTER(hough_geometry), I, I, I, I, C.POINTER(P)]
     lib.hough_pipeline_destroy.restype = C.c_int
     lib.hough_pipeline_destroy.argtypes = [P]
+    lib.hough_pipeline_set_option.restype = C.c_int
+    lib.hough_pipeline_set_option.argtypes = [P, C.c_char_p, I]
     lib.hough_pipeline_run_host.restype = C.c_int
     lib.hough_pipeline_run_host.argtypes = [P, P, I, P, I, I, I, I, P, P, P, I, P, P, P]
     lib.hough_window_table.restype = C.c_int
@@ -225,6 +227,9 @@ class HoughPipeline:
             self.close()
         except Exception:
             pass
+
+    def set_option(self, key: str, value: int):
+        _check(self.lib.hough_pipeline_set_option(self._h, key.encode(), int(value)), "hough_pipeline_set_option")
 
     def run_host(self, hits_xy, event_offsets, threshold, assoc_dj, min_hits, hit_to_cand, cand_offsets, cands,
                  cand_capacity, cand_nhits, cand_keep) -> bool:

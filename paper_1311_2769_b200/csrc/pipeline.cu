@@ -11,6 +11,7 @@
 // t is issued when tile t + n_streams is about to reuse the lane, so n_streams - 1 tiles are always in flight while
 // the host waits for a count.  Host buffers should be pinned (copies are cudaMemcpyAsync).
 #include <algorithm>
+#include <cstring>
 #include <new>
 #include <vector>
 
@@ -28,6 +29,82 @@ __global__ void __launch_bounds__(256) rebase_kernel(int32_t* __restrict__ hit_t
     if (t < n_cands) cands[t].event += event_base;
 }
 
+// ---- "kept_only" mode: compact the candidates that survive duplicate removal (D9) on the device -------------------
+constexpr int KEEP_BLOCK = 4096;                      // candidates per compaction block (256 threads x 16)
+
+// kept candidates per block of KEEP_BLOCK; n_c = min(cand_off[n_ev], cap) is read on the device
+__global__ void __launch_bounds__(256) keep_count_kernel(const uint8_t* __restrict__ keep, const int32_t* __restrict__ cand_off,
+                                                         int n_ev, int cap, int32_t* __restrict__ blk) {
+    const int n_c = min(cand_off[n_ev], cap);
+    const int base = blockIdx.x * KEEP_BLOCK + threadIdx.x * 16;
+    int cnt = 0;
+    if (base + 16 <= n_c) {
+        const uint4 q = *reinterpret_cast<const uint4*>(keep + base);            // flags are 0 / 1
+        cnt = __popc(q.x) + __popc(q.y) + __popc(q.z) + __popc(q.w);
+    } else {
+        for (int c = base; c < min(base + 16, n_c); ++c) cnt += keep[c];
+    }
+    cnt = __reduce_add_sync(0xffffffffu, cnt);
+    __shared__ int s[8];
+    if ((threadIdx.x & 31) == 0) s[threadIdx.x >> 5] = cnt;
+    __syncthreads();
+    if (threadIdx.x == 0) blk[blockIdx.x] = s[0] + s[1] + s[2] + s[3] + s[4] + s[5] + s[6] + s[7];
+}
+
+__global__ void __launch_bounds__(1024) keep_scan_kernel(int32_t* blk, int n_blk) {
+    cta_exclusive_scan(blk, n_blk, blk + n_blk);          // blk[n_blk] = kept candidates of the tile
+}
+
+// pre[c] = kept candidates before c (for every c < n_c); kept records and their hit counts move to rank pre[c]
+__global__ void __launch_bounds__(256) keep_compact_kernel(const uint8_t* __restrict__ keep, const int32_t* __restrict__ cand_off,
+                                                           int n_ev, int cap, const int32_t* __restrict__ blk,
+                                                           const hough_candidate* __restrict__ cands, const int32_t* __restrict__ nh,
+                                                           int32_t* __restrict__ pre, hough_candidate* __restrict__ kcands,
+                                                           int32_t* __restrict__ knh) {
+    const int n_c = min(cand_off[n_ev], cap);
+    const int base = blockIdx.x * KEEP_BLOCK + threadIdx.x * 16;
+    int cnt = 0;
+    for (int c = base; c < min(base + 16, n_c); ++c) cnt += keep[c];
+    int x = cnt;                                          // inclusive scan over the block's 256 threads
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const int y = __shfl_up_sync(0xffffffffu, x, o);
+        if ((threadIdx.x & 31) >= o) x += y;
+    }
+    __shared__ int s[8];
+    if ((threadIdx.x & 31) == 31) s[threadIdx.x >> 5] = x;
+    __syncthreads();
+    int run = blk[blockIdx.x] + x - cnt;
+    for (int w = 0; w < (int)(threadIdx.x >> 5); ++w) run += s[w];
+    for (int c = base; c < min(base + 16, n_c); ++c) {
+        pre[c] = run;
+        if (keep[c]) {
+            const int4* src = reinterpret_cast<const int4*>(cands + c);
+            int4* dst = reinterpret_cast<int4*>(kcands + run);
+            dst[0] = src[0];
+            dst[1] = src[1];
+            knh[run] = nh[c];
+            ++run;
+        }
+    }
+}
+
+// per-event offsets of the kept list and hit -> kept rank (hits of dropped candidates are already -1, D9)
+__global__ void __launch_bounds__(256) keep_finish_kernel(const int32_t* __restrict__ cand_off, int n_ev, int cap,
+                                                          const int32_t* __restrict__ blk, int n_blk, const int32_t* __restrict__ pre,
+                                                          int32_t* __restrict__ kept_off, int32_t* __restrict__ h2c, int n_hits) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    const int n_c = min(cand_off[n_ev], cap);
+    if (t <= n_ev) {
+        const int c = cand_off[t];
+        kept_off[t] = c < n_c ? pre[c] : blk[n_blk];
+    }
+    if (t < n_hits) {
+        const int c = h2c[t];
+        if (c >= 0) h2c[t] = pre[c];
+    }
+}
+
 struct Lane {
     cudaStream_t st = nullptr;
     hough_plan* plan = nullptr;
@@ -41,6 +118,13 @@ struct Lane {
     uint8_t* d_keep = nullptr;
     int32_t* h_off = nullptr;        // pinned: tile-relative event offsets
     int32_t* h_cand_off = nullptr;   // pinned: the tile's exclusive per-event candidate offsets
+    // kept_only mode
+    int32_t* d_pre = nullptr;        // [cap] kept candidates before each candidate
+    int32_t* d_blk = nullptr;        // [cap / KEEP_BLOCK + 2]
+    hough_candidate* d_kcands = nullptr;
+    int32_t* d_knh = nullptr;
+    int32_t* d_kept_off = nullptr;   // [tile_events + 1]
+    int32_t* h_kept_off = nullptr;   // pinned
     cudaEvent_t counted = nullptr;
     cudaGraphExec_t exec = nullptr;
     bool warmed = false;             // first tile of a lane runs un-captured (lazy kernel attributes)
@@ -55,6 +139,7 @@ struct hough_pipeline {
     int32_t tile_events, max_hits, tile_cap, n_streams;
     std::vector<Lane> lanes;
     int use_graphs;
+    int kept_only;
 };
 
 static void pipeline_free(hough_pipeline* p) {
@@ -67,6 +152,8 @@ static void pipeline_free(hough_pipeline* p) {
         cudaFree(l.d_h2c); cudaFree(l.d_nh); cudaFree(l.d_keep);
         if (l.h_off) cudaFreeHost(l.h_off);
         if (l.h_cand_off) cudaFreeHost(l.h_cand_off);
+        cudaFree(l.d_pre); cudaFree(l.d_blk); cudaFree(l.d_kcands); cudaFree(l.d_knh); cudaFree(l.d_kept_off);
+        if (l.h_kept_off) cudaFreeHost(l.h_kept_off);
         if (l.st) cudaStreamDestroy(l.st);
     }
     delete p;
@@ -87,6 +174,7 @@ extern "C" int hough_pipeline_create(const hough_binning* b, const hough_geometr
     p->n_streams = n_streams;
     const char* env = getenv("HOUGH_PIPELINE_NO_GRAPHS");
     p->use_graphs = (env && env[0] == '1') ? 0 : 1;
+    p->kept_only = 0;
     p->lanes.resize(n_streams);
     int rc = HOUGH_OK;
     for (Lane& l : p->lanes) {
@@ -110,6 +198,29 @@ extern "C" int hough_pipeline_create(const hough_binning* b, const hough_geometr
     }
     if (rc != HOUGH_OK) { pipeline_free(p); return rc; }
     *out = p;
+    return HOUGH_OK;
+}
+
+extern "C" int hough_pipeline_set_option(hough_pipeline* p, const char* key, int32_t value) {
+    if (!p || !key) return HOUGH_ERR_INVALID_ARG;
+    if (strcmp(key, "graphs") == 0) { p->use_graphs = value ? 1 : 0; return HOUGH_OK; }
+    if (strcmp(key, "kept_only") != 0) return HOUGH_ERR_INVALID_ARG;
+    if (value && !p->lanes.empty() && !p->lanes[0].d_pre) {          // buffers of the compaction, once
+        const size_t cap = (size_t)std::max(p->tile_cap, 1);
+        for (Lane& l : p->lanes) {
+            bool ok = cudaMalloc((void**)&l.d_pre, sizeof(int32_t) * cap) == cudaSuccess;
+            ok = ok && cudaMalloc((void**)&l.d_blk, sizeof(int32_t) * (cap / KEEP_BLOCK + 2)) == cudaSuccess;
+            ok = ok && cudaMalloc((void**)&l.d_kcands, sizeof(hough_candidate) * cap) == cudaSuccess;
+            ok = ok && cudaMalloc((void**)&l.d_knh, sizeof(int32_t) * cap) == cudaSuccess;
+            ok = ok && cudaMalloc((void**)&l.d_kept_off, sizeof(int32_t) * ((size_t)p->tile_events + 1)) == cudaSuccess;
+            ok = ok && cudaMallocHost((void**)&l.h_kept_off, sizeof(int32_t) * ((size_t)p->tile_events + 1)) == cudaSuccess;
+            if (!ok) { (void)cudaGetLastError(); return HOUGH_ERR_ALLOC; }
+        }
+    }
+    p->kept_only = value ? 1 : 0;
+    for (Lane& l : p->lanes) {                           // another node list: the lanes' graphs are rebuilt
+        if (l.exec) { cudaGraphExecDestroy(l.exec); l.exec = nullptr; }
+    }
     return HOUGH_OK;
 }
 
@@ -137,6 +248,20 @@ static int enqueue_part_a(hough_pipeline* p, Lane& l, const float* h_hits_xy, in
     if (rc != HOUGH_OK) return rc;
     HOUGH_CUDA_TRY(cudaMemcpyAsync(l.h_cand_off, l.d_cand_off, sizeof(int32_t) * ((size_t)n_ev + 1), cudaMemcpyDeviceToHost,
                                    l.st));
+    if (p->kept_only && p->tile_cap > 0) {
+        const int n_blk = p->tile_cap / KEEP_BLOCK + 1;
+        keep_count_kernel<<<n_blk, 256, 0, l.st>>>(l.d_keep, l.d_cand_off, n_ev, p->tile_cap, l.d_blk);
+        keep_scan_kernel<<<1, 1024, 0, l.st>>>(l.d_blk, n_blk);
+        keep_compact_kernel<<<n_blk, 256, 0, l.st>>>(l.d_keep, l.d_cand_off, n_ev, p->tile_cap, l.d_blk, l.d_cands, l.d_nh, l.d_pre,
+                                                     l.d_kcands, l.d_knh);
+        const int n_thr = std::max(n_h, n_ev + 1);
+        keep_finish_kernel<<<(n_thr + 255) / 256, 256, 0, l.st>>>(l.d_cand_off, n_ev, p->tile_cap, l.d_blk, n_blk, l.d_pre,
+                                                                 l.d_kept_off, l.d_h2c, n_h);
+        HOUGH_CUDA_TRY(cudaGetLastError());
+        hough_count_launches(4);
+        HOUGH_CUDA_TRY(cudaMemcpyAsync(l.h_kept_off, l.d_kept_off, sizeof(int32_t) * ((size_t)n_ev + 1), cudaMemcpyDeviceToHost,
+                                       l.st));
+    }
     return HOUGH_OK;
 }
 
@@ -198,11 +323,15 @@ extern "C" int hough_pipeline_run_host(hough_pipeline* p, const float* h_hits_xy
         if (l.tile < 0) return HOUGH_OK;
         HOUGH_CUDA_TRY(cudaEventSynchronize(l.counted));
         const int n_ev = l.e1 - l.e0, n_h = l.h1 - l.h0;
-        const int total = l.h_cand_off[n_ev];
-        const int n_c = std::min(total, p->tile_cap);
-        if (total > p->tile_cap && h_overflowed) *h_overflowed = 1;
+        const bool kept = p->kept_only && p->tile_cap > 0;
+        const int32_t* toff = kept ? l.h_kept_off : l.h_cand_off;        // offsets of the list that goes to the caller
+        if (l.h_cand_off[n_ev] > p->tile_cap && h_overflowed) *h_overflowed = 1;
+        const int total = toff[n_ev];
+        const int n_c = kept ? total : std::min(total, p->tile_cap);
+        const hough_candidate* d_rec = kept ? l.d_kcands : l.d_cands;
+        const int32_t* d_rnh = kept ? l.d_knh : l.d_nh;
         for (int i = 1; i <= n_ev; ++i)
-            h_cand_offsets[l.e0 + i] = (int32_t)std::min<long long>(cand_base + l.h_cand_off[i], 0x7fffffffLL);
+            h_cand_offsets[l.e0 + i] = (int32_t)std::min<long long>(cand_base + toff[i], 0x7fffffffLL);
         // records that fit the caller's capacity
         const long long room = std::max<long long>(0, (long long)cand_capacity - cand_base);
         const int n_out = (int)std::min<long long>(n_c, room);
@@ -210,17 +339,18 @@ extern "C" int hough_pipeline_run_host(hough_pipeline* p, const float* h_hits_xy
         const int n_thr = std::max(n_h, n_c);
         if (n_thr > 0) {
             rebase_kernel<<<(n_thr + 255) / 256, 256, 0, l.st>>>(l.d_h2c, n_h, (int)std::min<long long>(cand_base, 0x7fffffffLL),
-                                                                l.d_cands, n_c, l.e0);
+                                                                const_cast<hough_candidate*>(d_rec), n_c, l.e0);
             HOUGH_CUDA_TRY(cudaGetLastError());
             hough_count_launches(1);
         }
         if (n_h > 0)
             HOUGH_CUDA_TRY(cudaMemcpyAsync(h_hit_to_cand + l.h0, l.d_h2c, sizeof(int32_t) * (size_t)n_h, cudaMemcpyDeviceToHost, l.st));
         if (n_out > 0) {
-            HOUGH_CUDA_TRY(cudaMemcpyAsync(h_cands + cand_base, l.d_cands, sizeof(hough_candidate) * (size_t)n_out,
+            HOUGH_CUDA_TRY(cudaMemcpyAsync(h_cands + cand_base, d_rec, sizeof(hough_candidate) * (size_t)n_out,
                                            cudaMemcpyDeviceToHost, l.st));
-            HOUGH_CUDA_TRY(cudaMemcpyAsync(h_cand_nhits + cand_base, l.d_nh, sizeof(int32_t) * (size_t)n_out, cudaMemcpyDeviceToHost, l.st));
-            HOUGH_CUDA_TRY(cudaMemcpyAsync(h_cand_keep + cand_base, l.d_keep, (size_t)n_out, cudaMemcpyDeviceToHost, l.st));
+            HOUGH_CUDA_TRY(cudaMemcpyAsync(h_cand_nhits + cand_base, d_rnh, sizeof(int32_t) * (size_t)n_out, cudaMemcpyDeviceToHost, l.st));
+            if (kept) memset(h_cand_keep + cand_base, 1, (size_t)n_out);        // every returned candidate is a kept one
+            else HOUGH_CUDA_TRY(cudaMemcpyAsync(h_cand_keep + cand_base, l.d_keep, (size_t)n_out, cudaMemcpyDeviceToHost, l.st));
         }
         cand_base += total;
         l.tile = -1;

@@ -12,11 +12,13 @@ from gpu_util import assert_centroids_close  # noqa: E402
 from paper_1311_2769_b200 import CAND_DTYPE, HoughPipeline  # noqa: E402
 
 
-def _run_pipeline(w, batch, tile_events, n_streams, tile_cap, cand_capacity, pinned=True):
+def _run_pipeline(w, batch, tile_events, n_streams, tile_cap, cand_capacity, pinned=True, kept_only=False):
     off = batch.event_offsets.astype(np.int64)
     tiles = [(e0, min(e0 + tile_events, batch.n_events)) for e0 in range(0, batch.n_events, tile_events)]
     max_hits = max(int(off[e1] - off[e0]) for e0, e1 in tiles)
     pipe = HoughPipeline.from_workload(w, tile_events, max(max_hits, 1), tile_cap, n_streams)
+    if kept_only:
+        pipe.set_option("kept_only", 1)
 
     def host(t):
         return t.pin_memory() if pinned else t
@@ -107,3 +109,26 @@ def test_pipeline_empty_batch_and_empty_events():
     h_ref, _, _ = o.assign_indexed(batch.hits_xy, batch.event_offsets, ref, w.assoc_dj, w.min_hits)
     assert np.array_equal(h2c[:batch.n_hits], h_ref)
     assert np.array_equal(h2c[batch.n_hits:], np.where(h_ref >= 0, h_ref + ref.total, -1))
+
+
+@pytest.mark.parametrize("tile_events,n_streams", [(3, 2), (16, 3)])
+def test_pipeline_kept_only_returns_the_compacted_kept_list(tile_events, n_streams):
+    """include/hough.h "kept_only": same work, only the candidates with cand_keep = 1 come back, compacted."""
+    w = get_workload(3)
+    batch = generate_events(w, events=list(range(20, 31)))
+    rec, h2c_ref, nh_ref, keep_ref, off_ref = _oracle_per_event(w, batch)
+    kmask = keep_ref.astype(bool)
+    new_index = np.cumsum(kmask) - 1
+    n_kept = int(kmask.sum())
+    assert 0 < n_kept < len(kmask)
+    koff = np.array([int(kmask[:o].sum()) for o in off_ref], np.int32)
+    h2c_kept = np.where(h2c_ref >= 0, new_index[np.maximum(h2c_ref, 0)], -1).astype(np.int32)
+    tile_cap = int(max(off_ref[min(e0 + tile_events, 11)] - off_ref[e0] for e0 in range(0, 11, tile_events))) + 3
+    over, h2c, coff, cands, nh, keep = _run_pipeline(w, batch, tile_events, n_streams, tile_cap, n_kept + 4, kept_only=True)
+    assert not over
+    assert np.array_equal(coff, koff)
+    for f in ("event", "k", "i", "j", "votes"):
+        assert np.array_equal(cands[f][:n_kept], rec[f][kmask]), f
+    assert_centroids_close(cands[:n_kept], rec[kmask], w.binning)
+    assert np.array_equal(h2c, h2c_kept)
+    assert np.array_equal(nh[:n_kept], nh_ref[kmask]) and (keep[:n_kept] == 1).all()
