@@ -16,7 +16,8 @@ assert CAND_DTYPE.itemsize == 32
 
 class _Binning(C.Structure):
     _fields_ = [("n_phi", C.c_int32), ("n_qpt", C.c_int32), ("n_d0", C.c_int32),
-                ("qpt_min", C.c_float), ("qpt_max", C.c_float), ("d0_min", C.c_float), ("d0_max", C.c_float)]
+                ("qpt_min", C.c_float), ("qpt_max", C.c_float), ("d0_min", C.c_float), ("d0_max", C.c_float),
+                ("model", C.c_int32)]
 
 
 _lib = None
@@ -61,8 +62,11 @@ class OracleCandidates:
 class Oracle:
     """One binning + field; methods mirror the C functions."""
 
-    def __init__(self, n_phi, n_qpt, n_d0, qpt_min=-1.0, qpt_max=1.0, d0_min=-20.0, d0_max=20.0, bz_tesla=3.8):
-        self.b = _Binning(n_phi, n_qpt, n_d0, qpt_min, qpt_max, d0_min, d0_max)
+    def __init__(self, n_phi, n_qpt, n_d0, qpt_min=-1.0, qpt_max=1.0, d0_min=-20.0, d0_max=20.0, bz_tesla=3.8, model=0):
+        """model 0: curved tracks, axis j = q/pT (D3); model 1: straight displaced tracks, axis j = d0 in cm over
+        [qpt_min, qpt_max) (D3L; n_d0 must be 1, the field is ignored)."""
+        self.b = _Binning(n_phi, n_qpt, n_d0, qpt_min, qpt_max, d0_min, d0_max, int(model))
+        self.model = int(model)
         self.bz = float(bz_tesla)
         self.n_phi, self.n_qpt, self.n_d0 = int(n_phi), int(n_qpt), int(n_d0)
         self.lib = _load()
@@ -70,7 +74,7 @@ class Oracle:
     @classmethod
     def from_binning(cls, binning, bz_tesla=3.8):
         return cls(binning.n_phi, binning.n_qpt, binning.n_d0, binning.qpt_min, binning.qpt_max,
-                   binning.d0_min, binning.d0_max, bz_tesla)
+                   binning.d0_min, binning.d0_max, bz_tesla, getattr(binning, "model", 0))
 
     @staticmethod
     def _hits(hits_xy):

@@ -36,6 +36,7 @@ typedef struct {
     int32_t n_phi, n_qpt, n_d0;
     float qpt_min, qpt_max;   // GeV^-1, half-open [min, max)
     float d0_min, d0_max;     // cm; ignored when n_d0 == 1
+    int32_t model;            // 0: curved tracks, solve q/pT (D3);  1: straight displaced tracks, solve d0 (D3L)
 } orc_binning;
 
 typedef struct {
@@ -55,16 +56,19 @@ struct Tables {
     std::vector<float> cosT, sinT;     // [n_phi]  phi0 column centres
     std::vector<float> d0c, td0, d0sq; // [n_d0]
     float A_f, qmin, inv_wq;
+    int model;
 };
 
 bool valid_binning(const orc_binning* b) {
     return b && b->n_phi > 0 && b->n_phi % 4 == 0 && b->n_qpt > 0 && b->n_d0 > 0 &&
-           b->qpt_max > b->qpt_min && (b->n_d0 == 1 || b->d0_max > b->d0_min);
+           b->qpt_max > b->qpt_min && (b->n_d0 == 1 || b->d0_max > b->d0_min) &&
+           (b->model == 0 || (b->model == 1 && b->n_d0 == 1));
 }
 
 Tables make_tables(const orc_binning& b, float bz) {
     Tables t;
     t.A_f = (float)(0.5 * kGeVPerTeslaCm * (double)bz);
+    t.model = b.model;
     t.qmin = b.qpt_min;
     t.inv_wq = (float)((double)b.n_qpt / ((double)b.qpt_max - (double)b.qpt_min));
     const int n = b.n_phi, q = n / 4;
@@ -106,6 +110,16 @@ inline int vote_bin(const Tables& t, int n_qpt, float x, float y, float r2, int 
     const float ys = y * s;
     const float f = xc + ys;                 // f = p . t_hat
     if (!(f > 0.0f)) return -1;              // forward branch only (S4)
+    if (t.model == 1) {
+        // D3L -- straight displaced track ("or straight displaced tracks"): the zero-curvature limit of D1.
+        // A straight line with direction phi0 and signed impact parameter d0 passes through p iff d0 = p . n_hat = w
+        // (the hits of one point trace the sinusoid d0 = -x sin(phi0) + y cos(phi0)).  The binned axis j
+        // is d0 over [qpt_min, qpt_max) cm (the struct's q/pT fields carry the range of the solved parameter).
+        const float dw = w - t.qmin;
+        const float tl = dw * t.inv_wq;
+        if (!(tl >= 0.0f && tl < (float)n_qpt)) return -1;
+        return (int)tl;
+    }
     const float num = t.d0c[k] - w;
     const float tw = t.td0[k] * w;
     const float d1 = r2 - tw;

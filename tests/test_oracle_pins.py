@@ -479,3 +479,111 @@ def test_paper_toy_workload_shape_and_physics_sanity():
         d = np.abs(((rec["i"] - a + bn.n_phi // 2) % bn.n_phi) - bn.n_phi // 2)
         found += bool(np.any((d <= 1) & (np.abs(rec["j"] - c) <= 2)))
     assert 0.25 < found / 500 < 1.0 and len(rec) < 500
+
+
+# ---- D3L: straight displaced tracks, two-parameter space (phi0, d0) ----------------
+def _line_oracle(n_phi, n_d, dmin, dmax):
+    return Oracle(n_phi, n_d, 1, dmin, dmax, model=1)
+
+
+@pytest.mark.parametrize("seed", [0, 1, 2])
+def test_v1l_line_bruteforce_double_geometry(seed):
+    """Brute force in double from the definition: a line of direction theta_i through p has impact parameter
+    d0 = p . n_hat; forward iff p . t_hat > 0.  Compared wherever the double value is away from a bin edge."""
+    rng = np.random.default_rng(seed)
+    n_phi, n_d, dmin, dmax = 16, 12, -9.0, 7.0
+    hits = rng.uniform(-40, 40, (9, 2)).astype(np.float32)
+    acc, votes = _line_oracle(n_phi, n_d, dmin, dmax).vote(hits)
+    exp = np.zeros((n_phi, n_d), np.int64)
+    unsafe = np.zeros((n_phi, n_d), bool)
+    for x, y in hits.astype(np.float64):
+        for i in range(n_phi):
+            th = (i + 0.5) * 2 * math.pi / n_phi
+            f = x * math.cos(th) + y * math.sin(th)
+            d0 = -x * math.sin(th) + y * math.cos(th)
+            t = (d0 - dmin) / ((dmax - dmin) / n_d)
+            near = abs(t - round(t)) < 1e-4 or abs(f) < 1e-5
+            j = int(math.floor(t))
+            if near:
+                for jj in (j - 1, j, j + 1):
+                    if 0 <= jj < n_d:
+                        unsafe[i, jj] = True
+            if f > 0 and 0 <= t < n_d:
+                exp[i, j] += 1
+    got = acc[0, 0].astype(np.int64)
+    assert votes == got.sum() and np.array_equal(got[~unsafe], exp[~unsafe]) and (~unsafe).mean() > 0.9
+
+
+@pytest.mark.parametrize("shape,ij", [((256, 128), (37, 100)), ((512, 256), (300, 17)), ((64, 32), (0, 31))])
+def test_v2l_noiseless_line_peaks_in_its_own_bin(shape, ij):
+    from workloads import LAYERS_PAPER_TOY, line_hits
+    n_phi, n_d = shape
+    dmin, dmax = -12.0, 12.0
+    i, j = ij
+    phi0 = (i + 0.5) * 2 * math.pi / n_phi
+    d0 = dmin + (j + 0.5) * (dmax - dmin) / n_d
+    hits = line_hits(phi0, d0, LAYERS_PAPER_TOY)
+    assert hits.shape[0] == 10
+    o = _line_oracle(n_phi, n_d, dmin, dmax)
+    acc, _ = o.vote(hits)
+    a = acc[0, 0]
+    assert a[i, j] == 10 and (a == 10).sum() == 1                     # every hit votes the true bin, nothing else reaches 10
+    ref = o.find_peaks(acc, 10)
+    assert ref.total == 1 and (ref.records["i"][0], ref.records["j"][0], ref.records["votes"][0]) == (i, j, 10)
+    h2c, nh, keep = o.assign_indexed(hits, None, ref, 1, 10)
+    assert (h2c == 0).all() and nh[0] == 10 and keep[0] == 1
+    # centroid: the `qpt` field carries d0 [cm] in this model; within one bin of the truth
+    assert abs(ref.records["qpt"][0] - d0) <= (dmax - dmin) / n_d and abs(ref.records["phi0"][0] - phi0) <= 2 * math.pi / n_phi
+
+
+def test_v3l_line_closed_form_vote_count_and_sinusoid():
+    """A hit at radius r votes in the columns with dmin <= r sin(phi - theta) < dmax on the forward half: their number is
+    n_phi (asin(min(dmax/r, 1)) - asin(max(dmin/r, -1))) / 2pi within +-1; the voted bins trace the sinusoid
+    d0 = -x sin(theta) + y cos(theta)."""
+    n_phi, n_d, dmin, dmax = 720, 64, -15.0, 10.0
+    rng = np.random.default_rng(5)
+    r = rng.uniform(3.0, 120.0, 40)
+    ph = rng.uniform(0, 2 * math.pi, 40)
+    hits = np.stack([r * np.cos(ph), r * np.sin(ph)], 1).astype(np.float32)
+    o = _line_oracle(n_phi, n_d, dmin, dmax)
+    per_hit = o.votes_per_hit(hits)
+    exp = n_phi * (np.arcsin(np.minimum(dmax / r, 1.0)) - np.arcsin(np.maximum(dmin / r, -1.0))) / (2 * math.pi)
+    assert np.all(np.abs(per_hit - exp) <= 1.0)
+    acc, votes = o.vote(hits[:1])
+    ii, jj = np.nonzero(acc[0, 0])
+    th = (ii + 0.5) * 2 * math.pi / n_phi
+    d0 = -float(hits[0, 0]) * np.sin(th) + float(hits[0, 1]) * np.cos(th)
+    assert votes == per_hit[0] and np.all(np.abs(dmin + (jj + 0.5) * (dmax - dmin) / n_d - d0) <= 0.5 * (dmax - dmin) / n_d + 1e-4)
+
+
+def test_v6l_line_quarter_turn_shifts_accumulator_exactly():
+    w = get_workload(6)
+    batch = generate_events(w)
+    o = Oracle.from_binning(w.binning, w.bz_tesla)
+    acc, _ = o.vote(batch.hits_xy, batch.event_offsets)
+    rot = np.stack([-batch.hits_xy[:, 1], batch.hits_xy[:, 0]], 1)    # (x, y) -> (-y, x): exact in fp32
+    acc_r, _ = o.vote(rot, batch.event_offsets)
+    assert np.array_equal(np.roll(acc, w.binning.n_phi // 4, axis=2), acc_r)
+
+
+def test_line_workload_vertices_show_as_sinusoids():
+    """PAPER.md:61 / Fig. 3: tracks from one displaced vertex (xv, yv) lie on d0 = -xv sin(phi0) + yv cos(phi0)."""
+    w = get_workload(6)
+    batch = generate_events(w, want_truth=True)
+    t = batch.truth[0]
+    sx, sy, psi = t["start_x"], t["start_y"], t["direction"]
+    d0_true = -sx * np.sin(psi) + sy * np.cos(psi)
+    assert np.allclose(d0_true[:w.n_prompt], 0.0) and np.abs(d0_true[w.n_prompt:]).max() < 12.0 + 1e-9
+    o = Oracle.from_binning(w.binning, w.bz_tesla)
+    acc, _ = o.vote(batch.hits_xy, batch.event_offsets)
+    ref = o.find_peaks(acc, w.threshold)
+    h2c, nh, keep = o.assign_indexed(batch.hits_xy, batch.event_offsets, ref, w.assoc_dj, w.min_hits)
+    rec = ref.records[keep.astype(bool)]
+    bn = w.binning
+    ti = np.floor(np.mod(psi, 2 * math.pi) / (2 * math.pi) * bn.n_phi).astype(int)
+    tj = np.floor((d0_true - bn.qpt_min) / (bn.qpt_max - bn.qpt_min) * bn.n_qpt).astype(int)
+    found = 0
+    for a, c in zip(ti, tj):
+        d = np.abs(((rec["i"] - a + bn.n_phi // 2) % bn.n_phi) - bn.n_phi // 2)
+        found += bool(np.any((d <= 1) & (np.abs(rec["j"] - c) <= 2)))
+    assert found / len(ti) > 0.2                                       # sanity only (binning-dependent)

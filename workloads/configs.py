@@ -32,6 +32,8 @@ class HoughBinning:
     d0_min: float = -20.0
     d0_max: float = 20.0
     accum_dtype: int = ACC_I32
+    model: int = 0               # 0: curved tracks (axis j = q/pT); 1: straight displaced tracks (axis j = d0 [cm] over
+                                 # [qpt_min, qpt_max), n_d0 = 1) -- PAPER.md:45
 
     @property
     def n_bins(self) -> int:
@@ -101,6 +103,14 @@ WORKLOADS = {
                      n_prompt=500, n_displaced=0, n_noise=0, pt_law="exp", pt_min=1.0, pt_max=0.0,
                      binning=HoughBinning(512, 256, 1, accum_dtype=ACC_I32), threshold=8,
                      sigma_rphi_cm=0.04, cite="P:L39"),
+    # straight displaced tracks in the two-parameter space (phi0, d0) ("or straight
+    # displaced tracks"; Fig. 3: "four displaced jets").  The paper's toy detector with the field off:
+    # 40 prompt tracks plus 160 tracks from 4 displaced vertices (round-robin, G4), 200 noise hits.  Binning (512 phi0 x
+    # 256 d0 bins over [-30, 30) cm) and threshold are this build's choices.
+    6: HoughWorkload(name="paper_toy_straight_displaced", seed=7, n_events=1, layers=LAYERS_PAPER_TOY,
+                     n_prompt=40, n_displaced=160, n_noise=200, pt_law="exp", pt_min=1.0, pt_max=0.0,
+                     binning=HoughBinning(512, 256, 1, qpt_min=-30.0, qpt_max=30.0, accum_dtype=ACC_I32, model=1),
+                     threshold=8, bz_tesla=0.0, sigma_rphi_cm=0.04, vertex_r_min=1.0, vertex_r_max=12.0, cite="P:L45, P:L61"),
 }
 
 

@@ -102,6 +102,32 @@ def _propagate_to_layers(px, py, psi, rho, radii):
     return x, y, reach & outside
 
 
+def _propagate_lines(px, py, psi, radii):
+    """Forward crossing of straight lines p + s (cos psi, sin psi), s > 0, with the barrel layers (zero field).
+
+    |p + s t|^2 = r^2  =>  s = -(p.t) + sqrt((p.t)^2 - |p|^2 + r^2); a layer inside the start radius is not crossed going
+    forward unless the root is real and positive.  Returns x, y [T, L] and the validity mask."""
+    px = np.asarray(px, np.float64)[:, None]
+    py = np.asarray(py, np.float64)[:, None]
+    psi = np.asarray(psi, np.float64)[:, None]
+    r = np.asarray(radii, np.float64)[None, :]
+    tx, ty = np.cos(psi), np.sin(psi)
+    pt_ = px * tx + py * ty
+    disc = pt_ * pt_ - (px * px + py * py) + r * r
+    ok = (disc > 0.0) & (r * r > px * px + py * py)
+    sq = np.sqrt(np.where(disc > 0.0, disc, 0.0))
+    sfwd = -pt_ + sq
+    ok = ok & (sfwd > 0.0)
+    return px + sfwd * tx, py + sfwd * ty, ok
+
+
+def line_hits(phi0: float, d0: float, radii: Sequence[float]) -> np.ndarray:
+    """Noiseless hits (float32 [n,2]) of ONE straight track: direction phi0, signed impact parameter d0 (SURVEY D1
+    convention: closest point = d0 * (-sin phi0, cos phi0)), followed forward from its closest point."""
+    x, y, ok = _propagate_lines([-d0 * np.sin(phi0)], [d0 * np.cos(phi0)], [phi0], radii)
+    return np.stack([x[0][ok[0]], y[0][ok[0]]], axis=1).astype(np.float32)
+
+
 def helix_hits(phi0: float, qpt: float, d0: float, radii: Sequence[float], bz_tesla: float) -> np.ndarray:
     """Noiseless hits (float32 [n,2]) of ONE track given at its point of closest approach.
 
@@ -176,7 +202,10 @@ def generate_event(w: HoughWorkload, event: int, want_truth: bool = False):
     rho = -(q / pt) * kb
 
     n_t = n_p + n_d
-    x, y, ok = _propagate_to_layers(px, py, psi, rho, radii)
+    if w.bz_tesla == 0.0:                                 # zero field: straight tracks
+        x, y, ok = _propagate_lines(px, py, psi, radii)
+    else:
+        x, y, ok = _propagate_to_layers(px, py, psi, rho, radii)
     # r-phi smear (G5): rotate about the origin by N(0, sigma) / r_layer
     delta = (s.normal(n_t * n_layers).reshape(n_t, n_layers) * w.sigma_rphi_cm) / radii[None, :]
     cd, sd = np.cos(delta), np.sin(delta)
