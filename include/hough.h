@@ -37,6 +37,11 @@ extern "C" {
 
 enum { HOUGH_OK = 0, HOUGH_ERR_INVALID_ARG = -1, HOUGH_ERR_CUDA = -2, HOUGH_ERR_ALLOC = -3, HOUGH_ERR_UNSUPPORTED = -4 };
 enum { HOUGH_ACC_I32 = 0, HOUGH_ACC_U16 = 1 };
+/* Track model = which parameter is solved per (hit, phi0 column).  HELIX: curved tracks, signed q/pT (D3; the space of
+ * B:L5).  LINE: straight displaced tracks ("or straight displaced tracks"; zero field): the impact
+ * parameter d0 = y cos(phi0) - x sin(phi0) is solved (D3L), n_d0 must be 1, the binned axis j is d0 in cm over
+ * [qpt_min, qpt_max) -- the q/pT fields of hough_binning and of hough_candidate then carry d0 -- and bz is ignored. */
+enum { HOUGH_MODEL_HELIX = 0, HOUGH_MODEL_LINE = 1 };
 
 /* Parameter-space binning (B:L5; D2).  n_phi % 4 == 0 (quadrant-symmetric trig tables).  n_d0 == 1 is the
  * two-parameter space of PAPER.md:45 (single d0 slice with centre exactly 0; d0_min/d0_max ignored). */
@@ -45,6 +50,7 @@ typedef struct {
     float qpt_min, qpt_max;       /* GeV^-1, half-open [min, max) */
     float d0_min, d0_max;         /* cm */
     int32_t accum_dtype;          /* HOUGH_ACC_I32 | HOUGH_ACC_U16 */
+    int32_t model;                /* HOUGH_MODEL_HELIX | HOUGH_MODEL_LINE */
 } hough_binning;
 
 /* Detector description.  bz_tesla enters the vote formula (A = K*Bz/2, K = 0.00299792458 GeV/(T cm)).
@@ -85,6 +91,8 @@ size_t hough_accum_bytes(const hough_plan* plan, int32_t n_events);
  *     num = d0_k - w;  den = (r2 - 2d0_k*w) + d0_k^2;  v = num * (1/(A*den));  t = (v - qmin)*inv_wq;
  *     vote only if 0 <= t < n_qpt;  j = (int)t;  accum[e][k][i][j] += 1
  * (each operation rounded to nearest-even, no FMA contraction, IEEE reciprocal).
+ * HOUGH_MODEL_LINE (D3L): same w, f and forward test, then  t = (w - qpt_min)*inv_w;  vote only if 0 <= t < n_qpt;
+ * j = (int)t;  accum[e][0][i][j] += 1.
  * Errors: INVALID_ARG (null pointers, n_hits > max_hits, n_events > max_events, negative sizes), CUDA. */
 int hough_vote(hough_plan* plan, const float* d_hits_xy, int32_t n_hits, const int32_t* d_event_offsets,
                int32_t n_events, void* d_accum, void* cuda_stream);

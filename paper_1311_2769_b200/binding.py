@@ -18,6 +18,8 @@ LIB_PATH = os.path.join(_HERE, "libhough_b200.so")
 HOUGH_OK = 0
 HOUGH_ACC_I32 = 0
 HOUGH_ACC_U16 = 1
+HOUGH_MODEL_HELIX = 0
+HOUGH_MODEL_LINE = 1
 
 CAND_DTYPE = np.dtype([("event", "<i4"), ("k", "<i4"), ("i", "<i4"), ("j", "<i4"), ("votes", "<i4"),
                        ("phi0", "<f4"), ("qpt", "<f4"), ("d0", "<f4")])
@@ -30,7 +32,7 @@ class HoughError(RuntimeError):
 class hough_binning(C.Structure):
     _fields_ = [("n_phi", C.c_int32), ("n_qpt", C.c_int32), ("n_d0", C.c_int32),
                 ("qpt_min", C.c_float), ("qpt_max", C.c_float), ("d0_min", C.c_float), ("d0_max", C.c_float),
-                ("accum_dtype", C.c_int32)]
+                ("accum_dtype", C.c_int32), ("model", C.c_int32)]
 
 
 class hough_geometry(C.Structure):
@@ -110,8 +112,8 @@ def _dptr(t: Optional[torch.Tensor]) -> Optional[int]:
     return t.data_ptr()
 
 
-def make_structs(n_phi, n_qpt, n_d0, qpt_min, qpt_max, d0_min, d0_max, accum_dtype, bz_tesla, layers):
-    b = hough_binning(n_phi, n_qpt, n_d0, qpt_min, qpt_max, d0_min, d0_max, accum_dtype)
+def make_structs(n_phi, n_qpt, n_d0, qpt_min, qpt_max, d0_min, d0_max, accum_dtype, bz_tesla, layers, model=0):
+    b = hough_binning(n_phi, n_qpt, n_d0, qpt_min, qpt_max, d0_min, d0_max, accum_dtype, int(model))
     arr = (C.c_float * max(len(layers), 1))(*[float(r) for r in layers])
     g = hough_geometry(float(bz_tesla), len(layers), C.cast(arr, C.POINTER(C.c_float)))
     return b, g, arr
@@ -123,7 +125,7 @@ class HoughPlan:
     def __init__(self, n_phi: int, n_qpt: int, n_d0: int, qpt_min: float = -1.0, qpt_max: float = 1.0,
                  d0_min: float = -20.0, d0_max: float = 20.0, accum_dtype: int = HOUGH_ACC_I32,
                  bz_tesla: float = 3.8, layers: Sequence[float] = (), max_hits: int = 1 << 20,
-                 max_events: int = 1):
+                 max_events: int = 1, model: int = HOUGH_MODEL_HELIX):
         self.lib = load_library()
         if not torch.cuda.is_available():
             raise HoughError("no CUDA device: libhough_b200 has no CPU fallback")
@@ -131,7 +133,7 @@ class HoughPlan:
         self.accum_dtype = int(accum_dtype)
         self.max_hits, self.max_events = int(max_hits), int(max_events)
         b, g, self._keep = make_structs(n_phi, n_qpt, n_d0, qpt_min, qpt_max, d0_min, d0_max, accum_dtype,
-                                        bz_tesla, layers)
+                                        bz_tesla, layers, model)
         h = C.c_void_p()
         _check(self.lib.hough_plan_create(C.byref(b), C.byref(g), self.max_hits, self.max_events, C.byref(h)),
                "hough_plan_create")
@@ -141,7 +143,8 @@ class HoughPlan:
     def from_workload(cls, w, max_hits: int, max_events: Optional[int] = None):
         bn = w.binning
         return cls(bn.n_phi, bn.n_qpt, bn.n_d0, bn.qpt_min, bn.qpt_max, bn.d0_min, bn.d0_max, bn.accum_dtype,
-                   w.bz_tesla, w.layers, max_hits=max_hits, max_events=max_events or w.n_events)
+                   w.bz_tesla, w.layers, max_hits=max_hits, max_events=max_events or w.n_events,
+                   model=getattr(bn, "model", 0))
 
     def close(self):
         if getattr(self, "_h", None):
@@ -199,12 +202,12 @@ class HoughPipeline:
 
     def __init__(self, n_phi, n_qpt, n_d0, qpt_min=-1.0, qpt_max=1.0, d0_min=-20.0, d0_max=20.0,
                  accum_dtype=HOUGH_ACC_I32, bz_tesla=3.8, layers=(), tile_events=64, max_hits_per_tile=1 << 20,
-                 tile_cand_capacity=1 << 20, n_streams=4):
+                 tile_cand_capacity=1 << 20, n_streams=4, model=HOUGH_MODEL_HELIX):
         self.lib = load_library()
         if not torch.cuda.is_available():
             raise HoughError("no CUDA device: libhough_b200 has no CPU fallback")
         b, g, self._keep = make_structs(n_phi, n_qpt, n_d0, qpt_min, qpt_max, d0_min, d0_max, accum_dtype,
-                                        bz_tesla, layers)
+                                        bz_tesla, layers, model)
         h = C.c_void_p()
         _check(self.lib.hough_pipeline_create(C.byref(b), C.byref(g), int(tile_events), int(max_hits_per_tile),
                                               int(tile_cand_capacity), int(n_streams), C.byref(h)),
@@ -215,7 +218,8 @@ class HoughPipeline:
     def from_workload(cls, w, tile_events, max_hits_per_tile, tile_cand_capacity, n_streams=4):
         bn = w.binning
         return cls(bn.n_phi, bn.n_qpt, bn.n_d0, bn.qpt_min, bn.qpt_max, bn.d0_min, bn.d0_max, bn.accum_dtype,
-                   w.bz_tesla, w.layers, tile_events, max_hits_per_tile, tile_cand_capacity, n_streams)
+                   w.bz_tesla, w.layers, tile_events, max_hits_per_tile, tile_cand_capacity, n_streams,
+                   model=getattr(bn, "model", 0))
 
     def close(self):
         if getattr(self, "_h", None):
@@ -250,10 +254,11 @@ class HoughPipeline:
         return bool(over.value)
 
 
-def window_table(n_phi, n_qpt, n_d0, qpt_min=-1.0, qpt_max=1.0, d0_min=-20.0, d0_max=20.0, bz_tesla=3.8, layers=()):
+def window_table(n_phi, n_qpt, n_d0, qpt_min=-1.0, qpt_max=1.0, d0_min=-20.0, d0_max=20.0, bz_tesla=3.8, layers=(),
+                 model=0):
     """hough_window_table (host only): (edge_r2 [n_class], lo_off [n_class, n_d0], steps [n_class, n_d0])."""
     lib = load_library()
-    b, g, _keep = make_structs(n_phi, n_qpt, n_d0, qpt_min, qpt_max, d0_min, d0_max, HOUGH_ACC_I32, bz_tesla, layers)
+    b, g, _keep = make_structs(n_phi, n_qpt, n_d0, qpt_min, qpt_max, d0_min, d0_max, HOUGH_ACC_I32, bz_tesla, layers, model)
     n = C.c_int32(0)
     edge = np.zeros(256, np.float32)
     lo = np.zeros(256 * n_d0, np.float32)

@@ -69,7 +69,7 @@ __global__ void __launch_bounds__(256) assign_fullscan_kernel(HoughConsts c, con
     unsigned long long best = 0ull;
     for (int k = 0; k < c.n_d0; ++k) {
         const float4 d = c.d0t[k];
-        const int jh = d3_bin_from_w(w, r2, d.x, d.y, d.z, c.A_f, c.qmin, c.inv_wq, c.nq_f);
+        const int jh = d3_bin_from_w(w, r2, d.x, d.y, d.z, c.A_f, c.qmin, c.inv_wq, c.nq_f, c.model != 0);
         if (jh < 0) continue;
         const int row = (k * c.n_phi + i) * c.n_qpt;
         const int j0 = max(jh - assoc_dj, 0), j1 = min(jh + assoc_dj, c.n_qpt - 1);

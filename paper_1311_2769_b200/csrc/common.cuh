@@ -30,6 +30,7 @@ struct HoughConsts {
     int32_t bins_per_event;       // n_d0 * n_phi * n_qpt
     int32_t words_per_event;      // ceil(bins_per_event / 32)  (peak bitmask)
     int32_t is_u16;
+    int32_t model;                // HOUGH_MODEL_HELIX | HOUGH_MODEL_LINE
     float A_f, qmin, inv_wq, nq_f;
     float qpt_min, d0_min;        // centroid (D7)
     float wq, wphi, wd, two_pi_f;
@@ -108,7 +109,12 @@ __device__ __forceinline__ void d3_wf(float x, float y, float c, float s, float&
 }
 
 __device__ __forceinline__ int d3_bin_from_w(float w, float r2, float d0c, float td0, float d0sq, float A_f,
-                                             float qmin, float inv_wq, float nq_f) {
+                                             float qmin, float inv_wq, float nq_f, bool line = false) {
+    if (line) {                                              // D3L: straight track, the solved parameter is d0 = w
+        const float tl = __fmul_rn(__fsub_rn(w, qmin), inv_wq);
+        if (!(tl >= 0.0f && tl < nq_f)) return -1;
+        return (int)tl;
+    }
     const float num = __fsub_rn(d0c, w);
     const float den = __fadd_rn(__fsub_rn(r2, __fmul_rn(td0, w)), d0sq);
     const float g = __fmul_rn(A_f, den);

@@ -62,6 +62,7 @@ extern "C" int hough_plan_create(const hough_binning* b, const hough_geometry* g
     if (!(b->qpt_max > b->qpt_min)) return HOUGH_ERR_INVALID_ARG;
     if (b->n_d0 > 1 && !(b->d0_max > b->d0_min)) return HOUGH_ERR_INVALID_ARG;
     if (b->accum_dtype != HOUGH_ACC_I32 && b->accum_dtype != HOUGH_ACC_U16) return HOUGH_ERR_INVALID_ARG;
+    if (b->model != HOUGH_MODEL_HELIX && !(b->model == HOUGH_MODEL_LINE && b->n_d0 == 1)) return HOUGH_ERR_INVALID_ARG;
     if (max_hits <= 0 || max_events <= 0) return HOUGH_ERR_INVALID_ARG;
     if (g->n_layers < 0 || g->n_layers > 64 || (g->n_layers > 0 && !g->layer_radius_cm)) return HOUGH_ERR_INVALID_ARG;
     if (!(g->bz_tesla == g->bz_tesla)) return HOUGH_ERR_INVALID_ARG;
@@ -94,6 +95,7 @@ extern "C" int hough_plan_create(const hough_binning* b, const hough_geometry* g
     c.bins_per_event = (int32_t)bins;
     c.words_per_event = (int32_t)((bins + 31) / 32);
     c.is_u16 = b->accum_dtype == HOUGH_ACC_U16;
+    c.model = b->model;
     c.A_f = (float)(0.5 * 0.00299792458 * (double)g->bz_tesla);
     c.qmin = b->qpt_min;
     c.inv_wq = (float)((double)b->n_qpt / ((double)b->qpt_max - (double)b->qpt_min));

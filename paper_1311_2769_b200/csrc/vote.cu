@@ -33,7 +33,7 @@ __global__ void __launch_bounds__(256) vote_fullscan_kernel(HoughConsts c, const
     const size_t ebase = (size_t)e * (size_t)c.bins_per_event;
     for (int k = 0; k < c.n_d0; ++k) {
         const float4 d = c.d0t[k];
-        const int j = d3_bin_from_w(w, r2, d.x, d.y, d.z, c.A_f, c.qmin, c.inv_wq, c.nq_f);
+        const int j = d3_bin_from_w(w, r2, d.x, d.y, d.z, c.A_f, c.qmin, c.inv_wq, c.nq_f, c.model != 0);
         if (j < 0) continue;
         const size_t bin = ebase + ((size_t)k * c.n_phi + i) * c.n_qpt + j;
         if (U16) {

@@ -94,11 +94,11 @@ static __device__ __noinline__ unsigned walk_lookup_votes(const hough_candidate*
 
 // The exact D3 bin of (hit, column) including the forward test; -1 = no vote.  Out of line: the rare path.
 static __device__ __noinline__ int d3_exact_bin(float x, float y, float r2, float cs_c, float cs_s, float d0c, float td0,
-                                                float d0sq, float A_f, float qmin, float inv_wq, float nq_f) {
+                                                float d0sq, float A_f, float qmin, float inv_wq, float nq_f, bool line) {
     float w, f;
     d3_wf(x, y, cs_c, cs_s, w, f);
     if (!(f > 0.0f)) return -1;
-    return d3_bin_from_w(w, r2, d0c, td0, d0sq, A_f, qmin, inv_wq, nq_f);
+    return d3_bin_from_w(w, r2, d0c, td0, d0sq, A_f, qmin, inv_wq, nq_f, line);
 }
 
 __device__ __forceinline__ float rcp_approx(float g) {
@@ -170,6 +170,7 @@ constexpr int WALK_MAGIC_BITS = 0x4B400000;
 struct FastK {
     float inv_wq, d0cq, ntd0A, d0sqA, c0h, a0, e_lin, d0abs, d0sq, A_f, inv_A_abs, t_max;
     bool usable;
+    bool line;        // HOUGH_MODEL_LINE: t~ = w inv_w + c0 -- the same loop with A den == 1 (gy = gx = 0, r2Ak = 1)
 };
 
 __device__ __forceinline__ FastK make_fastk(const HoughConsts& c, float4 d) {
@@ -188,6 +189,8 @@ __device__ __forceinline__ FastK make_fastk(const HoughConsts& c, float4 d) {
     k.inv_A_abs = 1.0f / fabsf(c.A_f);
     k.t_max = fmaxf(fabsf(c0), fabsf(c.nq_f - c0)) + 2.0f;
     // the rint trick needs |t| < 2^22; a zero / non-finite field constant or range has no usable bound
+    k.line = c.model != 0;
+    if (k.line) k.inv_A_abs = 1.0f;                     // no denominator: |rinv| = 1
     k.usable = c.n_qpt < (1 << 20) && k.inv_A_abs < 3.0e38f && k.t_max < 4.0e6f && k.e_lin < 3.0e38f;
     return k;
 }
@@ -197,6 +200,11 @@ __device__ __forceinline__ FastK make_fastk(const HoughConsts& c, float4 d) {
 struct FastHit { float gy, gx, ny, nx, r2Ak; };
 __device__ __forceinline__ FastHit make_fasthit(const FastK& fk, float x, float y, float r2) {
     FastHit h;
+    if (fk.line) {                                                          // numq = w inv_w = (inv_w y) c - (inv_w x) s
+        h.gy = 0.0f;  h.gx = 0.0f;  h.r2Ak = 1.0f;
+        h.ny = __fmul_rn(fk.inv_wq, y);  h.nx = -__fmul_rn(fk.inv_wq, x);
+        return h;
+    }
     h.gy = __fmul_rn(fk.ntd0A, y);  h.gx = -__fmul_rn(fk.ntd0A, x);       // A den ~ gy c + gx s + r2Ak
     h.ny = -__fmul_rn(fk.inv_wq, y);  h.nx = __fmul_rn(fk.inv_wq, x);      // numq  ~ ny c + nx s + d0cq
     h.r2Ak = __fmaf_rn(r2, fk.A_f, fk.d0sqA);
@@ -312,7 +320,7 @@ __device__ __noinline__ void walk_redo_pair(const HoughConsts& c, const FastK& f
         const float cs_c = w ? T.y : T.x, cs_s = w ? T.w : T.z;
         if (MODE == WALK_VOTE)
             tile_add_slot<TILE32>(tl.s_tile, tl.stride, cc + w, min(fast_slot(fk, fh, cs_c, cs_s), hmax), -1);
-        const int j = d3_exact_bin(hv.x, hv.y, r2, cs_c, cs_s, d.x, d.y, d.z, c.A_f, c.qmin, c.inv_wq, c.nq_f);
+        const int j = d3_exact_bin(hv.x, hv.y, r2, cs_c, cs_s, d.x, d.y, d.z, c.A_f, c.qmin, c.inv_wq, c.nq_f, c.model != 0);
         if (j >= 0)
             walk_apply<MODE, TILE32>(tl.s_tile, tl.stride, c.n_qpt, cc + w, j, tl.legacy, a.assoc_dj, a.cands, tl.cand_first,
                                      tl.cand_end, tl.c0, tl.row_lin0, best);
@@ -335,7 +343,7 @@ __device__ __noinline__ void walk_exact_window(const HoughConsts& c, float4 d, c
         if (col < cols) {
             const float4 T = tl.s_pair[col >> 1];
             const int j = d3_exact_bin(hv.x, hv.y, r2, (col & 1) ? T.y : T.x, (col & 1) ? T.w : T.z, d.x, d.y, d.z, c.A_f, c.qmin,
-                                       c.inv_wq, c.nq_f);
+                                       c.inv_wq, c.nq_f, c.model != 0);
             if (j >= 0)
                 walk_apply<MODE, TILE32>(tl.s_tile, tl.stride, c.n_qpt, col, j, tl.legacy, a.assoc_dj, a.cands, tl.cand_first,
                                          tl.cand_end, tl.c0, tl.row_lin0, best);
@@ -443,8 +451,8 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(HoughConsts
             float dr = (fk.d0abs >= ra && fk.d0abs <= rb) ? 0.0f : fminf(fabsf(ra - fk.d0abs), fabsf(rb - fk.d0abs));
             dr = fmaxf(dr - 1.0e-6f * rb, 0.0f);                              // den >= (r - |d0|)^2 >= dr^2
             const float S = 8.0f * fk.d0abs * L + rb * rb + fk.d0sq;
-            const float inv_dr2 = 1.000001f / (dr * dr);
-            const float arel = WALK_U * (6.0f * S * inv_dr2 + 24.0f);
+            const float inv_dr2 = fk.line ? 1.0f : 1.000001f / (dr * dr);       // line model: no denominator at all
+            const float arel = WALK_U * ((fk.line ? 0.0f : 6.0f * S * inv_dr2) + 24.0f);
             const float elin = fk.e_lin * (L + fk.d0abs);
             const float m = fk.inv_A_abs * inv_dr2 * elin + arel * fk.t_max + fk.a0;
             if (m < 0.45f) hm = 0.5f - m;                                     // false for NaN / inf

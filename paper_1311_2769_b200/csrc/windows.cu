@@ -94,7 +94,30 @@ int hough_build_windows(const hough_binning& b, float bz, int n_layers, const fl
             float& lo = out.lo_off[(size_t)c * nd + k];
             int& st = out.steps[(size_t)c * nd + k];
             lo = full_lo; st = full_steps;           // default: the whole forward half (always contains the run)
-            if (open || !(A > 0.0)) continue;
+            if (open) continue;
+            if (b.model == HOUGH_MODEL_LINE) {
+                // D3L: qmin <= r s < qmax (cm), s = sin(phi - phi0): s in [qmin / r, qmax / r) over the class's radii
+                if (!(ra > 0.0)) continue;
+                const double eps_d = 1.0e-5 * (std::fabs(qmin) + std::fabs(qmax));
+                double s_lo = std::min((qmin - eps_d) / ra, (qmin - eps_d) / rb);
+                double s_hi = std::max((qmax + eps_d) / ra, (qmax + eps_d) / rb);
+                s_lo -= 1.0e-5 + 1.0e-6 * std::fabs(s_lo);
+                s_hi += 1.0e-5 + 1.0e-6 * std::fabs(s_hi);
+                if (s_lo > 1.0 || s_hi < -1.0 || s_lo > s_hi) { lo = 0.0f; st = 0; continue; }
+                const double d_lo = -std::asin(std::min(s_hi, 1.0));
+                const double d_hi = -std::asin(std::max(s_lo, -1.0));
+                const double lo_c = d_lo / dphi - margin_cols, hi_c = d_hi / dphi + margin_cols;
+                const int steps = (int)std::floor(hi_c - lo_c) + 1;
+                if (steps >= full_steps) continue;
+                lo = (float)lo_c;
+                if ((double)lo > lo_c) lo = std::nextafterf(lo, -1.0e30f);
+                st = steps + 1;
+                const double lim = 89.0 / 360.0 * (double)nphi;
+                if (c > 0 && (double)lo - 2.0 >= -lim && (double)lo + (double)st + 3.0 <= lim)
+                    out.fwd_safe[(size_t)c * nd + k] = 1;
+                continue;
+            }
+            if (!(A > 0.0)) continue;
             double d0 = 0.0;
             if (nd > 1)
                 d0 = (double)(float)((double)b.d0_min + ((double)k + 0.5) * ((double)b.d0_max - (double)b.d0_min) / (double)nd);

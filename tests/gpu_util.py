@@ -31,7 +31,7 @@ def run_cuda(binning, bz, layers, hits_xy, event_offsets, threshold, assoc_dj, m
     if own:
         plan = HoughPlan(binning.n_phi, binning.n_qpt, binning.n_d0, binning.qpt_min, binning.qpt_max, binning.d0_min,
                          binning.d0_max, binning.accum_dtype, bz, layers, max_hits=max(n_hits, 1),
-                         max_events=max(n_events, 1))
+                         max_events=max(n_events, 1), model=getattr(binning, "model", 0))
     if fullscan:
         plan.set_option("fullscan", 1)
     for key in options:
@@ -122,7 +122,7 @@ def run_vote(binning, bz, layers, hits_xy, event_offsets, max_hits=None, misalig
     n_events = int(event_offsets.shape[0] - 1)
     plan = HoughPlan(binning.n_phi, binning.n_qpt, binning.n_d0, binning.qpt_min, binning.qpt_max, binning.d0_min,
                      binning.d0_max, binning.accum_dtype, bz, layers, max_hits=max_hits or max(n_hits, 1),
-                     max_events=max(n_events, 1))
+                     max_events=max(n_events, 1), model=getattr(binning, "model", 0))
     if fullscan:
         plan.set_option("fullscan", 1)
     for key in options:
@@ -149,7 +149,7 @@ def run_assign(binning, bz, layers, hits_xy, event_offsets, records, cand_offset
     n_events = int(event_offsets.shape[0] - 1)
     plan = HoughPlan(binning.n_phi, binning.n_qpt, binning.n_d0, binning.qpt_min, binning.qpt_max, binning.d0_min,
                      binning.d0_max, binning.accum_dtype, bz, layers, max_hits=max_hits or max(n_hits, 1),
-                     max_events=max(n_events, 1))
+                     max_events=max(n_events, 1), model=getattr(binning, "model", 0))
     if fullscan:
         plan.set_option("fullscan", 1)
     for key in options:

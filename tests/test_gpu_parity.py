@@ -187,11 +187,14 @@ def test_random_configurations_bit_exact(seed):
     n_phi = 4 * int(rng.integers(2, 160))
     n_qpt = int(rng.choice([8, 24, 37, 64, 128, 200, 256, 333]))
     n_d0 = int(rng.choice([1, 2, 3, 5, 8]))
-    qa, qb = sorted(rng.uniform(-1.5, 1.5, 2))
+    model = 1 if seed % 5 == 3 else 0                      # straight-track space (phi0, d0): range in cm, one slice
+    if model:
+        n_d0 = 1
+    qa, qb = sorted(rng.uniform(-1.5, 1.5, 2) * (25.0 if model else 1.0))
     if seed % 4 == 0:
         qa = 0.0                                           # one-sided range: c0 = 0
-    if qb - qa < 0.2:
-        qb = qa + 0.2
+    if qb - qa < 0.2 * (25.0 if model else 1.0):
+        qb = qa + 0.2 * (25.0 if model else 1.0)
     da, db = sorted(rng.uniform(-25.0, 25.0, 2))
     if db - da < 2.0:
         db = da + 2.0
@@ -199,7 +202,7 @@ def test_random_configurations_bit_exact(seed):
     bz = float(rng.choice([3.8, 2.0, -3.8, 1.0]))
     layers = LAYERS_10 if seed % 3 else ()
     bn = HoughBinning(n_phi, n_qpt, n_d0, float(np.float32(qa)), float(np.float32(qb)), float(np.float32(da)),
-                      float(np.float32(db)), dtype)
+                      float(np.float32(db)), dtype, model)
     hits, off = _mixed_hits(5000 + seed, 2500, LAYERS_10)
     o = Oracle.from_binning(bn, bz)
     acc, votes = o.vote(hits, off)
@@ -400,3 +403,43 @@ def test_invalid_arguments_are_rejected():
     with pytest.raises(HoughError):
         plan.vote(hits, off, plan.alloc_accum(1))   # n_hits > max_hits
     plan.close()
+
+
+# ---- HOUGH_MODEL_LINE: straight displaced tracks, two-parameter space (phi0, d0) ----
+def test_line_model_workload_bit_exact():
+    w = get_workload(6)
+    for fullscan, options in ((False, ()), (True, ()), (False, ("exact_walk",))):
+        got, ref = _compare_all(w, generate_events(w), fullscan=fullscan, options=options)
+        assert ref.total > 100
+
+
+@pytest.mark.parametrize("shape,dtype,max_hits,drange,layers", [
+    ((256, 128, 1), ACC_U16, None, (-20.0, 20.0), LAYERS_10),      # full-phi packed tile
+    ((1024, 512, 1), ACC_I32, None, (-30.0, 10.0), LAYERS_10),     # phi slabs, asymmetric range
+    ((256, 64, 1), ACC_I32, 70000, (0.0, 25.0), ()),               # 32-bit tile, one-sided range, no geometry
+    ((100, 37, 1), ACC_U16, None, (-5.0, 5.0), LAYERS_10),         # odd sizes
+])
+def test_line_model_variants_bit_exact(shape, dtype, max_hits, drange, layers):
+    bn = HoughBinning(shape[0], shape[1], 1, drange[0], drange[1], accum_dtype=dtype, model=1)
+    hits, off = _mixed_hits(shape[0] + 7, 3000, LAYERS_10)
+    o = Oracle.from_binning(bn, 0.0)
+    acc, votes = o.vote(hits, off)
+    got = run_vote(bn, 0.0, layers, hits, off, max_hits=max_hits)
+    assert votes > 0 and np.array_equal(got.astype(np.int32), acc)
+    thr = 3
+    ref = o.find_peaks(acc, thr)
+    cap = ref.total + 5
+    res = run_cuda(bn, 0.0, layers, hits, off, thr, 1, 2, cap)
+    assert res.total == ref.total and np.array_equal(res.offsets, ref.offsets)
+    for f in ("event", "k", "i", "j", "votes"):
+        assert np.array_equal(res.records[f], ref.records[f]), f
+    assert_centroids_close(res.records, ref.records, bn)
+    h2c, nh, keep = o.assign_indexed(hits, off, ref, 1, 2, capacity=cap)
+    assert np.array_equal(res.hit_to_cand, h2c)
+    assert np.array_equal(res.cand_nhits[:ref.total], nh) and np.array_equal(res.cand_keep[:ref.total], keep)
+
+
+def test_line_model_rejects_a_d0_axis():
+    from paper_1311_2769_b200 import HoughError, HoughPlan
+    with pytest.raises(HoughError):
+        HoughPlan(64, 32, 4, -10.0, 10.0, model=1)

@@ -97,3 +97,23 @@ def test_windows_negative_field_and_zero_field_fall_back_to_the_forward_half():
     edge, lo, steps = window_table(64, 32, 4, bz_tesla=-3.8, layers=LAYERS_10)
     cov, _ = _covered_columns(hits, 64, edge, lo, steps)
     assert valid.any() and not (valid & ~cov).any()
+
+
+@pytest.mark.parametrize("shape,layers,dr", [
+    ((64, 32), LAYERS_10, (-20.0, 20.0)),
+    ((256, 64), LAYERS_14, (-30.0, 5.0)),                  # asymmetric d0 range
+    ((128, 16), (), (2.0, 40.0)),                          # no geometry; range excluding 0 and wider than inner radii
+])
+def test_line_model_windows_never_miss_a_vote(shape, layers, dr):
+    """HOUGH_MODEL_LINE (D3L): the windows of the straight-track space (phi0, d0) contain every voting column."""
+    n_phi, n_d = shape
+    rng = np.random.default_rng(n_phi + n_d)
+    hits = _random_hits(rng, 260, layers or LAYERS_10)
+    o = Oracle(n_phi, n_d, 1, dr[0], dr[1], bz_tesla=0.0, model=1)
+    valid = _valid_columns(o, hits)
+    edge, lo, steps = window_table(n_phi, n_d, 1, dr[0], dr[1], bz_tesla=0.0, layers=layers, model=1)
+    cov, _ = _covered_columns(hits, n_phi, edge, lo, steps)
+    assert valid.any() and not (valid & ~cov).any(), "a window misses a voting column"
+    on_layer = np.isin(np.round(np.hypot(hits[:, 0], hits[:, 1]), 3), np.round(np.asarray(layers or LAYERS_10), 3))
+    if layers:
+        assert cov[on_layer].sum() < 3.0 * valid[on_layer].sum() + 4 * on_layer.sum()      # and they are not wasteful
