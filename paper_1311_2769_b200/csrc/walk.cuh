@@ -169,8 +169,9 @@ constexpr int WALK_MAGIC_BITS = 0x4B400000;
 //   |t~ - t_D3| < m_h = rmax_h * elin_h + arel_h * Tmax + a0   for every column whose t~ lies in [-1, nq + 1]
 struct FastK {
     float inv_wq, d0cq, ntd0A, d0sqA, c0h, a0, e_lin, d0abs, d0sq, A_f, inv_A_abs, t_max;
+    float nq_s;       // numq = nq_s (y c - x s) + d0cq:  -inv_wq (helix: (d0c - w) inv_wq),  +inv_wq (line: w inv_w)
     bool usable;
-    bool line;        // HOUGH_MODEL_LINE: t~ = w inv_w + c0 -- the same loop with A den == 1 (gy = gx = 0, r2Ak = 1)
+    bool line;        // HOUGH_MODEL_LINE: t~ = w inv_w + c0 -- the same loop with A den == 1 (ntd0A = A = 0, d0sqA = 1)
 };
 
 __device__ __forceinline__ FastK make_fastk(const HoughConsts& c, float4 d) {
@@ -190,7 +191,8 @@ __device__ __forceinline__ FastK make_fastk(const HoughConsts& c, float4 d) {
     k.t_max = fmaxf(fabsf(c0), fabsf(c.nq_f - c0)) + 2.0f;
     // the rint trick needs |t| < 2^22; a zero / non-finite field constant or range has no usable bound
     k.line = c.model != 0;
-    if (k.line) k.inv_A_abs = 1.0f;                     // no denominator: |rinv| = 1
+    k.nq_s = k.line ? c.inv_wq : -c.inv_wq;
+    if (k.line) { k.inv_A_abs = 1.0f; k.ntd0A = 0.0f; k.A_f = 0.0f; k.d0sqA = 1.0f; }   // no denominator: A den == 1
     k.usable = c.n_qpt < (1 << 20) && k.inv_A_abs < 3.0e38f && k.t_max < 4.0e6f && k.e_lin < 3.0e38f;
     return k;
 }
@@ -199,14 +201,9 @@ __device__ __forceinline__ FastK make_fastk(const HoughConsts& c, float4 d) {
 // reproduce the hot loop's slot bit for bit: explicit intrinsics, no contraction, one definition.
 struct FastHit { float gy, gx, ny, nx, r2Ak; };
 __device__ __forceinline__ FastHit make_fasthit(const FastK& fk, float x, float y, float r2) {
-    FastHit h;
-    if (fk.line) {                                                          // numq = w inv_w = (inv_w y) c - (inv_w x) s
-        h.gy = 0.0f;  h.gx = 0.0f;  h.r2Ak = 1.0f;
-        h.ny = __fmul_rn(fk.inv_wq, y);  h.nx = -__fmul_rn(fk.inv_wq, x);
-        return h;
-    }
+    FastHit h;                                                              // (line model: gy = gx = 0, r2Ak = 1)
     h.gy = __fmul_rn(fk.ntd0A, y);  h.gx = -__fmul_rn(fk.ntd0A, x);       // A den ~ gy c + gx s + r2Ak
-    h.ny = -__fmul_rn(fk.inv_wq, y);  h.nx = __fmul_rn(fk.inv_wq, x);      // numq  ~ ny c + nx s + d0cq
+    h.ny = __fmul_rn(fk.nq_s, y);  h.nx = -__fmul_rn(fk.nq_s, x);          // numq  ~ ny c + nx s + d0cq
     h.r2Ak = __fmaf_rn(r2, fk.A_f, fk.d0sqA);
     return h;
 }
