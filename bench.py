@@ -410,8 +410,8 @@ def run_ours(args, rank, world, local_rank):
     bins_per_launch = bn.n_bins * run.tile_events
     hbm_bytes = hits_per_launch * 8 + bins_per_launch * bn.bin_bytes            # hits in + accumulator out
     # dram__bytes_read.sum + dram__bytes_write.sum of the walk kernel in the ncu --set full capture of this very
-    # launch configuration (profiles/r1_final.md): 20.3 MB + 340.9 MB per 128-event launch of cfg 3
-    traffic = 361.2e6 if (args.config == 3 and run.tile_events == 128) else None
+    # launch configuration (profiles/r1_final.md): 20.0 MB + 350.8 MB per 128-event launch of cfg 3
+    traffic = 370.8e6 if (args.config == 3 and run.tile_events == 128) else None
     roofline = {"bound": "alu", "kernel": "hough_vote (stage + vote + flush)", "achieved": achieved, "peak": alu_peak,
                 "unit": "Gvotes/s", "frac": achieved / alu_peak, "traffic": traffic,
                 "peak_source": f"{sms} SMs x {FP32_LANES_PER_SM} fp32 lanes x {sm_max_mhz:.0f} MHz / "
