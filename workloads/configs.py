@@ -64,6 +64,7 @@ class HoughWorkload:
     vertex_r_max: float = 20.0
     pt_exp_scale: float = 2.0
     assoc_dj: int = 1
+    n_vertices: int = 0              # displaced vertices; 0: ceil(n_displaced / 4) (G4)
     cite: str = ""
 
     @property
@@ -110,7 +111,8 @@ WORKLOADS = {
     6: HoughWorkload(name="paper_toy_straight_displaced", seed=7, n_events=1, layers=LAYERS_PAPER_TOY,
                      n_prompt=40, n_displaced=160, n_noise=200, pt_law="exp", pt_min=1.0, pt_max=0.0,
                      binning=HoughBinning(512, 256, 1, qpt_min=-30.0, qpt_max=30.0, accum_dtype=ACC_I32, model=1),
-                     threshold=8, bz_tesla=0.0, sigma_rphi_cm=0.04, vertex_r_min=1.0, vertex_r_max=12.0, cite="P:L45, P:L61"),
+                     threshold=8, bz_tesla=0.0, sigma_rphi_cm=0.04, vertex_r_min=2.0, vertex_r_max=12.0, n_vertices=4,
+                     cite="P:L45, P:L61"),
 }
 
 

@@ -186,7 +186,7 @@ def generate_event(w: HoughWorkload, event: int, want_truth: bool = False):
     p_pt = draw_pt(n_p)
     # displaced tracks (G4)
     n_d = w.n_displaced
-    n_v = (n_d + 3) // 4
+    n_v = w.n_vertices if w.n_vertices > 0 else (n_d + 3) // 4
     v_r = w.vertex_r_min + (w.vertex_r_max - w.vertex_r_min) * s.uniform(n_v)
     v_az = _TWO_PI * s.uniform(n_v)
     d_vtx = np.arange(n_d) % max(n_v, 1)
