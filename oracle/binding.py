@@ -44,6 +44,9 @@ def _load():
             f.restype = C.c_int
             f.argtypes = [C.POINTER(_Binning), C.c_float, P, C.c_int32, P, C.c_int32, P, P, C.c_longlong,
                           C.c_int32, C.c_int32, C.c_int32, P, P, P]
+        lib.orc_vertex_vote.restype = C.c_longlong
+        lib.orc_vertex_vote.argtypes = [C.POINTER(_Binning), C.c_float, P, P, C.c_int32, C.c_longlong, P, C.c_float, C.c_int32,
+                                        C.c_float, P]
         _lib = lib
     return _lib
 
@@ -162,6 +165,18 @@ class Oracle:
                 int(apply_dedup), _ptr(h2c), _ptr(nh), _ptr(keep))
         assert rc == 0
         return h2c, nh[:n_c], keep[:n_c]
+
+    def vertex_vote(self, cands: "OracleCandidates", keep, d_abs_min: float, n_r: int, r_max: float, capacity=None):
+        """orc_vertex_vote (D10): int32 [n_events, n_phi, n_r] vertex accumulator (Phi_v x R_v) and the number of votes."""
+        rec = np.ascontiguousarray(cands.records)
+        off = np.ascontiguousarray(cands.offsets, dtype=np.int32)
+        cap = int(rec.shape[0]) if capacity is None else int(capacity)
+        keep = None if keep is None else np.ascontiguousarray(keep, dtype=np.uint8)
+        vacc = np.empty((off.shape[0] - 1, self.n_phi, int(n_r)), np.int32)
+        votes = self.lib.orc_vertex_vote(C.byref(self.b), self.bz, _ptr(rec), _ptr(off), off.shape[0] - 1, cap, _ptr(keep),
+                                         float(d_abs_min), int(n_r), float(r_max), _ptr(vacc))
+        assert votes >= 0, "orc_vertex_vote: bad arguments"
+        return vacc, int(votes)
 
     def assign_brute(self, hits_xy, event_offsets, cands, assoc_dj=1, min_hits=0, apply_dedup=True, capacity=None):
         return self._assign(self.lib.orc_assign_brute, hits_xy, event_offsets, cands, assoc_dj, min_hits,

@@ -412,4 +412,50 @@ int orc_assign_indexed(const orc_binning* b, float bz, const float* hits_xy, int
     return 0;
 }
 
+// D10 -- second Hough transform: displaced vertices from the found straight tracks ("apply a Hough
+// transform to the track maxima"; Fig. 3: the tracks of one vertex lie on a sinusoid in (phi0, d0)).  A vertex at polar
+// position (R, Phi) is on the line (phi0, d0) iff d0 = R sin(Phi - phi0).  Every kept candidate (column i, d0 bin j) of a
+// LINE-model track space votes, for every vertex-azimuth column m (the SAME n_phi column centres as the track space), for
+// the one compatible radius -- each fp32 operation individually rounded, in this order:
+//     tj = (float)j + 0.5f;  dd = tj * wq;  d = qmin + dd;              // centre of the candidate's d0 bin
+//     skip the candidate unless keep[c] != 0 and |d| >= d_abs_min       // prompt tracks constrain no vertex
+//     sd = sin_m * cos_i - cos_m * sin_i                                 // sin(Phi_m - phi0_i): two products, one subtraction
+//     R = d / sd;  t = R * inv_wr;  vote iff 0 <= t < n_r;  n = (int)t;  vacc[e][m][n] += 1
+// (R < 0, sd == 0, NaN fall out at the range test; of the two representations (Phi, R), (Phi + pi, -R) exactly one votes).
+// vacc: int32 [n_events][n_phi][n_r], zeroed here.  Returns the number of votes, < 0 on bad arguments.
+long long orc_vertex_vote(const orc_binning* b, float bz, const orc_candidate* cands, const int32_t* cand_offsets,
+                          int32_t n_events, long long capacity, const uint8_t* keep, float d_abs_min, int32_t n_r,
+                          float r_max, int32_t* vacc) {
+    if (!valid_binning(b) || b->model != 1 || !cand_offsets || !vacc || n_events < 0 || n_r <= 0 || !(r_max > 0.0f)) return -1;
+    const Tables t = make_tables(*b, bz);
+    const int nphi = b->n_phi;
+    const float wq = (float)(((double)b->qpt_max - (double)b->qpt_min) / (double)b->n_qpt);
+    const float inv_wr = (float)((double)n_r / (double)r_max);
+    std::memset(vacc, 0, sizeof(int32_t) * (size_t)n_events * nphi * n_r);
+    long long votes = 0;
+    for (int e = 0; e < n_events; ++e) {
+        const long long c0 = cand_offsets[e] < capacity ? cand_offsets[e] : capacity;
+        const long long c1 = cand_offsets[e + 1] < capacity ? cand_offsets[e + 1] : capacity;
+        for (long long c = c0; c < c1; ++c) {
+            if (keep && !keep[c]) continue;
+            const float tj = (float)cands[c].j + 0.5f;
+            const float dd = tj * wq;
+            const float d = b->qpt_min + dd;
+            if (!(std::fabs(d) >= d_abs_min)) continue;
+            const float ci = t.cosT[cands[c].i], si = t.sinT[cands[c].i];
+            for (int m = 0; m < nphi; ++m) {
+                const float a1 = t.sinT[m] * ci;
+                const float a2 = t.cosT[m] * si;
+                const float sd = a1 - a2;
+                const float R = d / sd;
+                const float tt = R * inv_wr;
+                if (!(tt >= 0.0f && tt < (float)n_r)) continue;
+                vacc[((size_t)e * nphi + m) * n_r + (int)tt] += 1;
+                ++votes;
+            }
+        }
+    }
+    return votes;
+}
+
 }  // extern "C"

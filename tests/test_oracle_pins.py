@@ -587,3 +587,98 @@ def test_line_workload_vertices_show_as_sinusoids():
         d = np.abs(((rec["i"] - a + bn.n_phi // 2) % bn.n_phi) - bn.n_phi // 2)
         found += bool(np.any((d <= 1) & (np.abs(rec["j"] - c) <= 2)))
     assert found / len(ti) > 0.2                                       # sanity only (binning-dependent)
+
+
+# ---- D10: second Hough transform, found straight tracks -> displaced vertices --------
+def _track_list(cols, bins, keep=None):
+    from oracle import CAND_DTYPE, OracleCandidates
+    rec = np.zeros(len(cols), CAND_DTYPE)
+    rec["i"] = cols
+    rec["j"] = bins
+    return OracleCandidates(rec, np.array([0, len(rec)], np.int32), len(rec)), (np.ones(len(rec), np.uint8) if keep is None else keep)
+
+
+def test_d10_bruteforce_double_and_closed_form_count():
+    """Definition in double: vertex (R, Phi) is on the line (phi0, d0) iff d0 = R sin(Phi - phi0); one vote per column with
+    0 <= R < r_max.  Per track the number of voting columns is n_phi (pi - 2 asin(|d0| / r_max)) / 2pi within +-1."""
+    rng = np.random.default_rng(3)
+    n_phi, n_d, dmin, dmax, n_r, r_max = 96, 64, -12.0, 12.0, 20, 15.0
+    o = _line_oracle(n_phi, n_d, dmin, dmax)
+    cols = rng.integers(0, n_phi, 12)
+    bins = rng.integers(0, n_d, 12)
+    cands, keep = _track_list(cols, bins)
+    keep[3] = 0
+    vacc, votes = o.vertex_vote(cands, keep, 0.5, n_r, r_max)
+    exp = np.zeros((n_phi, n_r), np.int64)
+    unsafe = np.zeros((n_phi, n_r), bool)
+    per_track = []
+    for c, (i, j) in enumerate(zip(cols, bins)):
+        d0 = dmin + (j + 0.5) * (dmax - dmin) / n_d
+        if not keep[c] or abs(d0) < 0.5:
+            continue
+        phi0 = (i + 0.5) * 2 * math.pi / n_phi
+        n_cols = 0
+        for m in range(n_phi):
+            sd = math.sin((m + 0.5) * 2 * math.pi / n_phi - phi0)
+            if abs(sd) < 1e-9:
+                continue
+            t = d0 / sd / (r_max / n_r)
+            if abs(t - round(t)) < 1e-4:
+                for nn in (int(math.floor(t)) - 1, int(math.floor(t)), int(math.floor(t)) + 1):
+                    if 0 <= nn < n_r:
+                        unsafe[m, nn] = True
+            if 0 <= t < n_r:
+                exp[m, int(math.floor(t))] += 1
+                n_cols += 1
+        per_track.append((d0, n_cols))
+    got = vacc[0].astype(np.int64)
+    assert votes == got.sum() and np.array_equal(got[~unsafe], exp[~unsafe]) and (~unsafe).mean() > 0.95
+    for d0, n_cols in per_track:
+        assert abs(n_cols - n_phi * (math.pi - 2 * math.asin(abs(d0) / r_max)) / (2 * math.pi)) <= 1.0
+
+
+def test_d10_lines_through_one_vertex_peak_at_the_vertex():
+    n_phi, n_d, dmin, dmax = 720, 1024, -16.0, 16.0
+    o = _line_oracle(n_phi, n_d, dmin, dmax)
+    r_v, phi_col = 7.3, 100                                 # vertex azimuth at a column centre
+    phi_v = (phi_col + 0.5) * 2 * math.pi / n_phi
+    xv, yv = r_v * math.cos(phi_v), r_v * math.sin(phi_v)
+    cols = np.arange(7, n_phi, 20)
+    th = (cols + 0.5) * 2 * math.pi / n_phi
+    d_true = -xv * np.sin(th) + yv * np.cos(th)
+    bins = np.floor((d_true - dmin) / ((dmax - dmin) / n_d)).astype(np.int32)
+    cands, keep = _track_list(cols, bins)
+    n_r, r_max = 64, 16.0
+    vacc, votes = o.vertex_vote(cands, keep, 0.5, n_r, r_max)
+    m_pk, n_pk = np.unravel_index(np.argmax(vacc[0]), vacc[0].shape)
+    displaced = int((np.abs(dmin + (bins + 0.5) * (dmax - dmin) / n_d) >= 0.5).sum())
+    assert m_pk == phi_col and n_pk == int(r_v / (r_max / n_r))
+    assert vacc[0].max() >= 0.8 * displaced
+    # quarter turn of every track: the vertex accumulator shifts by n_phi / 4 columns exactly (table symmetry, D2)
+    cands_r, _ = _track_list((cols + n_phi // 4) % n_phi, bins)
+    vacc_r, _ = o.vertex_vote(cands_r, keep, 0.5, n_r, r_max)
+    assert np.array_equal(np.roll(vacc, n_phi // 4, axis=1), vacc_r)
+
+
+def test_d10_workload_6_vertex_directions():
+    """Sanity on the full chain (hits -> tracks -> vertices) of workload 6: the strongest vertex candidates point at true
+    vertices.  (Radial resolution is poor for jets that fly radially -- their lines are almost parallel to the vertex's
+    position vector -- so only the azimuth is checked; this is physics sanity, not a parity pin.)"""
+    w = get_workload(6)
+    batch = generate_events(w, want_truth=True)
+    t = batch.truth[0]
+    verts = np.unique(np.round(np.stack([t["start_x"][w.n_prompt:], t["start_y"][w.n_prompt:]], 1), 9), axis=0)
+    assert verts.shape == (4, 2)
+    o = Oracle.from_binning(w.binning, w.bz_tesla)
+    acc, _ = o.vote(batch.hits_xy, batch.event_offsets)
+    ref = o.find_peaks(acc, w.threshold)
+    h2c, nh, keep = o.assign_indexed(batch.hits_xy, batch.event_offsets, ref, w.assoc_dj, w.min_hits)
+    vacc, votes = o.vertex_vote(ref, keep, 0.6, 32, 16.0)
+    assert votes > 1000
+    vs = Oracle(w.binning.n_phi, 32, 1, 0.0, 16.0, bz_tesla=0.0, model=1)
+    vref = vs.find_peaks(vacc[:, None], 6)
+    rec = vref.records[np.argsort(-vref.records["votes"])[:6]]
+    az_true = np.arctan2(verts[:, 1], verts[:, 0])
+    for ph in rec["phi0"]:
+        dphi = np.abs(np.angle(np.exp(1j * (az_true - float(ph)))))
+        assert dphi.min() < math.radians(20.0)
