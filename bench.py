@@ -428,6 +428,32 @@ def run_ours(args, rank, world, local_rank):
                                                "on this pool's B200 (profiles/r1_microbench.txt); ncu: the walk kernel "
                                                "keeps the shared-memory wavefront pipe 82 % busy (profiles/r1_final.md)"}}
 
+    # second Hough transform (tracks -> displaced vertices; D10): line-model workloads only
+    vertex = None
+    if getattr(bn, "model", 0) == 1:
+        from paper_1311_2769_b200 import HoughPlan, alloc_candidates, hough_vertex_vote
+        n_r, r_max, thr_v = 32, 16.0, 6
+        (e0, e1, h0, h1) = run.tiles[0]
+        n_ev = e1 - e0
+        run.step()                                      # leaves the first tile's candidates / keep flags on the device
+        vacc = torch.empty((n_ev, bn.n_phi, n_r), dtype=torch.int32, device="cuda")
+        vplan = HoughPlan(bn.n_phi, n_r, 1, 0.0, r_max, bz_tesla=0.0, max_hits=1, max_events=n_ev, model=1)
+        vcands = alloc_candidates(1 << 16)
+        vcoff = torch.zeros(n_ev + 1, dtype=torch.int32, device="cuda")
+        vt = []
+        for it in range(25):
+            a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+            a.record()
+            hough_vertex_vote(run.plan, run.cands, run.cand_off, n_ev, run.cap, run.keep, 0.6, n_r, r_max, vacc)
+            vplan.find_peaks(vacc, n_ev, thr_v, vcands, 1 << 16, vcoff)
+            b.record(); b.synchronize()
+            if it >= 5:
+                vt.append(a.elapsed_time(b))
+        vertex = {"ms_median": statistics.median(vt), "vertex_votes": int(vacc.to(torch.int64).sum().item()),
+                  "vertex_candidates": int(vcoff[n_ev].item()), "binning": [bn.n_phi, n_r], "r_max_cm": r_max,
+                  "threshold": thr_v, "api": "hough_vertex_vote + hough_find_peaks on the vertex space (D10)"}
+        vplan.close()
+
     n_ref = oracle_events_for_seconds(w, args.cpu_seconds)
     o_votes, o_events, o_secs = oracle_sample(w, batch, n_ref)
     cpu = {"value": o_votes / o_secs, "unit": UNIT, "cores": 1, "kind": "oracle",
@@ -459,6 +485,8 @@ def run_ours(args, rank, world, local_rank):
                               "candidate_overflow": bool(k_over)},
             "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks,
             "candidate_overflow": peaks_overflow}
+    if vertex is not None:
+        line["vertex"] = vertex
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

@@ -118,6 +118,20 @@ int hough_assign_hits(hough_plan* plan, const float* d_hits_xy, int32_t n_hits, 
                       int32_t capacity, int32_t assoc_dj, int32_t min_hits, int32_t* d_hit_to_cand,
                       int32_t* d_cand_nhits, uint8_t* d_cand_keep, void* cuda_stream);
 
+/* hough_vertex_vote ("apply a Hough transform to the track maxima" -- displaced vertices; D10).
+ * `plan` is the HOUGH_MODEL_LINE plan of the TRACK space that produced d_cands.  Every candidate with d_cand_keep[c] != 0
+ * (all candidates when d_cand_keep is NULL), rank < capacity and |d| >= d0_abs_min votes, for every vertex-azimuth
+ * column m (the plan's own n_phi column centres), for the radius R = d / sin(Phi_m - phi0_i), where d is the centre of the
+ * candidate's d0 bin:  d = qpt_min + ((float)j + 0.5f) * w;  sd = sin_m cos_i - cos_m sin_i;  R = d / sd;  t = R * n_r /
+ * r_max;  vote iff 0 <= t < n_r  (each fp32 operation rounded, IEEE division).
+ * OVERWRITES d_vertex_accum: int32 [n_events][n_phi][n_r], i.e. the layout of an accumulator with binning
+ * {n_phi, n_qpt = n_r, n_d0 = 1, qpt range [0, r_max), int32}: its peaks (hough_find_peaks on such a plan) are the vertex
+ * candidates (phi0 field = vertex azimuth, qpt field = vertex radius in cm).
+ * Errors: INVALID_ARG (null pointers, plan not of the line model, bad sizes), CUDA. */
+int hough_vertex_vote(hough_plan* plan, const hough_candidate* d_cands, const int32_t* d_cand_offsets, int32_t n_events,
+                      int32_t capacity, const uint8_t* d_cand_keep, float d0_abs_min, int32_t n_r, float r_max,
+                      int32_t* d_vertex_accum, void* cuda_stream);
+
 /* Plan options (debug / tuning; results never change).  key "fullscan": 1 = evaluate every (hit,i,k) with
  * no windowing and vote straight into global memory (the bisecting path of SURVEY section 5; also read once at
  * plan creation from the environment: HOUGH_DEBUG_FULLSCAN=1).  "exact_walk": 1 = the windowed walk runs the

@@ -40,7 +40,7 @@ class hough_geometry(C.Structure):
 
 
 EXPORTS = ["hough_plan_create", "hough_plan_destroy", "hough_accum_bytes", "hough_vote", "hough_find_peaks",
-           "hough_assign_hits", "hough_plan_set_option", "hough_pipeline_create", "hough_pipeline_destroy",
+           "hough_assign_hits", "hough_vertex_vote", "hough_plan_set_option", "hough_pipeline_create", "hough_pipeline_destroy",
            "hough_pipeline_run_host", "hough_pipeline_set_option", "hough_window_table", "hough_microbench", "hough_kernel_launches", "hough_status_string",
            "hough_version"]
 
@@ -69,6 +69,8 @@ def load_library() -> C.CDLL:
     lib.hough_find_peaks.argtypes = [P, P, I, I, P, I, P, P]
     lib.hough_assign_hits.restype = C.c_int
     lib.hough_assign_hits.argtypes = [P, P, I, P, I, P, P, I, I, I, P, P, P, P]
+    lib.hough_vertex_vote.restype = C.c_int
+    lib.hough_vertex_vote.argtypes = [P, P, P, I, I, P, C.c_float, I, C.c_float, P, P]
     lib.hough_plan_set_option.restype = C.c_int
     lib.hough_plan_set_option.argtypes = [P, C.c_char_p, I]
     lib.hough_pipeline_create.restype = C.c_int
@@ -252,6 +254,15 @@ class HoughPipeline:
                                                 cand_nhits.data_ptr(), cand_keep.data_ptr(), C.byref(over)),
                "hough_pipeline_run_host")
         return bool(over.value)
+
+
+def hough_vertex_vote(plan: "HoughPlan", cands, cand_offsets, n_events, capacity, cand_keep, d0_abs_min, n_r, r_max,
+                      vertex_accum, stream=None):
+    """include/hough.h hough_vertex_vote: vertex_accum int32 [n_events, n_phi, n_r] on the device (overwritten)."""
+    assert vertex_accum.dtype == torch.int32 and vertex_accum.numel() >= n_events * plan.n_phi * n_r
+    _check(plan.lib.hough_vertex_vote(plan._h, _dptr(cands), _dptr(cand_offsets), int(n_events), int(capacity),
+                                      _dptr(cand_keep), float(d0_abs_min), int(n_r), float(r_max), _dptr(vertex_accum),
+                                      _stream_ptr(stream)), "hough_vertex_vote")
 
 
 def window_table(n_phi, n_qpt, n_d0, qpt_min=-1.0, qpt_max=1.0, d0_min=-20.0, d0_max=20.0, bz_tesla=3.8, layers=(),
