@@ -47,6 +47,8 @@ def _load():
         lib.orc_vertex_vote.restype = C.c_longlong
         lib.orc_vertex_vote.argtypes = [C.POINTER(_Binning), C.c_float, P, P, C.c_int32, C.c_longlong, P, C.c_float, C.c_int32,
                                         C.c_float, P]
+        lib.orc_fit_circles.restype = C.c_int
+        lib.orc_fit_circles.argtypes = [C.POINTER(_Binning), C.c_float, P, C.c_int32, P, P, C.c_longlong, P, P, P]
         _lib = lib
     return _lib
 
@@ -177,6 +179,19 @@ class Oracle:
                                          float(d_abs_min), int(n_r), float(r_max), _ptr(vacc))
         assert votes >= 0, "orc_vertex_vote: bad arguments"
         return vacc, int(votes)
+
+    def fit_circles(self, hits_xy, hit_to_cand, cands: "OracleCandidates", keep=None):
+        """orc_fit_circles (D11): float64 [n_cands, 4] = {phi0, qpt, d0, R} and int32 [n_cands] hits used (< 0: fit not ok)."""
+        h = self._hits(hits_xy)
+        rec = np.ascontiguousarray(cands.records)
+        h2c = np.ascontiguousarray(hit_to_cand, dtype=np.int32)
+        keep = None if keep is None else np.ascontiguousarray(keep, dtype=np.uint8)
+        fit = np.zeros((max(len(rec), 1), 4), np.float64)
+        nfit = np.zeros(max(len(rec), 1), np.int32)
+        rc = self.lib.orc_fit_circles(C.byref(self.b), self.bz, _ptr(h), h.shape[0], _ptr(h2c), _ptr(rec), len(rec), _ptr(keep),
+                                      _ptr(fit), _ptr(nfit))
+        assert rc == 0
+        return fit[:len(rec)], nfit[:len(rec)]
 
     def assign_brute(self, hits_xy, event_offsets, cands, assoc_dj=1, min_hits=0, apply_dedup=True, capacity=None):
         return self._assign(self.lib.orc_assign_brute, hits_xy, event_offsets, cands, assoc_dj, min_hits,

@@ -458,4 +458,69 @@ long long orc_vertex_vote(const orc_binning* b, float bz, const orc_candidate* c
     return votes;
 }
 
+// D11 -- circle fit of the hits assigned to each kept candidate ("further computations (e.g., a full Kalman
+// fit) can be performed to confirm the existence of the track and obtain the best measurement of the track parameters";
+// an algebraic circle fit stands in for the Kalman fit).  Kasa fit, everything in double:
+// over the hits h with hit_to_cand[h] == c (x, y = the fp32 coordinates widened to double, z = x x + y y) accumulate
+//     n, Sx, Sy, Sz, Sxx, Sxy, Syy, Sxz, Syz
+// and minimise sum (z + B x + C y + D)^2:   [Sxx Sxy Sx; Sxy Syy Sy; Sx Sy n] (B, C, D)^T = -(Sxz, Syz, Sz)^T   (Cramer's rule).
+// Centre (xc, yc) = (-B/2, -C/2), R^2 = xc^2 + yc^2 - D.  ok = (n >= 3, |det| > 1e-9 * Sxx Syy n scale, R^2 > 0, |centre| > 0).
+// Track parameters in the D1 convention, orientation taken from the candidate's column (theta_i in double):
+//     p0 = centre (1 - R / |centre|)                      point of the circle closest to the origin
+//     t  = +-(-yc, xc) / |centre|, the sign with t . (cos theta_i, sin theta_i) >= 0;   phi0 = atan2(t_y, t_x) in [0, 2pi)
+//     n = (-t_y, t_x);   d0 = p0 . n;   1/rho = (centre - p0) . n;   q/pT = -rho / (K Bz)   (0 when Bz == 0)
+// out: double fit[c][4] = {phi0, qpt, d0, R};  int32 n_fit[c] = hits used, or -n when the fit is not ok (0: no hits / dropped).
+int orc_fit_circles(const orc_binning* b, float bz, const float* hits_xy, int32_t n_hits, const int32_t* hit_to_cand,
+                    const orc_candidate* cands, long long n_cands, const uint8_t* keep, double* fit, int32_t* n_fit) {
+    if (!valid_binning(b) || !hit_to_cand || !fit || !n_fit || n_hits < 0 || n_cands < 0) return -1;
+    std::vector<double> m((size_t)n_cands * 9, 0.0);
+    for (int h = 0; h < n_hits; ++h) {
+        const long long c = hit_to_cand[h];
+        if (c < 0 || c >= n_cands) continue;
+        const double x = (double)hits_xy[2 * h], y = (double)hits_xy[2 * h + 1];
+        const double z = x * x + y * y;
+        double* a = &m[(size_t)c * 9];
+        a[0] += 1.0; a[1] += x; a[2] += y; a[3] += z; a[4] += x * x; a[5] += x * y; a[6] += y * y; a[7] += x * z; a[8] += y * z;
+    }
+    const double kb = kGeVPerTeslaCm * (double)bz;
+    for (long long c = 0; c < n_cands; ++c) {
+        double* f = fit + 4 * c;
+        f[0] = f[1] = f[2] = f[3] = 0.0;
+        n_fit[c] = 0;
+        if (keep && !keep[c]) continue;
+        const double* a = &m[(size_t)c * 9];
+        const double n = a[0], Sx = a[1], Sy = a[2], Sz = a[3], Sxx = a[4], Sxy = a[5], Syy = a[6], Sxz = a[7], Syz = a[8];
+        const int ni = (int)n;
+        if (ni == 0) continue;
+        n_fit[c] = -ni;
+        if (ni < 3) continue;
+        const double det = Sxx * (Syy * n - Sy * Sy) - Sxy * (Sxy * n - Sy * Sx) + Sx * (Sxy * Sy - Syy * Sx);
+        if (!(std::fabs(det) > 1.0e-9 * std::fabs(Sxx * Syy * n))) continue;
+        const double r1 = -Sxz, r2 = -Syz, r3 = -Sz;
+        const double B = (r1 * (Syy * n - Sy * Sy) - Sxy * (r2 * n - Sy * r3) + Sx * (r2 * Sy - Syy * r3)) / det;
+        const double Cc = (Sxx * (r2 * n - r3 * Sy) - r1 * (Sxy * n - Sy * Sx) + Sx * (Sxy * r3 - r2 * Sx)) / det;
+        const double D = (Sxx * (Syy * r3 - Sy * r2) - Sxy * (Sxy * r3 - r2 * Sx) + r1 * (Sxy * Sy - Syy * Sx)) / det;
+        const double xc = -0.5 * B, yc = -0.5 * Cc;
+        const double R2 = xc * xc + yc * yc - D;
+        const double cn = std::sqrt(xc * xc + yc * yc);
+        if (!(R2 > 0.0) || !(cn > 0.0)) continue;
+        const double R = std::sqrt(R2);
+        const double theta = ((double)cands[c].i + 0.5) * (2.0 * kPi / (double)b->n_phi);
+        double tx = -yc / cn, ty = xc / cn;
+        if (tx * std::cos(theta) + ty * std::sin(theta) < 0.0) { tx = -tx; ty = -ty; }
+        const double s = 1.0 - R / cn;
+        const double p0x = xc * s, p0y = yc * s;
+        const double nx = -ty, ny = tx;
+        double phi0 = std::atan2(ty, tx);
+        if (phi0 < 0.0) phi0 += 2.0 * kPi;
+        const double inv_rho = (xc - p0x) * nx + (yc - p0y) * ny;
+        f[0] = phi0;
+        f[1] = (kb != 0.0) ? -(1.0 / inv_rho) / kb : 0.0;
+        f[2] = p0x * nx + p0y * ny;
+        f[3] = R;
+        n_fit[c] = ni;
+    }
+    return 0;
+}
+
 }  // extern "C"

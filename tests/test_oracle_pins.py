@@ -682,3 +682,43 @@ def test_d10_workload_6_vertex_directions():
     for ph in rec["phi0"]:
         dphi = np.abs(np.angle(np.exp(1j * (az_true - float(ph)))))
         assert dphi.min() < math.radians(20.0)
+
+
+# ---- D11: circle fit of the assigned hits ("obtain the best measurement of the track parameters"; f4) ------
+@pytest.mark.parametrize("seed", [0, 1, 2, 3, 4, 5])
+def test_d11_circle_fit_recovers_noiseless_helices(seed):
+    """Noiseless hits of a helix (phi0, q/pT, d0) generated from the D1 geometry: the fit returns the parameters."""
+    from oracle import CAND_DTYPE, OracleCandidates
+    rng = np.random.default_rng(seed)
+    n_phi = 256
+    o = Oracle(n_phi, 128, 64)
+    phi0 = rng.uniform(0, 2 * math.pi)
+    qpt = rng.uniform(0.1, 0.9) * rng.choice([-1.0, 1.0])
+    d0 = rng.uniform(-8.0, 8.0)
+    hits = helix_hits(phi0, qpt, d0, LAYERS_14, 3.8)
+    assert hits.shape[0] >= 5
+    rec = np.zeros(2, CAND_DTYPE)
+    rec["i"][1] = int(phi0 / (2 * math.pi) * n_phi)         # the candidate's column orients the fitted circle
+    cands = OracleCandidates(rec, np.array([0, 2], np.int32), 2)
+    h2c = np.ones(hits.shape[0], np.int32)                  # every hit assigned to candidate 1, none to candidate 0
+    fit, nfit = o.fit_circles(hits, h2c, cands, np.array([1, 1], np.uint8))
+    assert nfit[0] == 0 and nfit[1] == hits.shape[0]
+    f = fit[1]
+    assert abs(np.angle(np.exp(1j * (f[0] - phi0)))) < 2e-5 and abs(f[1] - qpt) < 2e-5 * max(1.0, abs(qpt)) and abs(f[2] - d0) < 2e-4
+    assert abs(f[3] - 1.0 / abs(qpt * K * 3.8)) < 1e-3 * f[3]
+
+
+def test_d11_fit_flags_and_textbook_circle():
+    from oracle import CAND_DTYPE, OracleCandidates
+    o = Oracle(64, 32, 1)
+    # 8 exact points on the circle centre (3, -4), R = 10 (contains the origin side: |centre| = 5 < R)
+    ang = np.linspace(0.1, 5.9, 8)
+    pts = np.stack([3 + 10 * np.cos(ang), -4 + 10 * np.sin(ang)], 1).astype(np.float32)
+    two = pts[:2]
+    hits = np.concatenate([pts, two])
+    rec = np.zeros(3, CAND_DTYPE)
+    cands = OracleCandidates(rec, np.array([0, 3], np.int32), 3)
+    h2c = np.array([0] * 8 + [1, 1], np.int32)
+    fit, nfit = o.fit_circles(hits, h2c, cands, np.array([1, 1, 0], np.uint8))
+    assert list(nfit) == [8, -2, 0]                          # ok; too few hits; dropped candidate
+    assert abs(fit[0, 3] - 10.0) < 1e-5 and abs(abs(fit[0, 2]) - 5.0) < 1e-5      # R and |d0| = | |centre| - R |
