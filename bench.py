@@ -454,6 +454,31 @@ def run_ours(args, rank, world, local_rank):
                   "threshold": thr_v, "api": "hough_vertex_vote + hough_find_peaks on the vertex space (D10)"}
         vplan.close()
 
+    # circle fit of the assigned hits (D11), first tile, outside the timed step
+    fit_info = None
+    try:
+        from paper_1311_2769_b200 import hough_fit_circles
+        (e0, e1, h0, h1) = run.tiles[0]
+        n_ev = e1 - e0
+        run.step()
+        work = torch.empty((run.cap, 9), dtype=torch.float64, device="cuda")
+        fitp = torch.empty((run.cap, 4), dtype=torch.float64, device="cuda")
+        nfit = torch.empty((run.cap,), dtype=torch.int32, device="cuda")
+        ft = []
+        for it in range(12):
+            a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+            a.record()
+            hough_fit_circles(run.plan, run.d_hits[h0:h1], run.h2c[:max(h1 - h0, 1)][:h1 - h0], run.cands, run.cand_off, n_ev,
+                              run.cap, run.keep, work, fitp, nfit)
+            b.record(); b.synchronize()
+            if it >= 2:
+                ft.append(a.elapsed_time(b))
+        fit_info = {"ms_median": statistics.median(ft), "events": n_ev, "tracks_fitted": int((nfit > 0).sum().item()),
+                    "api": "hough_fit_circles on the first tile (D11), not part of the timed step"}
+        del work, fitp, nfit
+    except Exception as exc:                              # noqa: BLE001 -- report, do not hide
+        print(f"bench.py: fit stage failed: {exc}", file=sys.stderr)
+
     n_ref = oracle_events_for_seconds(w, args.cpu_seconds)
     o_votes, o_events, o_secs = oracle_sample(w, batch, n_ref)
     cpu = {"value": o_votes / o_secs, "unit": UNIT, "cores": 1, "kind": "oracle",
@@ -487,6 +512,8 @@ def run_ours(args, rank, world, local_rank):
             "candidate_overflow": peaks_overflow}
     if vertex is not None:
         line["vertex"] = vertex
+    if fit_info is not None:
+        line["fit"] = fit_info
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

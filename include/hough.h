@@ -132,6 +132,20 @@ int hough_vertex_vote(hough_plan* plan, const hough_candidate* d_cands, const in
                       int32_t capacity, const uint8_t* d_cand_keep, float d0_abs_min, int32_t n_r, float r_max,
                       int32_t* d_vertex_accum, void* cuda_stream);
 
+/* hough_fit_circles ("further computations (e.g., a full Kalman fit) can be performed to confirm the existence
+ * of the track and obtain the best measurement of the track parameters"; D11: an algebraic circle fit in double stands in).
+ * For every candidate c < min(d_cand_offsets[n_events], capacity) with d_cand_keep[c] != 0 (all when NULL): Kasa fit
+ * (minimise sum (x^2 + y^2 + B x + C y + D)^2) of the hits h with d_hit_to_cand[h] == c, then the D1 parameters of the
+ * circle, oriented by the candidate's phi0 column: d_fit[c] = {phi0 [rad, 0..2pi), q/pT [1/GeV; 0 when Bz = 0], d0 [cm],
+ * radius [cm]}; d_n_fit[c] = hits used, -(hits) when the fit is not ok (< 3 hits, singular, R^2 <= 0), 0 when no hits /
+ * dropped / beyond the list (d_fit then zero).  d_work: caller's scratch, 9 doubles per candidate of `capacity`.
+ * Moments are summed with double atomics, so results agree with a sequential sum to ~1e-9 relative, not bit for bit. */
+typedef struct { double phi0, qpt, d0, radius; } hough_track_fit;
+int hough_fit_circles(hough_plan* plan, const float* d_hits_xy, int32_t n_hits, const int32_t* d_hit_to_cand,
+                      const hough_candidate* d_cands, const int32_t* d_cand_offsets, int32_t n_events, int32_t capacity,
+                      const uint8_t* d_cand_keep, double* d_work, hough_track_fit* d_fit, int32_t* d_n_fit,
+                      void* cuda_stream);
+
 /* Plan options (debug / tuning; results never change).  key "fullscan": 1 = evaluate every (hit,i,k) with
  * no windowing and vote straight into global memory (the bisecting path of SURVEY section 5; also read once at
  * plan creation from the environment: HOUGH_DEBUG_FULLSCAN=1).  "exact_walk": 1 = the windowed walk runs the
