@@ -410,8 +410,8 @@ def run_ours(args, rank, world, local_rank):
     bins_per_launch = bn.n_bins * run.tile_events
     hbm_bytes = hits_per_launch * 8 + bins_per_launch * bn.bin_bytes            # hits in + accumulator out
     # dram__bytes_read.sum + dram__bytes_write.sum of the walk kernel in the ncu --set full capture of this very
-    # launch configuration (profiles/r1_final.md): 20.0 MB + 350.8 MB per 128-event launch of cfg 3
-    traffic = 370.8e6 if (args.config == 3 and run.tile_events == 128) else None
+    # launch configuration (profiles/r1_final.md): 39.6 MB + 756.0 MB per 256-event launch of cfg 3 (20.0 + 350.8 MB at 128)
+    traffic = {256: 795.6e6, 128: 370.8e6}.get(run.tile_events) if args.config == 3 else None
     roofline = {"bound": "alu", "kernel": "hough_vote (stage + vote + flush)", "achieved": achieved, "peak": alu_peak,
                 "unit": "Gvotes/s", "frac": achieved / alu_peak, "traffic": traffic,
                 "peak_source": f"{sms} SMs x {FP32_LANES_PER_SM} fp32 lanes x {sm_max_mhz:.0f} MHz / "
@@ -594,7 +594,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=3)
     ap.add_argument("--events", type=int, default=0, help="events per GPU (default: the workload's own count)")
-    ap.add_argument("--tile-events", type=int, default=128, help="events per call of the device-resident loop")
+    ap.add_argument("--tile-events", type=int, default=256, help="events per call of the device-resident loop")
     ap.add_argument("--e2e-tile-events", type=int, default=32, help="events per tile of the batched host pipeline")
     ap.add_argument("--cand-per-bin", type=float, default=1.0 / 16.0, help="candidate capacity per accumulator bin")
     ap.add_argument("--e2e-steps", type=int, default=2)
