@@ -3,7 +3,9 @@
 // Kasa circle fit in double precision stands in for the Kalman fit).
 //   K-fit-a  zero the moment rows of the candidates in use
 //   K-fit-b  one thread per hit: 9 double atomicAdds {n, Sx, Sy, Sz, Sxx, Sxy, Syy, Sxz, Syz} into its candidate's row
-//   K-fit-c  one thread per candidate: 3x3 normal equations by Cramer's rule, centre / radius, D1 parameters
+//   K-fit-c  one thread per candidate: moments about the hits' centroid, 2x2 solve for the centre, D1 parameters in
+//            closed form from (centre, R, orientation) -- written from the definition, independently of the oracle's
+//            3x3 Cramer solve and vector construction
 #include <cmath>
 
 #include "common.cuh"
@@ -44,36 +46,41 @@ __global__ void __launch_bounds__(128) fit_solve_kernel(HoughConsts c, double kb
     int nf = 0;
     const int n_c = min(cand_off[n_events], capacity);
     if (ci < n_c && (!keep || keep[ci])) {
+        // Raw sums of the candidate's hits: m0 = count, m1 = (Sx, Sy), Sz = sum |p|^2, second moments, and sum p |p|^2.
         const double* a = work + (size_t)ci * 9;
-        const double n = a[0], Sx = a[1], Sy = a[2], Sz = a[3], Sxx = a[4], Sxy = a[5], Syy = a[6], Sxz = a[7], Syz = a[8];
-        const int ni = (int)n;
-        nf = -ni;
-        if (ni >= 3) {
-            const double det = Sxx * (Syy * n - Sy * Sy) - Sxy * (Sxy * n - Sy * Sx) + Sx * (Sxy * Sy - Syy * Sx);
-            if (fabs(det) > 1.0e-9 * fabs(Sxx * Syy * n)) {
-                const double r1 = -Sxz, r2 = -Syz, r3 = -Sz;
-                const double B = (r1 * (Syy * n - Sy * Sy) - Sxy * (r2 * n - Sy * r3) + Sx * (r2 * Sy - Syy * r3)) / det;
-                const double Cc = (Sxx * (r2 * n - r3 * Sy) - r1 * (Sxy * n - Sy * Sx) + Sx * (Sxy * r3 - r2 * Sx)) / det;
-                const double D = (Sxx * (Syy * r3 - Sy * r2) - Sxy * (Sxy * r3 - r2 * Sx) + r1 * (Sxy * Sy - Syy * Sx)) / det;
-                const double xc = -0.5 * B, yc = -0.5 * Cc;
-                const double R2 = xc * xc + yc * yc - D;
-                const double cn = sqrt(xc * xc + yc * yc);
-                if (R2 > 0.0 && cn > 0.0) {
-                    const double R = sqrt(R2);
-                    const double theta = ((double)cands[ci].i + 0.5) * (2.0 * 3.14159265358979323846 / (double)c.n_phi);
-                    double tx = -yc / cn, ty = xc / cn;
-                    if (tx * cos(theta) + ty * sin(theta) < 0.0) { tx = -tx; ty = -ty; }
-                    const double s = 1.0 - R / cn;
-                    const double p0x = xc * s, p0y = yc * s;
-                    const double nx = -ty, ny = tx;
-                    double phi0 = atan2(ty, tx);
-                    if (phi0 < 0.0) phi0 += 2.0 * 3.14159265358979323846;
-                    const double inv_rho = (xc - p0x) * nx + (yc - p0y) * ny;
-                    f.phi0 = phi0;
-                    f.qpt = (kb != 0.0) ? -(1.0 / inv_rho) / kb : 0.0;
-                    f.d0 = p0x * nx + p0y * ny;
-                    f.radius = R;
-                    nf = ni;
+        const double m0 = a[0];
+        const int cnt = (int)m0;
+        nf = -cnt;
+        if (cnt >= 3) {
+            // Work about the centroid g = m1 / m0 (u = p - g).  Centred second moments and the centred cubic sums
+            // T = sum u |u|^2 follow from the raw sums; the Kasa minimum has its centre at g + c with
+            //     [Cuu Cuv; Cuv Cvv] c = T / 2        and       R^2 = |c|^2 + (Cuu + Cvv) / m0.
+            const double gx = a[1] / m0, gy = a[2] / m0, gg = gx * gx + gy * gy;
+            const double Cuu = a[4] - gx * a[1], Cuv = a[5] - gx * a[2], Cvv = a[6] - gy * a[2];
+            const double zc = a[3] - 2.0 * (gx * a[1] + gy * a[2]) + m0 * gg;                      // sum |u|^2 = Cuu + Cvv
+            const double Tu = a[7] - 2.0 * (gx * a[4] + gy * a[5]) + gg * a[1] - gx * zc;
+            const double Tv = a[8] - 2.0 * (gx * a[5] + gy * a[6]) + gg * a[2] - gy * zc;
+            const double dd = Cuu * Cvv - Cuv * Cuv;                     // (3x3 normal-equation determinant) / m0
+            if (fabs(dd) > 1.0e-9 * fabs(a[4] * a[6])) {                 // D11's singularity test, divided by m0
+                const double cu = 0.5 * (Tu * Cvv - Tv * Cuv) / dd, cv = 0.5 * (Tv * Cuu - Tu * Cuv) / dd;
+                const double ox = gx + cu, oy = gy + cv;                // circle centre
+                const double rr = cu * cu + cv * cv + zc / m0;
+                const double oc = hypot(ox, oy);
+                if (rr > 0.0 && oc > 0.0) {
+                    // D1: the centre is (d0 + 1/rho) n_hat with n_hat = (-sin phi0, cos phi0).  Of the two orientations
+                    // n_hat = +-centre/|centre| take the one whose direction of travel (n_y, -n_x) points along the
+                    // candidate's column; then 1/rho = s R (|d0| < R), d0 = s (|centre| - R).
+                    const double rad = sqrt(rr);
+                    double sn, cs;
+                    sincos(((double)cands[ci].i + 0.5) * (6.283185307179586476925 / (double)c.n_phi), &sn, &cs);
+                    const double s = (oy * cs - ox * sn) >= 0.0 ? 1.0 : -1.0;
+                    double ph = atan2(-s * ox, s * oy);
+                    if (ph < 0.0) ph += 6.283185307179586476925;
+                    f.phi0 = ph;
+                    f.qpt = kb != 0.0 ? -s / (rad * kb) : 0.0;
+                    f.d0 = s * (oc - rad);
+                    f.radius = rad;
+                    nf = cnt;
                 }
             }
         }

@@ -82,3 +82,53 @@ def test_fit_without_keep_flags_and_empty_inputs():
     assert np.array_equal(nfit.cpu().numpy(), nfit_ref)
     assert np.allclose(fit.cpu().numpy(), fit_ref, rtol=1e-7, atol=1e-7)
     plan.close()
+
+
+def test_fit_recovers_analytic_helices_without_the_oracle():
+    """The fit kernel against the geometry itself (no oracle on the expected side): noiseless helices generated from
+    their D1 parameters (both charges, d0 of both signs and zero, all quadrants of phi0) must come back; the fp32
+    rounding of the hit coordinates (~1e-7 relative) limits the agreement, not the solve."""
+    import math
+    from workloads import LAYERS_14, helix_hits
+    rng = np.random.default_rng(11)
+    bz = 3.8
+    n_phi = 256
+    tracks, hits, h2c = [], [], []
+    for t in range(64):
+        phi0 = rng.uniform(0, 2 * math.pi)
+        qpt = rng.choice([-1.0, 1.0]) * rng.uniform(0.05, 0.9)
+        d0 = 0.0 if t % 4 == 0 else rng.uniform(-3.0, 3.0)
+        p = helix_hits(phi0, qpt, d0, LAYERS_14, bz)
+        if len(p) < 5:
+            continue
+        tracks.append((phi0, qpt, d0, len(p)))
+        hits.append(p)
+        h2c += [len(tracks) - 1] * len(p)
+    n_t = len(tracks)
+    assert n_t > 40
+    hits = np.concatenate(hits)
+    perm = rng.permutation(len(hits))
+    hits, h2c = hits[perm], np.asarray(h2c, np.int32)[perm]
+    rec = np.zeros(n_t, dtype=[("event", "<i4"), ("k", "<i4"), ("i", "<i4"), ("j", "<i4"), ("votes", "<i4"),
+                               ("phi0", "<f4"), ("qpt", "<f4"), ("d0", "<f4")])
+    for c, (phi0, _, _, _) in enumerate(tracks):
+        rec[c]["i"] = int(phi0 / (2 * math.pi) * n_phi) % n_phi        # the candidate's column orients the circle
+    plan = HoughPlan(n_phi, 128, 1, -1.0, 1.0, -20.0, 20.0, 0, bz, LAYERS_14, max_hits=len(hits), max_events=1)
+    cands = alloc_candidates(n_t)
+    cands[:n_t].copy_(torch.from_numpy(rec.view(np.uint8).reshape(n_t, 32)))
+    coff = torch.tensor([0, n_t], dtype=torch.int32, device="cuda")
+    work = torch.empty((n_t, 9), dtype=torch.float64, device="cuda")
+    fit = torch.empty((n_t, 4), dtype=torch.float64, device="cuda")
+    nfit = torch.empty((n_t,), dtype=torch.int32, device="cuda")
+    hough_fit_circles(plan, torch.from_numpy(hits).cuda(), torch.from_numpy(h2c).cuda(), cands, coff, 1, n_t, None, work,
+                      fit, nfit)
+    torch.cuda.synchronize()
+    f, n = fit.cpu().numpy(), nfit.cpu().numpy()
+    K = 0.00299792458
+    for c, (phi0, qpt, d0, nh) in enumerate(tracks):
+        assert n[c] == nh
+        assert abs(np.angle(np.exp(1j * (f[c, 0] - phi0)))) < 2e-5, (c, f[c], tracks[c])
+        assert abs(f[c, 1] - qpt) < 2e-5 * max(1.0, abs(qpt)) + 2e-5
+        assert abs(f[c, 2] - d0) < 2e-4
+        assert abs(f[c, 3] - 1.0 / (abs(qpt) * K * bz)) < 2e-5 * f[c, 3] + 1e-3
+    plan.close()

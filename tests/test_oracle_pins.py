@@ -352,6 +352,99 @@ def test_v7_centroid_integer_moments():
     assert r["d0"] == 0.0
 
 
+def test_v7_centroid_d0_term_asymmetric_neighbourhood():
+    """D7, the d0 offset: a constructed 3-D volume whose three moments differ in sign and size, values by hand.
+    centre 6 at (k,i,j) = (1,4,4); 2 at k+1; 1 at k-1; 1 at i-1  ->  S = 10, Sk = +1, Si = -1, Sj = 0."""
+    o = Oracle(8, 8, 4, qpt_min=-1.0, qpt_max=1.0, d0_min=-20.0, d0_max=20.0, bz_tesla=BZ)
+    acc = np.zeros((1, 4, 8, 8), np.int32)
+    acc[0, 1, 4, 4] = 6
+    acc[0, 2, 4, 4] = 2          # +dk
+    acc[0, 0, 4, 4] = 1          # -dk
+    acc[0, 1, 3, 4] = 1          # -di
+    c = o.find_peaks(acc, 6)
+    assert c.total == 1 and tuple(c.records[0][["k", "i", "j", "votes"]]) == (1, 4, 4, 6)
+    r = c.records[0]
+    wd, wq, wphi = 10.0, 0.25, 2 * math.pi / 8
+    assert abs(r["d0"] - (-20.0 + (1.5 + 1.0 / 10.0) * wd)) < 2e-6          # = -4.0: Sk enters with +, scaled by wd
+    assert abs(r["phi0"] - ((4.5 - 1.0 / 10.0) * wphi)) < 1e-6
+    assert abs(r["qpt"] - (-1.0 + 4.5 * wq)) < 1e-6
+    # the mirrored volume moves d0 the other way (a sign error in Sk cannot satisfy both)
+    acc[0, 2, 4, 4], acc[0, 0, 4, 4] = 1, 2
+    r = o.find_peaks(acc, 6).records[0]
+    assert abs(r["d0"] - (-20.0 + (1.5 - 1.0 / 10.0) * wd)) < 2e-6
+    # peak on the k = 0 face: the missing slice contributes nothing (clipped, S10)
+    acc = np.zeros((1, 4, 8, 8), np.int32)
+    acc[0, 0, 2, 2] = 7
+    acc[0, 1, 2, 2] = 3
+    r = o.find_peaks(acc, 7).records[0]
+    assert abs(r["d0"] - (-20.0 + (0.5 + 3.0 / 10.0) * wd)) < 2e-6
+
+
+def test_v7_centroid_phi_wrap_both_branches():
+    """D7: "phi0 ... wrapped into [0, 2pi) by one +-2pi".  A peak at i = 0 whose weight sits at i = n_phi - 1 has
+    (i + 0.5 + Si/S) < 0 and must come back just below 2pi; the mirror case at i = n_phi - 1 comes back just above 0."""
+    n = 8
+    o = Oracle(n, 8, 1, bz_tesla=BZ)
+    wphi = 2 * math.pi / n
+    acc = np.zeros((1, 1, n, 8), np.int32)
+    acc[0, 0, 0, 4] = 5
+    acc[0, 0, n - 1, 3:6] = 4        # three "before" neighbours, each < 5, together heavier than the centre
+    c = o.find_peaks(acc, 5)
+    assert c.total == 1 and tuple(c.records[0][["i", "j"]]) == (0, 4)
+    ti = 0.5 - 12.0 / 17.0           # S = 17, Si = -12
+    assert ti < 0
+    exp = ti * wphi + 2 * math.pi
+    assert 2 * math.pi - wphi <= c.records[0]["phi0"] < np.float32(2 * math.pi)
+    assert abs(c.records[0]["phi0"] - exp) < 2e-6
+    acc = np.zeros((1, 1, n, 8), np.int32)
+    acc[0, 0, n - 1, 4] = 5
+    acc[0, 0, 0, 3:6] = 4            # three "after" neighbours
+    c = o.find_peaks(acc, 5)
+    assert c.total == 1 and tuple(c.records[0][["i", "j"]]) == (n - 1, 4)
+    ti = n - 0.5 + 12.0 / 17.0
+    assert ti > n
+    exp = ti * wphi - 2 * math.pi
+    assert 0.0 <= c.records[0]["phi0"] < wphi
+    assert abs(c.records[0]["phi0"] - exp) < 2e-6
+
+
+def test_s5_top_edge_is_decided_on_t():
+    """S5: the range test is on t itself.  q/pT = 1 - 2^-24 (the fp32 just below q_max = 1) is inside [q_min, q_max)
+    mathematically, but (v - q_min) = 2 - 2^-24 rounds to 2.0, t = n_qpt, and the vote is DROPPED; v = 1 - 2^-23
+    lands in the last bin.  Hits are searched (seeded) on the column's q/pT = 1 circle; fp32 numpy mirrors D3 only to
+    pick which of the candidate hits realise those two values; the assertions are the reading's."""
+    n_phi, n_qpt, i = 64, 32, 5
+    o = Oracle(n_phi, n_qpt, 1, bz_tesla=BZ)
+    t = o.tables()
+    c, s, A = np.float32(t["cosT"][i]), np.float32(t["sinT"][i]), np.float32(t["A_f"])
+    th = (i + 0.5) * 2 * math.pi / n_phi
+    Rc = 1.0 / (K * float(np.float32(BZ)) * 1.0)                 # radius of the q/pT = +1 circle through the origin
+    rng = np.random.default_rng(5)
+    a = rng.uniform(0.02, 0.6, 400000)                          # tangent-chord angle; hit = chord of length 2 R sin(a)
+    r = 2 * Rc * np.sin(a)
+    ang = th - a                                                # positive charge bends clockwise (D1)
+    x = (r * np.cos(ang)).astype(np.float32)
+    y = (r * np.sin(ang)).astype(np.float32)
+    r2 = x * x + y * y
+    w = y * c - x * s
+    v = (np.float32(0.0) - w) * (np.float32(1.0) / (A * r2))
+    below1 = np.nextafter(np.float32(1.0), np.float32(0.0))
+    below2 = np.nextafter(below1, np.float32(0.0))
+    drop = np.nonzero(v == below1)[0][:16]
+    keep = np.nonzero(v == below2)[0][:16]
+    assert len(drop) >= 4 and len(keep) >= 4
+    for h in drop:
+        hit = np.array([[x[h], y[h]]], np.float32)
+        # in range in exact arithmetic on the fp32 value v = 1 - 2^-24 < q_max ...
+        assert float(below1) < 1.0
+        # ... yet no vote: t == n_qpt exactly
+        assert o.vote_columns(hit, None, [[0, 0, i]]).sum() == 0
+    for h in keep:
+        hit = np.array([[x[h], y[h]]], np.float32)
+        row = o.vote_columns(hit, None, [[0, 0, i]])[0]
+        assert row.sum() == 1 and row[n_qpt - 1] == 1
+
+
 def test_v7_slab_peaks_equal_full_volume():
     w = get_workload(1)
     hits = generate_events(w).hits_xy
