@@ -273,6 +273,7 @@ def test_assign_tile_variants_bit_exact(shape, dtype, max_hits, dj):
     ((64, 64, 40), ACC_U16, False, "regs"),     # packed walk with register-held rows (no cp.async ring)
     ((256, 128, 1), ACC_U16, False, "regs"),
     ((512, 1024, 3), ACC_U16, False, False),    # cp.async ring: two rows per CTA (128 chunks per row)
+    ((512, 2048, 3), ACC_U16, False, False),    # rows too long for the ring: packed register walk (peak_kwalk16)
     ((32, 8, 5), ACC_U16, False, False),        # packed slice walk, one chunk per row (both q/pT faces in one thread)
 ])
 def test_peaks_tile_variants_bit_exact(shape, dtype, fullscan, tiled):
