@@ -16,9 +16,12 @@ One JSON line goes to stdout (rank 0):
   events_per_s     the same step expressed in events/s (the metric's second figure)
   e2e              the same metric through hough_pipeline_run_host (T2-event tiles on S streams, CUDA graphs): pinned
                    HOST buffers in, HOST results out, host<->device copies inside the timed region
-  roofline         dominant kernel (vote): algorithmic votes per launch / average launch duration (CUDA events
-                   on the launching stream, inside the timed region) against the ALU issue bound derived in
-                   DESIGN.md; the atomic and HBM ceilings of SURVEY 8(d) are quoted beside it
+  roofline         hough_vote: algorithmic votes per launch / average launch duration (CUDA events on the launching
+                   stream, inside the timed region) against the LOWEST of three ceilings, picked by rule in the run:
+                   ALU issue, shared-memory atomics (hough_microbench, measured in this process), HBM
+                   (MEASURED_PEAKS.json); all three fractions are in the object
+  roofline_assign  hough_assign_hits and hough_find_peaks timed the same way (per-position ALU ceiling; HBM bytes)
+  roofline_peaks
   cpu_baseline     the CPU oracle as it stands, one thread, on a bounded sample of the same workload
   --impl reference times the oracle instead (this tier's reference arm).
 
@@ -129,6 +132,21 @@ def load_peaks():
             p = json.load(f)
         return float(p["hbm_gbs"]), float(p.get("sm_max_mhz", 1965.0)), "measured (MEASURED_PEAKS.json)"
     return 6650.0, 1965.0, "fallback (B200_PROFILING.md)"
+
+
+def load_traffic():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture
+    (profiles/r2_traffic.csv: kernel,tile_events,dram_bytes; the command is in profiles/r2_traffic.md).  ({}, None) if absent."""
+    path = os.path.join(ROOT, "profiles", "r2_traffic.csv")
+    tab = {}
+    if not os.path.exists(path):
+        return tab, None
+    with open(path) as f:
+        for line in f:
+            p = [x.strip() for x in line.split(",")]
+            if len(p) >= 3 and p[1].isdigit():
+                tab[(p[0], int(p[1]))] = float(p[2])
+    return tab, "profiles/r2_traffic.csv (ncu --set full capture of this launch configuration; see profiles/r2_traffic.md)"
 
 
 # ----------------------------------------------------------------------------------------------
@@ -250,26 +268,34 @@ class DeviceRun:
         self.keep = torch.empty(self.cap, dtype=torch.uint8, device="cuda")
         self.totals = torch.zeros(len(self.tiles), dtype=torch.int32, device="cuda")
 
-    def step(self, vote_events=None):
-        """One pass over all tiles on the current stream.  vote_events: list to append (start, end) CUDA
-        events bracketing each hough_vote call."""
+    def step_tile(self, t, call_events=None):
+        """vote -> find_peaks -> assign_hits of tile t on the current stream.  call_events: dict of lists
+        {"vote", "peaks", "assign"} to append (start, end) CUDA events bracketing each C-ABI call."""
         torch = self.torch
         w = self.w
-        for t, (e0, e1, h0, h1) in enumerate(self.tiles):
-            hits = self.d_hits[h0:h1]
-            offs = self.d_offs[t]
-            n_ev = e1 - e0
-            if vote_events is not None:
-                a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
-                a.record()
-            self.plan.vote(hits, offs, self.accum)
-            if vote_events is not None:
-                b.record()
-                vote_events.append((a, b))
-            self.plan.find_peaks(self.accum, n_ev, w.threshold, self.cands, self.cap, self.cand_off)
-            self.plan.assign_hits(hits, offs, self.cands, self.cand_off, self.cap, w.assoc_dj, w.min_hits,
-                                  self.h2c[:max(h1 - h0, 1)], self.nh, self.keep)
-            self.totals[t:t + 1].copy_(self.cand_off[n_ev:n_ev + 1])
+        (e0, e1, h0, h1) = self.tiles[t]
+        hits = self.d_hits[h0:h1]
+        offs = self.d_offs[t]
+        n_ev = e1 - e0
+
+        def timed(name, fn):
+            if call_events is None:
+                fn()
+                return
+            a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+            a.record(); fn(); b.record()
+            call_events[name].append((a, b))
+
+        timed("vote", lambda: self.plan.vote(hits, offs, self.accum))
+        timed("peaks", lambda: self.plan.find_peaks(self.accum, n_ev, w.threshold, self.cands, self.cap, self.cand_off))
+        timed("assign", lambda: self.plan.assign_hits(hits, offs, self.cands, self.cand_off, self.cap, w.assoc_dj,
+                                                      w.min_hits, self.h2c[:max(h1 - h0, 1)], self.nh, self.keep))
+        self.totals[t:t + 1].copy_(self.cand_off[n_ev:n_ev + 1])
+
+    def step(self, call_events=None):
+        """One pass over all tiles on the current stream."""
+        for t in range(len(self.tiles)):
+            self.step_tile(t, call_events)
 
     def count_votes(self) -> int:
         """Votes cast per step = sum of all accumulator bins (counted once, outside the timed region)."""
@@ -363,20 +389,21 @@ def run_ours(args, rank, world, local_rank):
         sampler.start()
         time.sleep(0.3)
     barrier()
-    vote_events = []
+    call_events = {"vote": [], "peaks": [], "assign": []}
     launches0 = kernel_launches()
     t_mark0 = time.time()
     ev0 = torch.cuda.Event(enable_timing=True); ev1 = torch.cuda.Event(enable_timing=True)
     ev0.record()
     for _ in range(args.steps):
-        run.step(vote_events)
+        run.step(call_events)
     ev1.record()
     barrier()
     t_mark1 = time.time()
     launches = kernel_launches() - launches0
     ms_total = ev0.elapsed_time(ev1)
     clocks = sampler.stop(t_mark0, t_mark1) if rank == 0 else None
-    vote_ms = [a.elapsed_time(b) for (a, b) in vote_events]
+    call_ms = {k: [a.elapsed_time(b) for (a, b) in v] for k, v in call_events.items()}
+    vote_ms = call_ms["vote"]
     peaks_overflow = bool((run.totals > run.cap).any().item())
 
     # max over ranks (device time), whole-job totals
@@ -401,32 +428,67 @@ def run_ours(args, rank, world, local_rank):
     hbm_gbs, sm_max_mhz, peak_src = load_peaks()
     sms = torch.cuda.get_device_properties(local_rank).multi_processor_count
     bn = w.binning
-    # dominant kernel = vote: one launch per tile
-    vote_ms_avg = sum(vote_ms) / len(vote_ms)
+    n_launch = len(run.tiles) * args.steps
     votes_per_launch = votes_per_step / len(run.tiles)
-    achieved = votes_per_launch / (vote_ms_avg * 1e-3) / 1e9                     # Gvotes/s
-    alu_peak = sms * FP32_LANES_PER_SM * sm_max_mhz * 1e6 / D3_MIN_ISSUE_SLOTS / 1e9
     hits_per_launch = batch.n_hits / len(run.tiles)
     bins_per_launch = bn.n_bins * run.tile_events
+    cands_per_launch = float(run.totals.sum().item()) / len(run.tiles)
+
+    # Ceilings measured in THIS process on THIS GPU (hough_microbench, outside the timed region): conflict-free and
+    # random-address shared-memory atomicAdd rates, and the issue rate of the exact D3 sequence.
+    from paper_1311_2769_b200 import microbench
+    mb = {"smem_atomic_conflict_free_gops": microbench(0, 0, 5) / 1e9, "smem_atomic_random_gops": microbench(1, 0, 5) / 1e9,
+          "d3_exact_eval_gops": microbench(4, 0, 5) / 1e9}
+    traffic_tab, traffic_src = load_traffic()
+
+    def avg(name):
+        return sum(call_ms[name]) / max(len(call_ms[name]), 1)
+
+    # --- hough_vote (stage + vote walk + flush).  Three ceilings in votes/s; `bound` is the LOWEST of them,
+    # chosen here by rule: ALU issue (12 issue slots per vote at the very least), shared-memory atomics (one per
+    # vote, conflict-free rate measured above), HBM (hit bytes in + accumulator bytes out at the measured copy rate).
+    vote_ms_avg = avg("vote")
+    achieved = votes_per_launch / (vote_ms_avg * 1e-3) / 1e9                     # Gvotes/s
     hbm_bytes = hits_per_launch * 8 + bins_per_launch * bn.bin_bytes            # hits in + accumulator out
-    # dram__bytes_read.sum + dram__bytes_write.sum of the walk kernel in the ncu --set full capture of this very
-    # launch configuration (profiles/r1_final.md): 39.6 MB + 756.0 MB per 256-event launch of cfg 3 (20.0 + 350.8 MB at 128)
-    traffic = {256: 795.6e6, 128: 370.8e6}.get(run.tile_events) if args.config == 3 else None
-    roofline = {"bound": "alu", "kernel": "hough_vote (stage + vote + flush)", "achieved": achieved, "peak": alu_peak,
-                "unit": "Gvotes/s", "frac": achieved / alu_peak, "traffic": traffic,
-                "peak_source": f"{sms} SMs x {FP32_LANES_PER_SM} fp32 lanes x {sm_max_mhz:.0f} MHz / "
-                               f"{D3_MIN_ISSUE_SLOTS} issue slots per vote (DESIGN.md); clocks {peak_src}",
-                "vote_ms_per_launch": vote_ms_avg, "votes_per_launch": votes_per_launch,
+    ceilings = {"alu": sms * FP32_LANES_PER_SM * sm_max_mhz * 1e6 / D3_MIN_ISSUE_SLOTS / 1e9,
+                "atomic": mb["smem_atomic_conflict_free_gops"],
+                "hbm": votes_per_launch / (hbm_bytes / (hbm_gbs * 1e9)) / 1e9}
+    bound = min(ceilings, key=ceilings.get)
+    roofline = {"bound": bound, "kernel": "hough_vote (stage + vote walk + flush)", "achieved": achieved,
+                "peak": ceilings[bound], "unit": "Gvotes/s", "frac": achieved / ceilings[bound],
+                "traffic": traffic_tab.get(("vote", run.tile_events)) if args.config == 3 else None,
+                "traffic_source": traffic_src,
+                "rule": "bound = the lowest of the three ceilings below, all in votes/s (SURVEY 8(d): report all three, "
+                        "say which binds); north_star's reading (slower of atomic and HBM) is frac_atomic / frac_hbm",
+                "ceilings_gvotes": ceilings,
+                "frac_alu": achieved / ceilings["alu"], "frac_atomic": achieved / ceilings["atomic"],
+                "frac_atomic_random": achieved / mb["smem_atomic_random_gops"], "frac_hbm": achieved / ceilings["hbm"],
+                "peak_source": f"alu: {sms} SMs x {FP32_LANES_PER_SM} fp32 lanes x {sm_max_mhz:.0f} MHz / "
+                               f"{D3_MIN_ISSUE_SLOTS} issue slots per vote (DESIGN.md), clocks {peak_src}; atomic: "
+                               "hough_microbench kind 0 measured in this run; hbm: copy rate " + peak_src,
+                "measured_in_run": mb, "vote_ms_per_launch": vote_ms_avg, "votes_per_launch": votes_per_launch,
                 "launches_timed": len(vote_ms),
                 "hbm": {"algorithmic_bytes_per_launch": hbm_bytes, "achieved_gbs": hbm_bytes / (vote_ms_avg * 1e-3) / 1e9,
-                        "peak_gbs": hbm_gbs, "frac": hbm_bytes / (vote_ms_avg * 1e-3) / 1e9 / hbm_gbs,
-                        "peak_source": peak_src},
-                "smem_atomic": {"peak_gops": args.smem_atomic_gops, "frac": achieved / args.smem_atomic_gops,
-                                "peak_random_gops": args.smem_atomic_random_gops,
-                                "frac_random": achieved / args.smem_atomic_random_gops,
-                                "peak_source": "hough_microbench kinds 0 (conflict-free) and 1 (random words of a 64 KB tile) "
-                                               "on this pool's B200 (profiles/r1_microbench.txt); ncu: the walk kernel "
-                                               "keeps the shared-memory wavefront pipe 82 % busy (profiles/r1_final.md)"}}
+                        "peak_gbs": hbm_gbs, "frac": hbm_bytes / (vote_ms_avg * 1e-3) / 1e9 / hbm_gbs}}
+    # --- hough_find_peaks: HBM-bound by construction (reads every bin once, writes the candidate records)
+    peaks_ms = avg("peaks")
+    peak_bytes = bins_per_launch * bn.bin_bytes + cands_per_launch * 32 + (run.tile_events + 1) * 4
+    roofline_peaks = {"bound": "hbm", "kernel": "hough_find_peaks (mask + scans + emit)", "achieved": peak_bytes / (peaks_ms * 1e-3) / 1e9,
+                      "peak": hbm_gbs, "unit": "GB/s", "frac": peak_bytes / (peaks_ms * 1e-3) / 1e9 / hbm_gbs,
+                      "algorithmic_bytes_per_launch": peak_bytes, "ms_per_launch": peaks_ms,
+                      "candidates_per_launch": cands_per_launch,
+                      "traffic": traffic_tab.get(("peaks", run.tile_events)) if args.config == 3 else None}
+    # --- hough_assign_hits: every vote position of every hit has to be held against the candidates (D8 as the indexed
+    # oracle states it), so the unit is the vote position and the ceiling the same ALU issue bound as the vote's
+    assign_ms = avg("assign")
+    a_ach = votes_per_launch / (assign_ms * 1e-3) / 1e9
+    roofline_assign = {"bound": "alu", "kernel": "hough_assign_hits (association + duplicate removal)", "achieved": a_ach,
+                       "peak": ceilings["alu"], "unit": "G vote positions/s", "frac": a_ach / ceilings["alu"],
+                       "ms_per_launch": assign_ms, "vote_positions_per_launch": votes_per_launch,
+                       "candidates_per_launch": cands_per_launch,
+                       "note": "unit = vote positions of the launch's hits (what D8 ranges over); an association that "
+                               "visits fewer positions than that can exceed the per-position ceiling"}
+    step_share = {k: sum(v) / (ms_total) for k, v in call_ms.items()}
 
     # second Hough transform (tracks -> displaced vertices; D10): line-model workloads only
     vertex = None
@@ -435,7 +497,7 @@ def run_ours(args, rank, world, local_rank):
         n_r, r_max, thr_v = 32, 16.0, 6
         (e0, e1, h0, h1) = run.tiles[0]
         n_ev = e1 - e0
-        run.step()                                      # leaves the first tile's candidates / keep flags on the device
+        run.step_tile(0)                                # leaves the first tile's candidates / keep flags on the device
         vacc = torch.empty((n_ev, bn.n_phi, n_r), dtype=torch.int32, device="cuda")
         vplan = HoughPlan(bn.n_phi, n_r, 1, 0.0, r_max, bz_tesla=0.0, max_hits=1, max_events=n_ev, model=1)
         vcands = alloc_candidates(1 << 16)
@@ -460,7 +522,7 @@ def run_ours(args, rank, world, local_rank):
         from paper_1311_2769_b200 import hough_fit_circles
         (e0, e1, h0, h1) = run.tiles[0]
         n_ev = e1 - e0
-        run.step()
+        run.step_tile(0)                                # hits, candidates and assignments of the SAME (first) tile
         work = torch.empty((run.cap, 9), dtype=torch.float64, device="cuda")
         fitp = torch.empty((run.cap, 4), dtype=torch.float64, device="cuda")
         nfit = torch.empty((run.cap,), dtype=torch.int32, device="cuda")
@@ -508,7 +570,8 @@ def run_ours(args, rank, world, local_rank):
                               "api": "the same pipeline with option kept_only: identical work, only the candidates that "
                                      "survive duplicate removal are compacted on the device and copied back",
                               "candidate_overflow": bool(k_over)},
-            "gpu_launches": int(launches), "roofline": roofline, "cpu_baseline": cpu, "clocks": clocks,
+            "gpu_launches": int(launches), "roofline": roofline, "roofline_assign": roofline_assign,
+            "roofline_peaks": roofline_peaks, "step_share": step_share, "cpu_baseline": cpu, "clocks": clocks,
             "candidate_overflow": peaks_overflow}
     if vertex is not None:
         line["vertex"] = vertex
@@ -601,9 +664,6 @@ def main():
     ap.add_argument("--streams", type=int, default=4, help="CUDA streams of the batched pipeline (B:L10: 4)")
     ap.add_argument("--cpu-seconds", type=float, default=15.0, help="target oracle time of the cpu_baseline sample")
     ap.add_argument("--ref-seconds-per-step", type=float, default=10.0)
-    ap.add_argument("--smem-atomic-random-gops", type=float, default=3304.0)
-    ap.add_argument("--smem-atomic-gops", type=float, default=7593.0,
-                    help="measured conflict-free shared atomicAdd rate, Gops/s (profiles/microbench_r1.md)")
     ap.add_argument("--sweep-tracks", action="store_true", help="Fig. 2-style sweep on the paper's toy detector (workload 5)")
     ap.add_argument("--sweep-reps", type=int, default=30)
     args = ap.parse_args()
