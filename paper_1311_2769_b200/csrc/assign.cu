@@ -190,34 +190,45 @@ extern "C" int hough_assign_hits(hough_plan* p, const float* d_hits_xy, int32_t 
     if (capacity > 0) HOUGH_CUDA_TRY(cudaMemsetAsync(d_cand_nhits, 0, sizeof(int32_t) * (size_t)capacity, st));
     if (n_hits > 0) HOUGH_CUDA_TRY(cudaMemsetAsync(p->d_best_key, 0, sizeof(unsigned long long) * (size_t)n_hits, st));
     if (tiled) {
+        bool by_index = false;
         if (n_hits > 0 && capacity > 0) {
             int rc = hough_stage_hits(p, d_hits_xy, n_hits, d_event_offsets, n_events, st, true);
             if (rc != HOUGH_OK) return rc;
-            WalkArgs a{};
-            a.staged = p->d_staged;
-            a.off = d_event_offsets;
-            a.key_start = p->d_stage_cnt;
-            walk_shape(p, n_events, a.n_slabs, a.slab_cols);
-            a.stride = p->tile_stride_words;
-            a.cands = d_cands;
-            a.slice = p->d_slice;
-            a.assoc_dj = assoc_dj;
-            a.best_key = p->d_best_key;
-            const long long tiles = (long long)n_events * p->c.n_d0 * a.n_slabs;
-            if (tiles > (long long)p->slice_len) return HOUGH_ERR_UNSUPPORTED;
-            cand_slice_kernel<<<(unsigned)((tiles + 255) / 256), 256, 0, st>>>(p->c, d_cands, d_cand_offsets, n_events,
-                                                                                capacity, a.n_slabs, a.slab_cols, p->d_slice);
-            HOUGH_CUDA_TRY(cudaGetLastError());
-            hough_count_launches(1);
-            rc = walk_dispatch<WALK_ASSIGN>(p, n_events, a, p->tile32 != 0, false, st);
-            if (rc != HOUGH_OK) return rc;
+            by_index = p->d_assoc_tab != nullptr && !p->assign_walk;
+            if (by_index) {
+                // candidate-centric association (assoc.cu): keys carry the candidate index
+                rc = hough_assoc_candidates(p, d_event_offsets, n_hits, n_events, d_cands, d_cand_offsets, capacity, assoc_dj,
+                                            d_hit_to_cand, d_cand_nhits, st);
+                if (rc != HOUGH_OK) return rc;
+            } else {
+                WalkArgs a{};
+                a.staged = p->d_staged;
+                a.off = d_event_offsets;
+                a.key_start = p->d_stage_cnt;
+                walk_shape(p, n_events, a.n_slabs, a.slab_cols);
+                a.stride = p->tile_stride_words;
+                a.cands = d_cands;
+                a.slice = p->d_slice;
+                a.assoc_dj = assoc_dj;
+                a.best_key = p->d_best_key;
+                const long long tiles = (long long)n_events * p->c.n_d0 * a.n_slabs;
+                if (tiles > (long long)p->slice_len) return HOUGH_ERR_UNSUPPORTED;
+                cand_slice_kernel<<<(unsigned)((tiles + 255) / 256), 256, 0, st>>>(p->c, d_cands, d_cand_offsets, n_events,
+                                                                                    capacity, a.n_slabs, a.slab_cols, p->d_slice);
+                HOUGH_CUDA_TRY(cudaGetLastError());
+                hough_count_launches(1);
+                rc = walk_dispatch<WALK_ASSIGN>(p, n_events, a, p->tile32 != 0, false, st);
+                if (rc != HOUGH_OK) return rc;
+            }
         }
         if (n_hits > 0) {
-            assign_decode_bin_kernel<<<(n_hits + 255) / 256, 256, 0, st>>>(p->c, p->d_best_key, n_hits, d_event_offsets,
-                                                                           n_events, d_cands, d_cand_offsets, capacity,
-                                                                           d_hit_to_cand, d_cand_nhits);
-            HOUGH_CUDA_TRY(cudaGetLastError());
-            hough_count_launches(1);
+            if (!by_index) {
+                assign_decode_bin_kernel<<<(n_hits + 255) / 256, 256, 0, st>>>(p->c, p->d_best_key, n_hits, d_event_offsets,
+                                                                               n_events, d_cands, d_cand_offsets, capacity,
+                                                                               d_hit_to_cand, d_cand_nhits);
+                HOUGH_CUDA_TRY(cudaGetLastError());
+                hough_count_launches(1);
+            }
         }
     } else {
         const size_t n_words = (size_t)n_events * p->c.words_per_event;

@@ -45,7 +45,7 @@ struct HoughConsts {
 };
 
 constexpr int HOUGH_MAX_CLASSES = 255;
-constexpr int HOUGH_SECTORS = 32;
+constexpr int HOUGH_SECTORS_MIN = 32, HOUGH_SECTORS_MAX = 1024;   // phi sectors of the staging sort: n_phi clamped to this range
 
 struct HoughWindows {             // host copy of the class / window tables
     int n_class = 0;
@@ -66,6 +66,7 @@ struct hough_plan {
     int peaks_regs;                    // 1: 16-bit packed peak walk with register-held rows instead of the cp.async ring
     int peaks_scalar;                  // 1: 16-bit accumulators use the unpacked slice-walk peak kernel (bisecting)
     int exact_walk;                    // 1: the walks evaluate the D3 sequence at every column (no fast path)
+    int assign_walk;                   // 1: hough_assign_hits re-walks the vote columns (walk.cuh) instead of the candidate-centric path
     int reuse_staging;                 // 1: hough_assign_hits may reuse the staging of the preceding hough_vote (same arguments)
     const void* staged_hits; const void* staged_off; int32_t staged_n_hits, staged_n_events; cudaStream_t staged_stream;
     HoughConsts c;
@@ -91,6 +92,9 @@ struct hough_plan {
     float4* d_staged;                  // [max_hits] {x, y, u, bitcast(original index)} sorted by (event, class, sector)
     int2* d_stage_tmp;                 // [max_hits] {key, rank within key}
     int32_t* d_stage_cnt;              // [max_events][n_keys + 1] key counters -> exclusive key starts
+    // candidate-centric association (assoc.cu)
+    float2* d_assoc_tab;               // [n_class][n_d0][n_qpt + 1] azimuth-offset hulls per bin edge; null: not built
+    int assoc_smem_configured;         // dynamic shared memory the kernel is configured for on this plan's device
     // vote tile shape (vote.cu)
     int32_t tile32;                    // 1: 32-bit bins in shared memory, 0: two 16-bit bins per word
     int32_t tile_stride_words;         // shared-memory row stride (odd)
@@ -167,6 +171,10 @@ __device__ __forceinline__ void cta_exclusive_scan(int32_t* data, int n, int32_t
 // internal entry points (defined in the .cu files)
 int hough_stage_hits(hough_plan* p, const float* d_hits_xy, int32_t n_hits, const int32_t* d_event_offsets,
                      int32_t n_events, cudaStream_t st, bool may_reuse);
+int hough_build_assoc_table(hough_plan* p);
+int hough_assoc_candidates(hough_plan* p, const int32_t* d_event_offsets, int32_t n_hits, int32_t n_events,
+                           const hough_candidate* d_cands, const int32_t* d_cand_offsets, int32_t capacity, int32_t assoc_dj,
+                           int32_t* d_hit_to_cand, int32_t* d_cand_nhits, cudaStream_t st);
 int hough_vote_fullscan(hough_plan* p, const float* d_hits_xy, int32_t n_hits, const int32_t* d_event_offsets,
                         int32_t n_events, void* d_accum, cudaStream_t st);
 int hough_vote_tiled(hough_plan* p, const float* d_hits_xy, int32_t n_hits, const int32_t* d_event_offsets,

@@ -52,6 +52,7 @@ static void plan_free(hough_plan* p) {
     cudaFree(p->d_slice);
     cudaFree(p->d_edge2);
     cudaFree(p->d_win);
+    cudaFree(p->d_assoc_tab);
     delete p;
 }
 
@@ -133,7 +134,10 @@ extern "C" int hough_plan_create(const hough_binning* b, const hough_geometry* g
     HoughWindows win;
     if (hough_build_windows(*b, g->bz_tesla, g->n_layers, g->layer_radius_cm, win) != HOUGH_OK) { delete p; return HOUGH_ERR_INVALID_ARG; }
     c.n_class = win.n_class;
-    { const char* es = getenv("HOUGH_SECTORS"); c.n_sector = es ? atoi(es) : HOUGH_SECTORS; if (c.n_sector < 1 || c.n_sector > 1024) c.n_sector = HOUGH_SECTORS; }
+    // one sector per phi0 column (clamped): fine enough for the candidate-centric association to read a candidate's
+    // hits off the key-start table, and the vote walk is insensitive to the count above 32 (profiles/r1_final.md)
+    c.n_sector = std::min(std::max(b->n_phi, HOUGH_SECTORS_MIN), HOUGH_SECTORS_MAX);
+    { const char* es = getenv("HOUGH_SECTORS"); if (es && atoi(es) >= 1 && atoi(es) <= HOUGH_SECTORS_MAX) c.n_sector = atoi(es); }
     c.n_keys = c.n_class * c.n_sector;
     c.u_scale = (float)((double)b->n_phi / (2.0 * kPi));
     c.sector_scale = (float)((double)c.n_sector / (2.0 * kPi));
@@ -205,6 +209,10 @@ extern "C" int hough_plan_create(const hough_binning* b, const hough_geometry* g
     c.d0t = p->d_d0t;
     c.edge2 = p->d_edge2;
     c.win = p->d_win;
+    if (p->tile_max_cols >= 1) {
+        const int rc = hough_build_assoc_table(p);
+        if (rc != HOUGH_OK) { plan_free(p); return rc; }
+    }
     *out = p;
     return HOUGH_OK;
 }
@@ -226,6 +234,7 @@ extern "C" int hough_plan_set_option(hough_plan* p, const char* key, int32_t val
     if (strcmp(key, "peaks_tiled") == 0) { p->peaks_tiled = value ? 1 : 0; return HOUGH_OK; }
     if (strcmp(key, "peaks_regs") == 0) { p->peaks_regs = value ? 1 : 0; return HOUGH_OK; }
     if (strcmp(key, "peaks_scalar") == 0) { p->peaks_scalar = value ? 1 : 0; return HOUGH_OK; }
+    if (strcmp(key, "assign_walk") == 0) { p->assign_walk = value ? 1 : 0; return HOUGH_OK; }
     if (strcmp(key, "exact_walk") == 0) { p->exact_walk = value ? 1 : 0; return HOUGH_OK; }
     if (strcmp(key, "reuse_staging") == 0) { p->reuse_staging = value ? 1 : 0; p->staged_hits = nullptr; return HOUGH_OK; }
     return HOUGH_ERR_INVALID_ARG;
