@@ -194,9 +194,9 @@ extern "C" int hough_assign_hits(hough_plan* p, const float* d_hits_xy, int32_t 
         if (n_hits > 0 && capacity > 0) {
             int rc = hough_stage_hits(p, d_hits_xy, n_hits, d_event_offsets, n_events, st, true);
             if (rc != HOUGH_OK) return rc;
-            by_index = p->d_assoc_tab != nullptr && !p->assign_walk;
+            by_index = p->d_assoc_tab != nullptr && p->assign_candidates;
             if (by_index) {
-                // candidate-centric association (assoc.cu): keys carry the candidate index
+                // plan option "assign_candidates": candidate-centric association (assoc.cu), keys carry the candidate index
                 rc = hough_assoc_candidates(p, d_event_offsets, n_hits, n_events, d_cands, d_cand_offsets, capacity, assoc_dj,
                                             d_hit_to_cand, d_cand_nhits, st);
                 if (rc != HOUGH_OK) return rc;

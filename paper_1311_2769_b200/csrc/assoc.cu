@@ -1,5 +1,5 @@
 // assoc.cu -- A5, candidate-centric hit association ("further computations ... to confirm the existence of the
-// track"; D8).  The default path of hough_assign_hits.
+// track"; D8).  Plan option "assign_candidates" (off by default: measured slower than the column walk, profiles/r2_assoc.md).
 //
 // D8 asks, for every hit, for the best candidate among those whose column (i, k) the hit votes in within assoc_dj bins
 // of the candidate's bin.  Candidates are few compared with vote positions (config 3: 2.6e4 candidates against 6.4e6

@@ -209,10 +209,6 @@ extern "C" int hough_plan_create(const hough_binning* b, const hough_geometry* g
     c.d0t = p->d_d0t;
     c.edge2 = p->d_edge2;
     c.win = p->d_win;
-    if (p->tile_max_cols >= 1) {
-        const int rc = hough_build_assoc_table(p);
-        if (rc != HOUGH_OK) { plan_free(p); return rc; }
-    }
     *out = p;
     return HOUGH_OK;
 }
@@ -234,7 +230,11 @@ extern "C" int hough_plan_set_option(hough_plan* p, const char* key, int32_t val
     if (strcmp(key, "peaks_tiled") == 0) { p->peaks_tiled = value ? 1 : 0; return HOUGH_OK; }
     if (strcmp(key, "peaks_regs") == 0) { p->peaks_regs = value ? 1 : 0; return HOUGH_OK; }
     if (strcmp(key, "peaks_scalar") == 0) { p->peaks_scalar = value ? 1 : 0; return HOUGH_OK; }
-    if (strcmp(key, "assign_walk") == 0) { p->assign_walk = value ? 1 : 0; return HOUGH_OK; }
+    if (strcmp(key, "assign_candidates") == 0) {
+        p->assign_candidates = value ? 1 : 0;
+        if (value && !p->d_assoc_tab && p->tile_max_cols >= 1) return hough_build_assoc_table(p);   // built once, on first use
+        return HOUGH_OK;
+    }
     if (strcmp(key, "exact_walk") == 0) { p->exact_walk = value ? 1 : 0; return HOUGH_OK; }
     if (strcmp(key, "reuse_staging") == 0) { p->reuse_staging = value ? 1 : 0; p->staged_hits = nullptr; return HOUGH_OK; }
     return HOUGH_ERR_INVALID_ARG;

@@ -40,7 +40,7 @@ constexpr int WALK_ASSIGN = 1;
 // 8 warps at 80 registers (profiles/r1_final.md)
 __host__ __device__ constexpr int walk_threads(int mode) { return mode == 0 ? 320 : 256; }
 constexpr int WALK_MAX_WARPS = 10;
-constexpr int WALK_CHUNK_PAIRS = 16;             // column pairs per chunk: 32 columns = the bits of the redo mask
+constexpr int WALK_CHUNK_PAIRS = 32;             // column pairs per chunk = the bits of the redo mask
 constexpr int WALK_WQ_CAP = 48;                  // entries of a warp's exact-redo queue (drained by the whole warp)
 
 struct WalkArgs {
@@ -372,7 +372,7 @@ template <int MODE, bool TILE32, bool OUT16, bool FULLPHI>
 __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(HoughConsts c, WalkArgs a) {
     constexpr int WALK_THREADS = walk_threads(MODE), WALK_WARPS = WALK_THREADS / 32;
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    __shared__ int s_meta[2];                           // number of batches of the tile
+    __shared__ int s_meta[2 + WALK_MAX_WARPS];          // number of batches of the tile; fill counts of the warps' redo queues
     const int n_slabs = a.n_slabs, slab_cols = a.slab_cols, stride = a.stride;
     const int slab = blockIdx.x % n_slabs;
     const int k = (blockIdx.x / n_slabs) % c.n_d0;
@@ -434,6 +434,7 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(HoughConsts
             s_pair[p] = make_float4(A.x, B.x, A.y, B.y);
         }
         if (tid < 32) reinterpret_cast<uint32_t*>(trash_ptr)[tid] = 0u;   // read (as empty entries) by association probes
+        if (tid < WALK_MAX_WARPS) s_meta[2 + tid] = 0;                     // redo queues start empty
     }
     // per class: column window and the fast path's error bound over the class's radius interval (DESIGN.md "Fast
     // path"): hm = 1/2 - m, or 0 when the class takes the exact sequence at every column
@@ -561,48 +562,25 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(HoughConsts
     WalkTile tl;
     tl.s_tile = s_tile; tl.s_pair = s_pair; tl.stride = stride; tl.c0 = c0; tl.cand_first = cand_first; tl.cand_end = cand_end;
     tl.row_lin0 = row_lin0; tl.legacy = legacy;
-    unsigned* wq = s_wq + warp * WALK_WQ_CAP;           // the warp's redo queue
-    int wq_n = 0;
+    unsigned* wq = s_wq + warp * WALK_WQ_CAP;           // the warp's redo queue; its fill count lives in s_meta[2 + warp]
+    int* wq_cnt = s_meta + 2 + warp;
     const bool wq_ok = ev_hits < (1 << 18) && slab_cols <= 2048;          // entries fit 32 bits (else: redo on the spot)
-    // batches ascend per warp (a running segment pointer).  PREFETCH (association walk, which has the registers): the
-    // staged hit of the warp's NEXT batch is loaded while the current one is walked.
-    constexpr bool PREFETCH = MODE == WALK_ASSIGN;
+    const unsigned dump = (unsigned)(lane & (WALK_DUMP - 1));
     int seg = 0;
-    int4 sg_n = make_int4(0, 0, 0, 0);
-    float4 hv_n = make_float4(1.f, 0.f, 0.f, 0.f);
-    if (PREFETCH && warp < n_batches) {
-        while (s_seg[seg + 1].w <= warp) ++seg;          // last segment with first batch <= bt (the sentinel ends the search)
-        sg_n = s_seg[seg];
-        const int in_n = (warp - sg_n.w) * 32 + lane;
-        if (in_n < sg_n.y) hv_n = __ldg(a.staged + ev_begin + sg_n.x + in_n);
-    }
     for (int bt = warp; bt < n_batches; bt += WALK_WARPS) {
-        int4 sg;
-        float4 hv;
-        if (PREFETCH) {
-            sg = sg_n;
-            hv = hv_n;
-        } else {
-            while (s_seg[seg + 1].w <= bt) ++seg;
-            sg = s_seg[seg];
-        }
+        while (s_seg[seg + 1].w <= bt) ++seg;            // last segment with first batch <= bt (the sentinel ends the search)
+        const int4 sg = s_seg[seg];                      // {first staged hit, hits, class, first batch}
+        // A batch = 32 consecutive staged hits of the segment (neighbours in azimuth: their cos/sin pairs sit in adjacent
+        // shared-memory words).  Dealing the hits of a segment to the lanes 4 or ~1 tile rows apart was measured and is
+        // slower (profiles/r2_walk.md: bank conflicts of the regular spacing outweigh the same-word votes it removes).
         const int in_seg = (bt - sg.w) * 32 + lane;
         const bool active = in_seg < sg.y;
         const float4 cw = s_cls[sg.z];
         const int steps = __float_as_int(cw.y);
         const float hm_c = cw.z;
         const int sidx = ev_begin + sg.x + in_seg;       // index of the lane's staged hit
-        if (!PREFETCH) {
-            hv = make_float4(1.f, 0.f, 0.f, 0.f);
-            if (active) hv = __ldg(a.staged + sidx);
-        } else if (bt + WALK_WARPS < n_batches) {
-            const int bn = bt + WALK_WARPS;
-            while (s_seg[seg + 1].w <= bn) ++seg;
-            sg_n = s_seg[seg];
-            const int in_n = (bn - sg_n.w) * 32 + lane;
-            hv_n = make_float4(1.f, 0.f, 0.f, 0.f);
-            if (in_n < sg_n.y) hv_n = __ldg(a.staged + ev_begin + sg_n.x + in_n);
-        }
+        float4 hv = make_float4(1.f, 0.f, 0.f, 0.f);
+        if (active) hv = __ldg(a.staged + sidx);
         const float x = hv.x, y = hv.y;
         const float r2 = d3_r2(x, y);
         int i_lo = (int)ceilf(hv.z + cw.x);
@@ -620,12 +598,13 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(HoughConsts
         } else {
             // ---- fast path: the lane's window, two columns at a time ----
             const FastHit fh = make_fasthit(fk, x, y, r2);
-            // first column (even, tile-relative) and number of columns of the lane's part of the tile
-            int start, my_n;
+            // first column (even, tile-relative) and number of column pairs of the lane's part of the tile
+            int start, my_n, np_total;
             if (FULLPHI) {
                 start = i_lo & ~1;                       // one column early when i_lo is odd; never past the window + 2
                 if (!active) start = (2 * lane) % nphi;  // lanes without work walk rows of their own (no same-word adds)
                 my_n = active ? ((steps + 2) & ~1) : 0;
+                np_total = (steps + 2) >> 1;             // the same for every hit of a class
             } else {
                 int rel = i_lo - c0;
                 if (rel < 0) rel += nphi;
@@ -636,10 +615,9 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(HoughConsts
                 const int se = start & ~1;
                 my_n = n > 0 ? n + (start - se) : 0;
                 start = se;
+                np_total = __reduce_max_sync(0xffffffffu, (my_n + 1) >> 1);
             }
-            const int np_total = __reduce_max_sync(0xffffffffu, (my_n + 1) >> 1);
             // lanes without work: every evaluation lands in guard slot 0 and none is ever "uncertain"
-            const unsigned dump = (unsigned)(lane & (WALK_DUMP - 1));
             const unsigned hmax_l = active ? (unsigned)nq + 2u + dump : 0u;
             const float hm_l = active ? hm_c : __int_as_float(0x7f800000);
             const f32x2 r2Ak2 = pk2(fh.r2Ak, fh.r2Ak);
@@ -655,81 +633,92 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(HoughConsts
                 unsigned rowaddr = tile_saddr + (TILE32 ? (unsigned)col * stride4 : (unsigned)(col >> 1) * stride4);
                 const int wrap_t = FULLPHI ? ((nphi - col) >> 1) : 0x7fffffff;   // pair of the chunk at which the lane wraps
                 unsigned cinv = EntryT<TILE32>::CINV0 - (unsigned)col;   // association: ~(running tile column of the pair)
-                unsigned slowmask = 0u;                  // bit (np - 1 - t): pair t of the chunk is uncertain
-                // One chunk of column pairs; WRAP: some lane of the warp passes column n_phi - 1 inside the chunk.
-                // The vote is unconditional: slot min(h, nq + 2 + dump) of the column's row (results outside [-1, nq]
-                // land in a dump slot).  A pair with an uncertain column is flagged; the redo takes the pair's two fast
-                // votes back (fast_slot reproduces them) and casts the exact ones.
-                auto run_chunk = [&](auto wrap_c) {
+                unsigned slowmask = 0u;                  // bit t: pair t of the chunk is uncertain
+                // One column pair.  The vote is unconditional: slot min(h, nq + 2 + dump) of the column's row (results
+                // outside [-1, nq] land in a dump slot).  A pair with an uncertain column is flagged; the redo takes the
+                // pair's two fast votes back (fast_slot reproduces them) and casts the exact ones.
+                auto pair_step = [&](auto wrap_c, int t, unsigned bit) {
                     constexpr bool WRAP = decltype(wrap_c)::value;
-#pragma unroll 2
-                    for (int t = 0; t < np; ++t) {
-                        if (WRAP && t == wrap_t) { rowaddr -= tile_bytes; cinv += (unsigned)nphi; }
-                        const float4 T = *pp++;          // {cosA, cosB, sinA, sinB}
-                        const f32x2 C2 = pk2(T.x, T.y), S2 = pk2(T.z, T.w);
-                        const f32x2 g2 = fma2(gx2, S2, fma2(gy2, C2, r2Ak2));
-                        const f32x2 n2 = fma2(nx2, S2, fma2(ny2, C2, d0cq2));
-                        float gA, gB;
-                        upk2(g2, gA, gB);
-                        const f32x2 th2 = fma2(n2, pk2(rcp_approx(gA), rcp_approx(gB)), c0h2);   // t~ - 1/2
-                        const f32x2 yb2 = add2(th2, magic2);
-                        const f32x2 dl2 = sub2(th2, add2(yb2, nmagic2));                          // (t~ - 1/2) - J
-                        float ybA, ybB, dA, dB;
-                        upk2(yb2, ybA, ybB);
-                        upk2(dl2, dA, dB);
-                        const unsigned hA = min((unsigned)(__float_as_int(ybA) - (WALK_MAGIC_BITS - 1)), hmax_l);   // slot J + 1
-                        const unsigned hB = min((unsigned)(__float_as_int(ybB) - (WALK_MAGIC_BITS - 1)), hmax_l);
-                        // uncertain: t~ within m of a bin edge, J <= t_D3 < J + 1 not proven (NaN never compares true)
-                        bool unsA = fabsf(dA) >= hm_l, unsB = fabsf(dB) >= hm_l;
-                        unsigned adA = addr_w(rowaddr, hA), adB = addr_w(TILE32 ? rowaddr + stride4 : rowaddr, hB);
-                        if (!FULLPHI) {                  // slab tiles: the lane's own part of the tile only
-                            const bool liveA = rem > 0, liveB = rem > 1;
-                            adA = liveA ? adA : trash_saddr;  adB = liveB ? adB : trash_saddr;   // rows past the tile: scratch word
-                            unsA = unsA && liveA;  unsB = unsB && liveB;
-                            rem -= 2;
-                        }
-                        const bool uns = unsA || unsB;
-                        if (MODE == WALK_VOTE) {
-                            red_shared(adA, 1u);
-                            red_shared(adB, TILE32 ? 1u : 65536u);
-                        } else {
-                            // best (entry >> 1, ~column) of the lane; the q/pT bin and the entry's sign bit are recovered
-                            // after the loop by re-evaluating the winning column (fast_slot)
-                            const unsigned entA = TILE32 ? lds_u32(adA) : lds_u16(adA);
-                            const unsigned entB = TILE32 ? lds_u32(adB) : lds_u16(adB + 2u);
-                            const typename EntryT<TILE32>::pkey_t pA = EntryT<TILE32>::pkey_inv(entA, cinv);
-                            const typename EntryT<TILE32>::pkey_t pB = EntryT<TILE32>::pkey_inv(entB, cinv - 1u);
-                            const typename EntryT<TILE32>::pkey_t pm = pA > pB ? pA : pB;      // ties: the smaller column
-                            if (!uns && pm > bestp) bestp = pm;      // flagged pairs are probed by the redo
-                            cinv -= 2u;
-                        }
-                        slowmask = slowmask * 2u + (uns ? 1u : 0u);
-                        rowaddr += TILE32 ? 2u * stride4 : stride4;
+                    if (WRAP && t == wrap_t) { rowaddr -= tile_bytes; cinv += (unsigned)nphi; }
+                    const float4 T = *pp++;              // {cosA, cosB, sinA, sinB}
+                    const f32x2 C2 = pk2(T.x, T.y), S2 = pk2(T.z, T.w);
+                    const f32x2 g2 = fma2(gx2, S2, fma2(gy2, C2, r2Ak2));
+                    const f32x2 n2 = fma2(nx2, S2, fma2(ny2, C2, d0cq2));
+                    float gA, gB;
+                    upk2(g2, gA, gB);
+                    const f32x2 th2 = fma2(n2, pk2(rcp_approx(gA), rcp_approx(gB)), c0h2);   // t~ - 1/2
+                    const f32x2 yb2 = add2(th2, magic2);
+                    const f32x2 dl2 = sub2(th2, add2(yb2, nmagic2));                          // (t~ - 1/2) - J
+                    float ybA, ybB, dA, dB;
+                    upk2(yb2, ybA, ybB);
+                    upk2(dl2, dA, dB);
+                    const unsigned hA = min((unsigned)(__float_as_int(ybA) - (WALK_MAGIC_BITS - 1)), hmax_l);   // slot J + 1
+                    const unsigned hB = min((unsigned)(__float_as_int(ybB) - (WALK_MAGIC_BITS - 1)), hmax_l);
+                    unsigned adA = addr_w(rowaddr, hA), adB = addr_w(TILE32 ? rowaddr + stride4 : rowaddr, hB);
+                    // uncertain: t~ within m of a bin edge, J <= t_D3 < J + 1 not proven (NaN never compares true)
+                    bool uns;
+                    if (FULLPHI) {
+                        uns = fmaxf(fabsf(dA), fabsf(dB)) >= hm_l;
+                    } else {                             // slab tiles: the lane's own part of the tile only
+                        const bool liveA = rem > 0, liveB = rem > 1;
+                        adA = liveA ? adA : trash_saddr;  adB = liveB ? adB : trash_saddr;   // rows past the tile: scratch word
+                        uns = (fabsf(dA) >= hm_l && liveA) || (fabsf(dB) >= hm_l && liveB);
+                        rem -= 2;
+                    }
+                    if (MODE == WALK_VOTE) {
+                        red_shared(adA, 1u);
+                        red_shared(adB, TILE32 ? 1u : 65536u);
+                    } else {
+                        // best (entry >> 1, ~column) of the lane; the q/pT bin and the entry's sign bit are recovered
+                        // after the loop by re-evaluating the winning column (fast_slot)
+                        const unsigned entA = TILE32 ? lds_u32(adA) : lds_u16(adA);
+                        const unsigned entB = TILE32 ? lds_u32(adB) : lds_u16(adB + 2u);
+                        const typename EntryT<TILE32>::pkey_t pA = EntryT<TILE32>::pkey_inv(entA, cinv);
+                        const typename EntryT<TILE32>::pkey_t pB = EntryT<TILE32>::pkey_inv(entB, cinv - 1u);
+                        const typename EntryT<TILE32>::pkey_t pm = pA > pB ? pA : pB;      // ties: the smaller column
+                        if (!uns && pm > bestp) bestp = pm;      // flagged pairs are probed by the redo
+                        cinv -= 2u;
+                    }
+                    if (uns) slowmask |= bit;
+                    rowaddr += TILE32 ? 2u * stride4 : stride4;
+                };
+                // a chunk in groups of four pairs (constant flag bits inside a group), then the tail; WRAP: some lane of
+                // the warp passes column n_phi - 1 inside the chunk (warp-uniform choice of the compiled variant)
+                auto run_chunk = [&](auto wrap_c) {
+                    int t = 0;
+#pragma unroll 1
+                    for (; t + 4 <= np; t += 4) {
+                        unsigned m4 = slowmask;
+                        slowmask = 0u;
+                        pair_step(wrap_c, t, 1u);
+                        pair_step(wrap_c, t + 1, 2u);
+                        pair_step(wrap_c, t + 2, 4u);
+                        pair_step(wrap_c, t + 3, 8u);
+                        slowmask = m4 | (slowmask << t);
+                    }
+#pragma unroll 1
+                    for (; t < np; ++t) {
+                        unsigned m4 = slowmask;
+                        slowmask = 0u;
+                        pair_step(wrap_c, t, 1u);
+                        slowmask = m4 | (slowmask << t);
                     }
                 };
                 if (FULLPHI && __any_sync(0xffffffffu, wrap_t < np)) run_chunk(std::true_type{});
                 else run_chunk(std::false_type{});
                 col += 2 * np;                           // FULLPHI: reduced modulo n_phi at the top of the next chunk
-                // uncertain pairs of the chunk -> the warp's redo queue, drained 32 at a time by the whole warp
-                while (__any_sync(0xffffffffu, slowmask != 0u)) {
-                    if (wq_n > WALK_WQ_CAP - 32) {
-                        walk_drain<MODE, TILE32>(c, fk, d, a, tl, wq, wq_n, ev_begin, lane);
-                        wq_n = 0;
-                    }
-                    const bool has = slowmask != 0u;
-                    const unsigned bal = __ballot_sync(0xffffffffu, has);
-                    if (has) {
-                        const int b = __ffs(slowmask) - 1;
-                        slowmask &= slowmask - 1u;
-                        const int t = np - 1 - b;
-                        int cc = col_chunk + 2 * t;
-                        if (FULLPHI && cc >= nphi) cc -= nphi;
-                        unsigned live = 3u;
-                        if (!FULLPHI) live = (rem_chunk - 2 * t > 0 ? 1u : 0u) | (rem_chunk - 2 * t > 1 ? 2u : 0u);
-                        if (wq_ok) wq[wq_n + __popc(bal & ((1u << lane) - 1u))] = wq_pack(sidx - ev_begin, cc, dump, live);
-                        else walk_redo_pair<MODE, TILE32>(c, fk, d, a, tl, sidx, cc, dump, live);
-                    }
-                    if (wq_ok) wq_n += __popc(bal);
+                // uncertain pairs of the chunk -> the warp's redo queue (a slot claimed with one shared atomic), drained 32
+                // at a time by the whole warp; a full queue or entries that do not fit 32 bits: redone on the spot
+                while (slowmask != 0u) {
+                    const int t = __ffs(slowmask) - 1;
+                    slowmask &= slowmask - 1u;
+                    int cc = col_chunk + 2 * t;
+                    if (FULLPHI && cc >= nphi) cc -= nphi;
+                    unsigned live = 3u;
+                    if (!FULLPHI) live = (rem_chunk - 2 * t > 0 ? 1u : 0u) | (rem_chunk - 2 * t > 1 ? 2u : 0u);
+                    const int slot = wq_ok ? atomicAdd(wq_cnt, 1) : WALK_WQ_CAP;
+                    if (slot < WALK_WQ_CAP) wq[slot] = wq_pack(sidx - ev_begin, cc, dump, live);
+                    else walk_redo_pair<MODE, TILE32>(c, fk, d, a, tl, sidx, cc, dump, live);
                 }
             }
         }
@@ -748,8 +737,20 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(HoughConsts
                 atomicMax(a.best_key + __float_as_int(hw.w), walk_key((ent >> 5) - 1u, adj, row_lin0 + (unsigned)(bcol * nq + jc)));
             }
         }
+        // the queue is drained when it may not take another batch's worth of entries
+        __syncwarp();
+        const int wq_n = *reinterpret_cast<volatile int*>(wq_cnt);
+        if (wq_n > WALK_WQ_CAP - 32) {
+            walk_drain<MODE, TILE32>(c, fk, d, a, tl, wq, min(wq_n, WALK_WQ_CAP), ev_begin, lane);
+            if (lane == 0) *wq_cnt = 0;
+            __syncwarp();
+        }
     }
-    if (wq_n > 0) walk_drain<MODE, TILE32>(c, fk, d, a, tl, wq, wq_n, ev_begin, lane);
+    {
+        __syncwarp();
+        const int wq_n = *reinterpret_cast<volatile int*>(wq_cnt);
+        if (wq_n > 0) walk_drain<MODE, TILE32>(c, fk, d, a, tl, wq, min(wq_n, WALK_WQ_CAP), ev_begin, lane);
+    }
     if (MODE == WALK_ASSIGN) return;
     __syncthreads();
 

@@ -61,8 +61,8 @@ def test_config_0_1_bit_exact(cfg, fullscan):
 def test_config_0_1_exact_walk_and_tiled_peaks(cfg):
     """The bisecting options: D3 at every window column (no fast path) and the halo-tile peak kernels."""
     w = get_workload(cfg)
-    _compare_all(w, generate_events(w), options=("exact_walk", "peaks_tiled", "assign_walk"))
-    _compare_all(w, generate_events(w), options=("assign_walk",))
+    _compare_all(w, generate_events(w), options=("exact_walk", "peaks_tiled"))
+    _compare_all(w, generate_events(w), options=("assign_candidates",))
 
 
 def test_paper_toy_workload_bit_exact():
@@ -83,6 +83,7 @@ def test_config_3_subset_of_events_bit_exact():
     w = get_workload(3)
     batch = generate_events(w, events=[0, 1, 513, 1023, 7])
     _compare_all(w, batch)
+    _compare_all(w, batch, options=("assign_candidates",))
 
 
 def test_config_3_fullscan_matches_tiled_on_more_events():
@@ -220,8 +221,8 @@ def test_random_configurations_bit_exact(seed):
     h2c, nh, keep = o.assign_indexed(hits, off, ref, dj, 2, capacity=cap)
     assert np.array_equal(got.hit_to_cand, h2c), "hit_to_cand differs"
     assert np.array_equal(got.cand_nhits[:ref.total], nh) and np.array_equal(got.cand_keep[:ref.total], keep)
-    got_w = run_assign(bn, bz, layers, hits, off, ref.records, ref.offsets, cap, dj, 2, options=("assign_walk",))
-    assert np.array_equal(got_w[0], h2c), "hit_to_cand differs (column walk)"
+    got_w = run_assign(bn, bz, layers, hits, off, ref.records, ref.offsets, cap, dj, 2, options=("assign_candidates",))
+    assert np.array_equal(got_w[0], h2c), "hit_to_cand differs (candidate-centric path)"
     assert votes > 0 or seed % 4 != 1
 
 
@@ -253,7 +254,7 @@ def test_assign_tile_variants_bit_exact(shape, dtype, max_hits, dj):
     ref = o.find_peaks(acc, thr)
     assert ref.total > 50
     h2c, nh, keep = o.assign_brute(hits, off, ref, dj, 2)
-    for options in ((), ("assign_walk",), ("assign_walk", "exact_walk")):     # candidate-centric (default) and the column walk
+    for options in ((), ("exact_walk",), ("assign_candidates",)):     # the column walk (default) and the candidate-centric path
         got = run_assign(bn, 3.8, LAYERS_10, hits, off, ref.records, ref.offsets, ref.total + 5, dj, 2, max_hits=max_hits,
                          options=options)
         assert np.array_equal(got[0], h2c), options
@@ -318,7 +319,7 @@ def test_assign_saturated_votes_and_truncated_list():
     mod = OracleCandidates(rec, ref.offsets, ref.total)
     for cap in (ref.total, ref.total // 2):
         h2c, nh, keep = o.assign_brute(batch.hits_xy, batch.event_offsets, mod, 1, 3, capacity=cap)
-        for options in ((), ("assign_walk",)):
+        for options in ((), ("assign_candidates",)):
             got = run_assign(bn, w.bz_tesla, w.layers, batch.hits_xy, batch.event_offsets, rec, ref.offsets, cap, 1, 3,
                              options=options)
             assert np.array_equal(got[0], h2c), (cap, options)
