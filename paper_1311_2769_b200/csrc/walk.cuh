@@ -303,8 +303,9 @@ struct WalkTile {
 };
 
 template <int MODE, bool TILE32>
-__device__ __noinline__ void walk_redo_pair(const HoughConsts& c, const FastK& fk, float4 d, const WalkArgs& a, const WalkTile& tl,
+__device__ __noinline__ void walk_redo_pair(const HoughConsts& c, float4 d, const WalkArgs& a, const WalkTile& tl,
                                             int sidx, int cc, unsigned dump, unsigned live) {
+    const FastK fk = make_fastk(c, d);                  // recomputed here: the rare path keeps nothing of the caller's on the stack
     const float4 hv = __ldg(a.staged + sidx);
     const unsigned hmax = (unsigned)c.n_qpt + 2u + dump;
     const float r2 = d3_r2(hv.x, hv.y);
@@ -357,21 +358,22 @@ __device__ __forceinline__ unsigned wq_pack(int in_event, int cc, unsigned dump,
 }
 
 template <int MODE, bool TILE32>
-__device__ __forceinline__ void walk_drain(const HoughConsts& c, const FastK& fk, float4 d, const WalkArgs& a, const WalkTile& tl,
+__device__ __forceinline__ void walk_drain(const HoughConsts& c, float4 d, const WalkArgs& a, const WalkTile& tl,
                                            const unsigned* wq, int n, int ev_begin, int lane) {
     __syncwarp();
     for (int q = lane; q < n; q += 32) {
         const unsigned en = wq[q];
-        walk_redo_pair<MODE, TILE32>(c, fk, d, a, tl, ev_begin + (int)(en & 0x3ffffu), (int)((en >> 18) & 0x3ffu) * 2, (en >> 28) & 3u,
+        walk_redo_pair<MODE, TILE32>(c, d, a, tl, ev_begin + (int)(en & 0x3ffffu), (int)((en >> 18) & 0x3ffu) * 2, (en >> 28) & 3u,
                                      en >> 30);
     }
     __syncwarp();
 }
 
 template <int MODE, bool TILE32, bool OUT16, bool FULLPHI>
-__global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(HoughConsts c, WalkArgs a) {
+__global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __grid_constant__ HoughConsts c, const __grid_constant__ WalkArgs a) {
     constexpr int WALK_THREADS = walk_threads(MODE), WALK_WARPS = WALK_THREADS / 32;
     extern __shared__ __align__(16) unsigned char smem_raw[];
+    __shared__ WalkTile s_tl;
     __shared__ int s_meta[2 + WALK_MAX_WARPS];          // number of batches of the tile; fill counts of the warps' redo queues
     const int n_slabs = a.n_slabs, slab_cols = a.slab_cols, stride = a.stride;
     const int slab = blockIdx.x % n_slabs;
@@ -435,6 +437,10 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(HoughConsts
         }
         if (tid < 32) reinterpret_cast<uint32_t*>(trash_ptr)[tid] = 0u;   // read (as empty entries) by association probes
         if (tid < WALK_MAX_WARPS) s_meta[2 + tid] = 0;                     // redo queues start empty
+        if (tid == 0) {
+            s_tl.s_tile = s_tile; s_tl.s_pair = s_pair; s_tl.stride = stride; s_tl.c0 = c0; s_tl.cand_first = cand_first;
+            s_tl.cand_end = cand_end; s_tl.row_lin0 = (unsigned)(k * nphi + c0) * (unsigned)nq; s_tl.legacy = legacy;
+        }
     }
     // per class: column window and the fast path's error bound over the class's radius interval (DESIGN.md "Fast
     // path"): hm = 1/2 - m, or 0 when the class takes the exact sequence at every column
@@ -557,11 +563,10 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(HoughConsts
     const int n_batches = s_meta[0];
     const unsigned row_lin0 = (unsigned)(k * nphi + c0) * (unsigned)nq;   // linear bin of (k, c0, 0) inside the event
     const unsigned tile_bytes = (unsigned)(walk_tile_words(cols, stride, TILE32) * 4);   // FULLPHI: the wrap distance
+    const unsigned tile_end = tile_saddr + tile_bytes;
     const f32x2 d0cq2 = pk2(fk.d0cq, fk.d0cq), c0h2 = pk2(fk.c0h, fk.c0h);
     const f32x2 magic2 = pk2(WALK_MAGIC, WALK_MAGIC), nmagic2 = pk2(-WALK_MAGIC, -WALK_MAGIC);
-    WalkTile tl;
-    tl.s_tile = s_tile; tl.s_pair = s_pair; tl.stride = stride; tl.c0 = c0; tl.cand_first = cand_first; tl.cand_end = cand_end;
-    tl.row_lin0 = row_lin0; tl.legacy = legacy;
+    const WalkTile& tl = s_tl;                          // what the out-of-line rare paths need of the tile (written in the prologue)
     unsigned* wq = s_wq + warp * WALK_WQ_CAP;           // the warp's redo queue; its fill count lives in s_meta[2 + warp]
     int* wq_cnt = s_meta + 2 + warp;
     const bool wq_ok = ev_hits < (1 << 18) && slab_cols <= 2048;          // entries fit 32 bits (else: redo on the spot)
@@ -639,7 +644,6 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(HoughConsts
                 // pair's two fast votes back (fast_slot reproduces them) and casts the exact ones.
                 auto pair_step = [&](auto wrap_c, int t, unsigned bit) {
                     constexpr bool WRAP = decltype(wrap_c)::value;
-                    if (WRAP && t == wrap_t) { rowaddr -= tile_bytes; cinv += (unsigned)nphi; }
                     const float4 T = *pp++;              // {cosA, cosB, sinA, sinB}
                     const f32x2 C2 = pk2(T.x, T.y), S2 = pk2(T.z, T.w);
                     const f32x2 g2 = fma2(gx2, S2, fma2(gy2, C2, r2Ak2));
@@ -681,6 +685,8 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(HoughConsts
                     }
                     if (uns) slowmask |= bit;
                     rowaddr += TILE32 ? 2u * stride4 : stride4;
+                    if (WRAP && rowaddr >= tile_end) { rowaddr -= tile_bytes; cinv += (unsigned)nphi; }   // past column n_phi - 1
+                    (void)t;
                 };
                 // a chunk in groups of four pairs (constant flag bits inside a group), then the tail; WRAP: some lane of
                 // the warp passes column n_phi - 1 inside the chunk (warp-uniform choice of the compiled variant)
@@ -718,7 +724,7 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(HoughConsts
                     if (!FULLPHI) live = (rem_chunk - 2 * t > 0 ? 1u : 0u) | (rem_chunk - 2 * t > 1 ? 2u : 0u);
                     const int slot = wq_ok ? atomicAdd(wq_cnt, 1) : WALK_WQ_CAP;
                     if (slot < WALK_WQ_CAP) wq[slot] = wq_pack(sidx - ev_begin, cc, dump, live);
-                    else walk_redo_pair<MODE, TILE32>(c, fk, d, a, tl, sidx, cc, dump, live);
+                    else walk_redo_pair<MODE, TILE32>(c, d, a, tl, sidx, cc, dump, live);
                 }
             }
         }
@@ -741,7 +747,7 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(HoughConsts
         __syncwarp();
         const int wq_n = *reinterpret_cast<volatile int*>(wq_cnt);
         if (wq_n > WALK_WQ_CAP - 32) {
-            walk_drain<MODE, TILE32>(c, fk, d, a, tl, wq, min(wq_n, WALK_WQ_CAP), ev_begin, lane);
+            walk_drain<MODE, TILE32>(c, d, a, tl, wq, min(wq_n, WALK_WQ_CAP), ev_begin, lane);
             if (lane == 0) *wq_cnt = 0;
             __syncwarp();
         }
@@ -749,7 +755,7 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(HoughConsts
     {
         __syncwarp();
         const int wq_n = *reinterpret_cast<volatile int*>(wq_cnt);
-        if (wq_n > 0) walk_drain<MODE, TILE32>(c, fk, d, a, tl, wq, min(wq_n, WALK_WQ_CAP), ev_begin, lane);
+        if (wq_n > 0) walk_drain<MODE, TILE32>(c, d, a, tl, wq, min(wq_n, WALK_WQ_CAP), ev_begin, lane);
     }
     if (MODE == WALK_ASSIGN) return;
     __syncthreads();
