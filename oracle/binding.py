@@ -44,6 +44,9 @@ def _load():
             f.restype = C.c_int
             f.argtypes = [C.POINTER(_Binning), C.c_float, P, C.c_int32, P, C.c_int32, P, P, C.c_longlong,
                           C.c_int32, C.c_int32, C.c_int32, P, P, P]
+        lib.orc_assign_rounds.restype = C.c_int
+        lib.orc_assign_rounds.argtypes = [C.POINTER(_Binning), C.c_float, P, C.c_int32, P, C.c_int32, P, P, C.c_longlong,
+                                          C.c_int32, C.c_int32, C.c_int32, P, P, P]
         lib.orc_vertex_vote.restype = C.c_longlong
         lib.orc_vertex_vote.argtypes = [C.POINTER(_Binning), C.c_float, P, P, C.c_int32, C.c_longlong, P, C.c_float, C.c_int32,
                                         C.c_float, P]
@@ -192,6 +195,22 @@ class Oracle:
                                       _ptr(fit), _ptr(nfit))
         assert rc == 0
         return fit[:len(rec)], nfit[:len(rec)]
+
+    def assign_rounds(self, hits_xy, event_offsets, cands, assoc_dj=1, min_hits=0, max_rounds=8, capacity=None):
+        """orc_assign_rounds (D12): (hit_to_cand, cand_nhits, cand_keep, rounds run)."""
+        h = self._hits(hits_xy)
+        off = self._offsets(event_offsets, h.shape[0])
+        rec = np.ascontiguousarray(cands.records)
+        cap = int(rec.shape[0]) if capacity is None else int(capacity)
+        n_c = min(cap, int(cands.offsets[-1]))
+        h2c = np.full(h.shape[0], -2, np.int32)
+        nh = np.zeros(max(n_c, 1), np.int32)
+        keep = np.zeros(max(n_c, 1), np.uint8)
+        rounds = self.lib.orc_assign_rounds(C.byref(self.b), self.bz, _ptr(h), h.shape[0], _ptr(off), off.shape[0] - 1,
+                                            _ptr(rec), _ptr(np.ascontiguousarray(cands.offsets, dtype=np.int32)), cap,
+                                            int(assoc_dj), int(min_hits), int(max_rounds), _ptr(h2c), _ptr(nh), _ptr(keep))
+        assert rounds >= 1, "orc_assign_rounds: bad arguments"
+        return h2c, nh[:n_c], keep[:n_c], int(rounds)
 
     def assign_brute(self, hits_xy, event_offsets, cands, assoc_dj=1, min_hits=0, apply_dedup=True, capacity=None):
         return self._assign(self.lib.orc_assign_brute, hits_xy, event_offsets, cands, assoc_dj, min_hits,

@@ -23,7 +23,8 @@
 // Pins (tests/test_oracle_*.py, run with -m "not gpu"): V1 brute force in double from the
 // tangent-chord construction, V2 noiseless helix -> its own bin, V3 closed-form vote count,
 // V4 linearity/permutation, V5 2-D special case, V6 quarter-turn shift, V7 peak definition on
-// constructed volumes, V8 brute-force vs indexed assignment.  No function here is "parity unpinned".
+// constructed volumes, V8 brute-force vs indexed assignment, V12 re-assignment rounds (hand-built shared-hit case,
+// rounds = 1 == D9, fixed point == brute force over the kept candidates).  No function here is "parity unpinned".
 
 #include <cmath>
 #include <cstdint>
@@ -410,6 +411,67 @@ int orc_assign_indexed(const orc_binning* b, float bz, const float* hits_xy, int
         dedup(n_hits, n_cands, min_hits, hit_to_cand, cand_nhits, cand_keep);
     }
     return 0;
+}
+
+// D12 -- re-assignment rounds ("all track candidates found ... are cleaned to select only the best candidate
+// ... and eliminate duplicate tracks"; "hits in these tracks are then removed, allowing later iterations";
+// SURVEY 8(f) f4).  D9 drops a candidate with fewer than min_hits hits and leaves its hits unassigned; here those hits
+// re-enter the association.  Round t = 1, 2, ...: every hit takes its best candidate (D8 key) among the candidates
+// ALIVE in this round (round 1: all of them); a candidate stays alive iff at least min_hits hits took it.  Stop when no
+// candidate was dropped in a round, or after max_rounds rounds.  Outputs: hit_to_cand = the last round's assignment, with
+// hits on a candidate dropped in that last round set to -1; cand_keep = alive after the last round; cand_nhits[c] = the
+// number of hits c had in the last round in which it was alive (so max_rounds = 1 is exactly D8 + D9).
+// Brute force over (hit, candidate) pairs, written out from the definition.  Returns the number of rounds run, < 0 on
+// bad arguments.
+int orc_assign_rounds(const orc_binning* b, float bz, const float* hits_xy, int32_t n_hits,
+                      const int32_t* event_offsets, int32_t n_events, const orc_candidate* cands,
+                      const int32_t* cand_offsets, long long capacity, int32_t assoc_dj, int32_t min_hits,
+                      int32_t max_rounds, int32_t* hit_to_cand, int32_t* cand_nhits, uint8_t* cand_keep) {
+    if (!valid_binning(b) || !event_offsets || !cand_offsets || !hit_to_cand || !cand_nhits || !cand_keep) return -1;
+    if (max_rounds < 1) return -1;
+    const Tables t = make_tables(*b, bz);
+    const long long n_cands = cand_offsets[n_events] < capacity ? cand_offsets[n_events] : capacity;
+    std::vector<uint8_t> alive((size_t)(n_cands > 0 ? n_cands : 1), 1);
+    std::vector<int32_t> count((size_t)(n_cands > 0 ? n_cands : 1), 0);
+    for (long long c = 0; c < n_cands; ++c) cand_nhits[c] = 0;
+    int rounds = 0;
+    for (;;) {
+        ++rounds;
+        for (int e = 0; e < n_events; ++e) {
+            long long c0 = cand_offsets[e], c1 = cand_offsets[e + 1];
+            if (c1 > capacity) c1 = capacity;
+            for (int h = event_offsets[e]; h < event_offsets[e + 1]; ++h) {
+                const float x = hits_xy[2 * (size_t)h], y = hits_xy[2 * (size_t)h + 1];
+                const float r2 = hit_r2(x, y);
+                uint64_t best = 0;
+                int32_t best_c = -1;
+                for (long long c = c0; c < c1; ++c) {
+                    if (!alive[(size_t)c]) continue;
+                    const int jh = vote_bin(t, b->n_qpt, x, y, r2, cands[c].i, cands[c].k);
+                    if (jh < 0) continue;
+                    const int adj = jh > cands[c].j ? jh - cands[c].j : cands[c].j - jh;
+                    if (adj > assoc_dj) continue;
+                    const uint64_t key = assign_key(cands[c].votes, adj, c);
+                    if (best_c < 0 || key > best) { best = key; best_c = (int32_t)c; }
+                }
+                hit_to_cand[h] = best_c;
+            }
+        }
+        for (long long c = 0; c < n_cands; ++c) count[(size_t)c] = 0;
+        for (int h = 0; h < n_hits; ++h)
+            if (hit_to_cand[h] >= 0) count[(size_t)hit_to_cand[h]] += 1;
+        bool dropped = false;
+        for (long long c = 0; c < n_cands; ++c) {
+            if (!alive[(size_t)c]) continue;
+            cand_nhits[c] = count[(size_t)c];
+            if (count[(size_t)c] < min_hits) { alive[(size_t)c] = 0; dropped = true; }
+        }
+        if (!dropped || rounds >= max_rounds) break;
+    }
+    for (long long c = 0; c < n_cands; ++c) cand_keep[c] = alive[(size_t)c];
+    for (int h = 0; h < n_hits; ++h)
+        if (hit_to_cand[h] >= 0 && !alive[(size_t)hit_to_cand[h]]) hit_to_cand[h] = -1;
+    return rounds;
 }
 
 // D10 -- second Hough transform: displaced vertices from the found straight tracks ("apply a Hough

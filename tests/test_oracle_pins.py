@@ -526,6 +526,126 @@ def test_v8_capacity_limits_participants():
     assert np.array_equal(h_b, h_i) and np.array_equal(nh_b, nh_i) and h_b.max() < cap and len(nh_b) == cap
 
 
+# ----------------------------------------------------------------------------- V12 (D12: re-assignment rounds)
+def _hit_bins(o, hits, k, i):
+    """q/pT bin of every hit in column (k, i), -1 = no vote: one single-hit accumulator column per hit (D3, pinned by V1-V6)."""
+    out = np.full(len(hits), -1, np.int64)
+    for h in range(len(hits)):
+        nz = np.nonzero(o.vote_columns(hits[h:h + 1], None, [[0, k, i]])[0])[0]
+        assert len(nz) <= 1
+        if len(nz):
+            out[h] = nz[0]
+    return out
+
+
+def _rounds_python(jh, votes, cj, dj, min_hits, max_rounds):
+    """D12 written out in numpy from its definition.  jh[h, c] = bin of hit h in candidate c's column."""
+    n_h, n_c = jh.shape
+    alive = np.ones(n_c, bool)
+    nh = np.zeros(n_c, np.int64)
+    rounds = 0
+    while True:
+        rounds += 1
+        h2c = np.full(n_h, -1, np.int64)
+        for h in range(n_h):
+            best = None
+            for c in range(n_c):
+                if not alive[c] or jh[h, c] < 0 or abs(jh[h, c] - cj[c]) > dj:
+                    continue
+                key = (votes[c], -abs(jh[h, c] - cj[c]), -c)
+                if best is None or key > best[0]:
+                    best = (key, c)
+            if best is not None:
+                h2c[h] = best[1]
+        cnt = np.bincount(h2c[h2c >= 0], minlength=n_c)
+        nh[alive] = cnt[alive]
+        drop = alive & (cnt < min_hits)
+        alive &= ~drop
+        if not drop.any() or rounds >= max_rounds:
+            break
+    h2c[(h2c >= 0) & ~alive[np.maximum(h2c, 0)]] = -1
+    return h2c, nh, alive, rounds
+
+
+def test_v12_shared_hit_case_by_hand():
+    """One noiseless helix, its own bin as candidate 0 (10 votes) and a neighbour-column candidate 1 with MORE votes
+    that only the outer hits reach.  D9 leaves the outer hits unassigned; the second round hands them to candidate 0."""
+    from oracle import CAND_DTYPE, OracleCandidates
+    o = Oracle(256, 256, 1, bz_tesla=BZ)
+    i, j = 40, 100
+    hits = helix_hits((i + 0.5) * 2 * math.pi / 256, -1.0 + (j + 0.5) * 2.0 / 256, 0.0, LAYERS_10, BZ)
+    own = _hit_bins(o, hits, 0, i)
+    assert (own == j).all()                                       # V2: every hit votes in the helix's own bin
+    nb = _hit_bins(o, hits, 0, i + 1)
+    j1 = int(nb[-1])                                              # where the outermost hit lands one column on
+    reach = np.abs(nb - j1) <= 1
+    n1 = int(reach.sum())
+    assert 1 <= n1 <= 4 and reach[-1] and not reach[0]            # only a few outer hits are compatible with candidate 1
+    rec = np.zeros(2, CAND_DTYPE)
+    rec[0]["i"], rec[0]["j"], rec[0]["votes"] = i, j, 10
+    rec[1]["i"], rec[1]["j"], rec[1]["votes"] = i + 1, j1, 12
+    c = OracleCandidates(rec, np.array([0, 2], np.int32), 2)
+    # D8 + D9: the outer hits prefer candidate 1 (12 votes), which then fails min_hits = 5 and strands them
+    h9, nh9, keep9 = o.assign_brute(hits, None, c, 1, 5)
+    assert np.array_equal(h9, np.where(reach, -1, 0)) and list(nh9) == [10 - n1, n1] and list(keep9) == [1, 0]
+    h1, nh1, keep1, r1 = o.assign_rounds(hits, None, c, 1, 5, max_rounds=1)
+    assert r1 == 1 and np.array_equal(h1, h9) and np.array_equal(nh1, nh9) and np.array_equal(keep1, keep9)
+    # D12: round 2 re-associates them with the surviving candidate
+    h2, nh2, keep2, r2 = o.assign_rounds(hits, None, c, 1, 5, max_rounds=8)
+    assert r2 == 2 and (h2 == 0).all() and list(nh2) == [10, n1] and list(keep2) == [1, 0]
+    # min_hits above what either can reach: both die in round 1, nothing to re-assign
+    h3, nh3, keep3, r3 = o.assign_rounds(hits, None, c, 1, 11, max_rounds=8)
+    assert r3 == 2 and (h3 == -1).all() and list(nh3) == [10 - n1, n1] and list(keep3) == [0, 0]
+
+
+@pytest.mark.parametrize("min_hits,dj", [(3, 1), (6, 1), (8, 2), (1, 0)])
+def test_v12_rounds_vs_python_bruteforce(min_hits, dj):
+    """Config 0 with its real candidate list plus decoys: every output and the round count against the definition
+    written out in numpy on top of the (pinned) per-hit vote bins."""
+    from oracle import OracleCandidates
+    w = get_workload(0)
+    b = generate_events(w)
+    o = Oracle.from_binning(w.binning, w.bz_tesla)
+    acc, _ = o.vote(b.hits_xy)
+    c = o.find_peaks(acc, 6)                                       # lower threshold: more (and more dubious) candidates
+    rec = c.records[:60].copy()
+    cands = OracleCandidates(rec, np.array([0, len(rec)], np.int32), len(rec))
+    hits = b.hits_xy[:120]
+    jh = np.stack([_hit_bins(o, hits, int(r["k"]), int(r["i"])) for r in rec], axis=1)
+    for max_rounds in (1, 2, 5):
+        exp = _rounds_python(jh, rec["votes"].astype(np.int64), rec["j"].astype(np.int64), dj, min_hits, max_rounds)
+        got = o.assign_rounds(hits, None, cands, dj, min_hits, max_rounds=max_rounds)
+        assert np.array_equal(got[0], exp[0]) and np.array_equal(got[1], exp[1])
+        assert np.array_equal(got[2].astype(bool), exp[2]) and got[3] == exp[3]
+
+
+@pytest.mark.parametrize("cfg", [0, 1, 5])
+def test_v12_fixed_point_properties(cfg):
+    """What must hold whatever the input: max_rounds = 1 is D9; the kept set is D9's kept set (a kept candidate only gains
+    hits); two rounds reach the fixed point; the result equals a brute-force D8 over the kept candidates alone."""
+    from oracle import OracleCandidates
+    w = get_workload(cfg)
+    b = generate_events(w)
+    o = Oracle.from_binning(w.binning, w.bz_tesla)
+    acc, _ = o.vote(b.hits_xy, b.event_offsets)
+    c = o.find_peaks(acc, w.threshold)
+    h9, nh9, keep9 = o.assign_indexed(b.hits_xy, b.event_offsets, c, w.assoc_dj, w.min_hits)
+    h1, nh1, keep1, r1 = o.assign_rounds(b.hits_xy, b.event_offsets, c, w.assoc_dj, w.min_hits, max_rounds=1)
+    assert r1 == 1 and np.array_equal(h1, h9) and np.array_equal(nh1, nh9) and np.array_equal(keep1, keep9)
+    hr, nhr, keepr, rr = o.assign_rounds(b.hits_xy, b.event_offsets, c, w.assoc_dj, w.min_hits, max_rounds=8)
+    assert rr <= 2 and np.array_equal(keepr, keep9)
+    kept = keep9.astype(bool)
+    assert (nhr[kept] >= nh9[kept]).all() and np.array_equal(nhr[~kept], nh9[~kept])
+    assert np.array_equal(hr[h9 >= 0], h9[h9 >= 0])               # hits that had a kept candidate keep it
+    assert np.array_equal(nhr[kept], np.bincount(hr[hr >= 0], minlength=c.total)[kept])
+    # brute-force D8 over the kept candidates alone, indices mapped back
+    idx = np.nonzero(kept)[0]
+    sub = OracleCandidates(c.records[idx].copy(), np.array([0, len(idx)], np.int32), len(idx))
+    hs, _, _ = o.assign_brute(b.hits_xy, b.event_offsets, sub, w.assoc_dj, 0, apply_dedup=False)
+    assert np.array_equal(hr, np.where(hs >= 0, idx[np.maximum(hs, 0)], -1))
+    assert (hr >= 0).sum() > (h9 >= 0).sum() or cfg == 0          # the rounds do recover hits on the busy workloads
+
+
 # ----------------------------------------------------------------------------- workload sanity
 def test_workload_shapes_match_baseline():
     """Hit counts of the generated configs sit where BASELINE.json says ("about 210", "about 33k" ...)."""
