@@ -118,6 +118,25 @@ int hough_assign_hits(hough_plan* plan, const float* d_hits_xy, int32_t n_hits, 
                       int32_t capacity, int32_t assoc_dj, int32_t min_hits, int32_t* d_hit_to_cand,
                       int32_t* d_cand_nhits, uint8_t* d_cand_keep, void* cuda_stream);
 
+/* hough_reassign_hits ("cleaned to select only the best candidate ... and eliminate duplicate tracks"; "hits in
+ * these tracks are then removed, allowing later iterations"; D12 re-assignment rounds).
+ * Call after hough_assign_hits with the same hits, offsets, candidates, capacity and assoc_dj, and with ITS outputs in
+ * d_hit_to_cand / d_cand_nhits / d_cand_keep.  D12: in round t every hit takes its best candidate (the D8 key of
+ * hough_assign_hits) among the candidates still alive, a candidate stays alive iff >= min_hits hits took it; rounds end
+ * when none was dropped or after max_rounds.  Round 1 is hough_assign_hits.  A kept candidate can only gain hits in round
+ * 2, so the kept set never changes again: round 2 is the fixed point, and this call runs exactly that round for
+ * max_rounds >= 2 (max_rounds == 1: returns at once).  Effect: every hit with d_hit_to_cand[h] == -1 gets the best
+ * candidate with d_cand_keep != 0 (or stays -1), d_cand_nhits of that candidate is incremented; hits that had a kept
+ * candidate, d_cand_nhits of dropped candidates and d_cand_keep are left as they are.
+ * Tiled plans take the candidate-centric association over the surviving candidates; its azimuth-interval table is built
+ * on the first call (one cudaMalloc + device synchronisation: make that call outside stream capture), or, if the table
+ * does not fit or the plan option "reassign_walk" is set, re-walk the vote columns against the surviving candidates.
+ * Errors: INVALID_ARG (null pointers, sizes, max_rounds < 1), UNSUPPORTED, CUDA. */
+int hough_reassign_hits(hough_plan* plan, const float* d_hits_xy, int32_t n_hits, const int32_t* d_event_offsets,
+                        int32_t n_events, const hough_candidate* d_cands, const int32_t* d_cand_offsets,
+                        int32_t capacity, int32_t assoc_dj, int32_t max_rounds, int32_t* d_hit_to_cand,
+                        int32_t* d_cand_nhits, const uint8_t* d_cand_keep, void* cuda_stream);
+
 /* hough_vertex_vote ("apply a Hough transform to the track maxima" -- displaced vertices; D10).
  * `plan` is the HOUGH_MODEL_LINE plan of the TRACK space that produced d_cands.  Every candidate with d_cand_keep[c] != 0
  * (all candidates when d_cand_keep is NULL), rank < capacity and |d| >= d0_abs_min votes, for every vertex-azimuth

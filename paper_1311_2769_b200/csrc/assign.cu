@@ -52,6 +52,7 @@ __global__ void __launch_bounds__(256) assign_fullscan_kernel(HoughConsts c, con
                                                               const hough_candidate* __restrict__ cands,
                                                               const uint32_t* __restrict__ mask,
                                                               const int32_t* __restrict__ word_rank, int assoc_dj,
+                                                              const uint8_t* __restrict__ keep,
                                                               unsigned long long* __restrict__ best_key) {
     const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     const int h = (int)(t / c.n_phi);
@@ -78,6 +79,7 @@ __global__ void __launch_bounds__(256) assign_fullscan_kernel(HoughConsts c, con
             const uint32_t m = __ldg(emask + (b >> 5));
             if (!((m >> (b & 31)) & 1u)) continue;
             const int ci = __ldg(erank + (b >> 5)) + __popc(m & ((1u << (b & 31)) - 1u));
+            if (keep && !__ldg(keep + ci)) continue;
             const int votes = __ldg(&cands[ci].votes);
             const unsigned long long key = make_key(votes, abs(jh - j), ci);
             best = key > best ? key : best;
@@ -171,6 +173,37 @@ __global__ void __launch_bounds__(256) unassign_kernel(int n_hits, const uint8_t
     if (ci >= 0 && !cand_keep[ci]) hit_to_cand[h] = -1;
 }
 
+// D12 decode: only hits left without a candidate take the key of the re-assignment round.  BY_BIN: the key's low word
+// is ~(linear bin) (column walk); else ~(candidate index) (full scan).
+template <bool BY_BIN>
+__global__ void __launch_bounds__(256) reassign_decode_kernel(HoughConsts c, const unsigned long long* __restrict__ best_key,
+                                                              int n_hits, const int32_t* __restrict__ off, int n_events,
+                                                              const hough_candidate* __restrict__ cands,
+                                                              const int32_t* __restrict__ cand_offsets, int capacity,
+                                                              int32_t* __restrict__ hit_to_cand,
+                                                              int32_t* __restrict__ cand_nhits) {
+    const int h = blockIdx.x * blockDim.x + threadIdx.x;
+    if (h >= n_hits) return;
+    if (hit_to_cand[h] >= 0) return;
+    const unsigned long long key = best_key[h];
+    if (!key) return;
+    const unsigned low = 0xFFFFFFFFu - (unsigned)(key & 0xFFFFFFFFull);
+    int ci = (int)low;
+    if (BY_BIN) {
+        const int e = find_event_a(off, n_events, h);
+        int lo = min(__ldg(cand_offsets + e), capacity), hi = min(__ldg(cand_offsets + e + 1), capacity);
+        while (lo < hi) {
+            const int mid = (lo + hi) >> 1;
+            const int4 q = __ldg(reinterpret_cast<const int4*>(cands + mid));
+            const unsigned lm = (unsigned)(q.y * c.n_phi + q.z) * (unsigned)c.n_qpt + (unsigned)q.w;
+            if (lm < low) lo = mid + 1; else hi = mid;
+        }
+        ci = lo;
+    }
+    hit_to_cand[h] = ci;
+    atomicAdd(cand_nhits + ci, 1);
+}
+
 }  // namespace
 
 extern "C" int hough_assign_hits(hough_plan* p, const float* d_hits_xy, int32_t n_hits, const int32_t* d_event_offsets,
@@ -198,7 +231,7 @@ extern "C" int hough_assign_hits(hough_plan* p, const float* d_hits_xy, int32_t 
             if (by_index) {
                 // plan option "assign_candidates": candidate-centric association (assoc.cu), keys carry the candidate index
                 rc = hough_assoc_candidates(p, d_event_offsets, n_hits, n_events, d_cands, d_cand_offsets, capacity, assoc_dj,
-                                            d_hit_to_cand, d_cand_nhits, st);
+                                            d_hit_to_cand, d_cand_nhits, st, nullptr);
                 if (rc != HOUGH_OK) return rc;
             } else {
                 WalkArgs a{};
@@ -247,7 +280,7 @@ extern "C" int hough_assign_hits(hough_plan* p, const float* d_hits_xy, int32_t 
             if (blocks > 0x7fffffffLL) return HOUGH_ERR_UNSUPPORTED;
             if (capacity > 0) {
                 assign_fullscan_kernel<<<(unsigned)blocks, 256, 0, st>>>(p->c, hits, n_hits, d_event_offsets, n_events, d_cands,
-                                                                         p->d_mask, p->d_word_rank, assoc_dj, p->d_best_key);
+                                                                         p->d_mask, p->d_word_rank, assoc_dj, nullptr, p->d_best_key);
                 HOUGH_CUDA_TRY(cudaGetLastError());
                 hough_count_launches(1);
             }
@@ -267,5 +300,80 @@ extern "C" int hough_assign_hits(hough_plan* p, const float* d_hits_xy, int32_t 
             hough_count_launches(1);
         }
     }
+    return HOUGH_OK;
+}
+
+
+// D12: one re-assignment round after hough_assign_hits.  A kept candidate only gains hits, so the kept
+// set does not change and this round is the fixed point of the rounds.
+extern "C" int hough_reassign_hits(hough_plan* p, const float* d_hits_xy, int32_t n_hits, const int32_t* d_event_offsets,
+                                   int32_t n_events, const hough_candidate* d_cands, const int32_t* d_cand_offsets,
+                                   int32_t capacity, int32_t assoc_dj, int32_t max_rounds, int32_t* d_hit_to_cand,
+                                   int32_t* d_cand_nhits, const uint8_t* d_cand_keep, void* cuda_stream) {
+    if (!p || !d_event_offsets || !d_cand_offsets) return HOUGH_ERR_INVALID_ARG;
+    if (n_hits < 0 || n_events < 0 || n_hits > p->max_hits || n_events > p->max_events) return HOUGH_ERR_INVALID_ARG;
+    if (capacity < 0 || assoc_dj < 0 || assoc_dj > 15 || max_rounds < 1) return HOUGH_ERR_INVALID_ARG;
+    if (n_hits > 0 && (!d_hits_xy || !d_hit_to_cand)) return HOUGH_ERR_INVALID_ARG;
+    if (capacity > 0 && (!d_cands || !d_cand_nhits || !d_cand_keep)) return HOUGH_ERR_INVALID_ARG;
+    if ((reinterpret_cast<uintptr_t>(d_hits_xy) & 7u) || (reinterpret_cast<uintptr_t>(d_cands) & 15u))
+        return HOUGH_ERR_INVALID_ARG;
+    if (n_events == 0) return n_hits == 0 ? HOUGH_OK : HOUGH_ERR_INVALID_ARG;
+    if (max_rounds < 2 || n_hits == 0 || capacity == 0) return HOUGH_OK;       // one round is D9 itself
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+    const bool tiled = !p->fullscan && p->tile_max_cols >= 1;
+    HOUGH_CUDA_TRY(cudaMemsetAsync(p->d_best_key, 0, sizeof(unsigned long long) * (size_t)n_hits, st));
+    if (tiled) {
+        int rc = hough_stage_hits(p, d_hits_xy, n_hits, d_event_offsets, n_events, st, true);
+        if (rc != HOUGH_OK) return rc;
+        if (!p->reassign_walk && !p->d_assoc_tab && !p->assoc_tab_tried) {      // first use: build the table (one device sync)
+            p->assoc_tab_tried = 1;
+            rc = hough_build_assoc_table(p);
+            if (rc != HOUGH_OK) return rc;
+        }
+        if (p->d_assoc_tab != nullptr && !p->reassign_walk)
+            // few candidates survive D9: the candidate-centric association (assoc.cu) visits only them
+            return hough_assoc_candidates(p, d_event_offsets, n_hits, n_events, d_cands, d_cand_offsets, capacity, assoc_dj,
+                                          d_hit_to_cand, d_cand_nhits, st, d_cand_keep);
+        WalkArgs a{};
+        a.staged = p->d_staged;
+        a.off = d_event_offsets;
+        a.key_start = p->d_stage_cnt;
+        walk_shape(p, n_events, a.n_slabs, a.slab_cols);
+        a.stride = p->tile_stride_words;
+        a.cands = d_cands;
+        a.slice = p->d_slice;
+        a.assoc_dj = assoc_dj;
+        a.best_key = p->d_best_key;
+        a.keep = d_cand_keep;
+        const long long tiles = (long long)n_events * p->c.n_d0 * a.n_slabs;
+        if (tiles > (long long)p->slice_len) return HOUGH_ERR_UNSUPPORTED;
+        cand_slice_kernel<<<(unsigned)((tiles + 255) / 256), 256, 0, st>>>(p->c, d_cands, d_cand_offsets, n_events, capacity,
+                                                                            a.n_slabs, a.slab_cols, p->d_slice);
+        HOUGH_CUDA_TRY(cudaGetLastError());
+        rc = walk_dispatch<WALK_ASSIGN>(p, n_events, a, p->tile32 != 0, false, st);
+        if (rc != HOUGH_OK) return rc;
+        reassign_decode_kernel<true><<<(n_hits + 255) / 256, 256, 0, st>>>(p->c, p->d_best_key, n_hits, d_event_offsets, n_events,
+                                                                           d_cands, d_cand_offsets, capacity, d_hit_to_cand,
+                                                                           d_cand_nhits);
+        HOUGH_CUDA_TRY(cudaGetLastError());
+        hough_count_launches(2);
+        return HOUGH_OK;
+    }
+    const size_t n_words = (size_t)n_events * p->c.words_per_event;
+    HOUGH_CUDA_TRY(cudaMemsetAsync(p->d_mask, 0, sizeof(uint32_t) * n_words, st));
+    const int blocks_c = min((capacity + 255) / 256, p->sm_count * 8);
+    cand_index_kernel<<<blocks_c, 256, 0, st>>>(p->c, d_cands, d_cand_offsets, n_events, capacity, p->d_mask, p->d_word_rank);
+    HOUGH_CUDA_TRY(cudaGetLastError());
+    const float2* hits = reinterpret_cast<const float2*>(d_hits_xy);
+    const long long blocks = ((long long)n_hits * p->c.n_phi + 255) / 256;
+    if (blocks > 0x7fffffffLL) return HOUGH_ERR_UNSUPPORTED;
+    assign_fullscan_kernel<<<(unsigned)blocks, 256, 0, st>>>(p->c, hits, n_hits, d_event_offsets, n_events, d_cands, p->d_mask,
+                                                             p->d_word_rank, assoc_dj, d_cand_keep, p->d_best_key);
+    HOUGH_CUDA_TRY(cudaGetLastError());
+    reassign_decode_kernel<false><<<(n_hits + 255) / 256, 256, 0, st>>>(p->c, p->d_best_key, n_hits, d_event_offsets, n_events,
+                                                                        d_cands, d_cand_offsets, capacity, d_hit_to_cand,
+                                                                        d_cand_nhits);
+    HOUGH_CUDA_TRY(cudaGetLastError());
+    hough_count_launches(3);
     return HOUGH_OK;
 }

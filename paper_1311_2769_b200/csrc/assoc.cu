@@ -99,6 +99,7 @@ struct AssocArgs {
     const int32_t* cand_off;         // [n_events + 1]
     const float2* tab;               // assoc table
     unsigned long long* best_key;    // [n_hits] by original hit index
+    const uint8_t* keep;             // optional [capacity]: only candidates with keep != 0 take part (D12)
     int capacity, assoc_dj, parts;
     int smem_hits;                   // entries of the shared best-key array (events with more hits fold into global memory)
     float margin_cols, sec_per_col;
@@ -232,10 +233,12 @@ __global__ void __launch_bounds__(ASSOC_THREADS, SMEM ? 3 : 2) assoc_cand_kernel
         if (__ldg(ks + (cl + 1) * NS) > __ldg(ks + cl * NS)) s_cls[atomicAdd(&s_ncl, 1)] = (short)cl;
     if (SMEM)
         for (int h = tid; h < ev_hits; h += ASSOC_THREADS) s_best[h] = 0ull;
-    for (int ci = c_begin + tid; ci < c_end; ci += ASSOC_THREADS) atomicAdd(&s_hist[min(max(__ldg(&a.cands[ci].votes), 0), ASSOC_HIST - 1)], 1);
+    for (int ci = c_begin + tid; ci < c_end; ci += ASSOC_THREADS)
+        if (!a.keep || __ldg(a.keep + ci)) atomicAdd(&s_hist[min(max(__ldg(&a.cands[ci].votes), 0), ASSOC_HIST - 1)], 1);
     __syncthreads();
     if (tid == 0) {                                        // vote levels: top ~1/16 and top ~1/3 of the chunk
-        const int total = c_end - c_begin;
+        int total = 0;
+        for (int v = 0; v < ASSOC_HIST; ++v) total += s_hist[v];
         int acc = 0, l0 = ASSOC_HIST, l1 = ASSOC_HIST;
         for (int v = ASSOC_HIST - 1; v >= 0; --v) {
             acc += s_hist[v];
@@ -260,7 +263,7 @@ __global__ void __launch_bounds__(ASSOC_THREADS, SMEM ? 3 : 2) assoc_cand_kernel
         for (int g = w_begin; g < w_end; g += 32) {
             const int ci = g + lane;
             bool sel = false;
-            if (ci < w_end) {
+            if (ci < w_end && (!a.keep || __ldg(a.keep + ci))) {
                 const int v = min(max(__ldg(&a.cands[ci].votes), 0), ASSOC_HIST - 1);
                 sel = v >= v_lo && v < v_hi;
             }
@@ -287,17 +290,21 @@ __global__ void __launch_bounds__(ASSOC_THREADS, SMEM ? 3 : 2) assoc_cand_kernel
 }
 
 // best key by staged position -> hit_to_cand by original hit index, and the per-candidate hit counts
+// ORPHANS (D12 re-assignment round): only hits still at -1 take the new key; the others and their counts stay.
+template <bool ORPHANS>
 __global__ void __launch_bounds__(256) assoc_decode_kernel(const unsigned long long* __restrict__ best_key, const float4* __restrict__ staged,
                                                            int n_hits, int32_t* __restrict__ hit_to_cand, int32_t* __restrict__ cand_nhits) {
     const int pos = blockIdx.x * blockDim.x + threadIdx.x;
     if (pos >= n_hits) return;
     const unsigned long long key = best_key[pos];
+    const int h = __float_as_int(__ldg(staged + pos).w);
+    if (ORPHANS && (!key || hit_to_cand[h] >= 0)) return;
     int ci = -1;
     if (key) {
         ci = (int)(0xFFFFFFFFu - (unsigned)(key & 0xFFFFFFFFull));
         atomicAdd(cand_nhits + ci, 1);
     }
-    hit_to_cand[__float_as_int(__ldg(staged + pos).w)] = ci;
+    hit_to_cand[h] = ci;
 }
 
 }  // namespace
@@ -324,8 +331,9 @@ int hough_build_assoc_table(hough_plan* p) {
 // STAGED position) and decodes them into d_hit_to_cand / d_cand_nhits.
 int hough_assoc_candidates(hough_plan* p, const int32_t* d_event_offsets, int32_t n_hits, int32_t n_events,
                            const hough_candidate* d_cands, const int32_t* d_cand_offsets, int32_t capacity, int32_t assoc_dj,
-                           int32_t* d_hit_to_cand, int32_t* d_cand_nhits, cudaStream_t st) {
+                           int32_t* d_hit_to_cand, int32_t* d_cand_nhits, cudaStream_t st, const uint8_t* d_keep_filter) {
     AssocArgs a{};
+    a.keep = d_keep_filter;
     a.staged = p->d_staged;
     a.off = d_event_offsets;
     a.key_start = p->d_stage_cnt;
@@ -366,7 +374,10 @@ int hough_assoc_candidates(hough_plan* p, const int32_t* d_event_offsets, int32_
         HOUGH_CUDA_TRY(cudaGetLastError());
         ++launches;
     }
-    assoc_decode_kernel<<<(n_hits + 255) / 256, 256, 0, st>>>(p->d_best_key, p->d_staged, n_hits, d_hit_to_cand, d_cand_nhits);
+    if (d_keep_filter)
+        assoc_decode_kernel<true><<<(n_hits + 255) / 256, 256, 0, st>>>(p->d_best_key, p->d_staged, n_hits, d_hit_to_cand, d_cand_nhits);
+    else
+        assoc_decode_kernel<false><<<(n_hits + 255) / 256, 256, 0, st>>>(p->d_best_key, p->d_staged, n_hits, d_hit_to_cand, d_cand_nhits);
     HOUGH_CUDA_TRY(cudaGetLastError());
     hough_count_launches(launches);
     return HOUGH_OK;

@@ -94,6 +94,8 @@ struct hough_plan {
     int32_t* d_stage_cnt;              // [max_events][n_keys + 1] key counters -> exclusive key starts
     // candidate-centric association (assoc.cu)
     float2* d_assoc_tab;               // [n_class][n_d0][n_qpt + 1] azimuth-offset hulls per bin edge; null: not built
+    int reassign_walk;                 // 1: hough_reassign_hits re-walks the vote columns instead of the candidate-centric path
+    int assoc_tab_tried;               // the assoc table was requested once (it may not fit: d_assoc_tab stays null)
     int assoc_smem_configured;         // dynamic shared memory the kernel is configured for on this plan's device
     // vote tile shape (vote.cu)
     int32_t tile32;                    // 1: 32-bit bins in shared memory, 0: two 16-bit bins per word
@@ -174,7 +176,7 @@ int hough_stage_hits(hough_plan* p, const float* d_hits_xy, int32_t n_hits, cons
 int hough_build_assoc_table(hough_plan* p);
 int hough_assoc_candidates(hough_plan* p, const int32_t* d_event_offsets, int32_t n_hits, int32_t n_events,
                            const hough_candidate* d_cands, const int32_t* d_cand_offsets, int32_t capacity, int32_t assoc_dj,
-                           int32_t* d_hit_to_cand, int32_t* d_cand_nhits, cudaStream_t st);
+                           int32_t* d_hit_to_cand, int32_t* d_cand_nhits, cudaStream_t st, const uint8_t* d_keep_filter);
 int hough_vote_fullscan(hough_plan* p, const float* d_hits_xy, int32_t n_hits, const int32_t* d_event_offsets,
                         int32_t n_events, void* d_accum, cudaStream_t st);
 int hough_vote_tiled(hough_plan* p, const float* d_hits_xy, int32_t n_hits, const int32_t* d_event_offsets,

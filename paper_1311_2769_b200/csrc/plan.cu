@@ -150,6 +150,7 @@ extern "C" int hough_plan_create(const hough_binning* b, const hough_geometry* g
     // packed 16-bit tiles are exact whenever no bin can exceed 65535: the U16 precondition, or at most 65535
     // hits per call (a hit casts at most one vote per (phi0, d0) column, D3)
     p->tile32 = (b->accum_dtype == HOUGH_ACC_I32 && max_hits > 65535) ? 1 : 0;
+    { const char* et = getenv("HOUGH_FORCE_TILE32"); if (et && et[0] == '1') p->tile32 = 1; }
     {
         // walk.cuh "Tile layout": a row (32-bit bins) or a row of column PAIRS (16-bit bins) has `stride` words.
         // Largest even column count whose whole shared-memory block lets 3 CTAs share an SM (228 KB, 1 KB reserved per
@@ -232,9 +233,10 @@ extern "C" int hough_plan_set_option(hough_plan* p, const char* key, int32_t val
     if (strcmp(key, "peaks_scalar") == 0) { p->peaks_scalar = value ? 1 : 0; return HOUGH_OK; }
     if (strcmp(key, "assign_candidates") == 0) {
         p->assign_candidates = value ? 1 : 0;
-        if (value && !p->d_assoc_tab && p->tile_max_cols >= 1) return hough_build_assoc_table(p);   // built once, on first use
+        if (value && !p->d_assoc_tab && p->tile_max_cols >= 1) { p->assoc_tab_tried = 1; return hough_build_assoc_table(p); }   // built once, on first use
         return HOUGH_OK;
     }
+    if (strcmp(key, "reassign_walk") == 0) { p->reassign_walk = value ? 1 : 0; return HOUGH_OK; }
     if (strcmp(key, "exact_walk") == 0) { p->exact_walk = value ? 1 : 0; return HOUGH_OK; }
     if (strcmp(key, "reuse_staging") == 0) { p->reuse_staging = value ? 1 : 0; p->staged_hits = nullptr; return HOUGH_OK; }
     return HOUGH_ERR_INVALID_ARG;

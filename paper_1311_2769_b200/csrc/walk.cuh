@@ -30,6 +30,7 @@
 // "exact_walk" take the exact sequence at every column.  The result is therefore the D3 bin in every case.
 #pragma once
 
+#include <cstdlib>
 #include <type_traits>
 
 #include "common.cuh"
@@ -56,6 +57,7 @@ struct WalkArgs {
     const int2* slice;               // [n_events * n_d0 * n_slabs] {first, end} candidate of each tile
     int assoc_dj;
     unsigned long long* best_key;    // [n_hits] by original hit index
+    const uint8_t* keep;             // optional [capacity]: only candidates with keep != 0 take part (D12 re-assignment round)
 };
 
 constexpr int WALK_DUMP = 4;                     // dump slots per row: where results outside [-1, nq] are added (by lane & 3)
@@ -420,8 +422,13 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
     bool legacy = false;
     if (MODE == WALK_ASSIGN) {
         int sat = 0;
-        for (int ci = cand_first + tid; ci < cand_end; ci += WALK_THREADS)
+        int any = 0;
+        for (int ci = cand_first + tid; ci < cand_end; ci += WALK_THREADS) {
+            if (a.keep && !__ldg(a.keep + ci)) continue;
+            any = 1;
             sat |= ((unsigned)__ldg(&a.cands[ci].votes) + 1u >= EntryT<TILE32>::VSAT) ? 1 : 0;
+        }
+        if (a.keep && !__syncthreads_or(any)) return;      // no surviving candidate in this tile
         legacy = __syncthreads_or(sat) != 0 || a.exact_only != 0;
     }
     const bool exact_mode = a.exact_only != 0 || !fk.usable || (MODE == WALK_ASSIGN && legacy);
@@ -525,6 +532,7 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
         __syncthreads();                                // the tile is zero
         if (legacy) {                                   // votes + 1 at the candidates' own bins
             for (int ci = cand_first + tid; ci < cand_end; ci += WALK_THREADS) {
+                if (a.keep && !__ldg(a.keep + ci)) continue;
                 const int4 q = __ldg(reinterpret_cast<const int4*>(a.cands + ci));          // event, k, i, j
                 const unsigned v = (unsigned)__ldg(&a.cands[ci].votes) + 1u;
                 const int col = q.z - c0;
@@ -534,6 +542,7 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
         } else {                                        // dilated entries: max over the candidates within assoc_dj
             const int dj = a.assoc_dj;
             for (int ci = cand_first + tid; ci < cand_end; ci += WALK_THREADS) {
+                if (a.keep && !__ldg(a.keep + ci)) continue;
                 const int4 q = __ldg(reinterpret_cast<const int4*>(a.cands + ci));
                 const unsigned v = ((unsigned)__ldg(&a.cands[ci].votes) + 1u) << 5;
                 const int col = q.z - c0;
@@ -762,7 +771,11 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
 
     // ---- flush: the tile is written to the global accumulator exactly once (A3); guard slots are dropped ----
     const size_t row0 = ((size_t)e * c.n_d0 + k) * (size_t)nphi + c0;      // first global row of the tile
-    if (TILE32) {
+    if (TILE32 && OUT16) {
+        unsigned short* g = reinterpret_cast<unsigned short*>(a.accum) + row0 * nq;
+        for (int ci = warp; ci < cols; ci += WALK_WARPS)
+            for (int j = lane; j < nq; j += 32) g[(size_t)ci * nq + j] = (unsigned short)s_tile[ci * stride + j + 1];
+    } else if (TILE32) {
         int* g = reinterpret_cast<int*>(a.accum) + row0 * nq;
         for (int ci = warp; ci < cols; ci += WALK_WARPS)
             for (int j = lane; j < nq; j += 32) g[(size_t)ci * nq + j] = (int)s_tile[ci * stride + j + 1];
@@ -798,6 +811,7 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
 inline void walk_shape(const hough_plan* p, int n_events, int& n_slabs, int& slab_cols) {
     const int nphi = p->c.n_phi;
     n_slabs = (nphi + p->tile_max_cols - 1) / p->tile_max_cols;
+    { const char* es = getenv("HOUGH_FORCE_SLABS"); if (es && atoi(es) > n_slabs) n_slabs = atoi(es); }
     const long long want = 3LL * p->sm_count;
     while ((long long)n_slabs * p->c.n_d0 * n_events < want && (nphi + n_slabs - 1) / n_slabs > 32) n_slabs *= 2;
     slab_cols = (nphi + n_slabs - 1) / n_slabs;
@@ -826,6 +840,9 @@ int walk_launch(hough_plan* p, int n_events, WalkArgs a, cudaStream_t st) {
 template <int MODE>
 int walk_dispatch(hough_plan* p, int n_events, WalkArgs a, bool tile32, bool out16, cudaStream_t st) {
     const bool full = a.n_slabs == 1;
+    if (tile32 && out16 && MODE == WALK_VOTE)
+        return full ? walk_launch<MODE, true, true, true>(p, n_events, a, st)
+                    : walk_launch<MODE, true, true, false>(p, n_events, a, st);
     if (tile32)
         return full ? walk_launch<MODE, true, false, true>(p, n_events, a, st)
                     : walk_launch<MODE, true, false, false>(p, n_events, a, st);
