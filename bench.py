@@ -649,6 +649,135 @@ def run_sweep(args):
         plan.close()
 
 
+def run_efficiency(args):
+    """Track-finding efficiency / fake / duplicate report against generator truth (Fig. 1: "track-finding
+    efficiency ... approximately 86%" on the toy detector of PAPER.md:39).  vote -> peaks -> assign (D9),
+    then the D12 re-assignment round, then the circle fit of the kept candidates, all through the library; the counting is
+    paper_1311_2769_b200.efficiency (host numpy).  Prints one JSON line per configuration (not the driver's bench line)."""
+    import math
+    import torch
+    from paper_1311_2769_b200 import HoughPlan, alloc_candidates, candidates_to_numpy, hough_fit_circles, load_library
+    from paper_1311_2769_b200.efficiency import efficiency_report, truth_parameters
+    from workloads import generate_events, get_workload
+    load_library()
+    torch.cuda.set_device(0)
+    from dataclasses import replace
+    todo = [(cfg, None) for cfg in args.efficiency]
+    if args.efficiency_scan:
+        # the paper's toy scenario (workload 5) under other binnings: PAPER.md:43 quotes its 86 % without stating the binning
+        todo = [(5, t) for t in ((512, 256, 8, 8, 1), (1024, 64, 8, 8, 1), (2048, 64, 8, 8, 1), (2048, 32, 8, 8, 1),
+                                 (4096, 64, 8, 8, 1), (2048, 64, 7, 7, 1), (2048, 64, 9, 8, 2), (4096, 32, 9, 8, 1),
+                                 (4096, 128, 7, 7, 2), (8192, 64, 8, 8, 1))]
+    for cfg, alt in todo:
+        w = get_workload(cfg)
+        if alt is not None:
+            w = replace(w, binning=replace(w.binning, n_phi=alt[0], n_qpt=alt[1]), threshold=alt[2], assoc_dj=alt[4],
+                        name=f"{w.name}_{alt[0]}x{alt[1]}_thr{alt[2]}_min{alt[3]}_dj{alt[4]}")
+            min_hits_alt = alt[3]
+        else:
+            min_hits_alt = None
+        if w.n_events > 1:
+            w = w.scaled(min(w.n_events, args.efficiency_events))
+        batch = generate_events(w, want_truth=True)
+        n_ev = w.n_events
+        bn = w.binning
+        plan = HoughPlan.from_workload(w, max_hits=max(batch.n_hits, 1), max_events=n_ev)
+        d_hits = torch.from_numpy(batch.hits_xy).cuda()
+        d_off = torch.from_numpy(batch.event_offsets).cuda()
+        accum = plan.alloc_accum(n_ev)
+        plan.vote(d_hits, d_off, accum)
+        coff = torch.zeros(n_ev + 1, dtype=torch.int32, device="cuda")
+        plan.find_peaks(accum, n_ev, w.threshold, None, 0, coff)
+        cap = int(coff[n_ev].item()) + 1
+        cands = alloc_candidates(cap)
+        plan.find_peaks(accum, n_ev, w.threshold, cands, cap, coff)
+        h2c = torch.empty(max(batch.n_hits, 1), dtype=torch.int32, device="cuda")
+        nh = torch.empty(cap, dtype=torch.int32, device="cuda")
+        keep = torch.empty(cap, dtype=torch.uint8, device="cuda")
+        min_hits = w.min_hits if min_hits_alt is None else min_hits_alt
+        plan.assign_hits(d_hits, d_off, cands, coff, cap, w.assoc_dj, min_hits, h2c, nh, keep)
+        torch.cuda.synchronize()
+        off = coff.cpu().numpy()
+        rec = candidates_to_numpy(cands, int(off[-1]))
+        keep_h = keep[:int(off[-1])].cpu().numpy()
+        h2c_d9 = h2c[:batch.n_hits].cpu().numpy()
+        plan.reassign_hits(d_hits, d_off, cands, coff, cap, w.assoc_dj, 2, h2c, nh, keep)
+        torch.cuda.synchronize()
+        h2c_d12 = h2c[:batch.n_hits].cpu().numpy()
+        # circle fit of the kept candidates on the re-assigned hits (D11)
+        work = torch.zeros(cap * 9, dtype=torch.float64, device="cuda")
+        fit = torch.zeros((cap, 4), dtype=torch.float64, device="cuda")
+        nfit = torch.zeros(cap, dtype=torch.int32, device="cuda")
+        hough_fit_circles(plan, d_hits, h2c, cands, coff, n_ev, cap, keep, work, fit, nfit)
+        torch.cuda.synchronize()
+        fit_h, nfit_h = fit.cpu().numpy(), nfit.cpu().numpy()
+
+        def total(h2c_all):
+            acc = None
+            for e in range(n_ev):
+                a, b = int(batch.event_offsets[e]), int(batch.event_offsets[e + 1])
+                c0, c1 = int(off[e]), int(off[e + 1])
+                local = np.where(h2c_all[a:b] >= 0, h2c_all[a:b] - c0, -1)
+                r = efficiency_report(bn, w.bz_tesla, batch.truth[e], rec[c0:c1], keep_h[c0:c1], local, min_hits)
+                if acc is None:
+                    acc = {k: r[k] for k in ("tracks", "reconstructable", "candidates", "kept", "hits_assigned", "hits_total")}
+                    acc["found_by_hits"] = r["by_hits"]["tracks_found"]
+                    acc["found_by_parameters"] = r["by_parameters"]["tracks_found"]
+                    acc["fake_by_hits"] = r["by_hits"]["fake_rate"] * max(r["kept"], 1)
+                    acc["dup_by_hits"] = r["by_hits"]["duplicate_rate"] * max(r["kept"], 1)
+                    acc["fake_by_parameters"] = r["by_parameters"]["fake_rate"] * max(r["kept"], 1)
+                    acc["dup_by_parameters"] = r["by_parameters"]["duplicate_rate"] * max(r["kept"], 1)
+                    acc["purity_sum"] = r["mean_purity"] * r["kept"]
+                else:
+                    for k in ("tracks", "reconstructable", "candidates", "kept", "hits_assigned", "hits_total"):
+                        acc[k] += r[k]
+                    acc["found_by_hits"] += r["by_hits"]["tracks_found"]
+                    acc["found_by_parameters"] += r["by_parameters"]["tracks_found"]
+                    acc["fake_by_hits"] += r["by_hits"]["fake_rate"] * max(r["kept"], 1)
+                    acc["dup_by_hits"] += r["by_hits"]["duplicate_rate"] * max(r["kept"], 1)
+                    acc["fake_by_parameters"] += r["by_parameters"]["fake_rate"] * max(r["kept"], 1)
+                    acc["dup_by_parameters"] += r["by_parameters"]["duplicate_rate"] * max(r["kept"], 1)
+                    acc["purity_sum"] += r["mean_purity"] * r["kept"]
+            kept = max(acc["kept"], 1)
+            reco = max(acc["reconstructable"], 1)
+            out = {k: acc[k] for k in ("tracks", "reconstructable", "candidates", "kept", "hits_assigned", "hits_total")}
+            out["mean_purity"] = acc["purity_sum"] / kept
+            for m in ("hits", "parameters"):
+                out["by_" + m] = {"efficiency": acc["found_by_" + m] / reco, "fake_rate": acc["fake_by_" + m] / kept,
+                                  "duplicate_rate": acc["dup_by_" + m] / kept}
+            return out
+
+        # q/pT resolution of the kept, hit-matched candidates: peak centroid (D7) vs circle fit (D11), against truth
+        res_c, res_f = [], []
+        for e in range(n_ev):
+            tp = truth_parameters(batch.truth[e], w.bz_tesla)
+            a, b = int(batch.event_offsets[e]), int(batch.event_offsets[e + 1])
+            lab = batch.truth[e]["hit_track"]
+            for c in range(int(off[e]), int(off[e + 1])):
+                if not keep_h[c] or nfit_h[c] < 3:
+                    continue
+                own = lab[np.nonzero(h2c_d12[a:b] == c)[0]]
+                own = own[own >= 0]
+                if len(own) == 0:
+                    continue
+                ids, cnt = np.unique(own, return_counts=True)
+                t = ids[np.argmax(cnt)]
+                if 2 * cnt.max() <= nfit_h[c] or bn.model != 0:
+                    continue
+                res_c.append(float(rec["qpt"][c]) - tp["qpt"][t])
+                res_f.append(fit_h[c, 1] - tp["qpt"][t])
+        line = {"report": "efficiency", "cite": "PAPER.md:43 (approx. 86 % on its toy detector, binning unstated), SURVEY 8(f) f4",
+                "config": {"workload": w.name, "events": n_ev, "n_phi": bn.n_phi, "n_qpt": bn.n_qpt, "n_d0": bn.n_d0,
+                           "threshold": w.threshold, "min_hits": min_hits, "assoc_dj": w.assoc_dj},
+                "d9_single_pass": total(h2c_d9), "d12_reassigned": total(h2c_d12),
+                "qpt_resolution": {"matched_candidates": len(res_c), "bin_width": (bn.qpt_max - bn.qpt_min) / bn.n_qpt,
+                                   "centroid_rms": float(np.sqrt(np.mean(np.square(res_c)))) if res_c else None,
+                                   "circle_fit_rms": float(np.sqrt(np.mean(np.square(res_f)))) if res_f else None,
+                                   "circle_fit_median_abs": float(np.median(np.abs(res_f))) if res_f else None}}
+        print(json.dumps(line), flush=True)
+        plan.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -666,7 +795,18 @@ def main():
     ap.add_argument("--ref-seconds-per-step", type=float, default=10.0)
     ap.add_argument("--sweep-tracks", action="store_true", help="Fig. 2-style sweep on the paper's toy detector (workload 5)")
     ap.add_argument("--sweep-reps", type=int, default=30)
+    ap.add_argument("--efficiency", type=int, nargs="*", default=None, metavar="CFG",
+                    help="efficiency / fake / duplicate report against generator truth for these workloads (PAPER.md:43)")
+    ap.add_argument("--efficiency-events", type=int, default=8)
+    ap.add_argument("--efficiency-scan", action="store_true", help="the paper's toy scenario under a list of other binnings")
     args = ap.parse_args()
+    if args.efficiency_scan and args.efficiency is None:
+        args.efficiency = [5]
+    if args.efficiency is not None:
+        if not args.efficiency:
+            args.efficiency = [5, 0, 1, 3]
+        run_efficiency(args)
+        return
     if args.sweep_tracks:
         run_sweep(args)
         return

@@ -229,8 +229,10 @@ def generate_event(w: HoughWorkload, event: int, want_truth: bool = False):
     hits = np.stack([hx[order], hy[order]], axis=1).astype(np.float32)
     if not want_truth:
         return hits, None
+    # generating track of every hit (after the shuffle), -1 = noise: for the efficiency / fake-rate report
+    track_of = np.concatenate([np.broadcast_to(np.arange(n_t)[:, None], ok.shape)[ok], np.full(n_noise, -1)])[order]
     truth = dict(start_x=px, start_y=py, direction=psi, charge=q, pt=pt, rho=rho,
-                 n_track_hits=n_track_hits, n_noise=n_noise, layer_hit_mask=ok)
+                 n_track_hits=n_track_hits, n_noise=n_noise, layer_hit_mask=ok, hit_track=track_of.astype(np.int32))
     return hits, truth
 
 
