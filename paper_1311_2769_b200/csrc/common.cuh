@@ -34,6 +34,7 @@ struct HoughConsts {
     float A_f, qmin, inv_wq, nq_f;
     float qpt_min, d0_min;        // centroid (D7)
     float wq, wphi, wd, two_pi_f;
+    float kappa, sd2;             // column-pair recurrence of the walk: 4 sin^2(wphi), 2 sin(wphi)  (walk.cuh "Recurrence")
     const float2* cs;             // [n_phi] {cos, sin} of the column centres
     const float4* d0t;            // [n_d0]  {d0c, 2*d0c, d0c^2, 0}
     // work sizing (windows.cu): never changes a result

@@ -107,6 +107,11 @@ extern "C" int hough_plan_create(const hough_binning* b, const hough_geometry* g
     c.wphi = (float)((2.0 * kPi) / (double)b->n_phi);
     c.wd = (float)(((double)b->d0_max - (double)b->d0_min) / (double)b->n_d0);
     c.two_pi_f = (float)(2.0 * kPi);
+    {
+        const double delta = 2.0 * kPi / (double)b->n_phi;
+        c.kappa = (float)(4.0 * sin(delta) * sin(delta));
+        c.sd2 = (float)(2.0 * sin(delta));
+    }
 
     std::vector<float2> cs(b->n_phi);
     const int q = b->n_phi / 4;
@@ -178,7 +183,7 @@ extern "C" int hough_plan_create(const hough_binning* b, const hough_geometry* g
         if (!ok) return;
         if (cudaMalloc(ptr, bytes ? bytes : 4) != cudaSuccess) { ok = false; (void)cudaGetLastError(); }
     };
-    A((void**)&p->d_cs, sizeof(float2) * b->n_phi);
+    A((void**)&p->d_cs, sizeof(float2) * ((size_t)b->n_phi + 2));      // two pad entries in front: c.cs[-1] = column n_phi - 1
     A((void**)&p->d_d0t, sizeof(float4) * b->n_d0);
     A((void**)&p->d_peak_block_cnt, sizeof(int32_t) * (size_t)max_events * p->peak_blocks_per_event);
     A((void**)&p->d_event_cnt, sizeof(int32_t) * ((size_t)max_events + 1));
@@ -198,7 +203,8 @@ extern "C" int hough_plan_create(const hough_binning* b, const hough_geometry* g
     A((void**)&p->d_edge2, sizeof(float) * win.n_class);
     A((void**)&p->d_win, sizeof(int2) * winT.size());
     if (!ok) { plan_free(p); return HOUGH_ERR_ALLOC; }
-    if (cudaMemcpy(p->d_cs, cs.data(), sizeof(float2) * b->n_phi, cudaMemcpyHostToDevice) != cudaSuccess ||
+    cs.insert(cs.begin(), 2, cs[b->n_phi - 1]);
+    if (cudaMemcpy(p->d_cs, cs.data(), sizeof(float2) * ((size_t)b->n_phi + 2), cudaMemcpyHostToDevice) != cudaSuccess ||
         cudaMemcpy(p->d_edge2, win.edge2.data(), sizeof(float) * win.n_class, cudaMemcpyHostToDevice) != cudaSuccess ||
         cudaMemcpy(p->d_win, winT.data(), sizeof(int2) * winT.size(), cudaMemcpyHostToDevice) != cudaSuccess ||
         cudaMemcpy(p->d_d0t, d0t.data(), sizeof(float4) * b->n_d0, cudaMemcpyHostToDevice) != cudaSuccess) {
@@ -206,7 +212,7 @@ extern "C" int hough_plan_create(const hough_binning* b, const hough_geometry* g
         plan_free(p);
         return HOUGH_ERR_CUDA;
     }
-    c.cs = p->d_cs;
+    c.cs = p->d_cs + 2;                       // 16-byte aligned; c.cs[-1] is the wrap-around column (walk.cuh wrec_init)
     c.d0t = p->d_d0t;
     c.edge2 = p->d_edge2;
     c.win = p->d_win;

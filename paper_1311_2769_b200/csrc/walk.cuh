@@ -42,7 +42,7 @@ constexpr int WALK_ASSIGN = 1;
 __host__ __device__ constexpr int walk_threads(int mode) { return mode == 0 ? 320 : 256; }
 constexpr int WALK_MAX_WARPS = 10;
 constexpr int WALK_CHUNK_PAIRS = 32;             // column pairs per chunk = the bits of the redo mask
-constexpr int WALK_WQ_CAP = 48;                  // entries of a warp's exact-redo queue (drained by the whole warp)
+constexpr int WALK_WQ_CAP = 64;                  // entries of a warp's redo queue: < 32 waiting + up to 32 new ones per round
 
 struct WalkArgs {
     const float4* staged;            // [n_hits] staged hits (stage.cu)
@@ -69,7 +69,6 @@ __host__ __device__ inline size_t walk_tile_words(int cols, int stride, bool til
 
 __host__ __device__ inline size_t walk_smem_bytes(int cols, int stride, bool tile32, int n_class, bool fullphi) {
     size_t b = (walk_tile_words(cols, stride, tile32) * 4 + 15) & ~(size_t)15;
-    b += (size_t)(cols / 2 + WALK_CHUNK_PAIRS + 1) * 16;               // column pairs {cosA, cosB, sinA, sinB}
     b += (size_t)n_class * 16;                                          // per class: window, error bound
     b += ((size_t)n_class * (fullphi ? 1 : 2) + 1) * 16;                // segments (a full-phi tile has one per class)
     b += (size_t)WALK_MAX_WARPS * WALK_WQ_CAP * 4;                      // redo queues
@@ -199,23 +198,68 @@ __device__ __forceinline__ FastK make_fastk(const HoughConsts& c, float4 d) {
     return k;
 }
 
-// Per-hit terms of the fast path.  Used by the hot loop (packed) and by the redo of queued pairs, which must
-// reproduce the hot loop's slot bit for bit: explicit intrinsics, no contraction, one definition.
-struct FastHit { float gy, gx, ny, nx, r2Ak; };
-__device__ __forceinline__ FastHit make_fasthit(const FastK& fk, float x, float y, float r2) {
-    FastHit h;                                                              // (line model: gy = gx = 0, r2Ak = 1)
-    h.gy = __fmul_rn(fk.ntd0A, y);  h.gx = -__fmul_rn(fk.ntd0A, x);       // A den ~ gy c + gx s + r2Ak
-    h.ny = __fmul_rn(fk.nq_s, y);  h.nx = -__fmul_rn(fk.nq_s, x);          // numq  ~ ny c + nx s + d0cq
-    h.r2Ak = __fmaf_rn(r2, fk.A_f, fk.d0sqA);
-    return h;
+// ---- Recurrence.  Both A den and the numerator are affine in ONE per-column quantity,
+//   w_i = y cos_i - x sin_i = r sin(phi_hit - theta_i):     A den ~ ntd0A w + r2Ak,    numq ~ nq_s w + d0cq,
+// and along the columns of a pair walk (step 2 columns = angle 2 wphi) w obeys  w_{n+1} = 2 cos(2 wphi) w_n - w_{n-1}.
+// In Reinsch's difference form (stable for small angles):  d_{n+1} = d_n - kappa w_n,  w_{n+1} = w_n + d_{n+1},
+// kappa = 4 sin^2(wphi): one FFMA2 + one FADD2 per column pair and NO table read in the hot loop.  The walk
+// re-initialises (w, d) from the cos/sin table at the first pair of every chunk of WALK_CHUNK_PAIRS pairs:
+//   w_0 = y c - x s at the pair's two columns,   d_0 = w_0 - w_{-1} = -2 sin(wphi) (x c' + y s') with (c', s') of the column
+//   before each (the half-way column of the step) -- no cancellation.
+// The rounding error the recurrence accumulates over a chunk enters the bound m through Ew (walk_kernel prologue).
+// One definition serves the hot loop and the replay of a queued pair (which must reproduce the hot loop's slots bit
+// for bit): explicit PTX operations, no contraction.
+struct WRec { f32x2 w2, d2; };
+__device__ __forceinline__ WRec wrec_init(const HoughConsts& c, float x, float y, int ca) {      // ca: absolute column, even
+    const float4 T = __ldg(reinterpret_cast<const float4*>(c.cs + ca));                          // {cosA, sinA, cosB, sinB}
+    const float2 M = __ldg(c.cs + ca - 1);                                                        // the column before A (cs[-1] = cs[n_phi - 1])
+    const float wA = __fmaf_rn(y, T.x, -__fmul_rn(x, T.y));
+    const float wB = __fmaf_rn(y, T.z, -__fmul_rn(x, T.w));
+    const float fM = __fmaf_rn(y, M.y, __fmul_rn(x, M.x));
+    const float fA = __fmaf_rn(y, T.y, __fmul_rn(x, T.x));
+    WRec r;
+    r.w2 = pk2(wA, wB);
+    r.d2 = pk2(-__fmul_rn(c.sd2, fM), -__fmul_rn(c.sd2, fA));
+    return r;
 }
-// slot h = J + 1 of one column, scalar form of the packed sequence of the hot loop (same operations, same rounding)
-__device__ __forceinline__ unsigned fast_slot(const FastK& fk, const FastHit& h, float cs_c, float cs_s) {
-    const float g = __fmaf_rn(h.gx, cs_s, __fmaf_rn(h.gy, cs_c, h.r2Ak));
-    const float n = __fmaf_rn(h.nx, cs_s, __fmaf_rn(h.ny, cs_c, fk.d0cq));
+__device__ __forceinline__ void wrec_step(WRec& r, f32x2 nkap2) {
+    r.d2 = fma2(nkap2, r.w2, r.d2);
+    r.w2 = add2(r.w2, r.d2);
+}
+// The fast-path bin of ONE column from the cos/sin table (no recurrence): true and J = the D3 bin when t~ is further than
+// the class's bound from a bin edge (the bound covers this sequence as well: its w carries 2 roundings, Ew allows for more).
+__device__ __forceinline__ bool fast_bin_direct(const FastK& fk, float x, float y, float r2Ak, float2 cs, float hm, int& J) {
+    const float w = __fmaf_rn(y, cs.x, -__fmul_rn(x, cs.y));
+    const float g = __fmaf_rn(fk.ntd0A, w, r2Ak);
+    const float n = __fmaf_rn(fk.nq_s, w, fk.d0cq);
     const float th = __fmaf_rn(n, rcp_approx(g), fk.c0h);
     const float yb = __fadd_rn(th, WALK_MAGIC);
-    return (unsigned)(__float_as_int(yb) - (WALK_MAGIC_BITS - 1));
+    const float dl = __fsub_rn(th, __fadd_rn(yb, -WALK_MAGIC));
+    J = __float_as_int(yb) - WALK_MAGIC_BITS;
+    return fabsf(dl) < hm;
+}
+// t~ - 1/2 of the pair's two columns
+__device__ __forceinline__ f32x2 wrec_th(f32x2 w2, f32x2 ntd0A2, f32x2 r2Ak2, f32x2 nqs2, f32x2 d0cq2, f32x2 c0h2) {
+    const f32x2 g2 = fma2(ntd0A2, w2, r2Ak2);
+    const f32x2 n2 = fma2(nqs2, w2, d0cq2);
+    float gA, gB;
+    upk2(g2, gA, gB);
+    return fma2(n2, pk2(rcp_approx(gA), rcp_approx(gB)), c0h2);
+}
+// slots h = J + 1 of the two columns of the pair `steps` pairs after the chunk start at absolute column ca0: the
+// replay of the hot loop (same functions, same operand values)
+__device__ __forceinline__ void wrec_replay_slots(const HoughConsts& c, const FastK& fk, float x, float y, float r2Ak, int ca0,
+                                                  int steps, unsigned& hA, unsigned& hB) {
+    WRec r = wrec_init(c, x, y, ca0);
+    const f32x2 nkap2 = pk2(-c.kappa, -c.kappa);
+    for (int t = 0; t < steps; ++t) wrec_step(r, nkap2);
+    const f32x2 th2 = wrec_th(r.w2, pk2(fk.ntd0A, fk.ntd0A), pk2(r2Ak, r2Ak), pk2(fk.nq_s, fk.nq_s), pk2(fk.d0cq, fk.d0cq),
+                              pk2(fk.c0h, fk.c0h));
+    const f32x2 yb2 = add2(th2, pk2(WALK_MAGIC, WALK_MAGIC));
+    float ybA, ybB;
+    upk2(yb2, ybA, ybB);
+    hA = (unsigned)(__float_as_int(ybA) - (WALK_MAGIC_BITS - 1));
+    hB = (unsigned)(__float_as_int(ybB) - (WALK_MAGIC_BITS - 1));
 }
 
 // Entry of an association tile: (min(votes, VCAP) + 1) << 5 | p,  p = (15 - |dj|) * 2 + (dj < 0), dj = j_cand - j_bin.
@@ -291,36 +335,31 @@ __device__ __forceinline__ void walk_apply(uint32_t* s_tile, int stride, int nq,
     }
 }
 
-// Redo of one flagged column pair with the exact D3 sequence.  `sidx` = staged hit, `cc` = tile column of the
-// pair, `dump` = the lane's dump slot, `live` = which columns of the pair belonged to the lane's part of the tile.
-// Vote: the hot loop has already cast the pair's fast votes at slots min(fast_slot, nq + 2 + dump); they are taken
-// back (integer adds commute, also across a transient 16-bit wrap) and the exact votes are cast.  Association: the
-// hot loop skipped the pair; its exact positions are probed and published here.
+// What the out-of-line rare paths need of the tile (written once per CTA into shared memory).
 struct WalkTile {
     uint32_t* s_tile;
-    const float4* s_pair;
     int stride, c0, cand_first, cand_end;
     unsigned row_lin0;
     bool legacy;
 };
 
+// Redo of one flagged column pair with the exact D3 sequence.  `sidx` = staged hit, `cc` = tile column of the pair,
+// `live` = which columns of the pair belong to the lane's part of the tile.  The hot loop did nothing for a flagged
+// pair (no vote, no probe): both columns are decided here.
 template <int MODE, bool TILE32>
 __device__ __noinline__ void walk_redo_pair(const HoughConsts& c, float4 d, const WalkArgs& a, const WalkTile& tl,
-                                            int sidx, int cc, unsigned dump, unsigned live) {
-    const FastK fk = make_fastk(c, d);                  // recomputed here: the rare path keeps nothing of the caller's on the stack
+                                            int sidx, int cc, unsigned live) {
     const float4 hv = __ldg(a.staged + sidx);
-    const unsigned hmax = (unsigned)c.n_qpt + 2u + dump;
     const float r2 = d3_r2(hv.x, hv.y);
-    const FastHit fh = make_fasthit(fk, hv.x, hv.y, r2);
-    const float4 T = tl.s_pair[cc >> 1];
+    int ca = tl.c0 + cc;                                // absolute column of the pair (even)
+    if (ca >= c.n_phi) ca -= c.n_phi;
+    const float4 T = __ldg(reinterpret_cast<const float4*>(c.cs + ca));     // {cosA, sinA, cosB, sinB}
     unsigned long long best = 0ull;
 #pragma unroll
     for (int w = 0; w < 2; ++w) {
         if (!((live >> w) & 1u)) continue;
-        const float cs_c = w ? T.y : T.x, cs_s = w ? T.w : T.z;
-        if (MODE == WALK_VOTE)
-            tile_add_slot<TILE32>(tl.s_tile, tl.stride, cc + w, min(fast_slot(fk, fh, cs_c, cs_s), hmax), -1);
-        const int j = d3_exact_bin(hv.x, hv.y, r2, cs_c, cs_s, d.x, d.y, d.z, c.A_f, c.qmin, c.inv_wq, c.nq_f, c.model != 0);
+        const int j = d3_exact_bin(hv.x, hv.y, r2, w ? T.z : T.x, w ? T.w : T.y, d.x, d.y, d.z, c.A_f, c.qmin, c.inv_wq, c.nq_f,
+                                   c.model != 0);
         if (j >= 0)
             walk_apply<MODE, TILE32>(tl.s_tile, tl.stride, c.n_qpt, cc + w, j, tl.legacy, a.assoc_dj, a.cands, tl.cand_first,
                                      tl.cand_end, tl.c0, tl.row_lin0, best);
@@ -341,8 +380,8 @@ __device__ __noinline__ void walk_exact_window(const HoughConsts& c, float4 d, c
     if (col < 0) col += nphi;
     for (int t = 0; t < steps; ++t) {
         if (col < cols) {
-            const float4 T = tl.s_pair[col >> 1];
-            const int j = d3_exact_bin(hv.x, hv.y, r2, (col & 1) ? T.y : T.x, (col & 1) ? T.w : T.z, d.x, d.y, d.z, c.A_f, c.qmin,
+            const float2 T = __ldg(c.cs + tl.c0 + col);
+            const int j = d3_exact_bin(hv.x, hv.y, r2, T.x, T.y, d.x, d.y, d.z, c.A_f, c.qmin,
                                        c.inv_wq, c.nq_f, c.model != 0);
             if (j >= 0)
                 walk_apply<MODE, TILE32>(tl.s_tile, tl.stride, c.n_qpt, col, j, tl.legacy, a.assoc_dj, a.cands, tl.cand_first,
@@ -354,19 +393,19 @@ __device__ __noinline__ void walk_exact_window(const HoughConsts& c, float4 d, c
     if (MODE == WALK_ASSIGN && best) atomicMax(a.best_key + __float_as_int(hv.w), best);
 }
 
-// Redo queue entry (32 bits): staged index inside the event (18 bits) | pair index inside the tile (10) | dump (2) | live (2)
-__device__ __forceinline__ unsigned wq_pack(int in_event, int cc, unsigned dump, unsigned live) {
-    return (unsigned)in_event | ((unsigned)(cc >> 1) << 18) | (dump << 28) | (live << 30);
+// Redo queue entry (32 bits): staged index inside the event (18 bits) | pair index inside the tile (10) | live (2)
+__device__ __forceinline__ unsigned wq_pack(int in_event, int cc, unsigned live) {
+    return (unsigned)in_event | ((unsigned)(cc >> 1) << 18) | (live << 28);
 }
 
+// the whole warp redoes n <= 32 queued pairs, one per lane
 template <int MODE, bool TILE32>
 __device__ __forceinline__ void walk_drain(const HoughConsts& c, float4 d, const WalkArgs& a, const WalkTile& tl,
                                            const unsigned* wq, int n, int ev_begin, int lane) {
     __syncwarp();
-    for (int q = lane; q < n; q += 32) {
-        const unsigned en = wq[q];
-        walk_redo_pair<MODE, TILE32>(c, d, a, tl, ev_begin + (int)(en & 0x3ffffu), (int)((en >> 18) & 0x3ffu) * 2, (en >> 28) & 3u,
-                                     en >> 30);
+    if (lane < n) {
+        const unsigned en = wq[lane];
+        walk_redo_pair<MODE, TILE32>(c, d, a, tl, ev_begin + (int)(en & 0x3ffffu), (int)((en >> 18) & 0x3ffu) * 2, (en >> 28) & 3u);
     }
     __syncwarp();
 }
@@ -376,7 +415,7 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
     constexpr int WALK_THREADS = walk_threads(MODE), WALK_WARPS = WALK_THREADS / 32;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ WalkTile s_tl;
-    __shared__ int s_meta[2 + WALK_MAX_WARPS];          // number of batches of the tile; fill counts of the warps' redo queues
+    __shared__ int s_meta[2];                           // number of batches of the tile
     const int n_slabs = a.n_slabs, slab_cols = a.slab_cols, stride = a.stride;
     const int slab = blockIdx.x % n_slabs;
     const int k = (blockIdx.x / n_slabs) % c.n_d0;
@@ -387,13 +426,11 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
     const int nq = c.n_qpt;
     const int nc = c.n_class;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    const int n_pair_tab = slab_cols / 2 + WALK_CHUNK_PAIRS + 1;
 
-    uint32_t* s_tile; float4* s_pair; unsigned* s_wq; float4* s_cls; int4* s_seg;
+    uint32_t* s_tile; unsigned* s_wq; float4* s_cls; int4* s_seg;
     {
         unsigned char* q = smem_raw;
         s_tile = reinterpret_cast<uint32_t*>(q);  q += (walk_tile_words(slab_cols, stride, TILE32) * 4 + 15) & ~(size_t)15;
-        s_pair = reinterpret_cast<float4*>(q);    q += (size_t)n_pair_tab * 16;
         s_cls = reinterpret_cast<float4*>(q);     q += (size_t)nc * 16;              // {lo_off, bits(steps | flags), hm, -}
         s_seg = reinterpret_cast<int4*>(q);       q += ((size_t)nc * (FULLPHI ? 1 : 2) + 1) * 16;   // {first staged hit, hits, class, first batch}
         s_wq = reinterpret_cast<unsigned*>(q);                                        // [WALK_WARPS][WALK_WQ_CAP]
@@ -436,16 +473,9 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
         uint4* t4 = reinterpret_cast<uint4*>(s_tile);
         const int n4 = (int)((walk_tile_words(cols, stride, TILE32) + 3) >> 2);
         for (int x = tid; x < n4; x += WALK_THREADS) t4[x] = make_uint4(0u, 0u, 0u, 0u);
-        for (int p = tid; p < n_pair_tab; p += WALK_THREADS) {
-            int ca = c0 + 2 * p;                         // the table runs past the tile / wraps: never an out-of-range read
-            while (ca >= nphi) ca -= nphi;
-            const float2 A = __ldg(c.cs + ca), B = __ldg(c.cs + ca + 1);
-            s_pair[p] = make_float4(A.x, B.x, A.y, B.y);
-        }
         if (tid < 32) reinterpret_cast<uint32_t*>(trash_ptr)[tid] = 0u;   // read (as empty entries) by association probes
-        if (tid < WALK_MAX_WARPS) s_meta[2 + tid] = 0;                     // redo queues start empty
         if (tid == 0) {
-            s_tl.s_tile = s_tile; s_tl.s_pair = s_pair; s_tl.stride = stride; s_tl.c0 = c0; s_tl.cand_first = cand_first;
+            s_tl.s_tile = s_tile; s_tl.stride = stride; s_tl.c0 = c0; s_tl.cand_first = cand_first;
             s_tl.cand_end = cand_end; s_tl.row_lin0 = (unsigned)(k * nphi + c0) * (unsigned)nq; s_tl.legacy = legacy;
         }
     }
@@ -463,8 +493,15 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
             dr = fmaxf(dr - 1.0e-6f * rb, 0.0f);                              // den >= (r - |d0|)^2 >= dr^2
             const float S = 8.0f * fk.d0abs * L + rb * rb + fk.d0sq;
             const float inv_dr2 = fk.line ? 1.0f : 1.000001f / (dr * dr);       // line model: no denominator at all
-            const float arel = WALK_U * ((fk.line ? 0.0f : 6.0f * S * inv_dr2) + 24.0f);
-            const float elin = fk.e_lin * (L + fk.d0abs);
+            // rounding error of the w recurrence at the end of a chunk (first order, x 1.5): initial values, one rounding of
+            // w and of d per pair, d's errors integrated over the remaining pairs
+            const float lo_f = __int_as_float(w.x);
+            const float Nf = (float)min(WALK_CHUNK_PAIRS, (steps + 3) >> 1);
+            const float Th = 2.0f * c.wphi;
+            const float wmax = rb * fminf(1.0f, (fmaxf(fabsf(lo_f), fabsf(lo_f + (float)steps)) + 3.0f) * c.wphi);
+            const float Ew = 1.5f * WALK_U * (2.0f * L + 4.0f * Nf * Th * L + Nf * wmax + 0.5f * Nf * Nf * Th * rb * (1.0f + Th));
+            const float arel = WALK_U * ((fk.line ? 0.0f : 6.0f * S * inv_dr2) + 24.0f) + (fk.line ? 0.0f : 3.0f * fk.d0abs * Ew * inv_dr2);
+            const float elin = fk.e_lin * (L + fk.d0abs) + fabsf(fk.inv_wq) * Ew;
             const float m = fk.inv_A_abs * inv_dr2 * elin + arel * fk.t_max + fk.a0;
             if (m < 0.45f) hm = 0.5f - m;                                     // false for NaN / inf
         }
@@ -574,10 +611,12 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
     const unsigned tile_bytes = (unsigned)(walk_tile_words(cols, stride, TILE32) * 4);   // FULLPHI: the wrap distance
     const unsigned tile_end = tile_saddr + tile_bytes;
     const f32x2 d0cq2 = pk2(fk.d0cq, fk.d0cq), c0h2 = pk2(fk.c0h, fk.c0h);
+    const f32x2 ntd0A2 = pk2(fk.ntd0A, fk.ntd0A), nqs2 = pk2(fk.nq_s, fk.nq_s), nkap2 = pk2(-c.kappa, -c.kappa);
     const f32x2 magic2 = pk2(WALK_MAGIC, WALK_MAGIC), nmagic2 = pk2(-WALK_MAGIC, -WALK_MAGIC);
     const WalkTile& tl = s_tl;                          // what the out-of-line rare paths need of the tile (written in the prologue)
-    unsigned* wq = s_wq + warp * WALK_WQ_CAP;           // the warp's redo queue; its fill count lives in s_meta[2 + warp]
-    int* wq_cnt = s_meta + 2 + warp;
+    unsigned* wq = s_wq + warp * WALK_WQ_CAP;           // the warp's redo queue
+    int wq_n = 0;                                       // its fill: warp-uniform, kept in a register
+    const unsigned lt = (1u << lane) - 1u;
     const bool wq_ok = ev_hits < (1 << 18) && slab_cols <= 2048;          // entries fit 32 bits (else: redo on the spot)
     const unsigned dump = (unsigned)(lane & (WALK_DUMP - 1));
     int seg = 0;
@@ -599,8 +638,7 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
         const float r2 = d3_r2(x, y);
         int i_lo = (int)ceilf(hv.z + cw.x);
         if (i_lo < 0) i_lo += nphi;
-        if (i_lo >= nphi) i_lo -= nphi;
-        if (!(i_lo >= 0 && i_lo < nphi)) i_lo = 0;
+        if (i_lo >= nphi) i_lo -= nphi;                  // (u is finite and in [-1/2, n_phi - 1/2): stage.cu; |lo| < n_phi)
 
         // dilated association: (entry >> 1) above ~column (equal votes and |dj| in two columns: the smaller linear
         // bin wins, D8)
@@ -611,7 +649,7 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
             if (active) walk_exact_window<MODE, TILE32>(c, d, a, tl, sidx, i_lo, steps, cols);
         } else {
             // ---- fast path: the lane's window, two columns at a time ----
-            const FastHit fh = make_fasthit(fk, x, y, r2);
+            const float r2Ak = __fmaf_rn(r2, fk.A_f, fk.d0sqA);
             // first column (even, tile-relative) and number of column pairs of the lane's part of the tile
             int start, my_n, np_total;
             if (FULLPHI) {
@@ -634,8 +672,7 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
             // lanes without work: every evaluation lands in guard slot 0 and none is ever "uncertain"
             const unsigned hmax_l = active ? (unsigned)nq + 2u + dump : 0u;
             const float hm_l = active ? hm_c : __int_as_float(0x7f800000);
-            const f32x2 r2Ak2 = pk2(fh.r2Ak, fh.r2Ak);
-            const f32x2 gy2 = pk2(fh.gy, fh.gy), gx2 = pk2(fh.gx, fh.gx), ny2 = pk2(fh.ny, fh.ny), nx2 = pk2(fh.nx, fh.nx);
+            const f32x2 r2Ak2 = pk2(r2Ak, r2Ak);
             int col = start;
             int rem = my_n;                              // columns left in the lane's part (slab tiles)
             for (int p0 = 0; p0 < np_total; p0 += WALK_CHUNK_PAIRS) {
@@ -643,39 +680,38 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
                 if (FULLPHI && col >= nphi) col -= nphi;
                 if (!FULLPHI && rem <= 0) col = 0;       // a finished lane idles at the first pair (table bounds)
                 const int col_chunk = col, rem_chunk = rem;
-                const float4* pp = s_pair + (col >> 1);
+                WRec wr = wrec_init(c, x, y, c0 + col);   // (w, d) of the chunk's first pair, from the cos/sin table
                 unsigned rowaddr = tile_saddr + (TILE32 ? (unsigned)col * stride4 : (unsigned)(col >> 1) * stride4);
                 const int wrap_t = FULLPHI ? ((nphi - col) >> 1) : 0x7fffffff;   // pair of the chunk at which the lane wraps
                 unsigned cinv = EntryT<TILE32>::CINV0 - (unsigned)col;   // association: ~(running tile column of the pair)
                 unsigned slowmask = 0u;                  // bit t: pair t of the chunk is uncertain
-                // One column pair.  The vote is unconditional: slot min(h, nq + 2 + dump) of the column's row (results
-                // outside [-1, nq] land in a dump slot).  A pair with an uncertain column is flagged; the redo takes the
-                // pair's two fast votes back (fast_slot reproduces them) and casts the exact ones.
+                // One column pair.  Slot min(h, nq + 2 + dump) of the column's row (results outside [-1, nq] land in a dump
+                // slot) -- no range test.  A pair with an uncertain column is flagged and does nothing here (predicated
+                // votes / no probe): the redo decides both of its columns with the exact D3 sequence.
                 auto pair_step = [&](auto wrap_c, int t, unsigned bit) {
                     constexpr bool WRAP = decltype(wrap_c)::value;
-                    const float4 T = *pp++;              // {cosA, cosB, sinA, sinB}
-                    const f32x2 C2 = pk2(T.x, T.y), S2 = pk2(T.z, T.w);
-                    const f32x2 g2 = fma2(gx2, S2, fma2(gy2, C2, r2Ak2));
-                    const f32x2 n2 = fma2(nx2, S2, fma2(ny2, C2, d0cq2));
-                    float gA, gB;
-                    upk2(g2, gA, gB);
-                    const f32x2 th2 = fma2(n2, pk2(rcp_approx(gA), rcp_approx(gB)), c0h2);   // t~ - 1/2
+                    const f32x2 th2 = wrec_th(wr.w2, ntd0A2, r2Ak2, nqs2, d0cq2, c0h2);       // t~ - 1/2
+                    wrec_step(wr, nkap2);                                                     // the next pair's w
                     const f32x2 yb2 = add2(th2, magic2);
                     const f32x2 dl2 = sub2(th2, add2(yb2, nmagic2));                          // (t~ - 1/2) - J
                     float ybA, ybB, dA, dB;
                     upk2(yb2, ybA, ybB);
                     upk2(dl2, dA, dB);
-                    const unsigned hA = min((unsigned)(__float_as_int(ybA) - (WALK_MAGIC_BITS - 1)), hmax_l);   // slot J + 1
-                    const unsigned hB = min((unsigned)(__float_as_int(ybB) - (WALK_MAGIC_BITS - 1)), hmax_l);
-                    unsigned adA = addr_w(rowaddr, hA), adB = addr_w(TILE32 ? rowaddr + stride4 : rowaddr, hB);
                     // uncertain: t~ within m of a bin edge, J <= t_D3 < J + 1 not proven (NaN never compares true)
                     bool uns;
                     if (FULLPHI) {
                         uns = fmaxf(fabsf(dA), fabsf(dB)) >= hm_l;
                     } else {                             // slab tiles: the lane's own part of the tile only
-                        const bool liveA = rem > 0, liveB = rem > 1;
-                        adA = liveA ? adA : trash_saddr;  adB = liveB ? adB : trash_saddr;   // rows past the tile: scratch word
-                        uns = (fabsf(dA) >= hm_l && liveA) || (fabsf(dB) >= hm_l && liveB);
+                        uns = (fabsf(dA) >= hm_l && rem > 0) || (fabsf(dB) >= hm_l && rem > 1);
+                    }
+                    // a flagged pair is sent to guard slot 0 of its rows (never flushed, empty in association tiles): the
+                    // redo decides both of its columns
+                    const unsigned hcap = (MODE == WALK_VOTE && uns) ? 0u : hmax_l;     // (association: the probe result is dropped instead)
+                    const unsigned hA = min((unsigned)(__float_as_int(ybA) - (WALK_MAGIC_BITS - 1)), hcap);   // slot J + 1
+                    const unsigned hB = min((unsigned)(__float_as_int(ybB) - (WALK_MAGIC_BITS - 1)), hcap);
+                    unsigned adA = addr_w(rowaddr, hA), adB = addr_w(TILE32 ? rowaddr + stride4 : rowaddr, hB);
+                    if (!FULLPHI) {
+                        adA = rem > 0 ? adA : trash_saddr;  adB = rem > 1 ? adB : trash_saddr;   // rows past the tile: scratch word
                         rem -= 2;
                     }
                     if (MODE == WALK_VOTE) {
@@ -722,50 +758,50 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
                 if (FULLPHI && __any_sync(0xffffffffu, wrap_t < np)) run_chunk(std::true_type{});
                 else run_chunk(std::false_type{});
                 col += 2 * np;                           // FULLPHI: reduced modulo n_phi at the top of the next chunk
-                // uncertain pairs of the chunk -> the warp's redo queue (a slot claimed with one shared atomic), drained 32
-                // at a time by the whole warp; a full queue or entries that do not fit 32 bits: redone on the spot
-                while (slowmask != 0u) {
-                    const int t = __ffs(slowmask) - 1;
-                    slowmask &= slowmask - 1u;
-                    int cc = col_chunk + 2 * t;
-                    if (FULLPHI && cc >= nphi) cc -= nphi;
-                    unsigned live = 3u;
-                    if (!FULLPHI) live = (rem_chunk - 2 * t > 0 ? 1u : 0u) | (rem_chunk - 2 * t > 1 ? 2u : 0u);
-                    const int slot = wq_ok ? atomicAdd(wq_cnt, 1) : WALK_WQ_CAP;
-                    if (slot < WALK_WQ_CAP) wq[slot] = wq_pack(sidx - ev_begin, cc, dump, live);
-                    else walk_redo_pair<MODE, TILE32>(c, d, a, tl, sidx, cc, dump, live);
+                // uncertain pairs of the chunk -> the warp's redo queue, one round per set bit: slots dealt by ballot, the
+                // queue drained 32 entries at a time by the whole warp; entries that do not fit 32 bits: redone on the spot
+                // (a prefix sum over the lanes' flag counts was measured slower than these rounds)
+                unsigned any = __ballot_sync(0xffffffffu, slowmask != 0u);
+                while (any != 0u) {
+                    if (slowmask != 0u) {
+                        const int t = __ffs(slowmask) - 1;
+                        slowmask &= slowmask - 1u;
+                        int cc = col_chunk + 2 * t;
+                        if (FULLPHI && cc >= nphi) cc -= nphi;
+                        unsigned live = 3u;
+                        if (!FULLPHI) live = (rem_chunk - 2 * t > 0 ? 1u : 0u) | (rem_chunk - 2 * t > 1 ? 2u : 0u);
+                        if (wq_ok) wq[wq_n + __popc(any & lt)] = wq_pack(sidx - ev_begin, cc, live);
+                        else walk_redo_pair<MODE, TILE32>(c, d, a, tl, sidx, cc, live);
+                    }
+                    if (wq_ok) {
+                        wq_n += __popc(any);
+                        if (wq_n >= 32) {
+                            wq_n -= 32;
+                            walk_drain<MODE, TILE32>(c, d, a, tl, wq + wq_n, 32, ev_begin, lane);
+                        }
+                    }
+                    any = __ballot_sync(0xffffffffu, slowmask != 0u);
                 }
             }
         }
         if (MODE == WALK_ASSIGN) {
             const unsigned eh = EntryT<TILE32>::ent_hi(bestp);          // entry >> 1: votes + 1 above (15 - |dj|)
             if (eh >> 4) {
-                // the winning column's slot again (an unflagged pair: the fast slot IS the D3 bin), then the full entry
+                // the winning column's bin again (an unflagged pair: the fast slot IS the D3 bin), then the full entry
                 const float4 hw = hv;
                 const int bcol = EntryT<TILE32>::col_of(bestp);
-                const float4 T = s_pair[bcol >> 1];
-                const FastHit fh = make_fasthit(fk, hw.x, hw.y, r2);
-                const int J = (int)fast_slot(fk, fh, (bcol & 1) ? T.y : T.x, (bcol & 1) ? T.w : T.z) - 1;
+                const float2 T = __ldg(c.cs + c0 + bcol);
+                int J;
+                if (!fast_bin_direct(fk, hw.x, hw.y, __fmaf_rn(r2, fk.A_f, fk.d0sqA), T, hm_c, J))
+                    J = d3_exact_bin(hw.x, hw.y, r2, T.x, T.y, d.x, d.y, d.z, c.A_f, c.qmin, c.inv_wq, c.nq_f, c.model != 0);
                 const unsigned ent = tile_entry<TILE32>(s_tile, stride, bcol, J);
                 const int adj = 15 - (int)((ent >> 1) & 15u);
                 const int jc = J + ((ent & 1u) ? -adj : adj);
                 atomicMax(a.best_key + __float_as_int(hw.w), walk_key((ent >> 5) - 1u, adj, row_lin0 + (unsigned)(bcol * nq + jc)));
             }
         }
-        // the queue is drained when it may not take another batch's worth of entries
-        __syncwarp();
-        const int wq_n = *reinterpret_cast<volatile int*>(wq_cnt);
-        if (wq_n > WALK_WQ_CAP - 32) {
-            walk_drain<MODE, TILE32>(c, d, a, tl, wq, min(wq_n, WALK_WQ_CAP), ev_begin, lane);
-            if (lane == 0) *wq_cnt = 0;
-            __syncwarp();
-        }
     }
-    {
-        __syncwarp();
-        const int wq_n = *reinterpret_cast<volatile int*>(wq_cnt);
-        if (wq_n > 0) walk_drain<MODE, TILE32>(c, d, a, tl, wq, min(wq_n, WALK_WQ_CAP), ev_begin, lane);
-    }
+    if (wq_n > 0) walk_drain<MODE, TILE32>(c, d, a, tl, wq, wq_n, ev_begin, lane);
     if (MODE == WALK_ASSIGN) return;
     __syncthreads();
 
