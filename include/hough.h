@@ -102,7 +102,8 @@ int hough_vote(hough_plan* plan, const float* d_hits_xy, int32_t n_hits, const i
  * q/pT and d0 clipped), a > b for neighbours at lexicographically smaller offset (dk,di,dj) and a >= b for
  * the others.  Records are written in ascending (event, k, i, j) order for global rank < capacity;
  * d_cand_offsets[n_events + 1] always receives the exclusive scan of the TRUE per-event counts (overflow is
- * not an error: compare d_cand_offsets[n_events] with capacity).  d_cands may be NULL when capacity == 0. */
+ * not an error: compare d_cand_offsets[n_events] with capacity).  d_cands may be NULL when capacity == 0.
+ * Limit: at most 65535 events per call (one grid row per event); more returns UNSUPPORTED -- split the batch. */
 int hough_find_peaks(hough_plan* plan, const void* d_accum, int32_t n_events, int32_t threshold,
                      hough_candidate* d_cands, int32_t capacity, int32_t* d_cand_offsets, void* cuda_stream);
 
@@ -146,7 +147,7 @@ int hough_reassign_hits(hough_plan* plan, const float* d_hits_xy, int32_t n_hits
  * OVERWRITES d_vertex_accum: int32 [n_events][n_phi][n_r], i.e. the layout of an accumulator with binning
  * {n_phi, n_qpt = n_r, n_d0 = 1, qpt range [0, r_max), int32}: its peaks (hough_find_peaks on such a plan) are the vertex
  * candidates (phi0 field = vertex azimuth, qpt field = vertex radius in cm).
- * Errors: INVALID_ARG (null pointers, plan not of the line model, bad sizes), CUDA. */
+ * Errors: INVALID_ARG (null pointers, plan not of the line model, bad sizes, more than 65535 events per call), CUDA. */
 int hough_vertex_vote(hough_plan* plan, const hough_candidate* d_cands, const int32_t* d_cand_offsets, int32_t n_events,
                       int32_t capacity, const uint8_t* d_cand_keep, float d0_abs_min, int32_t n_r, float r_max,
                       int32_t* d_vertex_accum, void* cuda_stream);
@@ -225,7 +226,10 @@ int hough_window_table(const hough_binning* binning, const hough_geometry* geome
  *   1 = shared-memory atomicAdd(u32), random addresses in a 64 KB tile
  *   2 = shared-memory load+add+store (non-atomic RMW), conflict-free
  *   3 = global red.add.u32 to random addresses in a region of `region_bytes` (L2- or HBM-resident)
- *   4 = fp32 issue rate of the D3 vote sequence (no memory), evaluations per second            */
+ *   4 = fp32 issue rate of the D3 vote sequence (no memory), evaluations per second
+ *   5 = shared-memory atomicAdd(u32), every warp adds to random bins of one 128-bin row (same-address collisions
+ *       included): the address pattern closest to the vote walk's
+ * Errors: INVALID_ARG (unknown kind, iters <= 0, NULL ops_per_s), CUDA. */
 int hough_microbench(int32_t kind, size_t region_bytes, int32_t iters, double* ops_per_s, void* cuda_stream);
 
 /* Process-wide number of CUDA kernel launches this library has issued so far (memsets/copies excluded). */

@@ -39,7 +39,11 @@ def _stale(target: str, deps) -> bool:
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, checks: bool = False) -> str:
+    """checks=True: the self-check build (-DHOUGH_CHECKS=1, device asserts; see csrc/common.cuh) into
+    libhough_b200_checks.so -- a debugging artefact, never loaded by the binding."""
+    if checks:
+        return _build_checks()
     os.makedirs(OBJ_DIR, exist_ok=True)
     headers = glob.glob(os.path.join(CSRC, "*.cuh")) + [os.path.join(HERE, "..", "include", "hough.h")]
     objs = []
@@ -70,5 +74,24 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return LIB
 
 
+def _build_checks() -> str:
+    out_dir = os.path.join(HERE, "build", "checks")
+    os.makedirs(out_dir, exist_ok=True)
+    lib = os.path.join(HERE, "libhough_b200_checks.so")
+    objs, procs = [], []
+    for src in sources():
+        obj = os.path.join(out_dir, os.path.basename(src)[:-3] + ".o")
+        objs.append(obj)
+        flags = [f for f in NVCC_FLAGS if f not in ("-Xptxas", "-v")]
+        procs.append((src, subprocess.Popen([_nvcc(), *flags, "-DHOUGH_CHECKS=1", "-c", src, "-o", obj], stdout=subprocess.PIPE,
+                                            stderr=subprocess.STDOUT, text=True)))
+    for src, p in procs:
+        out, _ = p.communicate()
+        if p.returncode != 0:
+            raise RuntimeError(f"nvcc failed: {src}\n{out}")
+    subprocess.run([_nvcc(), "-shared", "-o", lib, *objs, "-gencode", "arch=compute_100a,code=sm_100a"], check=True)
+    return lib
+
+
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv, checks="--checks" in sys.argv))

@@ -21,6 +21,17 @@
         }                                            \
     } while (0)
 
+// Self-check build (-DHOUGH_CHECKS=1, `python -m paper_1311_2769_b200.build --checks`): device-side asserts on every
+// shared-memory address, queue slot and table index the walk and the peak ring compute.  compute-sanitizer is not
+// available on the GPU pool this was developed on; the parity suite is run once against this build instead
+// (profiles/r2_checks.md).  Compiled out otherwise.
+#ifdef HOUGH_CHECKS
+#include <cassert>
+#define HOUGH_CHECK(cond) assert(cond)
+#else
+#define HOUGH_CHECK(cond) ((void)0)
+#endif
+
 void hough_set_last_cuda_error(cudaError_t e, const char* what);
 void hough_count_launches(int n);   // process-wide count of kernel launches issued by the library
 
@@ -46,6 +57,7 @@ struct HoughConsts {
 };
 
 constexpr int HOUGH_MAX_CLASSES = 255;
+constexpr int HOUGH_MAX_DEVICES = 64;       // per-device caches of kernel attributes (a device index beyond it: set every call)
 constexpr int HOUGH_SECTORS_MIN = 32, HOUGH_SECTORS_MAX = 1024;   // phi sectors of the staging sort: n_phi clamped to this range
 
 struct HoughWindows {             // host copy of the class / window tables

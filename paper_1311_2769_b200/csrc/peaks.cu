@@ -768,6 +768,7 @@ __global__ void __launch_bounds__(256, 3) peak_stream16_kernel(HoughConsts c, co
             else ps_commit();
         }
         const unsigned short* st = s_base + (size_t)(it % PS_STAGES) * stage_halfwords + rl * nq;
+        HOUGH_CHECK((size_t)((it % PS_STAGES) * stage_halfwords + (rl + 2) * nq + j0 + 8) * 2 <= (size_t)PS_STAGES * (R + 2) * nq * 2);
         const Row6 Nm = ps_load_row(st, j0, nq);
         const Row6 N0 = ps_load_row(st + nq, j0, nq);
         const Row6 Np = ps_load_row(st + 2 * nq, j0, nq);
@@ -796,6 +797,7 @@ __global__ void __launch_bounds__(256, 3) peak_stream16_kernel(HoughConsts c, co
             flags |= (ge_hi && !le_hi ? 1u : 0u) << (2 * (w - 1) + 1);
         }
         const size_t bin0 = ((size_t)k * nphi + i) * nq + j0;
+        HOUGH_CHECK(k >= 0 && k < nd && i >= 0 && i < nphi && bin0 + 8 <= (size_t)c.bins_per_event);
         mask_bytes[bin0 >> 3] = (unsigned char)flags;
         const int cnt = __reduce_add_sync(0xffffffffu, __popc(flags));     // a warp = 256 consecutive bins of one peak block
         if ((tid & 31) == 0 && cnt)
@@ -846,10 +848,11 @@ extern "C" int hough_find_peaks(hough_plan* p, const void* d_accum, int32_t n_ev
         if (stream16) {
             const int R = 256 / cpr16;
             const size_t smem = (size_t)PS_STAGES * (R + 2) * p->c.n_qpt * 2;
-            static bool configured = false;
-            if (!configured) {
+            static bool configured[HOUGH_MAX_DEVICES] = {};          // per device: the attribute belongs to the device's copy of the function
+            const int dev = p->device >= 0 && p->device < HOUGH_MAX_DEVICES ? p->device : 0;
+            if (!configured[dev] || p->device >= HOUGH_MAX_DEVICES) {
                 HOUGH_CUDA_TRY(cudaFuncSetAttribute(peak_stream16_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 64 * 1024));
-                configured = true;
+                configured[dev] = true;
             }
             const long long nb = (long long)(p->c.n_phi / R) * n_seg * n_events;
             if (nb > 0x7fffffffLL) return HOUGH_ERR_UNSUPPORTED;
@@ -865,8 +868,10 @@ extern "C" int hough_find_peaks(hough_plan* p, const void* d_accum, int32_t n_ev
             peak_kwalk_kernel<false><<<(unsigned)nblk, 256, 0, st>>>(p->c, d_accum, threshold, n_events, kseg, n_seg, bpe,
                                                                      p->d_mask, p->d_peak_block_cnt);
     } else if (tiled) {
-        static bool smem_configured = false;        // the tiled path never needs more than 100 KB
-        if (!smem_configured) {
+        static bool smem_configured_dev[HOUGH_MAX_DEVICES] = {};     // per device; the tiled path never needs more than 100 KB
+        const int dev = p->device >= 0 && p->device < HOUGH_MAX_DEVICES ? p->device : 0;
+        bool& smem_configured = smem_configured_dev[dev];
+        if (!smem_configured || p->device >= HOUGH_MAX_DEVICES) {
             const int cap = 100 * 1024;
             HOUGH_CUDA_TRY(cudaFuncSetAttribute(peak_tile_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap));
             HOUGH_CUDA_TRY(cudaFuncSetAttribute(peak_tile_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, cap));

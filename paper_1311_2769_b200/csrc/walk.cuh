@@ -211,6 +211,7 @@ __device__ __forceinline__ FastK make_fastk(const HoughConsts& c, float4 d) {
 // for bit): explicit PTX operations, no contraction.
 struct WRec { f32x2 w2, d2; };
 __device__ __forceinline__ WRec wrec_init(const HoughConsts& c, float x, float y, int ca) {      // ca: absolute column, even
+    HOUGH_CHECK(ca >= 0 && ca + 1 < c.n_phi && (ca & 1) == 0);
     const float4 T = __ldg(reinterpret_cast<const float4*>(c.cs + ca));                          // {cosA, sinA, cosB, sinB}
     const float2 M = __ldg(c.cs + ca - 1);                                                        // the column before A (cs[-1] = cs[n_phi - 1])
     const float wA = __fmaf_rn(y, T.x, -__fmul_rn(x, T.y));
@@ -290,6 +291,7 @@ template <> struct EntryT<true> {                    // 32-bit entries: 27 bits 
 // ---- tile accessors by (tile column, q/pT bin J in [0, nq)) ----
 template <bool TILE32>
 __device__ __forceinline__ void tile_vote(uint32_t* s_tile, int stride, int col, int J) {
+    HOUGH_CHECK(col >= 0 && J >= 0 && J + 1 < stride);
     if (TILE32) atomicAdd(s_tile + col * stride + J + 1, 1u);
     else atomicAdd(s_tile + (col >> 1) * stride + J + 1, 1u << (16 * (col & 1)));
 }
@@ -301,6 +303,7 @@ __device__ __forceinline__ void tile_add_slot(uint32_t* s_tile, int stride, int 
 }
 template <bool TILE32>
 __device__ __forceinline__ unsigned tile_entry(const uint32_t* s_tile, int stride, int col, int J) {
+    HOUGH_CHECK(col >= 0 && J >= 0 && J + 1 < stride);
     if (TILE32) return s_tile[col * stride + J + 1];
     return (unsigned)reinterpret_cast<const unsigned short*>(s_tile)[(((col >> 1) * stride + J + 1) << 1) + (col & 1)];
 }
@@ -353,6 +356,7 @@ __device__ __noinline__ void walk_redo_pair(const HoughConsts& c, float4 d, cons
     const float r2 = d3_r2(hv.x, hv.y);
     int ca = tl.c0 + cc;                                // absolute column of the pair (even)
     if (ca >= c.n_phi) ca -= c.n_phi;
+    HOUGH_CHECK(ca >= 0 && ca + 1 < c.n_phi && (ca & 1) == 0 && cc >= 0);
     const float4 T = __ldg(reinterpret_cast<const float4*>(c.cs + ca));     // {cosA, sinA, cosB, sinB}
     unsigned long long best = 0ull;
 #pragma unroll
@@ -610,6 +614,8 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
     const unsigned row_lin0 = (unsigned)(k * nphi + c0) * (unsigned)nq;   // linear bin of (k, c0, 0) inside the event
     const unsigned tile_bytes = (unsigned)(walk_tile_words(cols, stride, TILE32) * 4);   // FULLPHI: the wrap distance
     const unsigned tile_end = tile_saddr + tile_bytes;
+    const unsigned tile_alloc_end = tile_saddr + (unsigned)(walk_tile_words(slab_cols, stride, TILE32) * 4);   // (HOUGH_CHECK only)
+    (void)tile_alloc_end;
     const f32x2 d0cq2 = pk2(fk.d0cq, fk.d0cq), c0h2 = pk2(fk.c0h, fk.c0h);
     const f32x2 ntd0A2 = pk2(fk.ntd0A, fk.ntd0A), nqs2 = pk2(fk.nq_s, fk.nq_s), nkap2 = pk2(-c.kappa, -c.kappa);
     const f32x2 magic2 = pk2(WALK_MAGIC, WALK_MAGIC), nmagic2 = pk2(-WALK_MAGIC, -WALK_MAGIC);
@@ -622,7 +628,9 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
     int seg = 0;
     for (int bt = warp; bt < n_batches; bt += WALK_WARPS) {
         while (s_seg[seg + 1].w <= bt) ++seg;            // last segment with first batch <= bt (the sentinel ends the search)
+        HOUGH_CHECK(seg >= 0 && seg < nc * (FULLPHI ? 1 : 2));
         const int4 sg = s_seg[seg];                      // {first staged hit, hits, class, first batch}
+        HOUGH_CHECK(sg.z >= 0 && sg.z < nc && sg.x >= 0 && sg.x + sg.y <= ev_hits);
         // A batch = 32 consecutive staged hits of the segment (neighbours in azimuth: their cos/sin pairs sit in adjacent
         // shared-memory words).  Dealing the hits of a segment to the lanes 4 or ~1 tile rows apart was measured and is
         // slower (profiles/r2_walk.md: bank conflicts of the regular spacing outweigh the same-word votes it removes).
@@ -714,6 +722,8 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
                         adA = rem > 0 ? adA : trash_saddr;  adB = rem > 1 ? adB : trash_saddr;   // rows past the tile: scratch word
                         rem -= 2;
                     }
+                    HOUGH_CHECK((adA >= tile_saddr && adA + 4u <= tile_alloc_end) || adA == trash_saddr);
+                    HOUGH_CHECK((adB >= tile_saddr && adB + 4u <= tile_alloc_end) || adB == trash_saddr);
                     if (MODE == WALK_VOTE) {
                         red_shared(adA, 1u);
                         red_shared(adB, TILE32 ? 1u : 65536u);
@@ -770,6 +780,8 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
                         if (FULLPHI && cc >= nphi) cc -= nphi;
                         unsigned live = 3u;
                         if (!FULLPHI) live = (rem_chunk - 2 * t > 0 ? 1u : 0u) | (rem_chunk - 2 * t > 1 ? 2u : 0u);
+                        HOUGH_CHECK(!wq_ok || (wq_n >= 0 && wq_n + __popc(any & lt) < WALK_WQ_CAP));
+                        HOUGH_CHECK(cc >= 0 && cc < slab_cols && (cc & 1) == 0);
                         if (wq_ok) wq[wq_n + __popc(any & lt)] = wq_pack(sidx - ev_begin, cc, live);
                         else walk_redo_pair<MODE, TILE32>(c, d, a, tl, sidx, cc, live);
                     }
@@ -859,10 +871,13 @@ template <int MODE, bool TILE32, bool OUT16, bool FULLPHI>
 int walk_launch(hough_plan* p, int n_events, WalkArgs a, cudaStream_t st) {
     const size_t smem = walk_smem_bytes(a.slab_cols, a.stride, TILE32, p->c.n_class, FULLPHI);
     auto kern = walk_kernel<MODE, TILE32, OUT16, FULLPHI>;
-    static size_t smem_configured = 0;              // per instantiation; raised only when a call needs more
-    if (smem > smem_configured) {
+    // opt-in shared memory is a per-device function attribute: one cached size per (instantiation, device), raised
+    // only when a call needs more (benign if two host threads race: both set a sufficient value)
+    static size_t smem_configured[HOUGH_MAX_DEVICES] = {};
+    const int dev = p->device >= 0 && p->device < HOUGH_MAX_DEVICES ? p->device : 0;
+    if (smem > smem_configured[dev] || p->device >= HOUGH_MAX_DEVICES) {
         HOUGH_CUDA_TRY(cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-        smem_configured = smem;
+        smem_configured[dev] = smem;
     }
     const long long grid = (long long)a.n_slabs * p->c.n_d0 * n_events;
     if (grid > 0x7fffffffLL) return HOUGH_ERR_UNSUPPORTED;
