@@ -292,6 +292,12 @@ class DeviceRun:
                                                       w.min_hits, self.h2c[:max(h1 - h0, 1)], self.nh, self.keep))
         self.totals[t:t + 1].copy_(self.cand_off[n_ev:n_ev + 1])
 
+    def reassign_tile(self, t):
+        """hough_reassign_hits (D12) on tile t, after step_tile(t) left its D9 outputs on the device."""
+        (e0, e1, h0, h1) = self.tiles[t]
+        self.plan.reassign_hits(self.d_hits[h0:h1], self.d_offs[t], self.cands, self.cand_off, self.cap, self.w.assoc_dj, 2,
+                                self.h2c[:max(h1 - h0, 1)], self.nh, self.keep)
+
     def step(self, call_events=None):
         """One pass over all tiles on the current stream."""
         for t in range(len(self.tiles)):
@@ -541,6 +547,30 @@ def run_ours(args, rank, world, local_rank):
     except Exception as exc:                              # noqa: BLE001 -- report, do not hide
         print(f"bench.py: fit stage failed: {exc}", file=sys.stderr)
 
+    # re-assignment round of the stranded hits (PAPER.md:33 / :29; D12), first tile, outside the timed step
+    reassign_info = None
+    try:
+        (e0, e1, h0, h1) = run.tiles[0]
+        n_ev = e1 - e0
+        rt = []
+        gained = 0
+        for it in range(8):
+            run.step_tile(0)                            # fresh D9 state of the first tile
+            before = int((run.h2c[:h1 - h0] >= 0).sum().item()) if it == 7 else 0
+            a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+            a.record()
+            run.reassign_tile(0)
+            b.record(); b.synchronize()
+            if it >= 2:
+                rt.append(a.elapsed_time(b))
+            if it == 7:
+                gained = int((run.h2c[:h1 - h0] >= 0).sum().item()) - before
+        reassign_info = {"ms_median": statistics.median(rt), "events": n_ev, "hits_recovered": gained,
+                         "api": "hough_reassign_hits on the first tile (D12, candidate-centric over the kept candidates), "
+                                "not part of the timed step"}
+    except Exception as exc:                              # noqa: BLE001 -- report, do not hide
+        print(f"bench.py: reassign stage failed: {exc}", file=sys.stderr)
+
     n_ref = oracle_events_for_seconds(w, args.cpu_seconds)
     o_votes, o_events, o_secs = oracle_sample(w, batch, n_ref)
     cpu = {"value": o_votes / o_secs, "unit": UNIT, "cores": 1, "kind": "oracle",
@@ -577,6 +607,8 @@ def run_ours(args, rank, world, local_rank):
         line["vertex"] = vertex
     if fit_info is not None:
         line["fit"] = fit_info
+    if reassign_info is not None:
+        line["reassign"] = reassign_info
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()
@@ -639,12 +671,32 @@ def run_sweep(args):
                 gtimes.append(a.elapsed_time(b))
         except Exception as exc:                          # noqa: BLE001 -- report, do not hide
             print(f"bench.py: graph capture failed: {exc}", file=sys.stderr)
+        # the same event through hough_event_run: one launch of a thread-block cluster (csrc/event.cu)
+        etimes = []
+        launches_event = None
+        try:
+            from paper_1311_2769_b200 import kernel_launches
+            for _ in range(5):
+                plan.event_run(d_hits, d_off, accum, w.threshold, cands, cap, coff, w.assoc_dj, w.min_hits, h2c, nh, keep)
+            torch.cuda.synchronize()
+            l0 = kernel_launches()
+            for _ in range(args.sweep_reps):
+                a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+                a.record()
+                plan.event_run(d_hits, d_off, accum, w.threshold, cands, cap, coff, w.assoc_dj, w.min_hits, h2c, nh, keep)
+                b.record(); b.synchronize()
+                etimes.append(a.elapsed_time(b))
+            launches_event = (kernel_launches() - l0) / float(args.sweep_reps)
+        except Exception as exc:                          # noqa: BLE001 -- report, do not hide
+            print(f"bench.py: hough_event_run failed: {exc}", file=sys.stderr)
         votes = int(accum.to(torch.int64).sum().item())
         n_c = int(coff[1].item())
         kept = int(keep[:min(n_c, cap)].sum().item())
         print(json.dumps({"sweep": "paper_toy_2d", "cite": "P:L39, P:L55", "n_tracks": n, "hits": batch.n_hits, "votes": votes,
                           "peaks": n_c, "kept": kept, "ms_median": statistics.median(times), "ms_min": min(times),
                           "ms_graph_median": statistics.median(gtimes) if gtimes else None,
+                          "ms_event_run_median": statistics.median(etimes) if etimes else None,
+                          "ms_event_run_min": min(etimes) if etimes else None, "event_run_launches": launches_event,
                           "reps": args.sweep_reps}), flush=True)
         plan.close()
 

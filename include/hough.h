@@ -119,6 +119,21 @@ int hough_assign_hits(hough_plan* plan, const float* d_hits_xy, int32_t n_hits, 
                       int32_t capacity, int32_t assoc_dj, int32_t min_hits, int32_t* d_hit_to_cand,
                       int32_t* d_cand_nhits, uint8_t* d_cand_keep, void* cuda_stream);
 
+/* hough_event_run (P:L37 vote -> local maxima -> further computations, for ONE event; "the two-parameter space";
+ * P:L55 / Fig. 2: time per event as a function of the number of tracks).
+ * Exactly hough_vote + hough_find_peaks + hough_assign_hits for a single event (n_events == 1, d_event_offsets = {0,
+ * n_hits} on the device), with the same outputs bit for bit: d_accum (one accumulator, overwritten), d_cands /
+ * d_cand_offsets[2], d_hit_to_cand, d_cand_nhits, d_cand_keep (see those calls for layouts and the capacity rule).
+ * For a two-parameter space (n_d0 == 1) whose 16-bit tile fits the shared memory of at most 8 SMs and an event of at
+ * most 2560 hits (about the measured break-even with the general path), the whole path runs in ONE launch of a thread-block cluster (accumulator slab in shared memory, steps
+ * separated by cluster barriers) -- what a latency-bound small event needs; every other case runs the three calls
+ * (plan option "event_general" = 1 forces that).  Enqueues on cuda_stream and returns; graph-capturable.
+ * Errors: INVALID_ARG (null / misaligned pointers, sizes, assoc_dj > 15), UNSUPPORTED, CUDA. */
+int hough_event_run(hough_plan* plan, const float* d_hits_xy, int32_t n_hits, const int32_t* d_event_offsets,
+                    void* d_accum, int32_t threshold, hough_candidate* d_cands, int32_t capacity,
+                    int32_t* d_cand_offsets, int32_t assoc_dj, int32_t min_hits, int32_t* d_hit_to_cand,
+                    int32_t* d_cand_nhits, uint8_t* d_cand_keep, void* cuda_stream);
+
 /* hough_reassign_hits ("cleaned to select only the best candidate ... and eliminate duplicate tracks"; "hits in
  * these tracks are then removed, allowing later iterations"; D12 re-assignment rounds).
  * Call after hough_assign_hits with the same hits, offsets, candidates, capacity and assoc_dj, and with ITS outputs in

@@ -40,7 +40,7 @@ class hough_geometry(C.Structure):
 
 
 EXPORTS = ["hough_plan_create", "hough_plan_destroy", "hough_accum_bytes", "hough_vote", "hough_find_peaks",
-           "hough_assign_hits", "hough_reassign_hits", "hough_vertex_vote", "hough_fit_circles", "hough_plan_set_option", "hough_pipeline_create", "hough_pipeline_destroy",
+           "hough_assign_hits", "hough_reassign_hits", "hough_event_run", "hough_vertex_vote", "hough_fit_circles", "hough_plan_set_option", "hough_pipeline_create", "hough_pipeline_destroy",
            "hough_pipeline_run_host", "hough_pipeline_set_option", "hough_window_table", "hough_microbench", "hough_kernel_launches", "hough_status_string",
            "hough_version"]
 
@@ -69,6 +69,8 @@ def load_library() -> C.CDLL:
     lib.hough_find_peaks.argtypes = [P, P, I, I, P, I, P, P]
     lib.hough_assign_hits.restype = C.c_int
     lib.hough_assign_hits.argtypes = [P, P, I, P, I, P, P, I, I, I, P, P, P, P]
+    lib.hough_event_run.restype = C.c_int
+    lib.hough_event_run.argtypes = [P, P, I, P, P, I, P, I, P, I, I, P, P, P, P]
     lib.hough_reassign_hits.restype = C.c_int
     lib.hough_reassign_hits.argtypes = [P, P, I, P, I, P, P, I, I, I, P, P, P, P]
     lib.hough_vertex_vote.restype = C.c_int
@@ -200,6 +202,15 @@ class HoughPlan:
                                           _dptr(cands), _dptr(cand_offsets), int(capacity), int(assoc_dj),
                                           int(min_hits), _dptr(hit_to_cand), _dptr(cand_nhits), _dptr(cand_keep),
                                           _stream_ptr(stream)), "hough_assign_hits")
+
+    def event_run(self, hits_xy, event_offsets, accum, threshold, cands, capacity, cand_offsets, assoc_dj, min_hits,
+                  hit_to_cand, cand_nhits, cand_keep, stream=None):
+        """include/hough.h hough_event_run: vote + find_peaks + assign_hits of ONE event, in one launch when it fits."""
+        assert int(event_offsets.shape[0]) == 2
+        _check(self.lib.hough_event_run(self._h, _dptr(hits_xy), int(hits_xy.shape[0]), _dptr(event_offsets), _dptr(accum),
+                                        int(threshold), _dptr(cands), int(capacity), _dptr(cand_offsets), int(assoc_dj),
+                                        int(min_hits), _dptr(hit_to_cand), _dptr(cand_nhits), _dptr(cand_keep),
+                                        _stream_ptr(stream)), "hough_event_run")
 
     def reassign_hits(self, hits_xy, event_offsets, cands, cand_offsets, capacity, assoc_dj, max_rounds, hit_to_cand,
                       cand_nhits, cand_keep, stream=None):

@@ -109,6 +109,7 @@ struct hough_plan {
     float2* d_assoc_tab;               // [n_class][n_d0][n_qpt + 1] azimuth-offset hulls per bin edge; null: not built
     int reassign_walk;                 // 1: hough_reassign_hits re-walks the vote columns instead of the candidate-centric path
     int assoc_tab_tried;               // the assoc table was requested once (it may not fit: d_assoc_tab stays null)
+    int event_general;                 // 1: hough_event_run always takes the three general calls (bisecting / comparison)
     int assoc_smem_configured;         // dynamic shared memory the kernel is configured for on this plan's device
     // vote tile shape (vote.cu)
     int32_t tile32;                    // 1: 32-bit bins in shared memory, 0: two 16-bit bins per word
@@ -145,6 +146,29 @@ __device__ __forceinline__ int d3_bin_from_w(float w, float r2, float d0c, float
 }
 
 __device__ __forceinline__ float d3_r2(float x, float y) { return __fadd_rn(__fmul_rn(x, x), __fmul_rn(y, y)); }
+
+// D7 centroid from the integer moments: every fp32 operation individually rounded.
+__device__ __forceinline__ void hough_write_candidate(const HoughConsts& c, hough_candidate* __restrict__ out, int e, int k, int i,
+                                                int j, int a, long long S, long long Sj, long long Si, long long Sk) {
+    const float fS = __ll2float_rn(S);
+    const float oj = __fdiv_rn(__ll2float_rn(Sj), fS);
+    const float oi = __fdiv_rn(__ll2float_rn(Si), fS);
+    const float ok = __fdiv_rn(__ll2float_rn(Sk), fS);
+    const float tj = __fadd_rn(__fadd_rn((float)j, 0.5f), oj);
+    const float qpt = __fadd_rn(c.qpt_min, __fmul_rn(tj, c.wq));
+    const float ti = __fadd_rn(__fadd_rn((float)i, 0.5f), oi);
+    float ph = __fmul_rn(ti, c.wphi);
+    if (ph < 0.0f) ph = __fadd_rn(ph, c.two_pi_f);
+    else if (ph >= c.two_pi_f) ph = __fsub_rn(ph, c.two_pi_f);
+    float d0 = 0.0f;
+    if (c.n_d0 > 1) {
+        const float tk = __fadd_rn(__fadd_rn((float)k, 0.5f), ok);
+        d0 = __fadd_rn(c.d0_min, __fmul_rn(tk, c.wd));
+    }
+    int4* o = reinterpret_cast<int4*>(out);
+    o[0] = make_int4(e, k, i, j);
+    o[1] = make_int4(a, __float_as_int(ph), __float_as_int(qpt), __float_as_int(d0));
+}
 
 // exclusive scan of n ints in place by one CTA of 1024 threads; the total goes to *total_out.
 __device__ __forceinline__ void cta_exclusive_scan(int32_t* data, int n, int32_t* total_out) {

@@ -103,29 +103,6 @@ __global__ void __launch_bounds__(1024) scan_events_kernel(int32_t* event_cnt, i
     if (threadIdx.x == 0) cand_offsets[n_events] = total;
 }
 
-// D7 centroid from the integer moments: every fp32 operation individually rounded.
-__device__ __forceinline__ void write_candidate(const HoughConsts& c, hough_candidate* __restrict__ out, int e, int k, int i,
-                                                int j, int a, long long S, long long Sj, long long Si, long long Sk) {
-    const float fS = __ll2float_rn(S);
-    const float oj = __fdiv_rn(__ll2float_rn(Sj), fS);
-    const float oi = __fdiv_rn(__ll2float_rn(Si), fS);
-    const float ok = __fdiv_rn(__ll2float_rn(Sk), fS);
-    const float tj = __fadd_rn(__fadd_rn((float)j, 0.5f), oj);
-    const float qpt = __fadd_rn(c.qpt_min, __fmul_rn(tj, c.wq));
-    const float ti = __fadd_rn(__fadd_rn((float)i, 0.5f), oi);
-    float ph = __fmul_rn(ti, c.wphi);
-    if (ph < 0.0f) ph = __fadd_rn(ph, c.two_pi_f);
-    else if (ph >= c.two_pi_f) ph = __fsub_rn(ph, c.two_pi_f);
-    float d0 = 0.0f;
-    if (c.n_d0 > 1) {
-        const float tk = __fadd_rn(__fadd_rn((float)k, 0.5f), ok);
-        d0 = __fadd_rn(c.d0_min, __fmul_rn(tk, c.wd));
-    }
-    int4* o = reinterpret_cast<int4*>(out);
-    o[0] = make_int4(e, k, i, j);
-    o[1] = make_int4(a, __float_as_int(ph), __float_as_int(qpt), __float_as_int(d0));
-}
-
 // One CTA = one peak block (PEAK_BLOCK_BINS bins = 128 mask words).  The block's candidates are dealt to the threads
 // by rank (thread t takes candidates t, t + 128, ...), so the lanes of a warp stay busy however the peaks cluster.
 template <bool U16>
@@ -202,7 +179,7 @@ __global__ void __launch_bounds__(128) peak_emit_kernel(HoughConsts c, const voi
                 }
             }
         }
-        write_candidate(c, cands + rank, e, k, i, j, a, (long long)S, (long long)Sj, (long long)Si, (long long)Sk);
+        hough_write_candidate(c, cands + rank, e, k, i, j, a, (long long)S, (long long)Sj, (long long)Si, (long long)Sk);
     }
 }
 
@@ -271,7 +248,7 @@ __device__ void peak_block_generic(const HoughConsts& c, const void* __restrict_
                     }
                 }
             }
-            write_candidate(c, cands + rank, e, k, i, j, a, S, Sj, Si, Sk);
+            hough_write_candidate(c, cands + rank, e, k, i, j, a, S, Sj, Si, Sk);
         }
         base += total;
         __syncthreads();
@@ -431,7 +408,7 @@ __global__ void __launch_bounds__(256) peak_tile_kernel(HoughConsts c, const voi
                 }
             }
         }
-        write_candidate(c, cands + rank, e, k, i, j, (int)tile[ci], S, Sj, Si, Sk);
+        hough_write_candidate(c, cands + rank, e, k, i, j, (int)tile[ci], S, Sj, Si, Sk);
     }
 }
 

@@ -242,6 +242,7 @@ extern "C" int hough_plan_set_option(hough_plan* p, const char* key, int32_t val
         if (value && !p->d_assoc_tab && p->tile_max_cols >= 1) { p->assoc_tab_tried = 1; return hough_build_assoc_table(p); }   // built once, on first use
         return HOUGH_OK;
     }
+    if (strcmp(key, "event_general") == 0) { p->event_general = value ? 1 : 0; return HOUGH_OK; }
     if (strcmp(key, "reassign_walk") == 0) { p->reassign_walk = value ? 1 : 0; return HOUGH_OK; }
     if (strcmp(key, "exact_walk") == 0) { p->exact_walk = value ? 1 : 0; return HOUGH_OK; }
     if (strcmp(key, "reuse_staging") == 0) { p->reuse_staging = value ? 1 : 0; p->staged_hits = nullptr; return HOUGH_OK; }
