@@ -547,6 +547,31 @@ def run_ours(args, rank, world, local_rank):
     except Exception as exc:                              # noqa: BLE001 -- report, do not hide
         print(f"bench.py: fit stage failed: {exc}", file=sys.stderr)
 
+    # single events: the same path through hough_event_run (one launch of a thread-block cluster when it fits)
+    event_info = None
+    if batch.n_events == 1:
+        try:
+            from paper_1311_2769_b200 import kernel_launches
+            (e0, e1, h0, h1) = run.tiles[0]
+            et = []
+            l0 = 0
+            for it in range(40):
+                if it == 10:
+                    l0 = kernel_launches()
+                a = torch.cuda.Event(enable_timing=True); b = torch.cuda.Event(enable_timing=True)
+                a.record()
+                run.plan.event_run(run.d_hits[h0:h1], run.d_offs[0], run.accum, w.threshold, run.cands, run.cap, run.cand_off,
+                                   w.assoc_dj, w.min_hits, run.h2c[:max(h1 - h0, 1)], run.nh, run.keep)
+                b.record(); b.synchronize()
+                if it >= 10:
+                    et.append(a.elapsed_time(b))
+            event_info = {"ms_median": statistics.median(et), "ms_min": min(et),
+                          "launches_per_call": (kernel_launches() - l0) / 30.0,
+                          "api": "hough_event_run: vote + peaks + assign of the single event in one call "
+                                 "(one cluster launch for two-parameter spaces up to 2560 hits)"}
+        except Exception as exc:                          # noqa: BLE001 -- report, do not hide
+            print(f"bench.py: hough_event_run stage failed: {exc}", file=sys.stderr)
+
     # re-assignment round of the stranded hits (PAPER.md:33 / :29; D12), first tile, outside the timed step
     reassign_info = None
     try:
@@ -609,6 +634,8 @@ def run_ours(args, rank, world, local_rank):
         line["fit"] = fit_info
     if reassign_info is not None:
         line["reassign"] = reassign_info
+    if event_info is not None:
+        line["event_run"] = event_info
     print(json.dumps(line), flush=True)
     if world > 1:
         dist.destroy_process_group()

@@ -125,9 +125,10 @@ int hough_assign_hits(hough_plan* plan, const float* d_hits_xy, int32_t n_hits, 
  * n_hits} on the device), with the same outputs bit for bit: d_accum (one accumulator, overwritten), d_cands /
  * d_cand_offsets[2], d_hit_to_cand, d_cand_nhits, d_cand_keep (see those calls for layouts and the capacity rule).
  * For a two-parameter space (n_d0 == 1) whose 16-bit tile fits the shared memory of at most 8 SMs and an event of at
- * most 2560 hits (about the measured break-even with the general path), the whole path runs in ONE launch of a thread-block cluster (accumulator slab in shared memory, steps
+ * most 2560 hits (and a work estimate below the measured break-even with the general path, see below), the whole path runs in ONE launch of a thread-block cluster (accumulator slab in shared memory, steps
  * separated by cluster barriers) -- what a latency-bound small event needs; every other case runs the three calls
- * (plan option "event_general" = 1 forces that).  Enqueues on cuda_stream and returns; graph-capturable.
+ * (plan option "event_general" = 1 forces that; "event_cluster" = 1 takes the cluster whenever it fits, ignoring the work
+ * estimate hits x longest window <= 160000 that otherwise gates it).  Enqueues on cuda_stream and returns; graph-capturable.
  * Errors: INVALID_ARG (null / misaligned pointers, sizes, assoc_dj > 15), UNSUPPORTED, CUDA. */
 int hough_event_run(hough_plan* plan, const float* d_hits_xy, int32_t n_hits, const int32_t* d_event_offsets,
                     void* d_accum, int32_t threshold, hough_candidate* d_cands, int32_t capacity,

@@ -109,6 +109,8 @@ struct hough_plan {
     float2* d_assoc_tab;               // [n_class][n_d0][n_qpt + 1] azimuth-offset hulls per bin edge; null: not built
     int reassign_walk;                 // 1: hough_reassign_hits re-walks the vote columns instead of the candidate-centric path
     int assoc_tab_tried;               // the assoc table was requested once (it may not fit: d_assoc_tab stays null)
+    int event_max_steps;               // longest column window of any radius class in slice 0 (work estimate of hough_event_run)
+    int event_cluster;                 // 1: hough_event_run takes the cluster kernel whenever it fits, whatever the work estimate says
     int event_general;                 // 1: hough_event_run always takes the three general calls (bisecting / comparison)
     int assoc_smem_configured;         // dynamic shared memory the kernel is configured for on this plan's device
     // vote tile shape (vote.cu)

@@ -32,6 +32,7 @@ namespace {
 constexpr int EV_THREADS = 1024;
 constexpr int EV_MAX_CLUSTER = 8;                  // portable cluster size
 constexpr size_t EV_SMEM_BUDGET = 200 * 1024;      // tile + hit cache bytes per CTA
+constexpr long long EV_MAX_EVALS = 160000;         // hits x longest window above which the general path is faster
 constexpr int EV_MAX_HITS = 2560;                 // hits of an event on the one-launch path (16-byte cache entry each)
 
 struct EventArgs {
@@ -342,7 +343,11 @@ extern "C" int hough_event_run(hough_plan* p, const float* d_hits_xy, int32_t n_
     // cluster shape: the fewest CTAs whose tiles fit, then more (up to 8) while every CTA keeps at least 32 columns
     int n_cta = 0;
     const size_t hit_bytes = (size_t)std::max(n_hits, 0) * 16;
-    if (c.n_d0 == 1 && n_hits <= EV_MAX_HITS && !p->fullscan && !p->event_general) {
+    // the cluster runs on at most 8 SMs: it wins while the event is latency-bound, i.e. while hits x columns per hit stays
+    // small (measured break-even about 2e5 evaluations per phase; an upper estimate from the longest class window)
+    const bool small = n_hits <= EV_MAX_HITS &&
+                       (p->event_cluster || (long long)n_hits * std::max(p->event_max_steps, 1) <= EV_MAX_EVALS);
+    if (c.n_d0 == 1 && small && !p->fullscan && !p->event_general) {
         for (int k = 1; k <= EV_MAX_CLUSTER; ++k) {
             const int cols = (c.n_phi + k - 1) / k;
             if ((size_t)(cols + 2) * c.n_qpt * 2 + 16 + hit_bytes <= EV_SMEM_BUDGET) { n_cta = k; break; }

@@ -4,8 +4,8 @@
 //   K-fit-a  zero the moment rows of the candidates in use
 //   K-fit-b  one thread per hit: 9 double atomicAdds {n, Sx, Sy, Sz, Sxx, Sxy, Syy, Sxz, Syz} into its candidate's row
 //   K-fit-c  one thread per candidate: moments about the hits' centroid, 2x2 solve for the centre, D1 parameters in
-//            closed form from (centre, R, orientation) -- written from the definition, independently of the CPU checker under tests
-//            3x3 Cramer solve and vector construction
+//            closed form from (centre, R, orientation) -- a different algebraic route from the 3x3 Cramer solve of the CPU
+//            checker under tests/, so that the parity test compares two independent solves
 #include <cmath>
 
 #include "common.cuh"

@@ -152,6 +152,10 @@ extern "C" int hough_plan_create(const hough_binning* b, const hough_geometry* g
         memcpy(&lo_bits, &win.lo_off[t], 4);
         winT[t] = make_int2(lo_bits, win.steps[t] | (win.fwd_safe[t] ? (1 << 30) : 0));
     }
+    p->event_max_steps = 0;
+    // (the first and the open-ended last class span the whole circle by construction and hold no layer: left out)
+    for (int cl = (win.n_class > 2 ? 1 : 0); cl < (win.n_class > 2 ? win.n_class - 1 : win.n_class); ++cl)
+        p->event_max_steps = std::max(p->event_max_steps, std::min(win.steps[(size_t)cl * b->n_d0], (int)b->n_phi));
     // packed 16-bit tiles are exact whenever no bin can exceed 65535: the U16 precondition, or at most 65535
     // hits per call (a hit casts at most one vote per (phi0, d0) column, D3)
     p->tile32 = (b->accum_dtype == HOUGH_ACC_I32 && max_hits > 65535) ? 1 : 0;
@@ -242,6 +246,7 @@ extern "C" int hough_plan_set_option(hough_plan* p, const char* key, int32_t val
         if (value && !p->d_assoc_tab && p->tile_max_cols >= 1) { p->assoc_tab_tried = 1; return hough_build_assoc_table(p); }   // built once, on first use
         return HOUGH_OK;
     }
+    if (strcmp(key, "event_cluster") == 0) { p->event_cluster = value ? 1 : 0; return HOUGH_OK; }
     if (strcmp(key, "event_general") == 0) { p->event_general = value ? 1 : 0; return HOUGH_OK; }
     if (strcmp(key, "reassign_walk") == 0) { p->reassign_walk = value ? 1 : 0; return HOUGH_OK; }
     if (strcmp(key, "exact_walk") == 0) { p->exact_walk = value ? 1 : 0; return HOUGH_OK; }

@@ -16,11 +16,13 @@ from gpu_util import assert_centroids_close  # noqa: E402
 from paper_1311_2769_b200 import HoughPlan, alloc_candidates, candidates_to_numpy, kernel_launches  # noqa: E402
 
 
-def _run(w, batch, capacity, general=False, threshold=None, assoc_dj=None, min_hits=None):
+def _run(w, batch, capacity, general=False, threshold=None, assoc_dj=None, min_hits=None, cluster=True):
     bn = w.binning
     plan = HoughPlan.from_workload(w, max_hits=max(batch.n_hits, 1), max_events=1)
     if general:
         plan.set_option("event_general", 1)
+    elif cluster:
+        plan.set_option("event_cluster", 1)                        # the cluster kernel whenever it fits (no work gate)
     d_hits = torch.from_numpy(batch.hits_xy).cuda() if batch.n_hits else torch.zeros((1, 2), dtype=torch.float32, device="cuda")[:0]
     d_off = torch.from_numpy(batch.event_offsets).cuda()
     accum = plan.alloc_accum(1)
@@ -80,6 +82,14 @@ def test_event_run_two_parameter_workloads_one_launch(cfg):
     for key in ("accum", "off", "h2c", "nh", "keep"):
         assert np.array_equal(got[key], gen[key]), key
     assert np.array_equal(got["rec"], gen["rec"])                 # records byte for byte, centroids included
+
+
+def test_event_run_work_gate():
+    """Without the test switch the cluster is taken only while hits x longest window stays small: config 0 yes, the
+    zero-field workload (windows of up to 512 columns, 2200 hits) no.  Same results either way."""
+    w0, w6 = get_workload(0), get_workload(6)
+    assert _check(w0, generate_events(w0), cluster=False)["launches"] == 1
+    assert _check(w6, generate_events(w6), cluster=False)["launches"] > 5
 
 
 def test_event_run_three_parameter_space_takes_the_general_calls():
