@@ -22,10 +22,11 @@
 // reciprocal, unfused multiplies).  The walk evaluates the same real-valued function with FMAs and MUFU.RCP (t~)
 // and owns, per (radius class, d0 slice), a bound m on |t~ - t_D3| (first-order rounding analysis of BOTH sequences
 // with a safety factor); if t~ is further than m from a bin edge the D3 bin is floor(t~) (or certainly out of range)
-// without running D3.  The hot loop casts the fast vote of every evaluation unconditionally; a column pair with an
-// uncertain evaluation (about 0.15 % of the pairs) goes to the warp's small shared-memory queue and is redone 32 at a
-// time by the whole warp: the pair's two fast votes are taken back (fast_slot reproduces them bit for bit) and the
-// votes of the exact D3 sequence (d3_exact_bin) are cast.  Classes whose bound is useless (r ~ |d0|, the open-ended
+// without running D3.  The per-column quantity w = y cos - x sin comes from a recurrence in registers (no table read in
+// the hot loop, see "Recurrence" below).  The hot loop has no branch: a column pair with an uncertain evaluation
+// (about 0.9 % of the pairs) sends both its votes / probes to guard slot 0 of their rows and goes to the warp's small
+// shared-memory queue, which the whole warp drains 32 pairs at a time with the exact D3 sequence (d3_exact_bin) for both
+// columns.  Classes whose bound is useless (r ~ |d0|, the open-ended
 // last class where non-finite coordinates land), classes whose window is not certainly forward, and the plan option
 // "exact_walk" take the exact sequence at every column.  The result is therefore the D3 bin in every case.
 #pragma once
@@ -729,7 +730,7 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
                         red_shared(adB, TILE32 ? 1u : 65536u);
                     } else {
                         // best (entry >> 1, ~column) of the lane; the q/pT bin and the entry's sign bit are recovered
-                        // after the loop by re-evaluating the winning column (fast_slot)
+                        // after the loop by re-evaluating the winning column (fast_bin_direct)
                         const unsigned entA = TILE32 ? lds_u32(adA) : lds_u16(adA);
                         const unsigned entB = TILE32 ? lds_u32(adB) : lds_u16(adB + 2u);
                         const typename EntryT<TILE32>::pkey_t pA = EntryT<TILE32>::pkey_inv(entA, cinv);
