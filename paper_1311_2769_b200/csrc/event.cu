@@ -85,6 +85,7 @@ __device__ __forceinline__ int ev_bin(const HoughConsts& c, float x, float y, fl
 }
 
 __device__ __forceinline__ void ev_tile_add(unsigned short* tile, int nq, int row, int j) {
+    HOUGH_CHECK(row >= 0 && j >= 0 && j < nq);
     const unsigned idx = (unsigned)row * (unsigned)nq + (unsigned)j;
     atomicAdd(reinterpret_cast<unsigned*>(tile) + (idx >> 1), 1u << (16 * (idx & 1u)));
 }
@@ -177,6 +178,7 @@ __global__ void __launch_bounds__(EV_THREADS, 1) event_kernel(const __grid_const
                 int col = halo_l + k;
                 if (col >= nphi) col -= nphi;
                 if (col >= nphi) col -= nphi;
+                HOUGH_CHECK(col >= 0 && col < nphi && k <= cols + 1);
                 const int j = ev_bin(c, hv.x, hv.y, r2, col);
                 if (j >= 0) ev_tile_add(tile, nq, k, j);
             }
@@ -257,6 +259,7 @@ __global__ void __launch_bounds__(EV_THREADS, 1) event_kernel(const __grid_const
     __syncthreads();
     for (int ci = first + tid; ci < end; ci += EV_THREADS) {
         const int4 q = *reinterpret_cast<const int4*>(a.cands + ci);          // event, k, i, j (written by this CTA)
+        HOUGH_CHECK(q.z >= c0 && q.z < c0 + cols && q.w >= 0 && q.w < nq);
         tile[(size_t)(q.z - c0 + 1) * nq + q.w] = 1;
     }
     __syncthreads();
