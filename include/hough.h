@@ -217,7 +217,9 @@ int hough_pipeline_destroy(hough_pipeline* p);
  * the KEPT list, h_hit_to_cand indexes it (hits of dropped candidates are -1 as always), h_cand_nhits follows it and
  * h_cand_keep is 1 for every returned candidate; cand_capacity then bounds the kept list.  All the work (vote, peaks,
  * association) is unchanged; only the result transfer shrinks (config 3: 1.0 GB -> 45 MB per 1024 events).
- * "graphs" = 0 / 1: CUDA graph capture off / on.  INVALID_ARG for unknown keys. */
+ * "graphs" = 0 / 1: CUDA graph capture off / on.  "reassign" = 1: every tile's association is followed by the D12
+ * re-assignment round (hough_reassign_hits), so h_hit_to_cand / h_cand_nhits are the fixed point of the rounds.
+ * INVALID_ARG for unknown keys. */
 int hough_pipeline_set_option(hough_pipeline* p, const char* key, int32_t value);
 int hough_pipeline_run_host(hough_pipeline* p, const float* h_hits_xy, int32_t n_hits,
                             const int32_t* h_event_offsets, int32_t n_events, int32_t threshold,

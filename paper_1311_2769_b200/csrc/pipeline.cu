@@ -140,6 +140,7 @@ struct hough_pipeline {
     std::vector<Lane> lanes;
     int use_graphs;
     int kept_only;
+    int reassign;                       // 1: hough_reassign_hits (D12) after the association of every tile
 };
 
 static void pipeline_free(hough_pipeline* p) {
@@ -175,6 +176,7 @@ extern "C" int hough_pipeline_create(const hough_binning* b, const hough_geometr
     const char* env = getenv("HOUGH_PIPELINE_NO_GRAPHS");
     p->use_graphs = (env && env[0] == '1') ? 0 : 1;
     p->kept_only = 0;
+    p->reassign = 0;
     p->lanes.resize(n_streams);
     int rc = HOUGH_OK;
     for (Lane& l : p->lanes) {
@@ -204,6 +206,14 @@ extern "C" int hough_pipeline_create(const hough_binning* b, const hough_geometr
 extern "C" int hough_pipeline_set_option(hough_pipeline* p, const char* key, int32_t value) {
     if (!p || !key) return HOUGH_ERR_INVALID_ARG;
     if (strcmp(key, "graphs") == 0) { p->use_graphs = value ? 1 : 0; return HOUGH_OK; }
+    if (strcmp(key, "reassign") == 0) {
+        p->reassign = value ? 1 : 0;
+        for (Lane& l : p->lanes) {                           // another node list: the lanes' graphs are rebuilt; the next tile of
+            if (l.exec) { cudaGraphExecDestroy(l.exec); l.exec = nullptr; }      // a lane runs un-captured once (the D12 table
+            l.warmed = false;                                                    // is built on first use, outside capture)
+        }
+        return HOUGH_OK;
+    }
     if (strcmp(key, "kept_only") != 0) return HOUGH_ERR_INVALID_ARG;
     if (value && !p->lanes.empty() && !p->lanes[0].d_pre) {          // buffers of the compaction, once
         const size_t cap = (size_t)std::max(p->tile_cap, 1);
@@ -246,6 +256,11 @@ static int enqueue_part_a(hough_pipeline* p, Lane& l, const float* h_hits_xy, in
     rc = hough_assign_hits(l.plan, l.d_hits, n_h, l.d_off, n_ev, l.d_cands, l.d_cand_off, p->tile_cap, assoc_dj, min_hits,
                            l.d_h2c, l.d_nh, l.d_keep, l.st);
     if (rc != HOUGH_OK) return rc;
+    if (p->reassign && p->tile_cap > 0) {                // D12: orphan hits take the best surviving candidate
+        rc = hough_reassign_hits(l.plan, l.d_hits, n_h, l.d_off, n_ev, l.d_cands, l.d_cand_off, p->tile_cap, assoc_dj, 2, l.d_h2c,
+                                 l.d_nh, l.d_keep, l.st);
+        if (rc != HOUGH_OK) return rc;
+    }
     HOUGH_CUDA_TRY(cudaMemcpyAsync(l.h_cand_off, l.d_cand_off, sizeof(int32_t) * ((size_t)n_ev + 1), cudaMemcpyDeviceToHost,
                                    l.st));
     if (p->kept_only && p->tile_cap > 0) {

@@ -12,13 +12,15 @@ from gpu_util import assert_centroids_close  # noqa: E402
 from paper_1311_2769_b200 import CAND_DTYPE, HoughPipeline  # noqa: E402
 
 
-def _run_pipeline(w, batch, tile_events, n_streams, tile_cap, cand_capacity, pinned=True, kept_only=False):
+def _run_pipeline(w, batch, tile_events, n_streams, tile_cap, cand_capacity, pinned=True, kept_only=False, reassign=False):
     off = batch.event_offsets.astype(np.int64)
     tiles = [(e0, min(e0 + tile_events, batch.n_events)) for e0 in range(0, batch.n_events, tile_events)]
     max_hits = max(int(off[e1] - off[e0]) for e0, e1 in tiles)
     pipe = HoughPipeline.from_workload(w, tile_events, max(max_hits, 1), tile_cap, n_streams)
     if kept_only:
         pipe.set_option("kept_only", 1)
+    if reassign:
+        pipe.set_option("reassign", 1)
 
     def host(t):
         return t.pin_memory() if pinned else t
@@ -37,14 +39,17 @@ def _run_pipeline(w, batch, tile_events, n_streams, tile_cap, cand_capacity, pin
     return over, h2c.numpy()[:batch.n_hits], coff.numpy(), cands.numpy().view(CAND_DTYPE).reshape(-1), nh.numpy(), keep.numpy()
 
 
-def _oracle_per_event(w, batch):
+def _oracle_per_event(w, batch, rounds=False):
     o = Oracle.from_binning(w.binning, w.bz_tesla)
     recs, h2cs, nhs, keeps, offs = [], [], [], [], [0]
     for e in range(batch.n_events):
         ev = batch.select([e])
         acc, _ = o.vote(ev.hits_xy, ev.event_offsets)
         ref = o.find_peaks(acc, w.threshold)
-        h2c, nh, keep = o.assign_indexed(ev.hits_xy, ev.event_offsets, ref, w.assoc_dj, w.min_hits)
+        if rounds:                                       # D12: the fixed point of the re-assignment rounds
+            h2c, nh, keep, _ = o.assign_rounds(ev.hits_xy, ev.event_offsets, ref, w.assoc_dj, w.min_hits, max_rounds=4)
+        else:
+            h2c, nh, keep = o.assign_indexed(ev.hits_xy, ev.event_offsets, ref, w.assoc_dj, w.min_hits)
         r = ref.records.copy()
         r["event"] = e
         recs.append(r)
@@ -132,3 +137,24 @@ def test_pipeline_kept_only_returns_the_compacted_kept_list(tile_events, n_strea
     assert_centroids_close(cands[:n_kept], rec[kmask], w.binning)
     assert np.array_equal(h2c, h2c_kept)
     assert np.array_equal(nh[:n_kept], nh_ref[kmask]) and (keep[:n_kept] == 1).all()
+
+
+@pytest.mark.parametrize("kept_only", [False, True])
+def test_pipeline_reassign_option_runs_the_d12_round(kept_only):
+    """Pipeline option "reassign": hit_to_cand / cand_nhits are the fixed point of the re-assignment rounds (D12)."""
+    w = get_workload(3)
+    batch = generate_events(w, events=[5, 6, 7])
+    rec, h2c_ref, nh_ref, keep_ref, off_ref = _oracle_per_event(w, batch, rounds=True)
+    total = int(off_ref[-1])
+    tile_cap = int(max(off_ref[min(e0 + 2, 3)] - off_ref[e0] for e0 in range(0, 3, 2))) + 3
+    over, h2c, coff, cands, nh, keep = _run_pipeline(w, batch, 2, 2, tile_cap, total + 5, kept_only=kept_only, reassign=True)
+    assert not over
+    if not kept_only:
+        assert np.array_equal(coff, off_ref) and np.array_equal(h2c, h2c_ref)
+        assert np.array_equal(nh[:total], nh_ref) and np.array_equal(keep[:total], keep_ref)
+    else:
+        kmask = keep_ref.astype(bool)
+        new_index = np.cumsum(kmask) - 1
+        assert np.array_equal(h2c, np.where(h2c_ref >= 0, new_index[np.maximum(h2c_ref, 0)], -1))
+        assert np.array_equal(nh[:int(kmask.sum())], nh_ref[kmask])
+    assert (h2c >= 0).sum() > (_oracle_per_event(w, batch)[1] >= 0).sum()     # the round did recover hits
