@@ -421,6 +421,10 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
     extern __shared__ __align__(16) unsigned char smem_raw[];
     __shared__ WalkTile s_tl;
     __shared__ int s_meta[2];                           // number of batches of the tile
+    // warp-uniform loop state kept in shared memory on purpose ({next batch, segment pointer, queue fill} per warp): at
+    // the kernels' register budgets the compiler otherwise spills exactly these to local memory, whose reloads miss the
+    // small L1 left beside 3 x 75 KB of tiles (measured: 10 % of the association walk's stall samples)
+    __shared__ int s_ws[WALK_MAX_WARPS][4];
     const int n_slabs = a.n_slabs, slab_cols = a.slab_cols, stride = a.stride;
     const int slab = blockIdx.x % n_slabs;
     const int k = (blockIdx.x / n_slabs) % c.n_d0;
@@ -622,13 +626,25 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
     const f32x2 magic2 = pk2(WALK_MAGIC, WALK_MAGIC), nmagic2 = pk2(-WALK_MAGIC, -WALK_MAGIC);
     const WalkTile& tl = s_tl;                          // what the out-of-line rare paths need of the tile (written in the prologue)
     unsigned* wq = s_wq + warp * WALK_WQ_CAP;           // the warp's redo queue
-    int wq_n = 0;                                       // its fill: warp-uniform, kept in a register
+    volatile int* ws = s_ws[warp];                      // [0] next batch, [1] segment pointer, [2] queue fill (all warp-uniform)
+    if (lane == 0) { ws[0] = warp; ws[1] = 0; ws[2] = 0; }
+    __syncwarp();
+    constexpr bool WS_SMEM = MODE == WALK_ASSIGN;       // the vote walk (64 registers, no spill) keeps them in registers: faster there
+    int bt_r = warp, seg_r = 0, wqn_r = 0;
     const unsigned lt = (1u << lane) - 1u;
     const bool wq_ok = ev_hits < (1 << 18) && slab_cols <= 2048;          // entries fit 32 bits (else: redo on the spot)
     const unsigned dump = (unsigned)(lane & (WALK_DUMP - 1));
-    int seg = 0;
-    for (int bt = warp; bt < n_batches; bt += WALK_WARPS) {
+    for (;;) {
+        const int bt = WS_SMEM ? ws[0] : bt_r;
+        if (bt >= n_batches) break;
+        int seg = WS_SMEM ? ws[1] : seg_r;
         while (s_seg[seg + 1].w <= bt) ++seg;            // last segment with first batch <= bt (the sentinel ends the search)
+        if (WS_SMEM) {
+            __syncwarp();
+            if (lane == 0) { ws[0] = bt + WALK_WARPS; ws[1] = seg; }
+        } else {
+            bt_r = bt + WALK_WARPS; seg_r = seg;
+        }
         HOUGH_CHECK(seg >= 0 && seg < nc * (FULLPHI ? 1 : 2));
         const int4 sg = s_seg[seg];                      // {first staged hit, hits, class, first batch}
         HOUGH_CHECK(sg.z >= 0 && sg.z < nc && sg.x >= 0 && sg.x + sg.y <= ev_hits);
@@ -643,6 +659,12 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
         const int sidx = ev_begin + sg.x + in_seg;       // index of the lane's staged hit
         float4 hv = make_float4(1.f, 0.f, 0.f, 0.f);
         if (active) hv = __ldg(a.staged + sidx);
+        // the warp's next batch is WALK_WARPS batches on: bring its staged hits into L1 while this one is walked (the
+        // address only has to be right most of the time; it stays inside the event's staged range)
+        {
+            const int nxt = sidx + 32 * WALK_WARPS;
+            if (nxt < ev_begin + ev_hits) asm volatile("prefetch.global.L1 [%0];" :: "l"(a.staged + nxt));
+        }
         const float x = hv.x, y = hv.y;
         const float r2 = d3_r2(x, y);
         int i_lo = (int)ceilf(hv.z + cw.x);
@@ -773,6 +795,8 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
                 // queue drained 32 entries at a time by the whole warp; entries that do not fit 32 bits: redone on the spot
                 // (a prefix sum over the lanes' flag counts was measured slower than these rounds)
                 unsigned any = __ballot_sync(0xffffffffu, slowmask != 0u);
+                int wq_n = WS_SMEM ? (any != 0u ? ws[2] : 0) : wqn_r;
+                const bool had_any = any != 0u;
                 while (any != 0u) {
                     if (slowmask != 0u) {
                         const int t = __ffs(slowmask) - 1;
@@ -795,6 +819,11 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
                     }
                     any = __ballot_sync(0xffffffffu, slowmask != 0u);
                 }
+                if (WS_SMEM) {
+                    if (had_any) { __syncwarp(); if (lane == 0) ws[2] = wq_n; __syncwarp(); }
+                } else {
+                    wqn_r = wq_n;
+                }
             }
         }
         if (MODE == WALK_ASSIGN) {
@@ -814,7 +843,11 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
             }
         }
     }
-    if (wq_n > 0) walk_drain<MODE, TILE32>(c, d, a, tl, wq, wq_n, ev_begin, lane);
+    __syncwarp();
+    {
+        const int wq_n = WS_SMEM ? ws[2] : wqn_r;
+        if (wq_n > 0) walk_drain<MODE, TILE32>(c, d, a, tl, wq, wq_n, ev_begin, lane);
+    }
     if (MODE == WALK_ASSIGN) return;
     __syncthreads();
 
