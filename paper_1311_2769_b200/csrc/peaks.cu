@@ -733,24 +733,31 @@ __global__ void __launch_bounds__(256, 3) peak_stream16_kernel(HoughConsts c, co
         if (v_first + s <= v_last) issue(v_first + s, s);
         else ps_commit();
     }
-    Row6 Vm, Rm, R0, Rp;
+    // Two register sets of rows (X, Y) swap roles every slice ("centre" <-> "next"), so no row is ever copied: the loop
+    // is unrolled by two with the names exchanged.
+    Row6 Vm, Xm, X0, Xp, Ym, Y0, Yp;
 #pragma unroll
-    for (int w = 0; w < 6; ++w) Vm.x[w] = Rm.x[w] = R0.x[w] = Rp.x[w] = 0u;
-    for (int it = 0, v = v_first; v <= v_last; ++it, ++v) {
+    for (int w = 0; w < 6; ++w) Vm.x[w] = Xm.x[w] = X0.x[w] = Xp.x[w] = Ym.x[w] = Y0.x[w] = Yp.x[w] = 0u;
+    // one slice step: wait for slice v (iteration it), refill the stage freed by the previous step, load its rows into
+    // (Nm, N0, Np) and, from the third step on, evaluate the centre slice held in (Rm, R0, Rp)
+    int sc = 0, sp = PS_STAGES - 1;                            // ring stage of this step and of the previous one (it % PS_STAGES, kept incrementally)
+    auto step = [&](int it, int v, Row6& Rm, Row6& R0, Row6& Rp, Row6& Nm, Row6& N0, Row6& Np) {
         ps_wait<PS_STAGES - 2>();                               // group `it` (slice v) has landed
         __syncthreads();                                        // ... for every thread; the previous stage is free
         if (it >= 1) {
             const int vn = v - 1 + PS_STAGES;
-            if (vn <= v_last) issue(vn, (it - 1) % PS_STAGES);
+            if (vn <= v_last) issue(vn, sp);
             else ps_commit();
         }
-        const unsigned short* st = s_base + (size_t)(it % PS_STAGES) * stage_halfwords + rl * nq;
-        HOUGH_CHECK((size_t)((it % PS_STAGES) * stage_halfwords + (rl + 2) * nq + j0 + 8) * 2 <= (size_t)PS_STAGES * (R + 2) * nq * 2);
-        const Row6 Nm = ps_load_row(st, j0, nq);
-        const Row6 N0 = ps_load_row(st + nq, j0, nq);
-        const Row6 Np = ps_load_row(st + 2 * nq, j0, nq);
-        if (it == 0) { Vm = k16_max3(Nm, N0, Np); continue; }
-        if (it == 1) { Rm = Nm; R0 = N0; Rp = Np; continue; }
+        const unsigned short* st = s_base + (size_t)sc * stage_halfwords + rl * nq;
+        HOUGH_CHECK(sc == it % PS_STAGES && (size_t)(sc * stage_halfwords + (rl + 2) * nq + j0 + 8) * 2 <= (size_t)PS_STAGES * (R + 2) * nq * 2);
+        sp = sc;
+        sc = sc + 1 == PS_STAGES ? 0 : sc + 1;
+        Nm = ps_load_row(st, j0, nq);
+        N0 = ps_load_row(st + nq, j0, nq);
+        Np = ps_load_row(st + 2 * nq, j0, nq);
+        if (it == 0) { Vm = k16_max3(Nm, N0, Np); return; }     // slice k0 - 1: only its column maximum is needed
+        if (it == 1) return;                                    // slice k0 becomes the centre of the next step
         const int k = v - 1;                                    // centre slice, k0 <= k < k1
         const Row6 B = k16_max2(Vm, Rm);                        // everything "before" the centre row, per q/pT bin
         const Row6 A = k16_max2(k16_max3(Nm, N0, Np), Rp);      // everything "after" it
@@ -780,7 +787,11 @@ __global__ void __launch_bounds__(256, 3) peak_stream16_kernel(HoughConsts c, co
         if ((tid & 31) == 0 && cnt)
             atomicAdd(block_cnt + (size_t)e * blocks_per_event + (int)(bin0 / PEAK_BLOCK_BINS), cnt);
         Vm = k16_max3(Rm, R0, Rp);
-        Rm = Nm; R0 = N0; Rp = Np;
+    };
+    // step 0 loads into Y, step 1 into X (the first centre), step 2 evaluates X against Y, step 3 Y against X, ...
+    for (int it = 0, v = v_first; v <= v_last; it += 2, v += 2) {
+        step(it, v, Xm, X0, Xp, Ym, Y0, Yp);
+        if (v + 1 <= v_last) step(it + 1, v + 1, Ym, Y0, Yp, Xm, X0, Xp);
     }
 }
 
