@@ -168,15 +168,16 @@ __global__ void __launch_bounds__(128) peak_emit_kernel(HoughConsts c, const voi
             for (int di = -1; di <= 1; ++di) {
                 int ii = i + di;
                 ii = ii < 0 ? ii + nphi : (ii >= nphi ? ii - nphi : ii);
-                const size_t row = ebase + ((size_t)kk * nphi + ii) * nq;
-#pragma unroll
-                for (int dj = -1; dj <= 1; ++dj) {
-                    const int jj = j + dj;
-                    if (jj < 0 || jj >= nq) continue;
-                    const int val = load_bin<U16>(acc, row + jj);
-                    S += val; Sj += (mom_t)val * dj; Si += (mom_t)val * di; Sk += (mom_t)val * dk;
-                    if (dk == 0 && di == 0 && dj == 0) a = val;
-                }
+                const size_t row = ebase + ((size_t)kk * nphi + ii) * nq + j;
+                // the row's three bins at once (missing q/pT neighbours count 0): row sum and left-right difference
+                const int vL = j > 0 ? load_bin<U16>(acc, row - 1) : 0;
+                const int vC = load_bin<U16>(acc, row);
+                const int vR = j + 1 < nq ? load_bin<U16>(acc, row + 1) : 0;
+                const mom_t rs = (mom_t)vL + vC + vR;
+                S += rs; Sj += (mom_t)(vR - vL);
+                if (di > 0) Si += rs; else if (di < 0) Si -= rs;
+                if (dk > 0) Sk += rs; else if (dk < 0) Sk -= rs;
+                if (dk == 0 && di == 0) a = vC;
             }
         }
         hough_write_candidate(c, cands + rank, e, k, i, j, a, (long long)S, (long long)Sj, (long long)Si, (long long)Sk);
