@@ -79,6 +79,7 @@ struct hough_plan {
     int peaks_regs;                    // 1: 16-bit packed peak walk with register-held rows instead of the cp.async ring
     int peaks_scalar;                  // 1: 16-bit accumulators use the unpacked slice-walk peak kernel (bisecting)
     int exact_walk;                    // 1: the walks evaluate the D3 sequence at every column (no fast path)
+    float m_scale;                     // 1 (HOUGH_DEBUG_M_SCALE: scales the fast path's error bound, to probe its margin)
     int assign_candidates;             // 1: hough_assign_hits takes the candidate-centric path (assoc.cu) instead of re-walking the vote columns
     int reuse_staging;                 // 1: hough_assign_hits may reuse the staging of the preceding hough_vote (same arguments)
     const void* staged_hits; const void* staged_off; int32_t staged_n_hits, staged_n_events; cudaStream_t staged_stream;

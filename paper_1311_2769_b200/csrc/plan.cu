@@ -84,6 +84,8 @@ extern "C" int hough_plan_create(const hough_binning* b, const hough_geometry* g
     p->fullscan = (env && env[0] == '1') ? 1 : 0;
     env = getenv("HOUGH_DEBUG_EXACT_WALK");
     p->exact_walk = (env && env[0] == '1') ? 1 : 0;
+    env = getenv("HOUGH_DEBUG_M_SCALE");
+    p->m_scale = (env && atof(env) >= 0.0) ? (float)atof(env) : 1.0f;
 
     cudaError_t ce = cudaGetDevice(&p->device);
     if (ce == cudaSuccess) ce = cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, p->device);

@@ -51,6 +51,7 @@ struct WalkArgs {
     const int32_t* key_start;        // [n_events][n_keys + 1] exclusive key starts
     int n_slabs, slab_cols, stride;  // tile shape (slab_cols even; stride = words per row / pair row, odd)
     int exact_only;                  // 1: never take the fast path (plan option "exact_walk", for bisecting)
+    float m_scale;                   // 1; HOUGH_DEBUG_M_SCALE scales the bound m (margin probe of the tests, profiles/r2_walk.md)
     // WALK_VOTE
     void* accum;
     // WALK_ASSIGN
@@ -512,7 +513,7 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
             const float arel = WALK_U * ((fk.line ? 0.0f : 6.0f * S * inv_dr2) + 24.0f) + (fk.line ? 0.0f : 3.0f * fk.d0abs * Ew * inv_dr2);
             const float elin = fk.e_lin * (L + fk.d0abs) + fabsf(fk.inv_wq) * Ew;
             const float m = fk.inv_A_abs * inv_dr2 * elin + arel * fk.t_max + fk.a0;
-            if (m < 0.45f) hm = 0.5f - m;                                     // false for NaN / inf
+            if (m < 0.45f) hm = 0.5f - m * a.m_scale;                         // false for NaN / inf
         }
         s_cls[cl] = make_float4(__int_as_float(w.x), __int_as_float(steps), hm, 0.0f);
     }
@@ -916,6 +917,7 @@ int walk_launch(hough_plan* p, int n_events, WalkArgs a, cudaStream_t st) {
     const long long grid = (long long)a.n_slabs * p->c.n_d0 * n_events;
     if (grid > 0x7fffffffLL) return HOUGH_ERR_UNSUPPORTED;
     a.exact_only = p->exact_walk;
+    a.m_scale = p->m_scale;
     kern<<<(unsigned)grid, walk_threads(MODE), smem, st>>>(p->c, a);
     HOUGH_CUDA_TRY(cudaGetLastError());
     hough_count_launches(1);
