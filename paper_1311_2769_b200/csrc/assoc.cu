@@ -17,6 +17,7 @@
 //     (one CTA works on one event) and merged into the global array with one atomicMax per touched hit at the end.
 //     Events with more hits than the shared-memory array holds fold straight into global memory (look first, then
 //     atomicMax).
+#include <algorithm>
 #include <cmath>
 
 #include "walk.cuh"
@@ -289,6 +290,96 @@ __global__ void __launch_bounds__(ASSOC_THREADS, SMEM ? 3 : 2) assoc_cand_kernel
     }
 }
 
+// ---- few candidates (D12 round: only the survivors of duplicate removal take part) -----------------------------------
+// With a keep filter a CTA's chunk holds a handful of participating candidates (config 3: 188 of 25 600 per event), far
+// too few to fill warps with lane = candidate.  Here the kept candidates of the chunk are compacted into shared memory
+// and the (candidate, class) ITEMS are dealt to the threads, so a few hundred candidates still give thousands of
+// independent items.  Keys are folded straight into the global best-key array (look first, then atomicMax).
+constexpr int ASSOC_KEPT_THREADS = 256;
+constexpr int ASSOC_KEPT_CHUNK = 4096;                // candidates examined per round: bounds the shared list
+
+__global__ void __launch_bounds__(ASSOC_KEPT_THREADS) assoc_kept_kernel(HoughConsts c, AssocArgs a) {
+    __shared__ int s_list[ASSOC_KEPT_CHUNK];
+    __shared__ int s_n, s_ncl;
+    __shared__ short s_cls[HOUGH_MAX_CLASSES + 1];
+    const int tid = threadIdx.x;
+    const int e = blockIdx.x / a.parts, part = blockIdx.x % a.parts;
+    const int first = min(__ldg(a.cand_off + e), a.capacity), end = min(__ldg(a.cand_off + e + 1), a.capacity);
+    const int n_c = end - first;
+    if (n_c <= 0) return;
+    const int chunk = (n_c + a.parts - 1) / a.parts;
+    const int c_begin = first + part * chunk, c_end = min(c_begin + chunk, end);
+    if (c_begin >= c_end) return;
+    const int ev_begin = __ldg(a.off + e);
+    const int ev_hits = __ldg(a.off + e + 1) - ev_begin;
+    if (ev_hits <= 0) return;
+    const int NS = c.n_sector, nc = c.n_class, nq = c.n_qpt, nq1 = nq + 1, dj = a.assoc_dj;
+    const int32_t* ks = a.key_start + (size_t)e * (c.n_keys + 1);
+    const bool line = c.model != 0;
+    if (tid == 0) s_ncl = 0;
+    __syncthreads();
+    for (int cl = tid; cl < nc; cl += ASSOC_KEPT_THREADS)
+        if (__ldg(ks + (cl + 1) * NS) > __ldg(ks + cl * NS)) s_cls[atomicAdd(&s_ncl, 1)] = (short)cl;
+    for (int r0 = c_begin; r0 < c_end; r0 += ASSOC_KEPT_CHUNK) {
+        __syncthreads();
+        if (tid == 0) s_n = 0;
+        __syncthreads();
+        const int r1 = min(r0 + ASSOC_KEPT_CHUNK, c_end);
+        for (int ci = r0 + tid; ci < r1; ci += ASSOC_KEPT_THREADS)
+            if (!a.keep || __ldg(a.keep + ci)) s_list[atomicAdd(&s_n, 1)] = ci;
+        __syncthreads();
+        const int ncl = s_ncl, items = s_n * ncl;
+        for (int item = tid; item < items; item += ASSOC_KEPT_THREADS) {
+            const int ci = s_list[item / ncl], cl = s_cls[item % ncl];
+            const int4 q = __ldg(reinterpret_cast<const int4*>(a.cands + ci));          // event, k, i, j
+            const int votes = __ldg(&a.cands[ci].votes);
+            const float2 cs = __ldg(c.cs + q.z);
+            const float4 d = __ldg(c.d0t + q.y);
+            const int e_lo = max(q.w - dj, 0), e_hi = min(q.w + dj + 1, nq);
+            const float2* tb = a.tab + ((size_t)cl * c.n_d0 + q.y) * nq1;
+            const float2 ta = __ldg(tb + e_lo), tz = __ldg(tb + e_hi);
+            const float col = (float)q.z;
+            const float ua = col + fminf(ta.x, tz.x) - a.margin_cols;
+            const float ub = col + fmaxf(ta.y, tz.y) + a.margin_cols;
+            const float fa = floorf((ua + 0.5f) * a.sec_per_col - 1.0e-3f);
+            const float fb = floorf((ub + 0.5f) * a.sec_per_col + 1.0e-3f);
+            const int base = cl * NS;
+            int p0, n0, p1 = 0, n1 = 0;
+            const float nsf = fb - fa + 1.0f;
+            if (!(nsf < (float)NS)) {
+                p0 = __ldg(ks + base);
+                n0 = __ldg(ks + base + NS) - p0;
+            } else {
+                const int ns = (int)nsf;
+                int sa = (int)fa % NS;
+                if (sa < 0) sa += NS;
+                p0 = __ldg(ks + base + sa);
+                if (sa + ns <= NS) {
+                    n0 = __ldg(ks + base + sa + ns) - p0;
+                } else {
+                    n0 = __ldg(ks + base + NS) - p0;
+                    p1 = __ldg(ks + base);
+                    n1 = __ldg(ks + base + sa + ns - NS) - p1;
+                }
+            }
+            const unsigned long long ub_key = assoc_key(votes, 0, ci);      // the best this candidate can offer any hit
+            for (int t = 0; t < n0 + n1; ++t) {
+                const int pos = t < n0 ? p0 + t : p1 + (t - n0);
+                unsigned long long* bp = a.best_key + ev_begin + pos;
+                if (!(ub_key > __ldcg(bp))) continue;
+                const float4 hv = __ldg(a.staged + ev_begin + pos);
+                const int jh = d3_exact_bin(hv.x, hv.y, d3_r2(hv.x, hv.y), cs.x, cs.y, d.x, d.y, d.z, c.A_f, c.qmin, c.inv_wq, c.nq_f,
+                                            line);
+                const int adj = abs(jh - q.w);
+                if (jh >= 0 && adj <= dj) {
+                    const unsigned long long key = assoc_key(votes, adj, ci);
+                    if (key > __ldcg(bp)) atomicMax(bp, key);
+                }
+            }
+        }
+    }
+}
+
 // best key by staged position -> hit_to_cand by original hit index, and the per-candidate hit counts
 // ORPHANS (D12 re-assignment round): only hits still at -1 take the new key; the others and their counts stay.
 template <bool ORPHANS>
@@ -364,6 +455,17 @@ int hough_assoc_candidates(hough_plan* p, const int32_t* d_event_offsets, int32_
     const long long grid = (long long)n_events * a.parts;
     if (grid > 0x7fffffffLL) return HOUGH_ERR_UNSUPPORTED;
     int launches = 1;
+    if (d_keep_filter) {
+        // D12 round: few survivors per event -> (candidate, class) items dealt to threads, keys straight into global memory
+        long long kp = (4LL * p->sm_count + n_events - 1) / n_events;
+        a.parts = (int)std::min<long long>(std::max<long long>(kp, 1), 64);
+        assoc_kept_kernel<<<(unsigned)((long long)n_events * a.parts), ASSOC_KEPT_THREADS, 0, st>>>(p->c, a);
+        HOUGH_CUDA_TRY(cudaGetLastError());
+        assoc_decode_kernel<true><<<(n_hits + 255) / 256, 256, 0, st>>>(p->d_best_key, p->d_staged, n_hits, d_hit_to_cand, d_cand_nhits);
+        HOUGH_CUDA_TRY(cudaGetLastError());
+        hough_count_launches(2);
+        return HOUGH_OK;
+    }
     if (smem_hits > 0) {
         assoc_cand_kernel<true><<<(unsigned)grid, ASSOC_THREADS, smem, st>>>(p->c, a);
         HOUGH_CUDA_TRY(cudaGetLastError());
