@@ -35,7 +35,8 @@
 extern "C" {
 #endif
 
-enum { HOUGH_OK = 0, HOUGH_ERR_INVALID_ARG = -1, HOUGH_ERR_CUDA = -2, HOUGH_ERR_ALLOC = -3, HOUGH_ERR_UNSUPPORTED = -4 };
+enum { HOUGH_OK = 0, HOUGH_ERR_INVALID_ARG = -1, HOUGH_ERR_CUDA = -2, HOUGH_ERR_ALLOC = -3, HOUGH_ERR_UNSUPPORTED = -4,
+       HOUGH_ERR_TOO_LARGE = -5 /* a size beyond the fixed limit of a no-allocation entry point */ };
 enum { HOUGH_ACC_I32 = 0, HOUGH_ACC_U16 = 1 };
 /* Track model = which parameter is solved per (hit, phi0 column).  HELIX: curved tracks, signed q/pT (D3; the space of
  * B:L5).  LINE: straight displaced tracks ("or straight displaced tracks"; zero field): the impact
@@ -181,6 +182,33 @@ int hough_fit_circles(hough_plan* plan, const float* d_hits_xy, int32_t n_hits, 
                       const hough_candidate* d_cands, const int32_t* d_cand_offsets, int32_t n_events, int32_t capacity,
                       const uint8_t* d_cand_keep, double* d_work, hough_track_fit* d_fit, int32_t* d_n_fit,
                       void* cuda_stream);
+
+/* hough_fit_circles_static -- hough_fit_circles for callers that cannot allocate device memory (same fit: PAPER.md:37, D11).
+ * Some users of this library may not call cudaMalloc where they need the fit: an event loop with a fixed time budget per
+ * event (a trigger; cudaMalloc / cudaFree take unbounded time and stall the whole device), or a plug-in inside an
+ * application whose GPU memory belongs to another memory manager and which is given only its input and output buffers.
+ * hough_fit_circles needs scratch from the caller (d_work) and a plan (whose creation allocates); this call needs neither:
+ * the moment sums go to a fixed array inside the library image, HOUGH_FIT_STATIC_MAX_CANDIDATES rows of 9 doubles
+ * (4.5 MiB), which every GPU that loads the library holds until the process exits.  The call itself allocates and frees
+ * nothing: no cudaMalloc, no cudaFree, no library routine that allocates.
+ * Arguments: n_phi and bz_tesla are the two plan values the fit uses (number of phi0 columns of the space the candidates
+ * come from; Bz in tesla, 0 gives q/pT = 0); all other arguments, outputs, alignment rules and tolerances are those of
+ * hough_fit_circles, computed by the same kernels.  Enqueues on cuda_stream and returns.
+ * Rules that follow from the shared array:
+ *   - capacity > HOUGH_FIT_STATIC_MAX_CANDIDATES returns HOUGH_ERR_TOO_LARGE and enqueues nothing (split the list, or use
+ *     hough_fit_circles with your own scratch);
+ *   - there is ONE array per GPU, shared by every call and keeping the last call's sums (each call zeroes the rows it
+ *     uses first): calls that can run on the GPU at the same time -- other streams, other threads -- race and give wrong
+ *     fits; issue them on one stream or order them with events;
+ *   - the first call on each GPU also looks up that GPU's copy of the array (cudaGetSymbolAddress, cached per device
+ *     afterwards): make one call per device at start-up (capacity >= 1; n_hits = 0 will do), with that device
+ *     current, before any stream capture begins.  cuda_stream must belong to the current device.
+ * Errors: INVALID_ARG (null / misaligned pointers, negative sizes, n_phi <= 0), TOO_LARGE, CUDA. */
+#define HOUGH_FIT_STATIC_MAX_CANDIDATES 65536
+int hough_fit_circles_static(int32_t n_phi, float bz_tesla, const float* d_hits_xy, int32_t n_hits,
+                             const int32_t* d_hit_to_cand, const hough_candidate* d_cands, const int32_t* d_cand_offsets,
+                             int32_t n_events, int32_t capacity, const uint8_t* d_cand_keep, hough_track_fit* d_fit,
+                             int32_t* d_n_fit, void* cuda_stream);
 
 /* Plan options (debug / tuning; results never change).  key "fullscan": 1 = evaluate every (hit,i,k) with
  * no windowing and vote straight into global memory (the bisecting path of SURVEY section 5; also read once at

@@ -3,7 +3,7 @@
 The product is `libhough_b200.so` (CUDA, sm_100a; C ABI in include/hough.h).  This package is its thin Python
 binding: same names as the C calls, argument marshalling only, PyTorch for device memory and streams.
 """
-from .binding import (HoughPlan, HoughPipeline, HoughError, hough_vertex_vote, hough_fit_circles, CAND_DTYPE, HOUGH_ACC_I32, HOUGH_ACC_U16, HOUGH_MODEL_HELIX, HOUGH_MODEL_LINE, alloc_candidates,
+from .binding import (HoughPlan, HoughPipeline, HoughError, hough_vertex_vote, hough_fit_circles, hough_fit_circles_static, FIT_STATIC_MAX_CANDIDATES, CAND_DTYPE, HOUGH_ACC_I32, HOUGH_ACC_U16, HOUGH_MODEL_HELIX, HOUGH_MODEL_LINE, alloc_candidates,
                       candidates_to_numpy, load_library, microbench, window_table, kernel_launches, version, LIB_PATH, EXPORTS)
 
 

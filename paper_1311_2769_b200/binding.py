@@ -40,7 +40,7 @@ class hough_geometry(C.Structure):
 
 
 EXPORTS = ["hough_plan_create", "hough_plan_destroy", "hough_accum_bytes", "hough_vote", "hough_find_peaks",
-           "hough_assign_hits", "hough_reassign_hits", "hough_event_run", "hough_vertex_vote", "hough_fit_circles", "hough_plan_set_option", "hough_pipeline_create", "hough_pipeline_destroy",
+           "hough_assign_hits", "hough_reassign_hits", "hough_event_run", "hough_vertex_vote", "hough_fit_circles", "hough_fit_circles_static", "hough_plan_set_option", "hough_pipeline_create", "hough_pipeline_destroy",
            "hough_pipeline_run_host", "hough_pipeline_set_option", "hough_window_table", "hough_microbench", "hough_kernel_launches", "hough_status_string",
            "hough_version"]
 
@@ -77,6 +77,8 @@ def load_library() -> C.CDLL:
     lib.hough_vertex_vote.argtypes = [P, P, P, I, I, P, C.c_float, I, C.c_float, P, P]
     lib.hough_fit_circles.restype = C.c_int
     lib.hough_fit_circles.argtypes = [P, P, I, P, P, P, I, I, P, P, P, P, P]
+    lib.hough_fit_circles_static.restype = C.c_int
+    lib.hough_fit_circles_static.argtypes = [I, C.c_float, P, I, P, P, P, I, I, P, P, P, P]
     lib.hough_plan_set_option.restype = C.c_int
     lib.hough_plan_set_option.argtypes = [P, C.c_char_p, I]
     lib.hough_pipeline_create.restype = C.c_int
@@ -296,6 +298,22 @@ def hough_fit_circles(plan: "HoughPlan", hits_xy, hit_to_cand, cands, cand_offse
     _check(plan.lib.hough_fit_circles(plan._h, _dptr(hits_xy), int(hits_xy.shape[0]), _dptr(hit_to_cand), _dptr(cands),
                                       _dptr(cand_offsets), int(n_events), int(capacity), _dptr(cand_keep), _dptr(work),
                                       _dptr(fit), _dptr(n_fit), _stream_ptr(stream)), "hough_fit_circles")
+
+
+FIT_STATIC_MAX_CANDIDATES = 65536   # include/hough.h HOUGH_FIT_STATIC_MAX_CANDIDATES
+
+
+def hough_fit_circles_static(n_phi, bz_tesla, hits_xy, hit_to_cand, cands, cand_offsets, n_events, capacity, cand_keep, fit,
+                             n_fit, stream=None):
+    """include/hough.h hough_fit_circles_static: the circle fit for callers that may not allocate device memory (a
+    fixed-latency event loop, a plug-in whose host application owns all GPU memory).  No plan and no work buffer: the moment
+    sums use a fixed per-GPU array inside the library, so capacity <= FIT_STATIC_MAX_CANDIDATES, calls on one GPU must not
+    overlap, and the first call per device (address look-up) belongs to start-up.  fit float64 [capacity, 4], n_fit int32."""
+    assert capacity == 0 or (fit.dtype == torch.float64 and n_fit.dtype == torch.int32)
+    _check(load_library().hough_fit_circles_static(int(n_phi), float(bz_tesla), _dptr(hits_xy), int(hits_xy.shape[0]),
+                                                   _dptr(hit_to_cand), _dptr(cands), _dptr(cand_offsets), int(n_events),
+                                                   int(capacity), _dptr(cand_keep), _dptr(fit), _dptr(n_fit),
+                                                   _stream_ptr(stream)), "hough_fit_circles_static")
 
 
 def window_table(n_phi, n_qpt, n_d0, qpt_min=-1.0, qpt_max=1.0, d0_min=-20.0, d0_max=20.0, bz_tesla=3.8, layers=(),

@@ -7,6 +7,7 @@
 //            closed form from (centre, R, orientation) -- a different algebraic route from the 3x3 Cramer solve of the CPU
 //            checker under tests/, so that the parity test compares two independent solves
 #include <cmath>
+#include <mutex>
 
 #include "common.cuh"
 
@@ -114,6 +115,90 @@ extern "C" int hough_fit_circles(hough_plan* p, const float* d_hits_xy, int32_t 
     }
     const double kb = 0.00299792458 * (double)p->bz;
     fit_solve_kernel<<<(capacity + 127) / 128, 128, 0, st>>>(p->c, kb, d_cands, d_cand_offsets, n_events, capacity, d_cand_keep,
+                                                            d_work, d_fit, d_n_fit);
+    HOUGH_CUDA_TRY(cudaGetLastError());
+    hough_count_launches(n_hits > 0 ? 3 : 2);
+    return HOUGH_OK;
+}
+
+// ---------------------------------------------------------------------------------------------------------------------
+// hough_fit_circles_static: the same three kernels, for callers that must not allocate device memory.
+//
+// Who that is.  (1) Trigger-style event loops (the paper's setting: a fixed time budget per event):
+// cudaMalloc / cudaFree take an unbounded time and stall every stream of the device while they run, so such a loop
+// may not reach them once it is live.  (2) Plug-ins inside a host application whose GPU memory is entirely managed by
+// someone else (a framework's caching pool, an experiment's memory manager with a fixed budget): they are handed
+// their input and output buffers and have nowhere to get 72 bytes of moment scratch per candidate from.
+//
+// The scratch therefore lives in the library image: one fixed array per GPU, reserved when the library's code is loaded
+// onto that GPU and held until the process exits (4.5 MiB).  Consequences a caller has to know:
+//   * capacity is limited to HOUGH_FIT_STATIC_MAX_CANDIDATES; larger requests are refused, nothing is enqueued;
+//   * all calls on one GPU share the array: two calls whose kernels can be in flight at the same time (different streams,
+//     or different host threads on different streams) corrupt each other's sums -- keep them on one stream or order them
+//     with events; the array also keeps the previous call's sums, which is why K-fit-a zeroes the rows in use every call;
+//   * the first call on each GPU looks up the array's device address (set-up, below); make that first call during
+//     start-up, on the device the later calls will use, and before any stream capture is begun.
+//
+// `g_fit_scratch` as written in host code is only a handle for the runtime's symbol table, NOT a device address:
+// handing it to a kernel would make the kernel read and write through a host pointer.  fit_static_scratch() turns it into
+// the real address with cudaGetSymbolAddress, per device, because every GPU holds its own copy at its own address.
+constexpr int FIT_STATIC_ROW = 9;   // doubles per candidate: {n, Sx, Sy, Sz, Sxx, Sxy, Syy, Sxz, Syz}
+static __device__ __align__(256) double g_fit_scratch[(size_t)HOUGH_FIT_STATIC_MAX_CANDIDATES * FIT_STATIC_ROW];
+
+namespace {
+
+std::mutex g_fit_static_mu;
+double* g_fit_static_ptr[HOUGH_MAX_DEVICES];   // per device: address of that GPU's copy of g_fit_scratch (null: not looked up)
+
+// Address of the CURRENT device's scratch array.  Cached per device; a device index beyond the cache asks every time.
+int fit_static_scratch(double** out) {
+    int dev = -1;
+    HOUGH_CUDA_TRY(cudaGetDevice(&dev));
+    std::lock_guard<std::mutex> lock(g_fit_static_mu);
+    if (dev >= 0 && dev < HOUGH_MAX_DEVICES && g_fit_static_ptr[dev]) {
+        *out = g_fit_static_ptr[dev];
+        return HOUGH_OK;
+    }
+    double* ptr = nullptr;
+    HOUGH_CUDA_TRY(cudaGetSymbolAddress(reinterpret_cast<void**>(&ptr), g_fit_scratch));
+    if (!ptr) return HOUGH_ERR_CUDA;
+    if (dev >= 0 && dev < HOUGH_MAX_DEVICES) g_fit_static_ptr[dev] = ptr;
+    *out = ptr;
+    return HOUGH_OK;
+}
+
+}  // namespace
+
+extern "C" int hough_fit_circles_static(int32_t n_phi, float bz_tesla, const float* d_hits_xy, int32_t n_hits,
+                                        const int32_t* d_hit_to_cand, const hough_candidate* d_cands,
+                                        const int32_t* d_cand_offsets, int32_t n_events, int32_t capacity,
+                                        const uint8_t* d_cand_keep, hough_track_fit* d_fit, int32_t* d_n_fit,
+                                        void* cuda_stream) {
+    if (!d_cand_offsets || n_phi <= 0) return HOUGH_ERR_INVALID_ARG;
+    if (n_hits < 0 || n_events < 0 || capacity < 0) return HOUGH_ERR_INVALID_ARG;
+    if (capacity > HOUGH_FIT_STATIC_MAX_CANDIDATES) return HOUGH_ERR_TOO_LARGE;   // the fixed scratch has no more rows
+    if (n_hits > 0 && (!d_hits_xy || !d_hit_to_cand)) return HOUGH_ERR_INVALID_ARG;
+    if (capacity > 0 && (!d_cands || !d_fit || !d_n_fit)) return HOUGH_ERR_INVALID_ARG;
+    if ((reinterpret_cast<uintptr_t>(d_hits_xy) & 7u) || (reinterpret_cast<uintptr_t>(d_cands) & 15u) ||
+        (reinterpret_cast<uintptr_t>(d_fit) & 7u))
+        return HOUGH_ERR_INVALID_ARG;
+    if (capacity == 0) return HOUGH_OK;
+    double* d_work = nullptr;
+    const int rc = fit_static_scratch(&d_work);
+    if (rc != HOUGH_OK) return rc;
+    cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
+    HoughConsts c{};                   // the solve reads n_phi only (orientation of the circle by the candidate's column)
+    c.n_phi = n_phi;
+    const long long cells = (long long)capacity * FIT_STATIC_ROW;
+    fit_zero_kernel<<<(unsigned)((cells + 255) / 256), 256, 0, st>>>(d_cand_offsets, n_events, capacity, d_work);
+    HOUGH_CUDA_TRY(cudaGetLastError());
+    if (n_hits > 0) {
+        fit_moments_kernel<<<(n_hits + 255) / 256, 256, 0, st>>>(reinterpret_cast<const float2*>(d_hits_xy), n_hits,
+                                                                 d_hit_to_cand, d_cand_offsets, n_events, capacity, d_work);
+        HOUGH_CUDA_TRY(cudaGetLastError());
+    }
+    const double kb = 0.00299792458 * (double)bz_tesla;
+    fit_solve_kernel<<<(capacity + 127) / 128, 128, 0, st>>>(c, kb, d_cands, d_cand_offsets, n_events, capacity, d_cand_keep,
                                                             d_work, d_fit, d_n_fit);
     HOUGH_CUDA_TRY(cudaGetLastError());
     hough_count_launches(n_hits > 0 ? 3 : 2);

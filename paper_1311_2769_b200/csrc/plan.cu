@@ -31,6 +31,8 @@ extern "C" const char* hough_status_string(int status) {
         case HOUGH_ERR_CUDA: return g_last_cuda[0] ? g_last_cuda : "CUDA error";
         case HOUGH_ERR_ALLOC: return "allocation failed";
         case HOUGH_ERR_UNSUPPORTED: return "unsupported configuration";
+        case HOUGH_ERR_TOO_LARGE:
+            return "size exceeds the fixed scratch of a no-allocation entry point (HOUGH_FIT_STATIC_MAX_CANDIDATES)";
         default: return "unknown status";
     }
 }
