@@ -146,9 +146,12 @@ int hough_event_run(hough_plan* plan, const float* d_hits_xy, int32_t n_hits, co
  * max_rounds >= 2 (max_rounds == 1: returns at once).  Effect: every hit with d_hit_to_cand[h] == -1 gets the best
  * candidate with d_cand_keep != 0 (or stays -1), d_cand_nhits of that candidate is incremented; hits that had a kept
  * candidate, d_cand_nhits of dropped candidates and d_cand_keep are left as they are.
- * Tiled plans take the candidate-centric association over the surviving candidates; its azimuth-interval table is built
- * on the first call (one cudaMalloc + device synchronisation: make that call outside stream capture), or, if the table
- * does not fit or the plan option "reassign_walk" is set, re-walk the vote columns against the surviving candidates.
+ * Tiled plans take the candidate-centric association over the surviving candidates, which needs an azimuth-interval table
+ * per plan.  Build it at set-up with hough_plan_set_option(plan, "prepare_reassign", 1) (one cudaMalloc + device
+ * synchronisation); the pipeline option "reassign" does so for its lanes.  Without that, the first call whose stream is NOT
+ * under capture builds it; a call on a capturing stream never allocates or synchronises -- while there is no table (not
+ * built yet, does not fit, build failed, or plan option "reassign_walk") the call re-walks the vote columns against the
+ * surviving candidates, with the same results.
  * Errors: INVALID_ARG (null pointers, sizes, max_rounds < 1), UNSUPPORTED, CUDA. */
 int hough_reassign_hits(hough_plan* plan, const float* d_hits_xy, int32_t n_hits, const int32_t* d_event_offsets,
                         int32_t n_events, const hough_candidate* d_cands, const int32_t* d_cand_offsets,
@@ -217,8 +220,10 @@ int hough_fit_circles_static(int32_t n_phi, float bz_tesla, const float* d_hits_
  * peak kernels; "peaks_scalar": 1 = the unpacked slice-walk peak kernel also for 16-bit bins, "peaks_regs": 1 = the packed
  * 16-bit walk with rows held in registers instead of the cp.async shared-memory ring.  "reuse_staging": 1 = the caller promises that a hough_assign_hits call whose hit pointer, offsets
  * pointer, sizes and stream equal those of the preceding hough_vote sees unchanged hits, so the staged (sorted)
- * copy of that vote is reused instead of rebuilt.
- * Environment (read at plan creation, work sizing only): HOUGH_SECTORS=n phi sectors of the staging sort (default 32). */
+ * copy of that vote is reused instead of rebuilt.  "prepare_reassign": 1 = build the table of hough_reassign_hits now
+ * (allocates and synchronises; always HOUGH_OK -- without a table that call re-walks the columns).
+ * Environment (read at plan creation, work sizing only): HOUGH_SECTORS=n phi sectors of the staging sort
+ * (default: n_phi clamped to [32, 1024], halved while the plan's key table max_events x classes x sectors exceeds 32 MiB). */
 int hough_plan_set_option(hough_plan* plan, const char* key, int32_t value);
 
 /* Batched multi-event pipeline (B:L5 "a batched multi-event path using CUDA streams and graphs"; B:L10).

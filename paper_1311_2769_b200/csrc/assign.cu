@@ -325,10 +325,13 @@ extern "C" int hough_reassign_hits(hough_plan* p, const float* d_hits_xy, int32_
     if (tiled) {
         int rc = hough_stage_hits(p, d_hits_xy, n_hits, d_event_offsets, n_events, st, true);
         if (rc != HOUGH_OK) return rc;
-        if (!p->reassign_walk && !p->d_assoc_tab && !p->assoc_tab_tried) {      // first use: build the table (one device sync)
-            p->assoc_tab_tried = 1;
-            rc = hough_build_assoc_table(p);
-            if (rc != HOUGH_OK) return rc;
+        if (!p->reassign_walk && !p->d_assoc_tab && !p->assoc_tab_tried) {
+            // No table yet and plan option "prepare_reassign" was not used.  Building it allocates and synchronises, which a
+            // stream under capture forbids: build only when `st` is not capturing, otherwise this call re-walks the columns
+            // (same results) and a later un-captured call builds.  A failed build is not an error either: walk instead.
+            cudaStreamCaptureStatus cs = cudaStreamCaptureStatusActive;
+            if (cudaStreamIsCapturing(st, &cs) != cudaSuccess) { (void)cudaGetLastError(); cs = cudaStreamCaptureStatusActive; }
+            if (cs == cudaStreamCaptureStatusNone) hough_prepare_reassign(p);
         }
         if (p->d_assoc_tab != nullptr && !p->reassign_walk)
             // few candidates survive D9: the candidate-centric association (assoc.cu) visits only them

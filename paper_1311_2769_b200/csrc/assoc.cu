@@ -418,6 +418,13 @@ int hough_build_assoc_table(hough_plan* p) {
     return HOUGH_OK;
 }
 
+int hough_prepare_reassign(hough_plan* p) {
+    if (p->d_assoc_tab || p->assoc_tab_tried || p->fullscan || p->tile_max_cols < 1) return HOUGH_OK;
+    p->assoc_tab_tried = 1;
+    if (hough_build_assoc_table(p) != HOUGH_OK) p->d_assoc_tab = nullptr;      // no table: the D12 round re-walks the columns
+    return HOUGH_OK;
+}
+
 // Candidate-centric association of a staged call: folds the D8 keys into p->d_best_key (zeroed by the caller, indexed by
 // STAGED position) and decodes them into d_hit_to_cand / d_cand_nhits.
 int hough_assoc_candidates(hough_plan* p, const int32_t* d_event_offsets, int32_t n_hits, int32_t n_events,

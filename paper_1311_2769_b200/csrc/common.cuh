@@ -59,6 +59,7 @@ struct HoughConsts {
 constexpr int HOUGH_MAX_CLASSES = 255;
 constexpr int HOUGH_MAX_DEVICES = 64;       // per-device caches of kernel attributes (a device index beyond it: set every call)
 constexpr int HOUGH_SECTORS_MIN = 32, HOUGH_SECTORS_MAX = 1024;   // phi sectors of the staging sort: n_phi clamped to this range
+constexpr long long HOUGH_STAGE_TABLE_BYTES = 32LL << 20;         // ... and halved until the per-call key-start table fits this
 
 struct HoughWindows {             // host copy of the class / window tables
     int n_class = 0;
@@ -79,7 +80,7 @@ struct hough_plan {
     int peaks_regs;                    // 1: 16-bit packed peak walk with register-held rows instead of the cp.async ring
     int peaks_scalar;                  // 1: 16-bit accumulators use the unpacked slice-walk peak kernel (bisecting)
     int exact_walk;                    // 1: the walks evaluate the D3 sequence at every column (no fast path)
-    float m_scale;                     // 1 (HOUGH_DEBUG_M_SCALE: scales the fast path's error bound, to probe its margin)
+    float m_scale;                     // 1 (self-check build: HOUGH_DEBUG_M_SCALE scales the fast path's error bound, to probe its margin)
     int assign_candidates;             // 1: hough_assign_hits takes the candidate-centric path (assoc.cu) instead of re-walking the vote columns
     int reuse_staging;                 // 1: hough_assign_hits may reuse the staging of the preceding hough_vote (same arguments)
     const void* staged_hits; const void* staged_off; int32_t staged_n_hits, staged_n_events; cudaStream_t staged_stream;
@@ -110,6 +111,7 @@ struct hough_plan {
     float2* d_assoc_tab;               // [n_class][n_d0][n_qpt + 1] azimuth-offset hulls per bin edge; null: not built
     int reassign_walk;                 // 1: hough_reassign_hits re-walks the vote columns instead of the candidate-centric path
     int assoc_tab_tried;               // the assoc table was requested once (it may not fit: d_assoc_tab stays null)
+    int assoc_tab_borrowed;            // d_assoc_tab belongs to another plan of the same binning / geometry (pipeline lanes): not freed here
     int event_max_steps;               // longest column window of any radius class in slice 0 (work estimate of hough_event_run)
     int event_cluster;                 // 1: hough_event_run takes the cluster kernel whenever it fits, whatever the work estimate says
     int event_general;                 // 1: hough_event_run always takes the three general calls (bisecting / comparison)
@@ -214,6 +216,10 @@ __device__ __forceinline__ void cta_exclusive_scan(int32_t* data, int n, int32_t
 int hough_stage_hits(hough_plan* p, const float* d_hits_xy, int32_t n_hits, const int32_t* d_event_offsets,
                      int32_t n_events, cudaStream_t st, bool may_reuse);
 int hough_build_assoc_table(hough_plan* p);
+// Builds the plan's assoc table now if it has none and none was tried (allocates + synchronises: never call it from a
+// stream-ordered entry point that may be under capture).  Always HOUGH_OK: a table that does not fit or cannot be built
+// leaves d_assoc_tab null, and hough_reassign_hits then re-walks the vote columns.
+int hough_prepare_reassign(hough_plan* p);
 int hough_assoc_candidates(hough_plan* p, const int32_t* d_event_offsets, int32_t n_hits, int32_t n_events,
                            const hough_candidate* d_cands, const int32_t* d_cand_offsets, int32_t capacity, int32_t assoc_dj,
                            int32_t* d_hit_to_cand, int32_t* d_cand_nhits, cudaStream_t st, const uint8_t* d_keep_filter);

@@ -208,9 +208,23 @@ extern "C" int hough_pipeline_set_option(hough_pipeline* p, const char* key, int
     if (strcmp(key, "graphs") == 0) { p->use_graphs = value ? 1 : 0; return HOUGH_OK; }
     if (strcmp(key, "reassign") == 0) {
         p->reassign = value ? 1 : 0;
-        for (Lane& l : p->lanes) {                           // another node list: the lanes' graphs are rebuilt; the next tile of
-            if (l.exec) { cudaGraphExecDestroy(l.exec); l.exec = nullptr; }      // a lane runs un-captured once (the D12 table
-            l.warmed = false;                                                    // is built on first use, outside capture)
+        if (value && !p->lanes.empty()) {
+            // The D12 round's azimuth table is built HERE, never inside a tile's (captured) sequence: once, on lane 0's plan;
+            // the other lanes' plans have the same binning and geometry and borrow it (read-only).  No table (it does not
+            // fit, or the build failed): every lane re-walks the vote columns instead.
+            hough_plan* first = p->lanes[0].plan;
+            hough_prepare_reassign(first);
+            for (size_t i = 1; i < p->lanes.size(); ++i) {
+                hough_plan* q = p->lanes[i].plan;
+                if (q->d_assoc_tab || q->assoc_tab_tried) continue;
+                q->assoc_tab_tried = 1;
+                q->d_assoc_tab = first->d_assoc_tab;
+                q->assoc_tab_borrowed = first->d_assoc_tab != nullptr;
+            }
+        }
+        for (Lane& l : p->lanes) {                           // another node list: the lanes' graphs are rebuilt, and the next
+            if (l.exec) { cudaGraphExecDestroy(l.exec); l.exec = nullptr; }      // tile of a lane runs un-captured once (lazy
+            l.warmed = false;                                                    // kernel attributes of the added kernels)
         }
         return HOUGH_OK;
     }

@@ -54,7 +54,7 @@ static void plan_free(hough_plan* p) {
     cudaFree(p->d_slice);
     cudaFree(p->d_edge2);
     cudaFree(p->d_win);
-    cudaFree(p->d_assoc_tab);
+    if (!p->assoc_tab_borrowed) cudaFree(p->d_assoc_tab);
     delete p;
 }
 
@@ -86,8 +86,13 @@ extern "C" int hough_plan_create(const hough_binning* b, const hough_geometry* g
     p->fullscan = (env && env[0] == '1') ? 1 : 0;
     env = getenv("HOUGH_DEBUG_EXACT_WALK");
     p->exact_walk = (env && env[0] == '1') ? 1 : 0;
+    p->m_scale = 1.0f;
+#ifdef HOUGH_CHECKS
+    // self-check build only (never in libhough_b200.so): scale the fast path's error bound to probe its margin -- values
+    // below 1 break bit-exactness on purpose (profiles/r2_walk.md)
     env = getenv("HOUGH_DEBUG_M_SCALE");
-    p->m_scale = (env && atof(env) >= 0.0) ? (float)atof(env) : 1.0f;
+    if (env && atof(env) >= 0.0) p->m_scale = (float)atof(env);
+#endif
 
     cudaError_t ce = cudaGetDevice(&p->device);
     if (ce == cudaSuccess) ce = cudaDeviceGetAttribute(&p->sm_count, cudaDevAttrMultiProcessorCount, p->device);
@@ -146,6 +151,13 @@ extern "C" int hough_plan_create(const hough_binning* b, const hough_geometry* g
     // one sector per phi0 column (clamped): fine enough for the candidate-centric association to read a candidate's
     // hits off the key-start table, and the vote walk is insensitive to the count above 32 (profiles/r1_final.md)
     c.n_sector = std::min(std::max(b->n_phi, HOUGH_SECTORS_MIN), HOUGH_SECTORS_MAX);
+    // ... but the key-start table [max_events][n_class * n_sector + 1] is cleared and scanned by every staging call: halve
+    // the sector count until the table is at most HOUGH_STAGE_TABLE_BYTES (a 1024-event plan with n_phi >= 1024 would
+    // otherwise clear ~290 MB per call, 32x the 32-sector table).  Coarser sectors only make the candidate-centric
+    // association read a few more hits per candidate.
+    while (c.n_sector > HOUGH_SECTORS_MIN &&
+           (long long)max_events * ((long long)c.n_class * c.n_sector + 1) * (long long)sizeof(int32_t) > HOUGH_STAGE_TABLE_BYTES)
+        c.n_sector = std::max(c.n_sector / 2, HOUGH_SECTORS_MIN);
     { const char* es = getenv("HOUGH_SECTORS"); if (es && atoi(es) >= 1 && atoi(es) <= HOUGH_SECTORS_MAX) c.n_sector = atoi(es); }
     c.n_keys = c.n_class * c.n_sector;
     c.u_scale = (float)((double)b->n_phi / (2.0 * kPi));
@@ -163,7 +175,9 @@ extern "C" int hough_plan_create(const hough_binning* b, const hough_geometry* g
     // packed 16-bit tiles are exact whenever no bin can exceed 65535: the U16 precondition, or at most 65535
     // hits per call (a hit casts at most one vote per (phi0, d0) column, D3)
     p->tile32 = (b->accum_dtype == HOUGH_ACC_I32 && max_hits > 65535) ? 1 : 0;
-    { const char* et = getenv("HOUGH_FORCE_TILE32"); if (et && et[0] == '1') p->tile32 = 1; }
+#ifdef HOUGH_CHECKS
+    { const char* et = getenv("HOUGH_FORCE_TILE32"); if (et && et[0] == '1') p->tile32 = 1; }   // layout experiments, checks build only
+#endif
     {
         // walk.cuh "Tile layout": a row (32-bit bins) or a row of column PAIRS (16-bit bins) has `stride` words.
         // Largest even column count whose whole shared-memory block lets 3 CTAs share an SM (228 KB, 1 KB reserved per
@@ -253,6 +267,7 @@ extern "C" int hough_plan_set_option(hough_plan* p, const char* key, int32_t val
     if (strcmp(key, "event_cluster") == 0) { p->event_cluster = value ? 1 : 0; return HOUGH_OK; }
     if (strcmp(key, "event_general") == 0) { p->event_general = value ? 1 : 0; return HOUGH_OK; }
     if (strcmp(key, "reassign_walk") == 0) { p->reassign_walk = value ? 1 : 0; return HOUGH_OK; }
+    if (strcmp(key, "prepare_reassign") == 0) return value ? hough_prepare_reassign(p) : HOUGH_OK;
     if (strcmp(key, "exact_walk") == 0) { p->exact_walk = value ? 1 : 0; return HOUGH_OK; }
     if (strcmp(key, "reuse_staging") == 0) { p->reuse_staging = value ? 1 : 0; p->staged_hits = nullptr; return HOUGH_OK; }
     return HOUGH_ERR_INVALID_ARG;

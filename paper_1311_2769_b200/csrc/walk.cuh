@@ -51,7 +51,7 @@ struct WalkArgs {
     const int32_t* key_start;        // [n_events][n_keys + 1] exclusive key starts
     int n_slabs, slab_cols, stride;  // tile shape (slab_cols even; stride = words per row / pair row, odd)
     int exact_only;                  // 1: never take the fast path (plan option "exact_walk", for bisecting)
-    float m_scale;                   // 1; HOUGH_DEBUG_M_SCALE scales the bound m (margin probe of the tests, profiles/r2_walk.md)
+    float m_scale;                   // 1; the self-check build's HOUGH_DEBUG_M_SCALE scales the bound m (margin probe, profiles/r2_walk.md)
     // WALK_VOTE
     void* accum;
     // WALK_ASSIGN
@@ -894,7 +894,9 @@ __global__ void __launch_bounds__(walk_threads(MODE), 3) walk_kernel(const __gri
 inline void walk_shape(const hough_plan* p, int n_events, int& n_slabs, int& slab_cols) {
     const int nphi = p->c.n_phi;
     n_slabs = (nphi + p->tile_max_cols - 1) / p->tile_max_cols;
-    { const char* es = getenv("HOUGH_FORCE_SLABS"); if (es && atoi(es) > n_slabs) n_slabs = atoi(es); }
+#ifdef HOUGH_CHECKS
+    { const char* es = getenv("HOUGH_FORCE_SLABS"); if (es && atoi(es) > n_slabs) n_slabs = atoi(es); }   // checks build only
+#endif
     const long long want = 3LL * p->sm_count;
     while ((long long)n_slabs * p->c.n_d0 * n_events < want && (nphi + n_slabs - 1) / n_slabs > 32) n_slabs *= 2;
     slab_cols = (nphi + n_slabs - 1) / n_slabs;

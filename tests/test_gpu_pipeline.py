@@ -158,3 +158,30 @@ def test_pipeline_reassign_option_runs_the_d12_round(kept_only):
         assert np.array_equal(h2c, np.where(h2c_ref >= 0, new_index[np.maximum(h2c_ref, 0)], -1))
         assert np.array_equal(nh[:int(kmask.sum())], nh_ref[kmask])
     assert (h2c >= 0).sum() > (_oracle_per_event(w, batch)[1] >= 0).sum()     # the round did recover hits
+
+
+@pytest.mark.parametrize("kept_only", [False, True])
+def test_pipeline_reassign_when_every_lane_starts_on_an_empty_tile(kept_only):
+    """Graphs on, option "reassign", and the FIRST tile of each lane has no hits (that tile runs un-captured and returns
+    before the D12 round): the round's table is built by set_option, so the following, captured tiles must not allocate."""
+    from workloads.generator import EventBatch
+    w = get_workload(3)
+    real = generate_events(w, events=[5, 6, 7])
+    n = [int(real.event_offsets[i + 1] - real.event_offsets[i]) for i in range(3)]
+    # events: empty, empty, e5, e6, empty, e7 -- tiles of one event on two lanes
+    off = np.cumsum([0, 0, 0, n[0], n[1], 0, n[2]]).astype(np.int32)
+    batch = EventBatch(real.hits_xy, off, None)
+    rec, h2c_ref, nh_ref, keep_ref, off_ref = _oracle_per_event(w, batch, rounds=True)
+    total = int(off_ref[-1])
+    tile_cap = int(np.diff(off_ref).max()) + 3
+    over, h2c, coff, cands, nh, keep = _run_pipeline(w, batch, 1, 2, tile_cap, total + 5, kept_only=kept_only, reassign=True)
+    assert not over
+    if not kept_only:
+        assert np.array_equal(coff, off_ref) and np.array_equal(h2c, h2c_ref)
+        assert np.array_equal(nh[:total], nh_ref) and np.array_equal(keep[:total], keep_ref)
+        assert np.array_equal(cands["event"][:total], rec["event"])
+    else:
+        kmask = keep_ref.astype(bool)
+        new_index = np.cumsum(kmask) - 1
+        assert np.array_equal(h2c, np.where(h2c_ref >= 0, new_index[np.maximum(h2c_ref, 0)], -1))
+        assert np.array_equal(nh[:int(kmask.sum())], nh_ref[kmask])
