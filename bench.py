@@ -141,12 +141,16 @@ def load_traffic():
     tab = {}
     if not os.path.exists(path):
         return tab, None
+    stamp = "unknown commit"
     with open(path) as f:
         for line in f:
             p = [x.strip() for x in line.split(",")]
-            if len(p) >= 3 and p[1].isdigit():
+            if len(p) >= 3 and p[0] == "# captured_at":
+                stamp = "kernels as of commit %s, %s" % (p[1], p[2].split(" ")[0])
+            elif len(p) >= 3 and p[1].isdigit():
                 tab[(p[0], int(p[1]))] = float(p[2])
-    return tab, "profiles/r2_traffic.csv (ncu --set full capture of this launch configuration; see profiles/r2_traffic.md)"
+    return tab, ("profiles/r2_traffic.csv (ncu --set full capture of this launch configuration, %s -- NOT measured in this "
+                 "run: stale if walk.cuh / peaks.cu changed since; see profiles/r2_traffic.md)" % stamp)
 
 
 # ----------------------------------------------------------------------------------------------
@@ -184,15 +188,28 @@ def oracle_sample(w, batch, n_sample_events: int):
     from oracle import Oracle
     sub = batch.select(list(range(min(n_sample_events, batch.n_events))))
     o = Oracle.from_binning(w.binning, w.bz_tesla)
-    t0 = time.perf_counter()
-    votes_total = 0
-    for e in range(sub.n_events):          # one event at a time keeps the oracle's int32 volume small
-        ev = sub.select([e])
-        acc, votes = o.vote(ev.hits_xy, ev.event_offsets)
-        cands = o.find_peaks(acc, w.threshold)
-        o.assign_indexed(ev.hits_xy, ev.event_offsets, cands, w.assoc_dj, w.min_hits)
-        votes_total += votes
-    return votes_total, sub.n_events, time.perf_counter() - t0
+    # the CPU baseline is timed on ONE core -- this thread is pinned to the core it is on for the duration
+    # (the oracle is single-threaded anyway; pinning only stops migrations) and released afterwards.
+    saved = None
+    try:
+        saved = os.sched_getaffinity(0)
+        os.sched_setaffinity(0, {sorted(saved)[-1]})
+    except (AttributeError, OSError):
+        saved = None
+    try:
+        t0 = time.perf_counter()
+        votes_total = 0
+        for e in range(sub.n_events):          # one event at a time keeps the oracle's int32 volume small
+            ev = sub.select([e])
+            acc, votes = o.vote(ev.hits_xy, ev.event_offsets)
+            cands = o.find_peaks(acc, w.threshold)
+            o.assign_indexed(ev.hits_xy, ev.event_offsets, cands, w.assoc_dj, w.min_hits)
+            votes_total += votes
+        secs = time.perf_counter() - t0
+    finally:
+        if saved is not None:
+            os.sched_setaffinity(0, saved)
+    return votes_total, sub.n_events, secs
 
 
 def oracle_events_for_seconds(w, target_s: float) -> int:
@@ -228,7 +245,7 @@ def run_reference(args, rank, world):
             "data": "synthetic", "events_per_s": n_ev * args.steps / secs,
             "config": {"workload": wl.name, "cite": wl.cite, "events_per_step": n_ev,
                        "note": "bounded sample of the workload; oracle single-threaded"},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample, "pinned_to_one_core": True},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
@@ -600,7 +617,7 @@ def run_ours(args, rank, world, local_rank):
     o_votes, o_events, o_secs = oracle_sample(w, batch, n_ref)
     cpu = {"value": o_votes / o_secs, "unit": UNIT, "cores": 1, "kind": "oracle",
            "sample": f"first {o_events} event(s) of {w.name}: vote (full scan) + peaks + indexed assignment, "
-                     f"{o_secs:.1f} s", "events_per_s": o_events / o_secs, "host_cores_available": os.cpu_count()}
+                     f"{o_secs:.1f} s", "events_per_s": o_events / o_secs, "host_cores_available": os.cpu_count(), "pinned_to_one_core": True}
 
     line = {"metric": METRIC, "value": job_votes / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world,
             "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True,
@@ -857,6 +874,40 @@ def run_efficiency(args):
         plan.close()
 
 
+def run_stage_probe(args):
+    """--stage-probe: hough_vote on a batched fine-phi plan (n_phi = 1024, 1024 events, 64 hits each: the staging sort and
+    its key-start table dominate) -- the cost of the staging sector count (plan.cu caps it by the table size; HOUGH_SECTORS=n
+    in the environment overrides).  One JSON line; not a bench value."""
+    import torch
+    from paper_1311_2769_b200 import HoughPlan
+    from workloads import LAYERS_14
+    n_ev, per = 1024, 64
+    rng = np.random.default_rng(3)
+    r = rng.choice(np.asarray(LAYERS_14), n_ev * per)
+    ph = rng.uniform(0, 2 * np.pi, n_ev * per)
+    hits = np.stack([r * np.cos(ph), r * np.sin(ph)], 1).astype(np.float32)
+    off = (np.arange(n_ev + 1) * per).astype(np.int32)
+    plan = HoughPlan(1024, 128, 1, -1.0, 1.0, -20.0, 20.0, 1, 3.8, LAYERS_14, max_hits=len(hits), max_events=n_ev)
+    d_hits, d_off = torch.from_numpy(hits).cuda(), torch.from_numpy(off).cuda()
+    acc = plan.alloc_accum(n_ev)
+    for _ in range(3):
+        plan.vote(d_hits, d_off, acc)
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ts = []
+    for _ in range(max(args.steps, 20)):
+        a.record()
+        plan.vote(d_hits, d_off, acc)
+        b.record()
+        b.synchronize()
+        ts.append(a.elapsed_time(b))
+    print(json.dumps({"probe": "stage_sectors", "HOUGH_SECTORS": os.environ.get("HOUGH_SECTORS", "default (capped by table size)"),
+                      "plan": "n_phi 1024 x n_qpt 128 x 1, u16, max_events 1024", "hits": len(hits),
+                      "hough_vote_ms_median": statistics.median(ts), "hough_vote_ms_min": min(ts),
+                      "votes": int(acc.to(torch.int64).sum().item())}), flush=True)
+    plan.close()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -878,7 +929,11 @@ def main():
                     help="efficiency / fake / duplicate report against generator truth for these workloads (PAPER.md:43)")
     ap.add_argument("--efficiency-events", type=int, default=8)
     ap.add_argument("--efficiency-scan", action="store_true", help="the paper's toy scenario under a list of other binnings")
+    ap.add_argument("--stage-probe", action="store_true", help="staging cost of a batched n_phi = 1024 plan (sector count)")
     args = ap.parse_args()
+    if args.stage_probe:
+        run_stage_probe(args)
+        return
     if args.efficiency_scan and args.efficiency is None:
         args.efficiency = [5]
     if args.efficiency is not None:

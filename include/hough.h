@@ -130,6 +130,10 @@ int hough_assign_hits(hough_plan* plan, const float* d_hits_xy, int32_t n_hits, 
  * separated by cluster barriers) -- what a latency-bound small event needs; every other case runs the three calls
  * (plan option "event_general" = 1 forces that; "event_cluster" = 1 takes the cluster whenever it fits, ignoring the work
  * estimate hits x longest window <= 160000 that otherwise gates it).  Enqueues on cuda_stream and returns; graph-capturable.
+ * d_event_offsets MUST hold {0, n_hits}: the cluster path takes the event as hits [0, n_hits) and does not read the array
+ * (no device->host read to validate it), the three calls do read it -- other contents give path-dependent results.
+ * A device (or MIG / MPS partition) on which a cluster of that shape cannot be co-scheduled, or a failing cluster launch,
+ * silently takes the three calls instead.
  * Errors: INVALID_ARG (null / misaligned pointers, sizes, assoc_dj > 15), UNSUPPORTED, CUDA. */
 int hough_event_run(hough_plan* plan, const float* d_hits_xy, int32_t n_hits, const int32_t* d_event_offsets,
                     void* d_accum, int32_t threshold, hough_candidate* d_cands, int32_t capacity,

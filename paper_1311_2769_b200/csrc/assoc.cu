@@ -1,5 +1,5 @@
 // assoc.cu -- A5, candidate-centric hit association ("further computations ... to confirm the existence of the
-// track"; D8).  Plan option "assign_candidates" (off by default: measured slower than the column walk, profiles/r2_assoc.md).
+// track"; D8).  Plan option "assign_candidates" (off by default: measured slower than the column walk: 4.6 vs 2.2 ms per 256-event call, profiles/r2_walk.md).
 //
 // D8 asks, for every hit, for the best candidate among those whose column (i, k) the hit votes in within assoc_dj bins
 // of the candidate's bin.  Candidates are few compared with vote positions (config 3: 2.6e4 candidates against 6.4e6
@@ -483,10 +483,7 @@ int hough_assoc_candidates(hough_plan* p, const int32_t* d_event_offsets, int32_
         HOUGH_CUDA_TRY(cudaGetLastError());
         ++launches;
     }
-    if (d_keep_filter)
-        assoc_decode_kernel<true><<<(n_hits + 255) / 256, 256, 0, st>>>(p->d_best_key, p->d_staged, n_hits, d_hit_to_cand, d_cand_nhits);
-    else
-        assoc_decode_kernel<false><<<(n_hits + 255) / 256, 256, 0, st>>>(p->d_best_key, p->d_staged, n_hits, d_hit_to_cand, d_cand_nhits);
+    assoc_decode_kernel<false><<<(n_hits + 255) / 256, 256, 0, st>>>(p->d_best_key, p->d_staged, n_hits, d_hit_to_cand, d_cand_nhits);
     HOUGH_CUDA_TRY(cudaGetLastError());
     hough_count_launches(launches);
     return HOUGH_OK;

@@ -358,15 +358,16 @@ extern "C" int hough_event_run(hough_plan* p, const float* d_hits_xy, int32_t n_
         // more CTAs than the tiles need: every per-bin pass (zero, flush, peaks) and the hit scans shrink with the slab
         while (n_cta > 0 && n_cta < EV_MAX_CLUSTER && (c.n_phi + n_cta) / (n_cta + 1) >= 16) ++n_cta;
     }
-    if (n_cta == 0) {
-        // general path: the three calls (same results)
+    // general path: the three calls (same results)
+    auto general = [&]() -> int {
         int rc = hough_vote(p, d_hits_xy, n_hits, d_event_offsets, 1, d_accum, cuda_stream);
         if (rc != HOUGH_OK) return rc;
         rc = hough_find_peaks(p, d_accum, 1, threshold, d_cands, capacity, d_cand_offsets, cuda_stream);
         if (rc != HOUGH_OK) return rc;
         return hough_assign_hits(p, d_hits_xy, n_hits, d_event_offsets, 1, d_cands, d_cand_offsets, capacity, assoc_dj, min_hits,
                                  d_hit_to_cand, d_cand_nhits, d_cand_keep, cuda_stream);
-    }
+    };
+    if (n_cta == 0) return general();
     EventArgs a{};
     a.hits = reinterpret_cast<const float2*>(d_hits_xy);
     a.n_hits = n_hits;
@@ -401,7 +402,24 @@ extern "C" int hough_event_run(hough_plan* p, const float* d_hits_xy, int32_t n_
     attr[0].val.clusterDim.z = 1;
     cfg.attrs = attr;
     cfg.numAttrs = 1;
-    HOUGH_CUDA_TRY(cudaLaunchKernelEx(&cfg, event_kernel, c, a));
+    // Can a cluster of n_cta such CTAs be co-scheduled on this device at all?  (Not under every MIG / MPS partition, nor on a
+    // GPC with fewer free SMs.)  Asked once per (device, cluster size) with the largest shared-memory block the path uses;
+    // 0 clusters, a failing query or a failing launch send this and later such calls to the general path: same results.
+    static signed char cluster_ok[HOUGH_MAX_DEVICES][EV_MAX_CLUSTER + 1] = {};       // 0: not asked, 1: fits, -1: does not
+    signed char& ok = cluster_ok[dev][n_cta];
+    if (ok == 0 || p->device >= HOUGH_MAX_DEVICES) {
+        cudaLaunchConfig_t q = cfg;
+        q.dynamicSmemBytes = EV_SMEM_BUDGET;
+        int n_clusters = 0;
+        if (cudaOccupancyMaxActiveClusters(&n_clusters, event_kernel, &q) != cudaSuccess) { (void)cudaGetLastError(); n_clusters = 0; }
+        ok = n_clusters > 0 ? 1 : -1;
+    }
+    if (ok < 0) return general();
+    if (cudaLaunchKernelEx(&cfg, event_kernel, c, a) != cudaSuccess) {
+        (void)cudaGetLastError();
+        ok = -1;
+        return general();
+    }
     hough_count_launches(1);
     return HOUGH_OK;
 }

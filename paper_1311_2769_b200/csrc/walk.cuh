@@ -209,8 +209,8 @@ __device__ __forceinline__ FastK make_fastk(const HoughConsts& c, float4 d) {
 //   w_0 = y c - x s at the pair's two columns,   d_0 = w_0 - w_{-1} = -2 sin(wphi) (x c' + y s') with (c', s') of the column
 //   before each (the half-way column of the step) -- no cancellation.
 // The rounding error the recurrence accumulates over a chunk enters the bound m through Ew (walk_kernel prologue).
-// One definition serves the hot loop and the replay of a queued pair (which must reproduce the hot loop's slots bit
-// for bit): explicit PTX operations, no contraction.
+// Nothing is ever replayed: a pair the fast path cannot decide votes into guard slot 0 and is redone with the exact D3
+// sequence from the table (walk_kernel "redo"), so the recurrence only has to stay inside the bound, not be reproducible.
 struct WRec { f32x2 w2, d2; };
 __device__ __forceinline__ WRec wrec_init(const HoughConsts& c, float x, float y, int ca) {      // ca: absolute column, even
     HOUGH_CHECK(ca >= 0 && ca + 1 < c.n_phi && (ca & 1) == 0);
@@ -249,22 +249,6 @@ __device__ __forceinline__ f32x2 wrec_th(f32x2 w2, f32x2 ntd0A2, f32x2 r2Ak2, f3
     upk2(g2, gA, gB);
     return fma2(n2, pk2(rcp_approx(gA), rcp_approx(gB)), c0h2);
 }
-// slots h = J + 1 of the two columns of the pair `steps` pairs after the chunk start at absolute column ca0: the
-// replay of the hot loop (same functions, same operand values)
-__device__ __forceinline__ void wrec_replay_slots(const HoughConsts& c, const FastK& fk, float x, float y, float r2Ak, int ca0,
-                                                  int steps, unsigned& hA, unsigned& hB) {
-    WRec r = wrec_init(c, x, y, ca0);
-    const f32x2 nkap2 = pk2(-c.kappa, -c.kappa);
-    for (int t = 0; t < steps; ++t) wrec_step(r, nkap2);
-    const f32x2 th2 = wrec_th(r.w2, pk2(fk.ntd0A, fk.ntd0A), pk2(r2Ak, r2Ak), pk2(fk.nq_s, fk.nq_s), pk2(fk.d0cq, fk.d0cq),
-                              pk2(fk.c0h, fk.c0h));
-    const f32x2 yb2 = add2(th2, pk2(WALK_MAGIC, WALK_MAGIC));
-    float ybA, ybB;
-    upk2(yb2, ybA, ybB);
-    hA = (unsigned)(__float_as_int(ybA) - (WALK_MAGIC_BITS - 1));
-    hB = (unsigned)(__float_as_int(ybB) - (WALK_MAGIC_BITS - 1));
-}
-
 // Entry of an association tile: (min(votes, VCAP) + 1) << 5 | p,  p = (15 - |dj|) * 2 + (dj < 0), dj = j_cand - j_bin.
 // Integer order of entries == D8 order among the candidates of one row that can serve bin j_bin.
 template <bool TILE32> struct EntryT {               // 16-bit entries: 11 bits of votes + 1
