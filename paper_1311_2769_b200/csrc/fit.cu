@@ -1,11 +1,12 @@
 // fit.cu -- circle fit of the hits assigned to each kept candidate ("further computations (e.g., a full
 // Kalman fit) ... obtain the best measurement of the track parameters"; reading D11: an algebraic
 // Kasa circle fit in double precision stands in for the Kalman fit).
-//   K-fit-a  zero the moment rows of the candidates in use
+//   K-fit-a  zero the moment rows of the candidates that will be fitted (kept ones, or all without keep flags)
 //   K-fit-b  one thread per hit: 9 double atomicAdds {n, Sx, Sy, Sz, Sxx, Sxy, Syy, Sxz, Syz} into its candidate's row
 //   K-fit-c  one thread per candidate: moments about the hits' centroid, 2x2 solve for the centre, D1 parameters in
 //            closed form from (centre, R, orientation) -- a different algebraic route from the 3x3 Cramer solve of the CPU
 //            checker under tests/, so that the parity test compares two independent solves
+#include <algorithm>
 #include <cmath>
 #include <mutex>
 
@@ -13,21 +14,28 @@
 
 namespace {
 
+// K-fit-a: one thread per candidate row (grid-stride over a fixed grid: the list length is only known on the device), and
+// only the rows that will be read -- of 6.6 M candidates per 256-event call of config 3, 48 k are kept.
 __global__ void __launch_bounds__(256) fit_zero_kernel(const int32_t* __restrict__ cand_off, int n_events, int capacity,
-                                                       double* __restrict__ work) {
+                                                       const uint8_t* __restrict__ keep, double* __restrict__ work) {
     const int n_c = min(cand_off[n_events], capacity);
-    const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-    if (t < (long long)n_c * 9) work[t] = 0.0;
+    for (long long ci = (long long)blockIdx.x * blockDim.x + threadIdx.x; ci < n_c; ci += (long long)gridDim.x * blockDim.x) {
+        if (keep && !keep[ci]) continue;
+        double* a = work + (size_t)ci * 9;
+#pragma unroll
+        for (int q = 0; q < 9; ++q) a[q] = 0.0;
+    }
 }
 
 __global__ void __launch_bounds__(256) fit_moments_kernel(const float2* __restrict__ hits, int n_hits,
                                                           const int32_t* __restrict__ hit_to_cand,
                                                           const int32_t* __restrict__ cand_off, int n_events, int capacity,
-                                                          double* __restrict__ work) {
+                                                          const uint8_t* __restrict__ keep, double* __restrict__ work) {
     const int h = blockIdx.x * blockDim.x + threadIdx.x;
     if (h >= n_hits) return;
     const int c = hit_to_cand[h];
     if (c < 0 || c >= min(cand_off[n_events], capacity)) return;
+    if (keep && !keep[c]) return;                            // that row was not zeroed and will not be read
     const float2 p = __ldg(hits + h);
     const double x = (double)p.x, y = (double)p.y;
     const double z = x * x + y * y;
@@ -90,6 +98,8 @@ __global__ void __launch_bounds__(128) fit_solve_kernel(HoughConsts c, double kb
     n_fit[ci] = nf;
 }
 
+inline unsigned fit_zero_blocks(int capacity) { return (unsigned)std::min((capacity + 255) / 256, 148 * 16); }
+
 }  // namespace
 
 extern "C" int hough_fit_circles(hough_plan* p, const float* d_hits_xy, int32_t n_hits, const int32_t* d_hit_to_cand,
@@ -105,12 +115,12 @@ extern "C" int hough_fit_circles(hough_plan* p, const float* d_hits_xy, int32_t 
         return HOUGH_ERR_INVALID_ARG;
     if (capacity == 0) return HOUGH_OK;
     cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
-    const long long cells = (long long)capacity * 9;
-    fit_zero_kernel<<<(unsigned)((cells + 255) / 256), 256, 0, st>>>(d_cand_offsets, n_events, capacity, d_work);
+    fit_zero_kernel<<<fit_zero_blocks(capacity), 256, 0, st>>>(d_cand_offsets, n_events, capacity, d_cand_keep, d_work);
     HOUGH_CUDA_TRY(cudaGetLastError());
     if (n_hits > 0) {
         fit_moments_kernel<<<(n_hits + 255) / 256, 256, 0, st>>>(reinterpret_cast<const float2*>(d_hits_xy), n_hits,
-                                                                 d_hit_to_cand, d_cand_offsets, n_events, capacity, d_work);
+                                                                 d_hit_to_cand, d_cand_offsets, n_events, capacity, d_cand_keep,
+                                                                 d_work);
         HOUGH_CUDA_TRY(cudaGetLastError());
     }
     const double kb = 0.00299792458 * (double)p->bz;
@@ -189,12 +199,12 @@ extern "C" int hough_fit_circles_static(int32_t n_phi, float bz_tesla, const flo
     cudaStream_t st = reinterpret_cast<cudaStream_t>(cuda_stream);
     HoughConsts c{};                   // the solve reads n_phi only (orientation of the circle by the candidate's column)
     c.n_phi = n_phi;
-    const long long cells = (long long)capacity * FIT_STATIC_ROW;
-    fit_zero_kernel<<<(unsigned)((cells + 255) / 256), 256, 0, st>>>(d_cand_offsets, n_events, capacity, d_work);
+    fit_zero_kernel<<<fit_zero_blocks(capacity), 256, 0, st>>>(d_cand_offsets, n_events, capacity, d_cand_keep, d_work);
     HOUGH_CUDA_TRY(cudaGetLastError());
     if (n_hits > 0) {
         fit_moments_kernel<<<(n_hits + 255) / 256, 256, 0, st>>>(reinterpret_cast<const float2*>(d_hits_xy), n_hits,
-                                                                 d_hit_to_cand, d_cand_offsets, n_events, capacity, d_work);
+                                                                 d_hit_to_cand, d_cand_offsets, n_events, capacity, d_cand_keep,
+                                                                 d_work);
         HOUGH_CUDA_TRY(cudaGetLastError());
     }
     const double kb = 0.00299792458 * (double)bz_tesla;
