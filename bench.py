@@ -908,6 +908,21 @@ def run_stage_probe(args):
     plan.close()
 
 
+def run_atoms_probe(args):
+    """--atoms-probe: shared-memory vote rates of hough_microbench kinds 0 / 1 / 5 / 6 / 7 on this GPU (one JSON line):
+    +1 votes (ATOMS.POPC.INC) against + 1 << 16 votes (ATOMS.ADD, the odd column of a packed pair word) on the same
+    addresses, and the latter warp-aggregated with __match_any_sync (B:L5).  Not a bench value."""
+    import torch
+    from paper_1311_2769_b200 import microbench
+    torch.cuda.init()
+    names = {0: "add_1_conflict_free", 1: "add_1_random_64KB", 5: "add_1_random_bin_of_one_row_per_warp",
+             6: "add_65536_same_addresses_as_5", 7: "add_65536_match_any_leader_same_addresses_as_5"}
+    out = {"probe": "shared_atomics", "unit": "Gops/s (lane operations)"}
+    for k, n in names.items():
+        out[n] = microbench(k, 0, 5) / 1e9
+    print(json.dumps(out), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -930,7 +945,11 @@ def main():
     ap.add_argument("--efficiency-events", type=int, default=8)
     ap.add_argument("--efficiency-scan", action="store_true", help="the paper's toy scenario under a list of other binnings")
     ap.add_argument("--stage-probe", action="store_true", help="staging cost of a batched n_phi = 1024 plan (sector count)")
+    ap.add_argument("--atoms-probe", action="store_true", help="shared-memory atomic rates: +1, +65536, match_any-aggregated")
     args = ap.parse_args()
+    if args.atoms_probe:
+        run_atoms_probe(args)
+        return
     if args.stage_probe:
         run_stage_probe(args)
         return

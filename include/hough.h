@@ -284,6 +284,8 @@ int hough_window_table(const hough_binning* binning, const hough_geometry* geome
  *   4 = fp32 issue rate of the D3 vote sequence (no memory), evaluations per second
  *   5 = shared-memory atomicAdd(u32), every warp adds to random bins of one 128-bin row (same-address collisions
  *       included): the address pattern closest to the vote walk's
+ *   6 = kind 5's addresses with atomicAdd(u32, 1 << 16): the vote of the odd column of a packed 16-bit pair word
+ *   7 = kind 6 warp-aggregated: __match_any_sync on the word, one leader adds (lanes << 16)   (B:L5 "warp-aggregated atomics")
  * Errors: INVALID_ARG (unknown kind, iters <= 0, NULL ops_per_s), CUDA. */
 int hough_microbench(int32_t kind, size_t region_bytes, int32_t iters, double* ops_per_s, void* cuda_stream);
 

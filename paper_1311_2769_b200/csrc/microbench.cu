@@ -42,6 +42,22 @@ __global__ void __launch_bounds__(MB_THREADS) mb_smem_atomic(int mode, unsigned*
             const unsigned row = ((threadIdx.x >> 5) * 16u + (it & 15)) * 128u;
             atomicAdd(&s_tile[(row + (state >> 27) * 1u) & (MB_WORDS - 1)], 1u);
         }
+    } else if (mode == 6) {     // kind 5's addresses, but the vote of the ODD column of a packed pair word: + 1 << 16
+#pragma unroll 8
+        for (int it = 0; it < MB_ITERS; ++it) {
+            state = state * 1664525u + 1013904223u;
+            const unsigned row = ((threadIdx.x >> 5) * 16u + (it & 15)) * 128u;
+            atomicAdd(&s_tile[(row + (state >> 27) * 1u) & (MB_WORDS - 1)], 65536u);
+        }
+    } else if (mode == 7) {     // kind 6 with warp-aggregated adds: __match_any_sync on the word, the leader adds count << 16
+#pragma unroll 8
+        for (int it = 0; it < MB_ITERS; ++it) {
+            state = state * 1664525u + 1013904223u;
+            const unsigned row = ((threadIdx.x >> 5) * 16u + (it & 15)) * 128u;
+            const unsigned word = (row + (state >> 27) * 1u) & (MB_WORDS - 1);
+            const unsigned peers = __match_any_sync(0xffffffffu, word);
+            if ((peers & ((1u << (threadIdx.x & 31)) - 1u)) == 0u) atomicAdd(&s_tile[word], (unsigned)__popc(peers) << 16);
+        }
     }
     __syncthreads();
     unsigned acc = 0;
@@ -96,7 +112,7 @@ extern "C" int hough_microbench(int32_t kind, size_t region_bytes, int32_t iters
         HOUGH_CUDA_TRY(cudaMalloc(&d_region, words * 4));
         HOUGH_CUDA_TRY(cudaMemsetAsync(d_region, 0, words * 4, st));
     }
-    if (kind == 0 || kind == 1 || kind == 2 || kind == 5)
+    if (kind == 0 || kind == 1 || kind == 2 || (kind >= 5 && kind <= 7))
         HOUGH_CUDA_TRY(cudaFuncSetAttribute(mb_smem_atomic, cudaFuncAttributeMaxDynamicSharedMemorySize, MB_WORDS * 4));
     HoughConsts c{};
     c.A_f = 0.0056960564f; c.qmin = -1.0f; c.inv_wq = 64.0f; c.nq_f = 128.0f;
@@ -104,7 +120,7 @@ extern "C" int hough_microbench(int32_t kind, size_t region_bytes, int32_t iters
     for (int it = 0; it < iters + 1; ++it) {
         HOUGH_CUDA_TRY(cudaEventRecord(e0, st));
         switch (kind) {
-            case 0: case 1: case 2: case 5:
+            case 0: case 1: case 2: case 5: case 6: case 7:
                 mb_smem_atomic<<<grid_smem, MB_THREADS, MB_WORDS * 4, st>>>(kind, d_sink);
                 ops = (double)grid_smem * MB_THREADS * MB_ITERS;
                 break;
