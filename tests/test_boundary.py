@@ -63,3 +63,24 @@ def test_product_does_not_import_oracle():
             src = open(os.path.join(ROOT, "oracle", f)).read()
             assert "import paper_1311_2769_b200" not in src and "from paper_1311_2769_b200" not in src
             assert "libhough_b200" not in src and "csrc" not in src
+
+
+def test_static_fit_refuses_oversized_lists_before_any_cuda_call(lib_path):
+    """hough_fit_circles_static keeps its scratch in a fixed array: a candidate capacity beyond
+    HOUGH_FIT_STATIC_MAX_CANDIDATES must come back as HOUGH_ERR_TOO_LARGE (-5) with a message that names the limit, and
+    plain argument errors as INVALID_ARG -- both decided on the host, so this runs without a GPU."""
+    header = open(os.path.join(ROOT, "include", "hough.h")).read()
+    limit = int(re.search(r"#define\s+HOUGH_FIT_STATIC_MAX_CANDIDATES\s+(\d+)", header).group(1))
+    from paper_1311_2769_b200 import FIT_STATIC_MAX_CANDIDATES, load_library
+    assert FIT_STATIC_MAX_CANDIDATES == limit
+    lib = load_library()
+    dummy = ctypes.create_string_buffer(64)                       # never dereferenced: the checks come first
+    p = ctypes.cast(dummy, ctypes.c_void_p)
+    rc = lib.hough_fit_circles_static(256, 3.8, None, 0, None, p, p, 1, limit + 1, None, p, p, None)
+    assert rc == -5
+    msg = lib.hough_status_string(rc)
+    assert b"HOUGH_FIT_STATIC_MAX_CANDIDATES" in msg and b"no-allocation" in msg
+    assert lib.hough_fit_circles_static(0, 3.8, None, 0, None, p, p, 1, 1, None, p, p, None) == -1      # n_phi <= 0
+    assert lib.hough_fit_circles_static(256, 3.8, None, 0, None, p, None, 1, 1, None, p, p, None) == -1  # no offsets
+    assert lib.hough_fit_circles_static(256, 3.8, None, 5, None, p, p, 1, 1, None, p, p, None) == -1     # hits without pointers
+    assert lib.hough_fit_circles_static(256, 3.8, None, 0, None, p, p, 1, 0, None, None, None, None) == 0  # capacity 0: no-op
