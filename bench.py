@@ -136,8 +136,8 @@ def load_peaks():
 
 def load_traffic():
     """dram__bytes_read.sum + dram__bytes_write.sum per launch from the committed ncu --set full capture
-    (profiles/r2_traffic.csv: kernel,tile_events,dram_bytes; the command is in profiles/r2_traffic.md).  ({}, None) if absent."""
-    path = os.path.join(ROOT, "profiles", "r2_traffic.csv")
+    (profiles/r3_traffic.csv: kernel,tile_events,dram_bytes; the command is in profiles/r3_traffic.md).  ({}, None) if absent."""
+    path = os.path.join(ROOT, "profiles", "r3_traffic.csv")
     tab = {}
     if not os.path.exists(path):
         return tab, None
@@ -149,8 +149,8 @@ def load_traffic():
                 stamp = "kernels as of commit %s, %s" % (p[1], p[2].split(" ")[0])
             elif len(p) >= 3 and p[1].isdigit():
                 tab[(p[0], int(p[1]))] = float(p[2])
-    return tab, ("profiles/r2_traffic.csv (ncu --set full capture of this launch configuration, %s -- NOT measured in this "
-                 "run: stale if walk.cuh / peaks.cu changed since; see profiles/r2_traffic.md)" % stamp)
+    return tab, ("profiles/r3_traffic.csv (ncu --set full capture of this launch configuration, %s -- NOT measured in this "
+                 "run: stale if walk.cuh / peaks.cu changed since; see profiles/r3_traffic.md)" % stamp)
 
 
 # ----------------------------------------------------------------------------------------------
